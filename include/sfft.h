@@ -1,0 +1,115 @@
+/* sfft.h -- C ABI of libsfft.so: B200 (sm_100a) SFFT image differencing of one aligned
+ * reference/science CCD pair.
+ *
+ * Method: PAPER.md:40 (§1) "formulates the image subtraction problem in the Fourier domain and
+ * accounts for spatial variations in the point-spread function ... convolution kernel is
+ * modeled with a delta-function basis"; used once per science image (§2.3.2).
+ * The paper prints no equations; BASELINE.json `north_star` fixes the problem, SURVEY.md §8.0
+ * and DESIGN.md ("Readings") fix every convention used below:
+ *
+ *   D = S - ( R (x) K(x,y) + B(x,y) ),  circular convolution on the H x W grid,
+ *   xi(x) = (2x+1-W)/W, eta(y) = (2y+1-H)/H, monomials P_t = xi^p eta^q ordered
+ *     for d in 0..D: for q in 0..d: p = d-q,
+ *   shifts s <-> (u,v), u,v in [-w,w], s = (v+w)(2w+1)+(u+w), u along x (fastest axis),
+ *   model  M(x,y) = sum_t sum_s a[s,t] (P_t R)((x-u) mod W,(y-v) mod H) + sum_t' beta[t'] P_t'(x,y)
+ *   coefficient vector c (length N = (2w+1)^2 (DK+1)(DK+2)/2 + (DB+1)(DB+2)/2):
+ *     c[t*L + s] = a[s,t]  (L = (2w+1)^2),  c[L*T_K + t'] = beta[t'],
+ *   fit: good-pixel indicator m = (mask==0); R~_t = m P_t R, S~ = m S, Psi_t' = m P_t';
+ *     A = G^T G, b = G^T S~ with G's columns the shifted R~_t and the Psi_t'  (normal equations,
+ *     no weights, no regularisation); c = A^-1 b by Cholesky.
+ *
+ * Memory: every image/matrix pointer below is a DEVICE pointer owned by the caller, 16-byte
+ * aligned, contiguous; images are H rows x W columns, row-major, element (y,x) at y*W+x, fp64.
+ * The library never allocates, frees or modifies caller buffers other than the stated outputs.
+ * The four hot calls only enqueue work on `stream` (a cudaStream_t passed as void*; NULL = the
+ * legacy default stream): they never synchronise the stream or the device.  A plan owns scratch
+ * memory and is NOT re-entrant: use one plan per stream in flight.  No call throws; every call
+ * returns an sfft_status.  There is no CPU fallback: without a CUDA device plan creation fails.
+ */
+#ifndef SFFT_H
+#define SFFT_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sfft_plan sfft_plan; /* opaque; owns workspace, twiddle and index tables */
+
+typedef enum {
+  SFFT_OK = 0,
+  SFFT_ERR_INVALID_ARG = 1, /* NULL where not allowed, misaligned pointer, bad sizes */
+  SFFT_ERR_UNSUPPORTED = 2, /* size/degree outside what this build supports */
+  SFFT_ERR_ALLOC = 3,       /* cudaMalloc / host allocation failed */
+  SFFT_ERR_CUDA = 4         /* a CUDA runtime call or launch failed (incl. no device) */
+} sfft_status;
+
+/* Create a plan for H x W images, kernel half-width w, polynomial degrees DK (kernel) and DB
+ * (background).  Supported: H, W powers of two, 16 <= H, W <= 4096; 0 <= w, 4w+1 <= min(H,W),
+ * w <= 15; 0 <= DK, DB <= 3.  Otherwise SFFT_ERR_UNSUPPORTED.  Allocates scratch on the current
+ * device and uploads tables; may synchronise.  *out is set to NULL on failure.
+ * (north_star: sfft_plan_create(H,W,w,DK,DB).) */
+sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int DB);
+
+/* Free a plan and its scratch.  The caller must have synchronised every stream that used it. */
+sfft_status sfft_plan_destroy(sfft_plan* p);
+
+/* N, the number of unknowns (length of b and coeffs, order of A).  -1 if p is NULL. */
+int sfft_num_coeffs(const sfft_plan* p);
+
+/* Bytes of device scratch the plan owns (0 if p is NULL). */
+size_t sfft_workspace_bytes(const sfft_plan* p);
+
+/* Static, human-readable name of a status code. */
+const char* sfft_status_string(sfft_status s);
+
+/* Build the normal equations (north_star subsystems (1)-(4)):
+ * weighted masked images -> batched fp64 2-D real FFTs -> Fourier-domain cross products and
+ * inverse transforms restricted to the lag window -> gather into A and b.
+ *   R, S  in : H*W fp64 (device).      mask in: H*W uint8 (device), nonzero = excluded; NULL = none.
+ *   A    out : N*N fp64 row-major, FULL symmetric matrix (both triangles written).
+ *   b    out : N fp64.
+ * Errors: INVALID_ARG on NULL p/R/S/A/b or misalignment; CUDA on a launch failure. */
+sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S,
+                              const unsigned char* mask, double* A, double* b, void* stream);
+
+/* Solve A c = b by blocked fp64 Cholesky + two triangular solves (north_star (5), a5).
+ *   A, b in (device, not modified; only the lower triangle of A is read), coeffs out: N fp64.
+ *   info out (device int, may be NULL): 0 = ok; k > 0 = the leading minor of order k is not
+ *   positive (A not positive definite; coeffs are then unspecified).  Reported on the device so
+ *   the stream is never stalled. */
+sfft_status sfft_solve(sfft_plan* p, const double* A, const double* b, double* coeffs,
+                       int* info, void* stream);
+
+/* Apply the fitted spatially varying kernel and background and subtract (north_star (6), a6):
+ * D = S - M, on EVERY pixel from the raw (unmasked) R and S.
+ *   R, S in: H*W fp64; coeffs in: N fp64 (device); D out: H*W fp64, must not alias R or S. */
+sfft_status sfft_subtract(sfft_plan* p, const double* R, const double* S, const double* coeffs,
+                          double* D, void* stream);
+
+/* ---- diagnostics (not on the hot path) ------------------------------------------------------ */
+
+/* Per-stage device times of the most recent build/solve/subtract calls are NOT recorded by the
+ * hot calls (they never synchronise).  This helper runs a dependent-free DFMA loop on every SM
+ * for `iters` iterations on `stream`, synchronises it, and returns the achieved fp64 rate in
+ * *tflops: the measured FP64-pipe peak used as the "alu" roofline denominator.
+ * kind = 0: DFMA (CUDA-core fp64 pipe); kind = 1: DMMA (mma.sync m8n8k4 f64). */
+sfft_status sfft_probe_fp64(int kind, int iters, double* tflops, double* elapsed_ms, void* stream);
+
+/* Number of kernel launches the last call of each hot entry point enqueued (host-side counter,
+ * for bench.py's "gpu_launches"): which = 0 build, 1 solve, 2 subtract.  -1 on bad arguments. */
+int sfft_last_launch_count(const sfft_plan* p, int which);
+
+/* Name and launch count of the dominant kernels, for bench.py's roofline section: fills
+ * flops/bytes the algorithmic model in DESIGN.md assigns to ONE call of entry point `which`
+ * (0 build, 1 solve, 2 subtract) at this plan's sizes.  Either output may be NULL. */
+sfft_status sfft_model_cost(const sfft_plan* p, int which, double* fp64_instr, double* hbm_bytes);
+
+/* Library version string, e.g. "sfft-b200 0.1 (sm_100a)". */
+const char* sfft_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SFFT_H */

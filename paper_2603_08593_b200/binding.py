@@ -1,0 +1,208 @@
+"""ctypes binding of libsfft.so (include/sfft.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI.  PyTorch is used for
+device memory and streams only.  There is NO CPU fallback: if the library is missing or no CUDA
+device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_NAME = "libsfft.so"
+
+# every symbol include/sfft.h declares (tests check the built library exports all of them)
+EXPORTED_SYMBOLS = [
+    "sfft_plan_create", "sfft_plan_destroy", "sfft_num_coeffs", "sfft_workspace_bytes",
+    "sfft_status_string", "sfft_build_system", "sfft_solve", "sfft_subtract",
+    "sfft_probe_fp64", "sfft_last_launch_count", "sfft_model_cost", "sfft_version",
+]
+
+
+class SfftError(RuntimeError):
+    def __init__(self, code: int, where: str, text: str):
+        super().__init__(f"{where}: {text} (sfft_status {code})")
+        self.code = code
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, _LIB_NAME)
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree libsfft.so and declare the prototypes.  Raises if it is not built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if not os.path.exists(path):
+        raise FileNotFoundError(
+            f"{path} is not built: run `python -c 'import __graft_entry__ as g; g.build()'` "
+            "(there is no CPU fallback for the SFFT hot path)")
+    lib = ctypes.CDLL(path)
+    vp, i32, dbl_p = ctypes.c_void_p, ctypes.c_int, ctypes.POINTER(ctypes.c_double)
+    lib.sfft_plan_create.argtypes = [ctypes.POINTER(vp), i32, i32, i32, i32, i32]
+    lib.sfft_plan_create.restype = i32
+    lib.sfft_plan_destroy.argtypes = [vp]
+    lib.sfft_plan_destroy.restype = i32
+    lib.sfft_num_coeffs.argtypes = [vp]
+    lib.sfft_num_coeffs.restype = i32
+    lib.sfft_workspace_bytes.argtypes = [vp]
+    lib.sfft_workspace_bytes.restype = ctypes.c_size_t
+    lib.sfft_status_string.argtypes = [i32]
+    lib.sfft_status_string.restype = ctypes.c_char_p
+    lib.sfft_build_system.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    lib.sfft_build_system.restype = i32
+    lib.sfft_solve.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.sfft_solve.restype = i32
+    lib.sfft_subtract.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.sfft_subtract.restype = i32
+    lib.sfft_probe_fp64.argtypes = [i32, i32, dbl_p, dbl_p, vp]
+    lib.sfft_probe_fp64.restype = i32
+    lib.sfft_last_launch_count.argtypes = [vp, i32]
+    lib.sfft_last_launch_count.restype = i32
+    lib.sfft_model_cost.argtypes = [vp, i32, dbl_p, dbl_p]
+    lib.sfft_model_cost.restype = i32
+    lib.sfft_version.argtypes = []
+    lib.sfft_version.restype = ctypes.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(lib, code: int, where: str):
+    if code != 0:
+        raise SfftError(code, where, lib.sfft_status_string(code).decode())
+
+
+def _stream_handle(stream) -> Optional[int]:
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+def _dev_ptr(t, dtype, numel, name):
+    import torch
+    if t is None:
+        return ctypes.c_void_p(0)
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name}: expected a CUDA tensor (device memory is the caller's)")
+    if t.dtype != dtype or not t.is_contiguous() or t.numel() != numel:
+        raise ValueError(f"{name}: need contiguous {dtype} with {numel} elements, got "
+                         f"{t.dtype} {tuple(t.shape)} contiguous={t.is_contiguous()}")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+class SfftPlan:
+    """sfft_plan_create / sfft_build_system / sfft_solve / sfft_subtract with torch CUDA tensors.
+
+    All methods only enqueue work on the given (default: current) torch stream.
+    """
+
+    def __init__(self, H: int, W: int, w: int, DK: int, DB: int):
+        self._lib = load_library()
+        self._p = ctypes.c_void_p(0)
+        _check(self._lib, self._lib.sfft_plan_create(ctypes.byref(self._p), H, W, w, DK, DB),
+               "sfft_plan_create")
+        self.H, self.W, self.w, self.DK, self.DB = H, W, w, DK, DB
+        self.N = self._lib.sfft_num_coeffs(self._p)
+
+    # -- lifetime
+    def close(self):
+        if getattr(self, "_p", None) is not None and self._p.value:
+            self._lib.sfft_plan_destroy(self._p)
+            self._p = ctypes.c_void_p(0)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    @property
+    def workspace_bytes(self) -> int:
+        return int(self._lib.sfft_workspace_bytes(self._p))
+
+    # -- the four hot calls
+    def build_system(self, R, S, mask, A=None, b=None, stream=None):
+        import torch
+        P = self.H * self.W
+        if A is None:
+            A = torch.empty((self.N, self.N), dtype=torch.float64, device=R.device)
+        if b is None:
+            b = torch.empty(self.N, dtype=torch.float64, device=R.device)
+        _check(self._lib, self._lib.sfft_build_system(
+            self._p, _dev_ptr(R, torch.float64, P, "R"), _dev_ptr(S, torch.float64, P, "S"),
+            _dev_ptr(mask, torch.uint8, P, "mask"), _dev_ptr(A, torch.float64, self.N * self.N, "A"),
+            _dev_ptr(b, torch.float64, self.N, "b"), _stream_handle(stream)), "sfft_build_system")
+        return A, b
+
+    def solve(self, A, b, coeffs=None, info=None, stream=None):
+        import torch
+        if coeffs is None:
+            coeffs = torch.empty(self.N, dtype=torch.float64, device=A.device)
+        if info is None:
+            info = torch.zeros(1, dtype=torch.int32, device=A.device)
+        _check(self._lib, self._lib.sfft_solve(
+            self._p, _dev_ptr(A, torch.float64, self.N * self.N, "A"),
+            _dev_ptr(b, torch.float64, self.N, "b"), _dev_ptr(coeffs, torch.float64, self.N, "coeffs"),
+            _dev_ptr(info, torch.int32, 1, "info"), _stream_handle(stream)), "sfft_solve")
+        return coeffs, info
+
+    def subtract(self, R, S, coeffs, D=None, stream=None):
+        import torch
+        P = self.H * self.W
+        if D is None:
+            D = torch.empty((self.H, self.W), dtype=torch.float64, device=R.device)
+        _check(self._lib, self._lib.sfft_subtract(
+            self._p, _dev_ptr(R, torch.float64, P, "R"), _dev_ptr(S, torch.float64, P, "S"),
+            _dev_ptr(coeffs, torch.float64, self.N, "coeffs"), _dev_ptr(D, torch.float64, P, "D"),
+            _stream_handle(stream)), "sfft_subtract")
+        return D
+
+    def difference(self, R, S, mask, stream=None):
+        """One pass of the whole hot path: build -> solve -> subtract (device tensors in/out)."""
+        A, b = self.build_system(R, S, mask, stream=stream)
+        c, info = self.solve(A, b, stream=stream)
+        D = self.subtract(R, S, c, stream=stream)
+        return A, b, c, info, D
+
+    def difference_host(self, R_host, S_host, mask_host, stream=None):
+        """End-to-end call with HOST (pinned) buffers: H2D copies, hot path, D2H of D and coeffs."""
+        import torch
+        dev = torch.device("cuda", torch.cuda.current_device())
+        R = R_host.to(dev, non_blocking=True)
+        S = S_host.to(dev, non_blocking=True)
+        mask = None if mask_host is None else mask_host.to(dev, non_blocking=True)
+        A, b, c, info, D = self.difference(R, S, mask, stream=stream)
+        return D.to("cpu", non_blocking=False), c.to("cpu"), info.to("cpu")
+
+    # -- diagnostics
+    def last_launch_count(self, which: int) -> int:
+        return int(self._lib.sfft_last_launch_count(self._p, which))
+
+    def model_cost(self, which: int):
+        fi, hb = ctypes.c_double(0), ctypes.c_double(0)
+        _check(self._lib, self._lib.sfft_model_cost(self._p, which, ctypes.byref(fi), ctypes.byref(hb)),
+               "sfft_model_cost")
+        return fi.value, hb.value
+
+
+def probe_fp64(kind: int = 0, iters: int = 4096, stream=None):
+    """Measured fp64 peak (TFLOP/s) of the DFMA (kind 0) or DMMA (kind 1) pipe."""
+    lib = load_library()
+    tf, ms = ctypes.c_double(0), ctypes.c_double(0)
+    _check(lib, lib.sfft_probe_fp64(kind, iters, ctypes.byref(tf), ctypes.byref(ms),
+                                    _stream_handle(stream)), "sfft_probe_fp64")
+    return tf.value, ms.value
