@@ -46,8 +46,8 @@ typedef enum {
 } sfft_status;
 
 /* Create a plan for H x W images, kernel half-width w, polynomial degrees DK (kernel) and DB
- * (background).  Supported: H, W powers of two, 16 <= H, W <= 4096; 0 <= w, 4w+1 <= min(H,W),
- * w <= 15; 0 <= DK, DB <= 3.  Otherwise SFFT_ERR_UNSUPPORTED.  Allocates scratch on the current
+ * (background).  Supported: H, W powers of two, 32 <= H, W <= 4096; 0 <= w <= 5 (this build),
+ * 4w+1 <= min(H,W); 0 <= DK, DB <= 3.  Otherwise SFFT_ERR_UNSUPPORTED.  Allocates scratch on the current
  * device and uploads tables; may synchronise.  *out is set to NULL on failure.
  * (north_star: sfft_plan_create(H,W,w,DK,DB).) */
 sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int DB);

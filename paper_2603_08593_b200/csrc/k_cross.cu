@@ -1,0 +1,275 @@
+// Fourier-domain cross products, lag-window inverse transforms and the gather into A, b
+// (north_star subsystems (3),(4)).
+//
+// Only the (2D+1)^2 lags |dy|,|dx| <= D (D = 2w for kernel-kernel pairs, w otherwise) of each
+// cross-correlation map C_{f,g} = irfft2(conj F_f . F_g) are ever read, so the inverse transform
+// is evaluated only there:
+//
+//  k_cross<D>   : for every column kx, Y[dy][kx] = sum_ky conj(F_f) F_g e^{+2 pi i ky dy/H}, |dy|<=D.
+//                 Output-pruned decimation: ky = b + (H/8) a, so
+//                 Y[dy] = sum_b e^{2 pi i b dy/H} Z_b[dy mod 8],  Z_b = 8-point inverse DFT over a.
+//                 One thread owns one column (lanes = adjacent kx -> 512-byte coalesced rows);
+//                 the 2D+1 accumulators live in registers; no shared memory, no reduction.
+//  k_lag_idft   : C[dy][dx] = (1/P) [ Re Y[dy][0] + (-1)^dx Re Y[dy][NC]
+//                                     + 2 sum_{kx=1}^{NC-1} Re( Y[dy][kx] e^{2 pi i kx dx/W} ) ].
+//  k_mom_final  : reduces the per-row moments of k_row_fwd to sum m xi^a eta^b and sum m xi^p eta^q S.
+//  k_gather     : A[tL+s, t'L+s'] = C_{t,t'}[(u-u', v-v')], b[tL+s] = C_{t,S}[(u,v)],
+//                 A[tL+s, B t'] = C_{t,Psi t'}[(u,v)], A[B,B] and b_B from the moments.
+#include "fft_smem.cuh"
+
+struct CrossParams {
+  const cplx* F;
+  cplx* Y;
+  const PairDesc* pairs;
+  int pair0, npair;   // pairs [pair0, pair0+npair) share the same D
+  int H, NC, pitch, nLag;
+  const cplx* twH;
+};
+
+template <int D>
+__global__ void __launch_bounds__(128) k_cross(CrossParams P) {
+  const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
+  const int pi = blockIdx.y * 4 + wrp;
+  if (pi >= P.npair) return;
+  const PairDesc pd = P.pairs[P.pair0 + pi];
+  int kx = blockIdx.x * 32 + lane;
+  const bool active = kx <= P.NC;
+  if (!active) kx = P.NC;
+  const size_t specStride = (size_t)P.H * P.pitch;
+  const cplx* Fa = P.F + pd.fa * specStride + kx;
+  const cplx* Fb = P.F + pd.fb * specStride + kx;
+  const int N1 = P.H >> 3;
+  const size_t rstep = (size_t)N1 * P.pitch;
+  cplx acc[2 * D + 1];
+#pragma unroll
+  for (int i = 0; i < 2 * D + 1; ++i) acc[i] = cmake(0.0, 0.0);
+  for (int b = 0; b < N1; ++b) {
+    cplx x[8];
+    const cplx* pa = Fa + (size_t)b * P.pitch;
+    const cplx* pb = Fb + (size_t)b * P.pitch;
+#pragma unroll
+    for (int a = 0; a < 8; ++a) x[a] = cmulc(ldg2(pa + a * rstep), ldg2(pb + a * rstep));
+    Dft<8, +1>::run(x);
+    acc[D] = cadd(acc[D], x[0]);
+#pragma unroll
+    for (int i = 1; i <= D; ++i) {
+      const cplx t = ldg2(P.twH + ((b * i) & (P.H - 1)));  // e^{-2 pi i b i/H}
+      cfmac(acc[D + i], t, x[i & 7]);                      // += e^{+...} * Z[i mod 8]
+      cfma(acc[D - i], t, x[(8 - (i & 7)) & 7]);           // += e^{-...} * Z[-i mod 8]
+    }
+  }
+  if (active) {
+    cplx* out = P.Y + ((size_t)(P.pair0 + pi) * P.nLag) * P.pitch + kx;
+#pragma unroll
+    for (int i = 0; i < 2 * D + 1; ++i) {
+      const int dy = i - D;  // the instantiated range may exceed the pair's own half-range pd.D
+      if (dy >= -pd.D && dy <= pd.D) out[(size_t)(dy + pd.D) * P.pitch] = acc[i];
+    }
+  }
+}
+
+template <int D>
+static sfft_status launch_cross_t(const CrossParams& P, cudaStream_t st) {
+  dim3 grid((P.NC + 1 + 31) / 32, (P.npair + 3) / 4);
+  k_cross<D><<<grid, 128, 0, st>>>(P);
+  SFFT_LAUNCH_CHECK();
+  return SFFT_OK;
+}
+
+static sfft_status launch_cross_D(int D, const CrossParams& P, cudaStream_t st) {
+  switch (D) {
+    case 0: case 1: return launch_cross_t<1>(P, st);
+    case 2: return launch_cross_t<2>(P, st);
+    case 3: return launch_cross_t<3>(P, st);
+    case 4: return launch_cross_t<4>(P, st);
+    case 5: return launch_cross_t<5>(P, st);
+    case 6: return launch_cross_t<6>(P, st);
+    case 7: case 8: return launch_cross_t<8>(P, st);
+    case 9: case 10: return launch_cross_t<10>(P, st);
+    default: return SFFT_ERR_UNSUPPORTED;
+  }
+}
+
+sfft_status sfft_launch_cross(sfft_plan* p, cudaStream_t st, int* nl) {
+  CrossParams P;
+  P.F = p->F; P.Y = p->Y; P.pairs = p->d_pairs; P.H = p->H; P.NC = p->NC; P.pitch = p->pitch;
+  P.nLag = p->nLag; P.twH = p->twH;
+  // pairs are sorted: kernel-kernel (D = 2w) first, then the D = w pairs
+  const int nKK = p->TK * (p->TK + 1) / 2;
+  P.pair0 = 0; P.npair = nKK;
+  ++*nl;
+  sfft_status s = launch_cross_D(2 * p->w, P, st);
+  if (s != SFFT_OK) return s;
+  P.pair0 = nKK; P.npair = p->nPair - nKK;
+  ++*nl;
+  return launch_cross_D(p->w, P, st);
+}
+
+// ------------------------------------------------------------------------------------------------
+
+struct LagParams {
+  const cplx* Y;
+  double* Cmap;  // [nPair][nLag][nLag]; pair with half-range D uses rows/cols [0, 2D]
+  const PairDesc* pairs;
+  int NC, W, pitch, nLag;
+  double invP;
+  const cplx* twW;
+};
+
+__global__ void __launch_bounds__(256) k_lag_idft(LagParams P) {
+  const int pair = blockIdx.x, dyi = blockIdx.y;
+  const int D = P.pairs[pair].D;
+  if (dyi > 2 * D) return;
+  const int lane = threadIdx.x & 31, slice = threadIdx.x >> 5;  // 8 slices over kx
+  const cplx* Yr = P.Y + ((size_t)pair * P.nLag + dyi) * P.pitch;
+  __shared__ double red[2][8][32];
+  double ap[2] = {0.0, 0.0}, am[2] = {0.0, 0.0};
+  const int dx = lane;
+  if (dx <= D) {
+    int it = 0;
+    for (int kx = 1 + slice; kx < P.NC; kx += 8, ++it) {
+      const cplx y = Yr[kx];
+      const cplx t = ldg2(P.twW + ((kx * dx) & (P.W - 1)));  // (c, -s)
+      const double pc = y.x * t.x, qs = y.y * (-t.y);
+      ap[it & 1] += pc - qs;  // Re(y e^{+i th})
+      am[it & 1] += pc + qs;  // Re(y e^{-i th})
+    }
+  }
+  red[0][slice][lane] = ap[0] + ap[1];
+  red[1][slice][lane] = am[0] + am[1];
+  __syncthreads();
+  if (slice == 0 && dx <= D) {
+    double sp = 0.0, sm = 0.0;
+    for (int k = 0; k < 8; k += 2) {
+      sp += red[0][k][lane] + red[0][k + 1][lane];
+      sm += red[1][k][lane] + red[1][k + 1][lane];
+    }
+    const double y0 = Yr[0].x, yn = Yr[P.NC].x;
+    const double sgn = (dx & 1) ? -1.0 : 1.0;
+    double* out = P.Cmap + ((size_t)pair * P.nLag + dyi) * P.nLag;
+    out[D + dx] = (y0 + sgn * yn + 2.0 * sp) * P.invP;
+    out[D - dx] = (y0 + sgn * yn + 2.0 * sm) * P.invP;
+  }
+}
+
+struct MomParams {
+  const double* rowMom;  // [nMomA + nMomS][H]
+  double* mom;           // [nMomA*nMomA] then [TB]
+  int H, nMomA, nMomS, TB;
+  int monoB[SFFT_MAX_T][2];
+};
+
+__global__ void __launch_bounds__(256) k_mom_final(MomParams P) {
+  // block q < nMomA^2: (a,b) = (q / nMomA, q % nMomA) -> sum_y eta^b rowMom[a][y]
+  // block q >= nMomA^2: background rhs t' -> sum_y eta^q rowMomS[p][y]
+  const int q = blockIdx.x;
+  int row, pw;
+  if (q < P.nMomA * P.nMomA) {
+    row = q / P.nMomA;
+    pw = q % P.nMomA;
+  } else {
+    const int t = q - P.nMomA * P.nMomA;
+    row = P.nMomA + P.monoB[t][0];
+    pw = P.monoB[t][1];
+  }
+  const double* src = P.rowMom + (size_t)row * P.H;
+  const double invH = 1.0 / (double)P.H;
+  double acc = 0.0;
+  for (int y = threadIdx.x; y < P.H; y += 256)
+    acc += ipow((double)(2 * y + 1 - P.H) * invH, pw) * src[y];
+  __shared__ double red[256];
+  red[threadIdx.x] = acc;
+  __syncthreads();
+  for (int off = 128; off > 0; off >>= 1) {
+    if (threadIdx.x < off) red[threadIdx.x] += red[threadIdx.x + off];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) P.mom[q] = red[0];
+}
+
+struct GatherParams {
+  const double* Cmap;
+  const double* mom;
+  double* A;
+  double* b;
+  int w, L, TK, TB, N, nLag, nMomA;
+  int monoB[SFFT_MAX_T][2];
+};
+
+__global__ void __launch_bounds__(256) k_gather(GatherParams P) {
+  const int N = P.N, L = P.L, w = P.w, S1 = 2 * w + 1;
+  const int nK = L * P.TK;
+  const int nKK = P.TK * (P.TK + 1) / 2;
+  const size_t lag2 = (size_t)P.nLag * P.nLag;
+  const size_t total = (size_t)N * N + N;
+  for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total;
+       e += (size_t)gridDim.x * blockDim.x) {
+    if (e >= (size_t)N * N) {  // right-hand side
+      const int i = (int)(e - (size_t)N * N);
+      double v;
+      if (i < nK) {
+        const int t = i / L, s = i - t * L;
+        const int u = s % S1 - w, vv = s / S1 - w;
+        const int pair = nKK + t * (1 + P.TB);  // (t, S)
+        v = P.Cmap[pair * lag2 + (size_t)(vv + w) * P.nLag + (u + w)];
+      } else {
+        v = P.mom[P.nMomA * P.nMomA + (i - nK)];
+      }
+      P.b[i] = v;
+      continue;
+    }
+    const int i = (int)(e / N), j = (int)(e - (size_t)i * N);
+    double v;
+    if (i < nK && j < nK) {
+      int t = i / L, s = i - t * L, t2 = j / L, s2 = j - t2 * L;
+      int du = (s % S1) - (s2 % S1), dv = (s / S1) - (s2 / S1);
+      if (t > t2) { int tmp = t; t = t2; t2 = tmp; du = -du; dv = -dv; }
+      // auto-correlation maps are even: read one canonical half so A is bitwise symmetric
+      if (t == t2 && (dv < 0 || (dv == 0 && du < 0))) { du = -du; dv = -dv; }
+      // pair index of (t,t2), t <= t2, in row-major upper-triangular order
+      const int pair = t * P.TK - t * (t - 1) / 2 + (t2 - t);
+      const int D = 2 * w;
+      v = P.Cmap[pair * lag2 + (size_t)(dv + D) * P.nLag + (du + D)];
+    } else if (i < nK || j < nK) {
+      const int ik = i < nK ? i : j, ib = (i < nK ? j : i) - nK;
+      const int t = ik / L, s = ik - t * L;
+      const int u = s % S1 - w, vv = s / S1 - w;
+      const int pair = nKK + t * (1 + P.TB) + 1 + ib;  // (t, Psi_ib)
+      v = P.Cmap[pair * lag2 + (size_t)(vv + w) * P.nLag + (u + w)];
+    } else {
+      const int a = i - nK, c = j - nK;
+      const int pa = P.monoB[a][0] + P.monoB[c][0], qa = P.monoB[a][1] + P.monoB[c][1];
+      v = P.mom[pa * P.nMomA + qa];
+    }
+    P.A[e] = v;
+  }
+}
+
+sfft_status sfft_launch_lag_gather(sfft_plan* p, double* A, double* b, cudaStream_t st, int* nl) {
+  LagParams LP;
+  LP.Y = p->Y; LP.Cmap = p->Cmap; LP.pairs = p->d_pairs; LP.NC = p->NC; LP.W = p->W;
+  LP.pitch = p->pitch; LP.nLag = p->nLag; LP.invP = 1.0 / ((double)p->H * (double)p->W);
+  LP.twW = p->twW;
+  dim3 g1(p->nPair, p->nLag);
+  k_lag_idft<<<g1, 256, 0, st>>>(LP);
+  SFFT_LAUNCH_CHECK();
+  ++*nl;
+  MomParams MP;
+  MP.rowMom = p->rowMom; MP.mom = p->mom; MP.H = p->H; MP.nMomA = p->nMomA; MP.nMomS = p->nMomS;
+  MP.TB = p->TB;
+  for (int t = 0; t < p->TB; ++t) { MP.monoB[t][0] = p->monoB[t][0]; MP.monoB[t][1] = p->monoB[t][1]; }
+  k_mom_final<<<p->nMomA * p->nMomA + p->TB, 256, 0, st>>>(MP);
+  SFFT_LAUNCH_CHECK();
+  ++*nl;
+  GatherParams GP;
+  GP.Cmap = p->Cmap; GP.mom = p->mom; GP.A = A; GP.b = b; GP.w = p->w; GP.L = p->L; GP.TK = p->TK;
+  GP.TB = p->TB; GP.N = p->N; GP.nLag = p->nLag; GP.nMomA = p->nMomA;
+  for (int t = 0; t < p->TB; ++t) { GP.monoB[t][0] = p->monoB[t][0]; GP.monoB[t][1] = p->monoB[t][1]; }
+  const size_t total = (size_t)p->N * p->N + p->N;
+  int blocks = (int)((total + 255) / 256);
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  k_gather<<<blocks, 256, 0, st>>>(GP);
+  SFFT_LAUNCH_CHECK();
+  ++*nl;
+  return SFFT_OK;
+}

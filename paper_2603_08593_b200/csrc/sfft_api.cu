@@ -1,0 +1,243 @@
+// C ABI of libsfft.so (include/sfft.h): plan management and stage scheduling on the caller stream.
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#include <new>
+#include <vector>
+
+#include "sfft_common.cuh"
+
+static bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+static int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
+
+static int fill_monomials(int D, int (*m)[2]) {
+  int n = 0;
+  for (int d = 0; d <= D; ++d)
+    for (int q = 0; q <= d; ++q) { m[n][0] = d - q; m[n][1] = q; ++n; }
+  return n;
+}
+
+static cudaError_t upload_twiddles(cplx** dst, int n) {
+  std::vector<cplx> h(n);
+  const long double twopi = 6.283185307179586476925286766559005768L;
+  for (int m = 0; m < n; ++m) {
+    // exact values on the axes and diagonals, long double elsewhere (rounded once to double)
+    const long double ang = -twopi * (long double)m / (long double)n;
+    long double c = cosl(ang), s = sinl(ang);
+    if ((4 * m) % n == 0) {
+      const int quad = (4 * m) / n;  // multiples of pi/2
+      c = (quad == 0) ? 1.0L : (quad == 2 ? -1.0L : 0.0L);
+      s = (quad == 1) ? -1.0L : (quad == 3 ? 1.0L : 0.0L);
+    }
+    h[m] = cmake((double)c, (double)s);
+  }
+  cudaError_t e = cudaMalloc((void**)dst, sizeof(cplx) * (size_t)n);
+  if (e != cudaSuccess) return e;
+  return cudaMemcpy(*dst, h.data(), sizeof(cplx) * (size_t)n, cudaMemcpyHostToDevice);
+}
+
+static void plan_free(sfft_plan* p) {
+  if (!p) return;
+  cudaFree(p->twNC); cudaFree(p->twW); cudaFree(p->twH); cudaFree(p->d_pairs);
+  cudaFree(p->T); cudaFree(p->F); cudaFree(p->Y); cudaFree(p->Cmap); cudaFree(p->rowMom);
+  cudaFree(p->mom); cudaFree(p->Lw); cudaFree(p->Ldiag); cudaFree(p->Etab); cudaFree(p->Mhat);
+  free(p->h_pairs);
+  delete p;
+}
+
+extern "C" {
+
+const char* sfft_version(void) { return "sfft-b200 0.1 (sm_100a)"; }
+
+const char* sfft_status_string(sfft_status s) {
+  switch (s) {
+    case SFFT_OK: return "SFFT_OK";
+    case SFFT_ERR_INVALID_ARG: return "SFFT_ERR_INVALID_ARG";
+    case SFFT_ERR_UNSUPPORTED: return "SFFT_ERR_UNSUPPORTED";
+    case SFFT_ERR_ALLOC: return "SFFT_ERR_ALLOC";
+    case SFFT_ERR_CUDA: return "SFFT_ERR_CUDA";
+    default: return "SFFT_ERR_UNKNOWN";
+  }
+}
+
+sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int DB) {
+  if (!out) return SFFT_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!is_pow2(H) || !is_pow2(W) || H < 32 || W < 32 || H > 4096 || W > 4096) return SFFT_ERR_UNSUPPORTED;
+  if (w < 0 || w > SFFT_MAX_W || 4 * w + 1 > (H < W ? H : W)) return SFFT_ERR_UNSUPPORTED;
+  if (w > 5) return SFFT_ERR_UNSUPPORTED;  // lag half-ranges above 10 need the split-range path (not built yet)
+  if (DK < 0 || DK > SFFT_MAX_DEG || DB < 0 || DB > SFFT_MAX_DEG) return SFFT_ERR_UNSUPPORTED;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return SFFT_ERR_CUDA; }
+
+  sfft_plan* p = new (std::nothrow) sfft_plan;
+  if (!p) return SFFT_ERR_ALLOC;
+  memset(p, 0, sizeof(*p));
+  p->H = H; p->W = W; p->w = w; p->DK = DK; p->DB = DB;
+  p->L = (2 * w + 1) * (2 * w + 1);
+  p->TK = fill_monomials(DK, p->monoK);
+  p->TB = fill_monomials(DB, p->monoB);
+  p->N = p->L * p->TK + p->TB;
+  p->NC = W / 2;
+  p->pitch = p->NC + SFFT_PITCH_PAD;
+  p->log2H = ilog2(H); p->log2NC = ilog2(p->NC);
+  p->nRowImg = (DK + 1) + 1 + (DB + 1);
+  p->nSpec = p->TK + 1 + p->TB;
+  p->nPair = p->TK * (p->TK + 1) / 2 + p->TK * (1 + p->TB);
+  p->Dmax = 2 * w;
+  p->nLag = 2 * p->Dmax + 1;
+  p->nMomA = 2 * DB + 1;
+  p->nMomS = DB + 1;
+  p->ldL = (p->N + 1 + 3) & ~3;
+  int dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, dev);
+
+  // pair list: kernel-kernel pairs (t <= t2) first, then for each t: (t,S), (t,Psi_0..)
+  p->h_pairs = (PairDesc*)malloc(sizeof(PairDesc) * p->nPair);
+  if (!p->h_pairs) { plan_free(p); return SFFT_ERR_ALLOC; }
+  int n = 0;
+  for (int t = 0; t < p->TK; ++t)
+    for (int t2 = t; t2 < p->TK; ++t2) { p->h_pairs[n].fa = t; p->h_pairs[n].fb = t2; p->h_pairs[n].D = 2 * w; ++n; }
+  for (int t = 0; t < p->TK; ++t) {
+    p->h_pairs[n].fa = t; p->h_pairs[n].fb = p->TK; p->h_pairs[n].D = w; ++n;
+    for (int t2 = 0; t2 < p->TB; ++t2) { p->h_pairs[n].fa = t; p->h_pairs[n].fb = p->TK + 1 + t2; p->h_pairs[n].D = w; ++n; }
+  }
+
+  size_t ws = 0;
+  bool ok = true;
+  auto dalloc = [&](void** ptr, size_t bytes) {
+    if (!ok) return;
+    if (cudaMalloc(ptr, bytes) != cudaSuccess) { cudaGetLastError(); ok = false; *ptr = nullptr; return; }
+    ws += bytes;
+  };
+  const size_t HN = (size_t)H * p->NC, HP = (size_t)H * p->pitch;
+  dalloc((void**)&p->T, sizeof(cplx) * HN * p->nRowImg);
+  dalloc((void**)&p->F, sizeof(cplx) * HP * p->nSpec);
+  dalloc((void**)&p->Y, sizeof(cplx) * (size_t)p->nPair * p->nLag * p->pitch);
+  dalloc((void**)&p->Cmap, sizeof(double) * (size_t)p->nPair * p->nLag * p->nLag);
+  dalloc((void**)&p->rowMom, sizeof(double) * (size_t)(p->nMomA + p->nMomS) * H);
+  dalloc((void**)&p->mom, sizeof(double) * (size_t)(p->nMomA * p->nMomA + p->TB));
+  dalloc((void**)&p->Lw, sizeof(double) * (size_t)(p->N + 1) * p->ldL);
+  dalloc((void**)&p->Ldiag, sizeof(double) * (size_t)((p->N + 31) / 32) * 32 * 32);
+  dalloc((void**)&p->Etab, sizeof(cplx) * (size_t)p->TK * (2 * w + 1) * p->NC);
+  dalloc((void**)&p->Mhat, sizeof(cplx) * HN);
+  dalloc((void**)&p->d_pairs, sizeof(PairDesc) * p->nPair);
+  if (!ok) { plan_free(p); return SFFT_ERR_ALLOC; }
+  if (upload_twiddles(&p->twNC, p->NC) != cudaSuccess || upload_twiddles(&p->twW, W) != cudaSuccess ||
+      upload_twiddles(&p->twH, H) != cudaSuccess ||
+      cudaMemcpy(p->d_pairs, p->h_pairs, sizeof(PairDesc) * p->nPair, cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemset(p->Y, 0, sizeof(cplx) * (size_t)p->nPair * p->nLag * p->pitch) != cudaSuccess ||
+      cudaMemset(p->Cmap, 0, sizeof(double) * (size_t)p->nPair * p->nLag * p->nLag) != cudaSuccess) {
+    cudaGetLastError();
+    plan_free(p);
+    return SFFT_ERR_CUDA;
+  }
+  ws += sizeof(cplx) * (size_t)(p->NC + W + H);
+  p->ws_bytes = ws;
+  if (cudaDeviceSynchronize() != cudaSuccess) { cudaGetLastError(); plan_free(p); return SFFT_ERR_CUDA; }
+  *out = p;
+  return SFFT_OK;
+}
+
+sfft_status sfft_plan_destroy(sfft_plan* p) {
+  if (!p) return SFFT_ERR_INVALID_ARG;
+  plan_free(p);
+  return SFFT_OK;
+}
+
+int sfft_num_coeffs(const sfft_plan* p) { return p ? p->N : -1; }
+size_t sfft_workspace_bytes(const sfft_plan* p) { return p ? p->ws_bytes : 0; }
+
+static bool aligned16(const void* q) { return (((uintptr_t)q) & 15) == 0; }
+
+sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
+                              double* A, double* b, void* stream) {
+  if (!p || !R || !S || !A || !b) return SFFT_ERR_INVALID_ARG;
+  if (!aligned16(R) || !aligned16(S) || !aligned16(A) || !aligned16(b) || (mask && (((uintptr_t)mask) & 1)))
+    return SFFT_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  int nl = 0;
+  // a1 + a2 (row pass): m xi^p R (p<=DK), m S, m xi^p (p<=DB), with the fused moment reductions
+  RowImage imgs[8];
+  int n = 0;
+  for (int q = 0; q <= p->DK; ++q) { imgs[n].src = 0; imgs[n].pxi = q; imgs[n].masked = 1; ++n; }
+  imgs[n].src = 1; imgs[n].pxi = 0; imgs[n].masked = 1; ++n;
+  for (int q = 0; q <= p->DB; ++q) { imgs[n].src = 2; imgs[n].pxi = q; imgs[n].masked = 1; ++n; }
+  sfft_status s = sfft_launch_row_fwd(p, R, S, mask, imgs, n, p->T, true, st, &nl);
+  if (s != SFFT_OK) return s;
+  s = sfft_launch_col_fwd(p, st, &nl);       // a2 (column pass, applies eta^q)
+  if (s != SFFT_OK) return s;
+  s = sfft_launch_cross(p, st, &nl);         // a3 (cross products + lag-pruned inverse along ky)
+  if (s != SFFT_OK) return s;
+  s = sfft_launch_lag_gather(p, A, b, st, &nl);  // a3 (inverse along kx on the lag rows) + a4
+  if (s != SFFT_OK) return s;
+  p->launches[0] = nl;
+  return SFFT_OK;
+}
+
+sfft_status sfft_solve(sfft_plan* p, const double* A, const double* b, double* coeffs, int* info, void* stream) {
+  if (!p || !A || !b || !coeffs) return SFFT_ERR_INVALID_ARG;
+  int nl = 0;
+  sfft_status s = sfft_launch_solve(p, A, b, coeffs, info, (cudaStream_t)stream, &nl);
+  if (s != SFFT_OK) return s;
+  p->launches[1] = nl;
+  return SFFT_OK;
+}
+
+sfft_status sfft_subtract(sfft_plan* p, const double* R, const double* S, const double* coeffs, double* D,
+                          void* stream) {
+  if (!p || !R || !S || !coeffs || !D) return SFFT_ERR_INVALID_ARG;
+  if (!aligned16(R) || !aligned16(S) || !aligned16(D) || D == R || D == S) return SFFT_ERR_INVALID_ARG;
+  int nl = 0;
+  sfft_status s = sfft_launch_subtract(p, R, S, coeffs, D, (cudaStream_t)stream, &nl);
+  if (s != SFFT_OK) return s;
+  p->launches[2] = nl;
+  return SFFT_OK;
+}
+
+sfft_status sfft_probe_fp64(int kind, int iters, double* tflops, double* elapsed_ms, void* stream) {
+  if (iters < 1 || kind < 0 || kind > 1) return SFFT_ERR_INVALID_ARG;
+  double tf = 0, ms = 0;
+  sfft_status s = sfft_run_probe(kind, iters, &tf, &ms, (cudaStream_t)stream);
+  if (tflops) *tflops = tf;
+  if (elapsed_ms) *elapsed_ms = ms;
+  return s;
+}
+
+int sfft_last_launch_count(const sfft_plan* p, int which) {
+  if (!p || which < 0 || which > 2) return -1;
+  return p->launches[which];
+}
+
+sfft_status sfft_model_cost(const sfft_plan* p, int which, double* fp64_instr, double* hbm_bytes) {
+  if (!p || which < 0 || which > 2) return SFFT_ERR_INVALID_ARG;
+  // Algorithmic model of DESIGN.md ("Cost model"): fp64 pipe instructions (DFMA/DADD/DMUL, one
+  // per lane) and compulsory HBM bytes of one call at this plan's sizes.
+  const double H = p->H, W = p->W, NC = p->NC, P = H * W;
+  const double fftH = 3.6 * H * p->log2H;      // instr per H-point complex FFT (radix-16/8 mix)
+  const double fftN = 3.6 * NC * p->log2NC + 10.0 * NC;  // per real row (W/2 complex FFT + split)
+  double fi = 0, hb = 0;
+  if (which == 0) {
+    const double nKK = p->TK * (p->TK + 1) / 2.0, nKO = p->TK * (1.0 + p->TB);
+    const double perColKK = H * 4.0 + (H / 8.0) * (56.0 + 8.0 * p->Dmax);   // product + DFT-8 + outer
+    const double perColKO = H * 4.0 + (H / 8.0) * (56.0 + 8.0 * p->w);
+    fi = p->nRowImg * H * fftN + p->nSpec * NC * fftH + (NC + 1) * (nKK * perColKK + nKO * perColKO);
+    hb = 2.0 * P * 8 + P            // R, S, mask read once
+         + 2.0 * p->nRowImg * P * 8   // row spectra written + read
+         + 2.0 * p->nSpec * P * 8     // spectra written + read once
+         + (double)p->N * p->N * 8;
+  } else if (which == 1) {
+    const double N = p->N;
+    fi = N * N * N / 6.0 + 2.0 * N * N;
+    hb = 2.0 * N * N * 8;
+  } else {
+    fi = (p->DK + 1) * H * fftN + H * fftN + P / 2.0 * (2 * p->w + 1) * (4.0 * (p->DK + 1) + 2.0 * (p->TK - 1 - p->DK) + 0.0);
+    hb = 3.0 * P * 8 + 2.0 * (p->DK + 1) * P * 8 + 2.0 * P * 8;
+  }
+  if (fp64_instr) *fp64_instr = fi;
+  if (hbm_bytes) *hbm_bytes = hb;
+  return SFFT_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,132 @@
+// Common definitions for the sm_100a SFFT kernels: plan layout, complex helpers, launch checks.
+// Conventions follow include/sfft.h.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/sfft.h"
+
+#define SFFT_MAX_DEG 3
+#define SFFT_MAX_T 10     // (3+1)(3+2)/2 monomials of degree <= 3
+#define SFFT_MAX_W 15
+#define SFFT_PITCH_PAD 8  // spectrum row pitch = W/2 + 8 complex (column W/2 = Nyquist)
+
+typedef double2 cplx;
+
+__host__ __device__ __forceinline__ cplx cmake(double a, double b) { return make_double2(a, b); }
+__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return cmake(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ cplx csub(cplx a, cplx b) { return cmake(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ cplx cconj(cplx a) { return cmake(a.x, -a.y); }
+__device__ __forceinline__ cplx cscale(cplx a, double s) { return cmake(a.x * s, a.y * s); }
+// a*b
+__device__ __forceinline__ cplx cmul(cplx a, cplx b) {
+  return cmake(fma(a.x, b.x, -(a.y * b.y)), fma(a.x, b.y, a.y * b.x));
+}
+// conj(a)*b
+__device__ __forceinline__ cplx cmulc(cplx a, cplx b) {
+  return cmake(fma(a.x, b.x, a.y * b.y), fma(a.x, b.y, -(a.y * b.x)));
+}
+// acc += a*b
+__device__ __forceinline__ void cfma(cplx& acc, cplx a, cplx b) {
+  acc.x = fma(a.x, b.x, acc.x);
+  acc.x = fma(-a.y, b.y, acc.x);
+  acc.y = fma(a.x, b.y, acc.y);
+  acc.y = fma(a.y, b.x, acc.y);
+}
+// acc += conj(a)*b
+__device__ __forceinline__ void cfmac(cplx& acc, cplx a, cplx b) {
+  acc.x = fma(a.x, b.x, acc.x);
+  acc.x = fma(a.y, b.y, acc.x);
+  acc.y = fma(a.x, b.y, acc.y);
+  acc.y = fma(-a.y, b.x, acc.y);
+}
+// multiply by +i / -i
+__device__ __forceinline__ cplx cmul_pi(cplx a) { return cmake(-a.y, a.x); }
+__device__ __forceinline__ cplx cmul_mi(cplx a) { return cmake(a.y, -a.x); }
+
+__device__ __forceinline__ cplx ldg2(const cplx* p) { return __ldg(p); }
+
+__device__ __forceinline__ double ipow(double x, int n) {
+  double r = 1.0;
+  for (int i = 0; i < n; ++i) r *= x;
+  return r;
+}
+
+// One image produced by the forward row pass: src (0 = R, 1 = S, 2 = all-ones), xi power, masked.
+struct RowImage {
+  int src;
+  int pxi;
+  int masked;
+};
+
+// A cross-correlation pair: spectra indices into the plan's spectrum array and its lag half-range.
+struct PairDesc {
+  int fa;   // spectrum index of f  (conj side)
+  int fb;   // spectrum index of g
+  int D;    // lags needed: dy,dx in [-D, D]
+};
+
+struct sfft_plan {
+  int H, W, w, DK, DB;
+  int L, TK, TB, N;
+  int NC;        // W/2
+  int pitch;     // spectrum row pitch (complex elements) = NC + SFFT_PITCH_PAD
+  int log2H, log2NC;
+  int nRowImg;   // forward row-pass images in build: R~ xi^p (DK+1), S~ (1), Psi xi^p (DB+1)
+  int nSpec;     // spectra: TK + 1 + TB
+  int nPair;     // TK(TK+1)/2 + TK + TK*TB
+  int Dmax;      // 2w
+  int nLag;      // 2*Dmax+1
+  int monoK[SFFT_MAX_T][2], monoB[SFFT_MAX_T][2];
+  int nMomA;     // 2*DB+1 row moments  sum_x m xi^a
+  int nMomS;     // DB+1 row moments     sum_x m xi^p S
+
+  // device tables
+  cplx* twNC;    // e^{-2 pi i m / NC}, m in [0, NC)
+  cplx* twW;     // e^{-2 pi i m / W},  m in [0, W)
+  cplx* twH;     // e^{-2 pi i m / H},  m in [0, H)
+  PairDesc* d_pairs;
+  PairDesc* h_pairs;
+
+  // device scratch
+  cplx* T;       // row-pass output  [nRowImg][H][NC]   (packed: column 0 = DC + i Nyquist)
+  cplx* F;       // spectra          [nSpec][H][pitch]  (column NC = Nyquist)
+  cplx* Y;       // lag rows         [nPair][nLag][pitch]
+  double* Cmap;  // lag windows      [nPair][nLag][nLag]
+  double* rowMom;   // [nMomA + nMomS][H]
+  double* mom;      // [(2DB+1)^2 + TB] reduced moments
+  double* Lw;       // Cholesky workspace (N+1) x ldL
+  double* Ldiag;    // factored diagonal blocks
+  cplx* Etab;       // subtract: E[TK][2w+1][NC]
+  cplx* Mhat;       // subtract: mixed row spectra [H][NC]
+  int ldL;
+  size_t ws_bytes;
+  int launches[3];
+  int num_sms;
+};
+
+#define SFFT_CUDA_TRY(expr)                          \
+  do {                                               \
+    cudaError_t _e = (expr);                         \
+    if (_e != cudaSuccess) return SFFT_ERR_CUDA;     \
+  } while (0)
+
+#define SFFT_LAUNCH_CHECK()                          \
+  do {                                               \
+    if (cudaPeekAtLastError() != cudaSuccess) {      \
+      cudaGetLastError();                            \
+      return SFFT_ERR_CUDA;                          \
+    }                                                \
+  } while (0)
+
+// ---- stage entry points implemented in the k_*.cu files (host functions) ----------------------
+sfft_status sfft_launch_row_fwd(sfft_plan* p, const double* R, const double* S,
+                                const unsigned char* mask, const RowImage* imgs, int nimg,
+                                cplx* Tout, bool moments, cudaStream_t st, int* nl);
+sfft_status sfft_launch_col_fwd(sfft_plan* p, cudaStream_t st, int* nl);
+sfft_status sfft_launch_cross(sfft_plan* p, cudaStream_t st, int* nl);
+sfft_status sfft_launch_lag_gather(sfft_plan* p, double* A, double* b, cudaStream_t st, int* nl);
+sfft_status sfft_launch_solve(sfft_plan* p, const double* A, const double* b, double* c, int* info,
+                              cudaStream_t st, int* nl);
+sfft_status sfft_launch_subtract(sfft_plan* p, const double* R, const double* S, const double* c,
+                                 double* D, cudaStream_t st, int* nl);
+sfft_status sfft_run_probe(int kind, int iters, double* tflops, double* ms, cudaStream_t st);

@@ -1,0 +1,189 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Tolerances (BASELINE.json north_star; norms per DESIGN.md reading A5):
+  A, b   : max|dA| <= 1e-10 max|A|  and per block (K-K, K-B, B-B, b_K, b_B) <= 1e-12 of the block max
+  coeffs : ||c_gpu - c_orc||_inf <= 1e-7 ||c_orc||_inf
+  D      : max|dD| <= 1e-6 sigma_sky
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import sfft_oracle as orc
+from paper_2603_08593_b200 import SfftPlan, synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_AB = 1e-10
+TOL_BLOCK = 1e-12
+TOL_C = 1e-7
+TOL_D = 1e-6
+
+
+def dev(x, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(x))
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.cuda()
+
+
+def check_system(A, b, Ao, bo, L, TK):
+    nK = L * TK
+    assert np.max(np.abs(A - Ao)) <= TOL_AB * np.max(np.abs(Ao))
+    assert np.max(np.abs(b - bo)) <= TOL_AB * np.max(np.abs(bo))
+    blocks = {
+        "KK": (A[:nK, :nK], Ao[:nK, :nK]), "KB": (A[:nK, nK:], Ao[:nK, nK:]),
+        "BK": (A[nK:, :nK], Ao[nK:, :nK]), "BB": (A[nK:, nK:], Ao[nK:, nK:]),
+        "bK": (b[:nK], bo[:nK]), "bB": (b[nK:], bo[nK:]),
+    }
+    for name, (g, o) in blocks.items():
+        scale = max(np.max(np.abs(o)), 1e-300)
+        err = np.max(np.abs(g - o))
+        assert err <= TOL_BLOCK * scale, (name, err / scale)
+    assert np.array_equal(A, A.T)
+
+
+def run_case(R, S, mask, w, DK, DB, sky_rms, full_D=True):
+    H, W = R.shape
+    Ao, bo = orc.build_system_fft(R, S, mask, w, DK, DB, workers=8)
+    co = orc.solve(Ao, bo)
+    with SfftPlan(H, W, w, DK, DB) as plan:
+        Rd, Sd = dev(R), dev(S)
+        Md = None if mask is None else dev(mask)
+        A, b, c, info, D = plan.difference(Rd, Sd, Md)
+        torch.cuda.synchronize()
+        A, b, c, D = A.cpu().numpy(), b.cpu().numpy(), c.cpu().numpy(), D.cpu().numpy()
+        assert int(info.item()) == 0
+        L = (2 * w + 1) ** 2
+        TK = (DK + 1) * (DK + 2) // 2
+        check_system(A, b, Ao, bo, L, TK)
+        assert np.max(np.abs(c - co)) <= TOL_C * np.max(np.abs(co))
+        # stage-isolated: oracle A, b -> sfft_solve; oracle c -> sfft_subtract
+        c2, info2 = plan.solve(dev(Ao), dev(bo))
+        assert int(info2.item()) == 0
+        assert np.max(np.abs(c2.cpu().numpy() - co)) <= TOL_C * np.max(np.abs(co))
+        D2 = plan.subtract(Rd, Sd, dev(co)).cpu().numpy()
+    if full_D:
+        Do = orc.subtract_rollsum(R, S, co, w, DK, DB)
+        assert np.max(np.abs(D2 - Do)) <= TOL_D * sky_rms
+        assert np.max(np.abs(D - Do)) <= TOL_D * sky_rms
+    else:
+        rng = np.random.default_rng(5)
+        ys = np.concatenate([rng.integers(0, H, 60), [0, 0, H - 1, H - 1, 3]])
+        xs = np.concatenate([rng.integers(0, W, 60), [0, W - 1, 0, W - 1, 2]])
+        Dp = orc.subtract_at_pixels(R, S, co, w, DK, DB, ys, xs)
+        assert np.max(np.abs(D2[ys, xs] - Dp)) <= TOL_D * sky_rms
+        assert np.max(np.abs(D[ys, xs] - Dp)) <= TOL_D * sky_rms
+        Df = orc.subtract_fft(R, S, co, w, DK, DB, workers=8)
+        assert np.max(np.abs(D2 - Df)) <= TOL_D * sky_rms
+        assert np.max(np.abs(D - Df)) <= TOL_D * sky_rms
+    return A, b, c, D
+
+
+def test_tiny_config():
+    pr = synth.make_pair("tiny")
+    run_case(pr.R, pr.S, pr.mask, pr.cfg.w, pr.cfg.DK, pr.cfg.DB, pr.sky_rms)
+
+
+def test_small_config():
+    pr = synth.make_pair("small", force_saturated=3)
+    assert pr.mask[10:-10, 10:-10].any()  # saturated cores are exercised
+    run_case(pr.R, pr.S, pr.mask, pr.cfg.w, pr.cfg.DK, pr.cfg.DB, pr.sky_rms)
+
+
+@pytest.mark.parametrize("H,W,w,DK,DB,masked", [
+    (32, 64, 1, 0, 3, True), (128, 32, 2, 3, 0, True), (64, 128, 3, 1, 2, False),
+    (512, 64, 0, 2, 1, True), (32, 32, 5, 1, 1, True)])
+def test_ragged_shapes_and_degrees(H, W, w, DK, DB, masked):
+    rng = np.random.default_rng(H * 7 + W)
+    R = 50.0 * rng.standard_normal((H, W)) + 500.0 * (rng.random((H, W)) > 0.98)
+    S = 0.7 * np.roll(R, (1 if w else 0, -1 if w else 0), (0, 1)) + 30.0 * rng.standard_normal((H, W)) + 200.0
+    mask = (rng.random((H, W)) < 0.05).astype(np.uint8) if masked else None
+    run_case(R, S, mask, w, DK, DB, 30.0)
+
+
+def test_mid_config():
+    pr = synth.make_pair("mid")
+    run_case(pr.R, pr.S, pr.mask, pr.cfg.w, pr.cfg.DK, pr.cfg.DB, pr.sky_rms, full_D=False)
+
+
+def test_full_config_and_sampled_definition_entries():
+    """BASELINE.json configs[3] at full size, in the launch configuration bench.py times; A is
+    compared entry by entry with the Fourier-route oracle and, on sampled entries, with direct
+    pixel sums of the definition."""
+    pr = synth.make_pair("full")
+    cfg = pr.cfg
+    A, b, c, D = run_case(pr.R, pr.S, pr.mask, cfg.w, cfg.DK, cfg.DB, pr.sky_rms, full_D=False)
+    rng = np.random.default_rng(9)
+    N = cfg.N
+    scale = np.max(np.abs(A))
+    for _ in range(12):
+        i, j = rng.integers(0, N, 2)
+        assert abs(A[i, j] - orc.normal_entry(pr.R, pr.S, pr.mask, cfg.w, cfg.DK, cfg.DB, i, j)) <= TOL_AB * scale
+    for i in (0, 60, 725, 731):
+        assert abs(b[i] - orc.normal_entry(pr.R, pr.S, pr.mask, cfg.w, cfg.DK, cfg.DB, i)) <= TOL_AB * np.max(np.abs(b))
+
+
+def test_transposed_ccd_orientation():
+    """H=4096, W=2048 (the physical DECam orientation; reading A4)."""
+    pr = synth.make_pair("full_t")
+    cfg = pr.cfg
+    run_case(pr.R, pr.S, pr.mask, cfg.w, cfg.DK, cfg.DB, pr.sky_rms, full_D=False)
+
+
+def test_exact_recovery_on_gpu():
+    """mask=NULL, S = M(R; c0): the CUDA path alone recovers c0 to 1e-9 relative and D = 0."""
+    H, W, w, DK, DB = 128, 256, 2, 2, 2
+    R, _ = synth.white_noise_pair(H, W, 77)
+    rng = np.random.default_rng(1)
+    L, TK, TB = 25, 6, 6
+    c0 = np.zeros(L * TK + TB)
+    c0[:L] = rng.random(L)
+    c0[:L] /= c0[:L].sum()
+    c0[L:L * TK] = 0.1 * rng.standard_normal(L * (TK - 1))
+    c0[L * TK:] = [300.0, 20.0, -10.0, 5.0, 3.0, -4.0]
+    S = orc.model_rollsum(R, c0, w, DK, DB)
+    with SfftPlan(H, W, w, DK, DB) as plan:
+        A, b, c, info, D = plan.difference(dev(R), dev(S), None)
+        assert int(info.item()) == 0
+        assert np.max(np.abs(c.cpu().numpy() - c0)) <= 1e-9 * np.max(np.abs(c0))
+        assert float(D.abs().max()) <= 1e-9 * np.max(np.abs(S))
+
+
+def test_not_positive_definite_reports_info():
+    H = W = 64
+    with SfftPlan(H, W, 1, 0, 0) as plan:
+        R = torch.zeros((H, W), dtype=torch.float64, device="cuda")
+        S = torch.ones((H, W), dtype=torch.float64, device="cuda")
+        A, b = plan.build_system(R, S, None)
+        c, info = plan.solve(A, b)
+        assert int(info.item()) == 1
+
+
+def test_degenerate_all_masked_and_plan_reuse():
+    pr = synth.make_pair("tiny")
+    cfg = pr.cfg
+    with SfftPlan(cfg.H, cfg.W, cfg.w, cfg.DK, cfg.DB) as plan:
+        allm = torch.ones((cfg.H, cfg.W), dtype=torch.uint8, device="cuda")
+        A, b = plan.build_system(dev(pr.R), dev(pr.S), allm)
+        assert float(A.abs().max()) == 0.0 and float(b.abs().max()) == 0.0
+        # the same plan gives the same answer when reused (scratch holds no state)
+        A1, b1 = plan.build_system(dev(pr.R), dev(pr.S), dev(pr.mask))
+        A2, b2 = plan.build_system(dev(pr.R), dev(pr.S), dev(pr.mask))
+        assert torch.equal(A1, A2) and torch.equal(b1, b2)
+        assert plan.last_launch_count(0) > 0
+
+
+def test_non_default_stream():
+    pr = synth.make_pair("tiny")
+    cfg = pr.cfg
+    st = torch.cuda.Stream()
+    with SfftPlan(cfg.H, cfg.W, cfg.w, cfg.DK, cfg.DB) as plan:
+        Rd, Sd, Md = dev(pr.R), dev(pr.S), dev(pr.mask)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(st):
+            A, b, c, info, D = plan.difference(Rd, Sd, Md, stream=st)
+        st.synchronize()
+        A0, b0, c0, info0, D0 = plan.difference(Rd, Sd, Md)
+        torch.cuda.synchronize()
+        assert torch.equal(D, D0) and torch.equal(c, c0)
