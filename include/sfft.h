@@ -97,14 +97,21 @@ sfft_status sfft_subtract(sfft_plan* p, const double* R, const double* S, const 
  * kind = 0: DFMA (CUDA-core fp64 pipe); kind = 1: DMMA (mma.sync m8n8k4 f64). */
 sfft_status sfft_probe_fp64(int kind, int iters, double* tflops, double* elapsed_ms, void* stream);
 
+/* Optional per-stage timing for benchmarks.  With profiling on, every hot call records a CUDA
+ * event pair on the caller stream around each stage (no synchronisation; at most 512 pending
+ * pairs between reads).  sfft_profile_read synchronises on the pending events, folds them into
+ * per-stage totals and returns the accumulated milliseconds and pair count of `stage`:
+ *   0 build: row pass (k_row_fwd)          1 build: column pass (k_col_fwd)
+ *   2 build: cross+pruned inverse, K-K     3 build: cross+pruned inverse, K-S and K-Psi
+ *   4 build: lag-row inverse + moments + gather      5 solve (all kernels)
+ *   6 subtract: row pass   7 subtract: phase table + y-mixing   8 subtract: inverse rows + D
+ * reset != 0 clears that stage's totals after reading. */
+sfft_status sfft_profile_enable(sfft_plan* p, int on);
+sfft_status sfft_profile_read(sfft_plan* p, int stage, double* total_ms, int* count, int reset);
+
 /* Number of kernel launches the last call of each hot entry point enqueued (host-side counter,
  * for bench.py's "gpu_launches"): which = 0 build, 1 solve, 2 subtract.  -1 on bad arguments. */
 int sfft_last_launch_count(const sfft_plan* p, int which);
-
-/* Name and launch count of the dominant kernels, for bench.py's roofline section: fills
- * flops/bytes the algorithmic model in DESIGN.md assigns to ONE call of entry point `which`
- * (0 build, 1 solve, 2 subtract) at this plan's sizes.  Either output may be NULL. */
-sfft_status sfft_model_cost(const sfft_plan* p, int which, double* fp64_instr, double* hbm_bytes);
 
 /* Library version string, e.g. "sfft-b200 0.1 (sm_100a)". */
 const char* sfft_version(void);

@@ -17,8 +17,12 @@ _LIB_NAME = "libsfft.so"
 EXPORTED_SYMBOLS = [
     "sfft_plan_create", "sfft_plan_destroy", "sfft_num_coeffs", "sfft_workspace_bytes",
     "sfft_status_string", "sfft_build_system", "sfft_solve", "sfft_subtract",
-    "sfft_probe_fp64", "sfft_last_launch_count", "sfft_model_cost", "sfft_version",
+    "sfft_probe_fp64", "sfft_last_launch_count", "sfft_version",
+    "sfft_profile_enable", "sfft_profile_read",
 ]
+
+STAGE_NAMES = ["build.row_fwd", "build.col_fwd", "build.cross_KK", "build.cross_KO",
+               "build.lag_gather", "solve", "subtract.row_fwd", "subtract.mix", "subtract.row_inv"]
 
 
 class SfftError(RuntimeError):
@@ -66,8 +70,10 @@ def load_library():
     lib.sfft_probe_fp64.restype = i32
     lib.sfft_last_launch_count.argtypes = [vp, i32]
     lib.sfft_last_launch_count.restype = i32
-    lib.sfft_model_cost.argtypes = [vp, i32, dbl_p, dbl_p]
-    lib.sfft_model_cost.restype = i32
+    lib.sfft_profile_enable.argtypes = [vp, i32]
+    lib.sfft_profile_enable.restype = i32
+    lib.sfft_profile_read.argtypes = [vp, i32, dbl_p, ctypes.POINTER(i32), i32]
+    lib.sfft_profile_read.restype = i32
     lib.sfft_version.argtypes = []
     lib.sfft_version.restype = ctypes.c_char_p
     _lib = lib
@@ -192,11 +198,18 @@ class SfftPlan:
     def last_launch_count(self, which: int) -> int:
         return int(self._lib.sfft_last_launch_count(self._p, which))
 
-    def model_cost(self, which: int):
-        fi, hb = ctypes.c_double(0), ctypes.c_double(0)
-        _check(self._lib, self._lib.sfft_model_cost(self._p, which, ctypes.byref(fi), ctypes.byref(hb)),
-               "sfft_model_cost")
-        return fi.value, hb.value
+    def profile_enable(self, on: bool = True):
+        _check(self._lib, self._lib.sfft_profile_enable(self._p, 1 if on else 0), "sfft_profile_enable")
+
+    def profile_read(self, reset: bool = True):
+        """{stage name: (total_ms, count)} accumulated since the last reset (synchronises)."""
+        out = {}
+        for i, name in enumerate(STAGE_NAMES):
+            ms, cnt = ctypes.c_double(0), ctypes.c_int(0)
+            _check(self._lib, self._lib.sfft_profile_read(self._p, i, ctypes.byref(ms), ctypes.byref(cnt),
+                                                          1 if reset else 0), "sfft_profile_read")
+            out[name] = (ms.value, cnt.value)
+        return out
 
 
 def probe_fp64(kind: int = 0, iters: int = 4096, stream=None):

@@ -98,11 +98,13 @@ sfft_status sfft_launch_cross(sfft_plan* p, cudaStream_t st, int* nl) {
   const int nKK = p->TK * (p->TK + 1) / 2;
   P.pair0 = 0; P.npair = nKK;
   ++*nl;
-  sfft_status s = launch_cross_D(2 * p->w, P, st);
+  sfft_status s;
+  { ProfScope ps(p, 2, st); s = launch_cross_D(2 * p->w, P, st); }
   if (s != SFFT_OK) return s;
   P.pair0 = nKK; P.npair = p->nPair - nKK;
   ++*nl;
-  return launch_cross_D(p->w, P, st);
+  { ProfScope ps(p, 3, st); s = launch_cross_D(p->w, P, st); }
+  return s;
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -111,8 +111,10 @@ sfft_status sfft_launch_subtract(sfft_plan* p, const double* R, const double* S,
   // 1. row spectra of xi^p R (unmasked), p = 0..DK, into the row-pass scratch
   RowImage imgs[SFFT_MAX_DEG + 1];
   for (int q = 0; q <= p->DK; ++q) { imgs[q].src = 0; imgs[q].pxi = q; imgs[q].masked = 0; }
-  sfft_status s = sfft_launch_row_fwd(p, R, S, nullptr, imgs, p->DK + 1, p->T, false, st, nl);
+  sfft_status s;
+  { ProfScope ps(p, 6, st); s = sfft_launch_row_fwd(p, R, S, nullptr, imgs, p->DK + 1, p->T, false, st, nl); }
   if (s != SFFT_OK) return s;
+  ProfScope* pmix = new ProfScope(p, 7, st);
   // 2. x-phase table of the kernel coefficients
   ETabParams EP;
   EP.coeffs = c; EP.E = p->Etab; EP.w = p->w; EP.L = p->L; EP.NC = p->NC; EP.W = p->W; EP.twW = p->twW;
@@ -137,8 +139,10 @@ sfft_status sfft_launch_subtract(sfft_plan* p, const double* R, const double* S,
   if (yt != MIX_YT) return SFFT_ERR_UNSUPPORTED;
   dim3 gm(p->NC / KT, p->H / MIX_YT);
   k_mix<<<gm, 256, smem, st>>>(MP);
+  delete pmix;
   SFFT_LAUNCH_CHECK();
   ++*nl;
   // 4. inverse rows + subtraction
-  return sfft_launch_row_inv_sub(p, S, c, D, st, nl);
+  { ProfScope ps(p, 8, st); s = sfft_launch_row_inv_sub(p, S, c, D, st, nl); }
+  return s;
 }

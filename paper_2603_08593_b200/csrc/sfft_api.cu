@@ -42,6 +42,7 @@ static void plan_free(sfft_plan* p) {
   cudaFree(p->T); cudaFree(p->F); cudaFree(p->Y); cudaFree(p->Cmap); cudaFree(p->rowMom);
   cudaFree(p->mom); cudaFree(p->Lw); cudaFree(p->Ldiag); cudaFree(p->Etab); cudaFree(p->Mhat);
   free(p->h_pairs);
+  for (int i = 0; i < 2 * SFFT_PROF_MAX; ++i) if (p->prof_ev[i]) cudaEventDestroy(p->prof_ev[i]);
   delete p;
 }
 
@@ -164,13 +165,14 @@ sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S, co
   for (int q = 0; q <= p->DK; ++q) { imgs[n].src = 0; imgs[n].pxi = q; imgs[n].masked = 1; ++n; }
   imgs[n].src = 1; imgs[n].pxi = 0; imgs[n].masked = 1; ++n;
   for (int q = 0; q <= p->DB; ++q) { imgs[n].src = 2; imgs[n].pxi = q; imgs[n].masked = 1; ++n; }
-  sfft_status s = sfft_launch_row_fwd(p, R, S, mask, imgs, n, p->T, true, st, &nl);
+  sfft_status s;
+  { ProfScope ps(p, 0, st); s = sfft_launch_row_fwd(p, R, S, mask, imgs, n, p->T, true, st, &nl); }
   if (s != SFFT_OK) return s;
-  s = sfft_launch_col_fwd(p, st, &nl);       // a2 (column pass, applies eta^q)
+  { ProfScope ps(p, 1, st); s = sfft_launch_col_fwd(p, st, &nl); }  // a2 (column pass, applies eta^q)
   if (s != SFFT_OK) return s;
   s = sfft_launch_cross(p, st, &nl);         // a3 (cross products + lag-pruned inverse along ky)
   if (s != SFFT_OK) return s;
-  s = sfft_launch_lag_gather(p, A, b, st, &nl);  // a3 (inverse along kx on the lag rows) + a4
+  { ProfScope ps(p, 4, st); s = sfft_launch_lag_gather(p, A, b, st, &nl); }  // a3 (kx inverse on lag rows) + a4
   if (s != SFFT_OK) return s;
   p->launches[0] = nl;
   return SFFT_OK;
@@ -179,7 +181,8 @@ sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S, co
 sfft_status sfft_solve(sfft_plan* p, const double* A, const double* b, double* coeffs, int* info, void* stream) {
   if (!p || !A || !b || !coeffs) return SFFT_ERR_INVALID_ARG;
   int nl = 0;
-  sfft_status s = sfft_launch_solve(p, A, b, coeffs, info, (cudaStream_t)stream, &nl);
+  sfft_status s;
+  { ProfScope ps(p, 5, (cudaStream_t)stream); s = sfft_launch_solve(p, A, b, coeffs, info, (cudaStream_t)stream, &nl); }
   if (s != SFFT_OK) return s;
   p->launches[1] = nl;
   return SFFT_OK;
@@ -205,39 +208,40 @@ sfft_status sfft_probe_fp64(int kind, int iters, double* tflops, double* elapsed
   return s;
 }
 
+sfft_status sfft_profile_enable(sfft_plan* p, int on) {
+  if (!p) return SFFT_ERR_INVALID_ARG;
+  if (on && !p->prof_ev[0]) {
+    for (int i = 0; i < 2 * SFFT_PROF_MAX; ++i)
+      if (cudaEventCreate(&p->prof_ev[i]) != cudaSuccess) { cudaGetLastError(); return SFFT_ERR_CUDA; }
+  }
+  p->prof_on = on ? 1 : 0;
+  return SFFT_OK;
+}
+
+sfft_status sfft_profile_read(sfft_plan* p, int stage, double* total_ms, int* count, int reset) {
+  if (!p || stage < 0 || stage >= SFFT_NSTAGE) return SFFT_ERR_INVALID_ARG;
+  // fold the pending event pairs into the per-stage totals (synchronises on those events)
+  for (int i = 0; i < p->prof_n; ++i) {
+    float ms = 0.f;
+    if (cudaEventSynchronize(p->prof_ev[2 * i + 1]) != cudaSuccess ||
+        cudaEventElapsedTime(&ms, p->prof_ev[2 * i], p->prof_ev[2 * i + 1]) != cudaSuccess) {
+      cudaGetLastError();
+      p->prof_n = 0;
+      return SFFT_ERR_CUDA;
+    }
+    p->prof_ms[p->prof_stage[i]] += ms;
+    p->prof_cnt[p->prof_stage[i]] += 1;
+  }
+  p->prof_n = 0;
+  if (total_ms) *total_ms = p->prof_ms[stage];
+  if (count) *count = p->prof_cnt[stage];
+  if (reset) { p->prof_ms[stage] = 0.0; p->prof_cnt[stage] = 0; }
+  return SFFT_OK;
+}
+
 int sfft_last_launch_count(const sfft_plan* p, int which) {
   if (!p || which < 0 || which > 2) return -1;
   return p->launches[which];
-}
-
-sfft_status sfft_model_cost(const sfft_plan* p, int which, double* fp64_instr, double* hbm_bytes) {
-  if (!p || which < 0 || which > 2) return SFFT_ERR_INVALID_ARG;
-  // Algorithmic model of DESIGN.md ("Cost model"): fp64 pipe instructions (DFMA/DADD/DMUL, one
-  // per lane) and compulsory HBM bytes of one call at this plan's sizes.
-  const double H = p->H, W = p->W, NC = p->NC, P = H * W;
-  const double fftH = 3.6 * H * p->log2H;      // instr per H-point complex FFT (radix-16/8 mix)
-  const double fftN = 3.6 * NC * p->log2NC + 10.0 * NC;  // per real row (W/2 complex FFT + split)
-  double fi = 0, hb = 0;
-  if (which == 0) {
-    const double nKK = p->TK * (p->TK + 1) / 2.0, nKO = p->TK * (1.0 + p->TB);
-    const double perColKK = H * 4.0 + (H / 8.0) * (56.0 + 8.0 * p->Dmax);   // product + DFT-8 + outer
-    const double perColKO = H * 4.0 + (H / 8.0) * (56.0 + 8.0 * p->w);
-    fi = p->nRowImg * H * fftN + p->nSpec * NC * fftH + (NC + 1) * (nKK * perColKK + nKO * perColKO);
-    hb = 2.0 * P * 8 + P            // R, S, mask read once
-         + 2.0 * p->nRowImg * P * 8   // row spectra written + read
-         + 2.0 * p->nSpec * P * 8     // spectra written + read once
-         + (double)p->N * p->N * 8;
-  } else if (which == 1) {
-    const double N = p->N;
-    fi = N * N * N / 6.0 + 2.0 * N * N;
-    hb = 2.0 * N * N * 8;
-  } else {
-    fi = (p->DK + 1) * H * fftN + H * fftN + P / 2.0 * (2 * p->w + 1) * (4.0 * (p->DK + 1) + 2.0 * (p->TK - 1 - p->DK) + 0.0);
-    hb = 3.0 * P * 8 + 2.0 * (p->DK + 1) * P * 8 + 2.0 * P * 8;
-  }
-  if (fp64_instr) *fp64_instr = fi;
-  if (hbm_bytes) *hbm_bytes = hb;
-  return SFFT_OK;
 }
 
 }  // extern "C"

@@ -8,7 +8,9 @@
 #define SFFT_MAX_DEG 3
 #define SFFT_MAX_T 10     // (3+1)(3+2)/2 monomials of degree <= 3
 #define SFFT_MAX_W 15
-#define SFFT_PITCH_PAD 8  // spectrum row pitch = W/2 + 8 complex (column W/2 = Nyquist)
+#define SFFT_PITCH_PAD 8
+#define SFFT_NSTAGE 9      // see sfft_profile_read in include/sfft.h
+#define SFFT_PROF_MAX 512  // spectrum row pitch = W/2 + 8 complex (column W/2 = Nyquist)
 
 typedef double2 cplx;
 
@@ -102,6 +104,26 @@ struct sfft_plan {
   size_t ws_bytes;
   int launches[3];
   int num_sms;
+  // optional per-stage CUDA-event timing (sfft_profile_*): events are recorded on the caller
+  // stream around each stage; nothing synchronises until sfft_profile_read.
+  int prof_on;
+  int prof_n;                       // recorded (stage, e0, e1) triples awaiting a read
+  int prof_stage[SFFT_PROF_MAX];
+  cudaEvent_t prof_ev[2 * SFFT_PROF_MAX];
+  double prof_ms[SFFT_NSTAGE];
+  int prof_cnt[SFFT_NSTAGE];
+};
+
+struct ProfScope {  // RAII: record an event pair around one stage when profiling is on
+  sfft_plan* p; cudaStream_t st; int slot;
+  ProfScope(sfft_plan* p_, int stage, cudaStream_t st_) : p(p_), st(st_), slot(-1) {
+    if (p->prof_on && p->prof_n < SFFT_PROF_MAX) {
+      slot = p->prof_n++;
+      p->prof_stage[slot] = stage;
+      cudaEventRecord(p->prof_ev[2 * slot], st);
+    }
+  }
+  ~ProfScope() { if (slot >= 0) cudaEventRecord(p->prof_ev[2 * slot + 1], st); }
 };
 
 #define SFFT_CUDA_TRY(expr)                          \
