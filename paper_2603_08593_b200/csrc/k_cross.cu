@@ -8,8 +8,9 @@
 //  k_cross<D>   : for every column kx, Y[dy][kx] = sum_ky conj(F_f) F_g e^{+2 pi i ky dy/H}, |dy|<=D.
 //                 Output-pruned decimation: ky = b + (H/8) a, so
 //                 Y[dy] = sum_b e^{2 pi i b dy/H} Z_b[dy mod 8],  Z_b = 8-point inverse DFT over a.
-//                 One thread owns one column (lanes = adjacent kx -> 512-byte coalesced rows);
-//                 the 2D+1 accumulators live in registers; no shared memory, no reduction.
+//                 One thread owns one (pair, column); a CTA owns 16 adjacent columns and a group of
+//                 <= 21 pairs whose spectra tiles are staged once in shared memory (cp.async,
+//                 double buffered); the 2D+1 accumulators live in registers.
 //  k_lag_idft   : C[dy][dx] = (1/P) [ Re Y[dy][0] + (-1)^dx Re Y[dy][NC]
 //                                     + 2 sum_{kx=1}^{NC-1} Re( Y[dy][kx] e^{2 pi i kx dx/W} ) ].
 //  k_mom_final  : reduces the per-row moments of k_row_fwd to sum m xi^a eta^b and sum m xi^p eta^q S.
@@ -20,90 +21,152 @@
 struct CrossParams {
   const cplx* F;
   cplx* Y;
-  const PairDesc* pairs;
-  int pair0, npair;   // pairs [pair0, pair0+npair) share the same D
+  const CrossGroup* groups;  // device array; blockIdx.y selects groups[g0 + blockIdx.y]
+  int g0;
   int H, NC, pitch, nLag;
+  int NB, log2NB;            // b values staged per pipeline stage (power of two, divides H/8)
   const cplx* twH;
 };
 
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gsrc));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+// One CTA = SFFT_CR_CT adjacent columns x one group of <= SFFT_CR_GP pairs; thread = (pair, column).
+// The group's spectra tiles are staged once in shared memory by cp.async (double buffered) and
+// shared by all of its pairs, so every spectrum element leaves L2 once per group instead of once
+// per pair.  Per staged b: x[a] = conj(F_f) F_g at ky = b + (H/8) a, 8-point inverse DFT over a,
+// then the 2D+1 twiddled accumulations in registers.
 template <int D>
-__global__ void __launch_bounds__(128) k_cross(CrossParams P) {
-  const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
-  const int pi = blockIdx.y * 4 + wrp;
-  if (pi >= P.npair) return;
-  const PairDesc pd = P.pairs[P.pair0 + pi];
-  int kx = blockIdx.x * 32 + lane;
-  const bool active = kx <= P.NC;
-  if (!active) kx = P.NC;
-  const size_t specStride = (size_t)P.H * P.pitch;
-  const cplx* Fa = P.F + pd.fa * specStride + kx;
-  const cplx* Fb = P.F + pd.fb * specStride + kx;
+__global__ void __launch_bounds__(SFFT_CR_GP * SFFT_CR_CT, 1) k_cross(CrossParams P) {
+  constexpr int CT = SFFT_CR_CT;
+  constexpr int NTH = SFFT_CR_GP * SFFT_CR_CT;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ CrossGroup G;
+  const int tid = threadIdx.x;
+  {
+    const int* src = reinterpret_cast<const int*>(P.groups + P.g0 + blockIdx.y);
+    int* dst = reinterpret_cast<int*>(&G);
+    for (int e = tid; e < (int)(sizeof(CrossGroup) / sizeof(int)); e += NTH) dst[e] = src[e];
+  }
+  __syncthreads();
+  const int ns = G.ns, NB = P.NB, lNB = P.log2NB;
+  const int pl = tid / CT, col = tid - pl * CT;
+  const bool has_pair = pl < G.np;
+  const int la = has_pair ? G.la[pl] : 0, lb = has_pair ? G.lb[pl] : 0;
+  const int kx0 = blockIdx.x * CT;
   const int N1 = P.H >> 3;
-  const size_t rstep = (size_t)N1 * P.pitch;
+  const size_t specStride = (size_t)P.H * P.pitch;
+  const int stageElems = ns * NB * 8 * CT;
+  cplx* buf0 = reinterpret_cast<cplx*>(smem_raw);
+  cplx* buf1 = buf0 + stageElems;
+
+  auto issue = [&](int b0, cplx* buf) {
+    for (int e = tid; e < stageElems; e += NTH) {
+      const int c = e % CT, r = e / CT;            // r = (s*NB + bb)*8 + a
+      const int a = r & 7, bb = (r >> 3) & (NB - 1), s = r >> (3 + lNB);
+      const cplx* src = P.F + (size_t)G.spec[s] * specStride + (size_t)(b0 + bb + a * N1) * P.pitch + kx0 + c;
+      cp_async16(buf + e, src);
+    }
+    cp_async_commit();
+  };
+
   cplx acc[2 * D + 1];
 #pragma unroll
   for (int i = 0; i < 2 * D + 1; ++i) acc[i] = cmake(0.0, 0.0);
-  for (int b = 0; b < N1; ++b) {
-    cplx x[8];
-    const cplx* pa = Fa + (size_t)b * P.pitch;
-    const cplx* pb = Fb + (size_t)b * P.pitch;
-#pragma unroll
-    for (int a = 0; a < 8; ++a) x[a] = cmulc(ldg2(pa + a * rstep), ldg2(pb + a * rstep));
-    Dft<8, +1>::run(x);
-    acc[D] = cadd(acc[D], x[0]);
-#pragma unroll
-    for (int i = 1; i <= D; ++i) {
-      const cplx t = ldg2(P.twH + ((b * i) & (P.H - 1)));  // e^{-2 pi i b i/H}
-      cfmac(acc[D + i], t, x[i & 7]);                      // += e^{+...} * Z[i mod 8]
-      cfma(acc[D - i], t, x[(8 - (i & 7)) & 7]);           // += e^{-...} * Z[-i mod 8]
+
+  const int nst = N1 >> lNB;
+  issue(0, buf0);
+  for (int st = 0; st < nst; ++st) {
+    cplx* cur = (st & 1) ? buf1 : buf0;
+    if (st + 1 < nst) {
+      issue((st + 1) << lNB, (st & 1) ? buf0 : buf1);
+      cp_async_wait<1>();
+    } else {
+      cp_async_wait<0>();
     }
+    __syncthreads();
+    if (has_pair) {
+      const cplx* pa = cur + (size_t)la * NB * 8 * CT + col;
+      const cplx* pb = cur + (size_t)lb * NB * 8 * CT + col;
+      for (int bb = 0; bb < NB; ++bb) {
+        const int b = (st << lNB) + bb;
+        cplx x[8];
+#pragma unroll
+        for (int a = 0; a < 8; ++a) x[a] = cmulc(pa[(bb * 8 + a) * CT], pb[(bb * 8 + a) * CT]);
+        Dft<8, +1>::run(x);
+        acc[D] = cadd(acc[D], x[0]);
+#pragma unroll
+        for (int i = 1; i <= D; ++i) {
+          const cplx t = ldg2(P.twH + ((b * i) & (P.H - 1)));  // e^{-2 pi i b i/H}
+          cfmac(acc[D + i], t, x[i & 7]);                      // += e^{+...} * Z[i mod 8]
+          cfma(acc[D - i], t, x[(8 - (i & 7)) & 7]);           // += e^{-...} * Z[-i mod 8]
+        }
+      }
+    }
+    __syncthreads();
   }
-  if (active) {
-    cplx* out = P.Y + ((size_t)(P.pair0 + pi) * P.nLag) * P.pitch + kx;
+  const int kx = kx0 + col;
+  if (has_pair && kx <= P.NC) {
+    const int Dp = G.D;  // the instantiated range may exceed the group's own half-range
+    cplx* out = P.Y + ((size_t)G.pair[pl] * P.nLag) * P.pitch + kx;
 #pragma unroll
     for (int i = 0; i < 2 * D + 1; ++i) {
-      const int dy = i - D;  // the instantiated range may exceed the pair's own half-range pd.D
-      if (dy >= -pd.D && dy <= pd.D) out[(size_t)(dy + pd.D) * P.pitch] = acc[i];
+      const int dy = i - D;
+      if (dy >= -Dp && dy <= Dp) out[(size_t)(dy + Dp) * P.pitch] = acc[i];
     }
   }
 }
 
 template <int D>
-static sfft_status launch_cross_t(const CrossParams& P, cudaStream_t st) {
-  dim3 grid((P.NC + 1 + 31) / 32, (P.npair + 3) / 4);
-  k_cross<D><<<grid, 128, 0, st>>>(P);
+static sfft_status launch_cross_t(const CrossParams& P, int ngroups, int maxns, cudaStream_t st) {
+  const size_t smem = (size_t)2 * maxns * P.NB * 8 * SFFT_CR_CT * sizeof(cplx);
+  SFFT_CUDA_TRY(cudaFuncSetAttribute(k_cross<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  dim3 grid(P.NC / SFFT_CR_CT + 1, ngroups);
+  k_cross<D><<<grid, SFFT_CR_GP * SFFT_CR_CT, smem, st>>>(P);
   SFFT_LAUNCH_CHECK();
   return SFFT_OK;
 }
 
-static sfft_status launch_cross_D(int D, const CrossParams& P, cudaStream_t st) {
+static sfft_status launch_cross_D(int D, const CrossParams& P, int ngroups, int maxns, cudaStream_t st) {
   switch (D) {
-    case 0: case 1: return launch_cross_t<1>(P, st);
-    case 2: return launch_cross_t<2>(P, st);
-    case 3: return launch_cross_t<3>(P, st);
-    case 4: return launch_cross_t<4>(P, st);
-    case 5: return launch_cross_t<5>(P, st);
-    case 6: return launch_cross_t<6>(P, st);
-    case 7: case 8: return launch_cross_t<8>(P, st);
-    case 9: case 10: return launch_cross_t<10>(P, st);
+    case 0: case 1: return launch_cross_t<1>(P, ngroups, maxns, st);
+    case 2: return launch_cross_t<2>(P, ngroups, maxns, st);
+    case 3: return launch_cross_t<3>(P, ngroups, maxns, st);
+    case 4: return launch_cross_t<4>(P, ngroups, maxns, st);
+    case 5: return launch_cross_t<5>(P, ngroups, maxns, st);
+    case 6: return launch_cross_t<6>(P, ngroups, maxns, st);
+    case 7: case 8: return launch_cross_t<8>(P, ngroups, maxns, st);
+    case 9: case 10: return launch_cross_t<10>(P, ngroups, maxns, st);
     default: return SFFT_ERR_UNSUPPORTED;
   }
 }
 
 sfft_status sfft_launch_cross(sfft_plan* p, cudaStream_t st, int* nl) {
   CrossParams P;
-  P.F = p->F; P.Y = p->Y; P.pairs = p->d_pairs; P.H = p->H; P.NC = p->NC; P.pitch = p->pitch;
+  P.F = p->F; P.Y = p->Y; P.groups = p->d_groups; P.H = p->H; P.NC = p->NC; P.pitch = p->pitch;
   P.nLag = p->nLag; P.twH = p->twH;
-  // pairs are sorted: kernel-kernel (D = 2w) first, then the D = w pairs
-  const int nKK = p->TK * (p->TK + 1) / 2;
-  P.pair0 = 0; P.npair = nKK;
-  ++*nl;
+  const int N1 = p->H / 8;
+  auto pickNB = [&](int maxns) {  // largest staged depth whose double buffer fits in shared memory
+    int nb = 4;
+    while (nb > 1 && ((size_t)2 * maxns * nb * 8 * SFFT_CR_CT * sizeof(cplx) > 200 * 1024 || nb > N1)) nb >>= 1;
+    return nb;
+  };
   sfft_status s;
-  { ProfScope ps(p, 2, st); s = launch_cross_D(2 * p->w, P, st); }
-  if (s != SFFT_OK) return s;
-  P.pair0 = nKK; P.npair = p->nPair - nKK;
+  // groups are sorted: kernel-kernel (D = 2w) first, then the D = w groups
+  P.g0 = 0;
+  P.NB = pickNB(p->maxnsKK); P.log2NB = P.NB == 4 ? 2 : (P.NB == 2 ? 1 : 0);
   ++*nl;
-  { ProfScope ps(p, 3, st); s = launch_cross_D(p->w, P, st); }
+  { ProfScope ps(p, 2, st); s = launch_cross_D(2 * p->w, P, p->nGroupKK, p->maxnsKK, st); }
+  if (s != SFFT_OK) return s;
+  P.g0 = p->nGroupKK;
+  P.NB = pickNB(p->maxnsKO); P.log2NB = P.NB == 4 ? 2 : (P.NB == 2 ? 1 : 0);
+  ++*nl;
+  { ProfScope ps(p, 3, st); s = launch_cross_D(p->w, P, p->nGroupKO, p->maxnsKO, st); }
   return s;
 }
 

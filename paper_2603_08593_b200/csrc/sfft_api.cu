@@ -38,7 +38,7 @@ static cudaError_t upload_twiddles(cplx** dst, int n) {
 
 static void plan_free(sfft_plan* p) {
   if (!p) return;
-  cudaFree(p->twNC); cudaFree(p->twW); cudaFree(p->twH); cudaFree(p->d_pairs);
+  cudaFree(p->twNC); cudaFree(p->twW); cudaFree(p->twH); cudaFree(p->d_pairs); cudaFree(p->d_groups);
   cudaFree(p->T); cudaFree(p->F); cudaFree(p->Y); cudaFree(p->Cmap); cudaFree(p->rowMom);
   cudaFree(p->mom); cudaFree(p->Lw); cudaFree(p->Ldiag); cudaFree(p->Etab); cudaFree(p->Mhat);
   free(p->h_pairs);
@@ -105,6 +105,28 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
     for (int t2 = 0; t2 < p->TB; ++t2) { p->h_pairs[n].fa = t; p->h_pairs[n].fb = p->TK + 1 + t2; p->h_pairs[n].D = w; ++n; }
   }
 
+  // k_cross groups: consecutive pairs (same D class) packed while the group holds <= SFFT_CR_GP
+  // pairs and <= SFFT_CR_MAXSPEC distinct spectra
+  std::vector<CrossGroup> groups;
+  const int nKKpairs = p->TK * (p->TK + 1) / 2;
+  for (int cls = 0; cls < 2; ++cls) {
+    const int lo = cls == 0 ? 0 : nKKpairs, hi = cls == 0 ? nKKpairs : p->nPair;
+    int maxns = 0, ng = 0;
+    CrossGroup g; memset(&g, 0, sizeof(g));
+    auto slot = [&](CrossGroup& gg, int spec) { for (int i = 0; i < gg.ns; ++i) if (gg.spec[i] == spec) return i; return -1; };
+    auto flush = [&]() { if (g.np) { groups.push_back(g); if (g.ns > maxns) maxns = g.ns; ++ng; } memset(&g, 0, sizeof(g)); };
+    for (int i = lo; i < hi; ++i) {
+      const PairDesc& pd = p->h_pairs[i];
+      int need = (slot(g, pd.fa) < 0) + (pd.fb != pd.fa && slot(g, pd.fb) < 0);
+      if (g.np == SFFT_CR_GP || g.ns + need > SFFT_CR_MAXSPEC) flush();
+      if (slot(g, pd.fa) < 0) g.spec[g.ns++] = pd.fa;
+      if (slot(g, pd.fb) < 0) g.spec[g.ns++] = pd.fb;
+      g.la[g.np] = slot(g, pd.fa); g.lb[g.np] = slot(g, pd.fb); g.pair[g.np] = i; g.D = pd.D; ++g.np;
+    }
+    flush();
+    if (cls == 0) { p->nGroupKK = ng; p->maxnsKK = maxns; } else { p->nGroupKO = ng; p->maxnsKO = maxns; }
+  }
+
   size_t ws = 0;
   bool ok = true;
   auto dalloc = [&](void** ptr, size_t bytes) {
@@ -124,10 +146,13 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   dalloc((void**)&p->Etab, sizeof(cplx) * (size_t)p->TK * (2 * w + 1) * p->NC);
   dalloc((void**)&p->Mhat, sizeof(cplx) * HN);
   dalloc((void**)&p->d_pairs, sizeof(PairDesc) * p->nPair);
+  dalloc((void**)&p->d_groups, sizeof(CrossGroup) * groups.size());
   if (!ok) { plan_free(p); return SFFT_ERR_ALLOC; }
   if (upload_twiddles(&p->twNC, p->NC) != cudaSuccess || upload_twiddles(&p->twW, W) != cudaSuccess ||
       upload_twiddles(&p->twH, H) != cudaSuccess ||
       cudaMemcpy(p->d_pairs, p->h_pairs, sizeof(PairDesc) * p->nPair, cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemcpy(p->d_groups, groups.data(), sizeof(CrossGroup) * groups.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemset(p->F, 0, sizeof(cplx) * HP * p->nSpec) != cudaSuccess ||
       cudaMemset(p->Y, 0, sizeof(cplx) * (size_t)p->nPair * p->nLag * p->pitch) != cudaSuccess ||
       cudaMemset(p->Cmap, 0, sizeof(double) * (size_t)p->nPair * p->nLag * p->nLag) != cudaSuccess) {
     cudaGetLastError();

@@ -8,9 +8,12 @@
 #define SFFT_MAX_DEG 3
 #define SFFT_MAX_T 10     // (3+1)(3+2)/2 monomials of degree <= 3
 #define SFFT_MAX_W 15
-#define SFFT_PITCH_PAD 8
+#define SFFT_PITCH_PAD 16   // spectrum row pitch = W/2 + 16 complex (column W/2 = Nyquist; a 16-column tile at W/2 stays in the row)
+#define SFFT_CR_CT 16        // k_cross: columns per CTA
+#define SFFT_CR_GP 21        // k_cross: pairs per CTA (threads = SFFT_CR_GP * SFFT_CR_CT)
+#define SFFT_CR_MAXSPEC 24   // k_cross: spectra a group may stage
 #define SFFT_NSTAGE 9      // see sfft_profile_read in include/sfft.h
-#define SFFT_PROF_MAX 512  // spectrum row pitch = W/2 + 8 complex (column W/2 = Nyquist)
+#define SFFT_PROF_MAX 512
 
 typedef double2 cplx;
 
@@ -67,6 +70,15 @@ struct PairDesc {
   int D;    // lags needed: dy,dx in [-D, D]
 };
 
+// A group of pairs handled by one k_cross CTA: the spectra it stages and, per pair, the local slots
+// of its two spectra and its row block in Y.  All pairs of a group share the lag half-range D.
+struct CrossGroup {
+  int ns, np, D, pad;
+  int spec[SFFT_CR_MAXSPEC];
+  int la[SFFT_CR_GP], lb[SFFT_CR_GP];
+  int pair[SFFT_CR_GP];
+};
+
 struct sfft_plan {
   int H, W, w, DK, DB;
   int L, TK, TB, N;
@@ -88,6 +100,8 @@ struct sfft_plan {
   cplx* twH;     // e^{-2 pi i m / H},  m in [0, H)
   PairDesc* d_pairs;
   PairDesc* h_pairs;
+  CrossGroup* d_groups;   // kernel-kernel groups first, then the D = w groups
+  int nGroupKK, nGroupKO, maxnsKK, maxnsKO;
 
   // device scratch
   cplx* T;       // row-pass output  [nRowImg][H][NC]   (packed: column 0 = DC + i Nyquist)
