@@ -1,182 +1,371 @@
 // Blocked fp64 Cholesky solve of the normal equations (north_star subsystem (5)).
 //
-// Right-looking blocked factorisation A = Lc Lc^T, block size NB = 32, on the augmented matrix
-// [A b; b^T .]: carrying b as row N through the panel solves yields z = Lc^-1 b for free (the
-// forward substitution), so only the back substitution Lc^T c = z remains.
-//   k_chol_load   : copy the lower triangle of A and b into the workspace (inputs stay untouched)
-//   k_chol_panel  : every CTA factors the 32x32 diagonal block in shared memory (redundantly, which
-//                   saves a launch), then solves its rows of the panel X Lkk^T = A_ik, one row per
-//                   thread, by substitution (backward stable; no explicit block inverse)
-//   k_chol_update : trailing update A22 -= L21 L21^T on 32x32 tiles of the lower triangle
-//   k_chol_back   : one CTA, blocked back substitution with the stored diagonal factors
+// One persistent cooperative kernel (k_chol_fused) runs the whole solve; the CTAs meet at a
+// software grid barrier between phases, so the 2*N/32 phase boundaries cost ~1 us each instead of
+// a kernel launch.  Right-looking blocked factorisation A = Lc Lc^T, block size NB = 32, on the
+// augmented matrix [A b; b^T .]: carrying b as row N through the panel solves yields
+// z = Lc^-1 b for free (the forward substitution), so only the back substitution Lc^T c = z remains.
+//   phase 0       : copy the lower triangle of A and b into the workspace (inputs stay untouched)
+//   panel phase k : every CTA factors the 32x32 diagonal block redundantly in shared memory
+//                   (square-root-free elimination, scaled afterwards), then solves its rows of the
+//                   panel X Lkk^T = A_ik, one row per warp, by substitution (backward stable; no
+//                   explicit block inverse)
+//   update phase k: trailing update A22 -= L21 L21^T on 32x32 tiles of the lower triangle
+//   k_chol_back   : one 1024-thread CTA, blocked back substitution (a second, tiny launch)
+// Square roots and divisions on the critical path are rsqrt + one fused Newton correction each
+// (<= 1 ulp), which keeps the 32 dependent steps of a diagonal block short.
 // info: 0, or the 1-based order of the first non-positive leading minor (no pivoting, no
 // regularisation: DESIGN.md reading A9).
 #include "sfft_common.cuh"
 
 #define CH_NB 32
+#define CH_THREADS 256
+#define CH_WARPS (CH_THREADS / 32)
 
-__global__ void __launch_bounds__(256) k_chol_load(const double* __restrict__ A,
-                                                    const double* __restrict__ b, double* Lw, int N,
-                                                    int ld, int* info) {
-  const size_t total = (size_t)(N + 1) * N;
-  if (blockIdx.x == 0 && threadIdx.x == 0 && info) *info = 0;
-  for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total;
-       e += (size_t)gridDim.x * blockDim.x) {
-    const int i = (int)(e / N), j = (int)(e - (size_t)i * N);
-    if (i == N) Lw[(size_t)N * ld + j] = b[j];
-    else if (j <= i) Lw[(size_t)i * ld + j] = A[e];
+// Optional phase timestamps (development builds only: -DSFFT_CHOL_TIMING): CTA 0 records
+// %globaltimer at every phase boundary into sfft_chol_dbg.
+#ifdef SFFT_CHOL_TIMING
+__device__ unsigned long long sfft_chol_dbg[256];
+#define CH_STAMP(i)                                                              \
+  if (blockIdx.x == 0 && threadIdx.x == 0 && (i) < 256) {                        \
+    unsigned long long t_;                                                       \
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));                       \
+    sfft_chol_dbg[i] = t_;                                                       \
   }
-}
+#else
+#define CH_STAMP(i)
+#endif
 
-__global__ void __launch_bounds__(128) k_chol_panel(double* Lw, double* Ldiag, int N, int ld, int k0,
-                                                     int* info) {
-  __shared__ double sd[CH_NB][CH_NB + 1];
-  const int tid = threadIdx.x;
-  const int nb = min(CH_NB, N - k0);
-  for (int e = tid; e < CH_NB * CH_NB; e += 128) {
-    const int i = e / CH_NB, j = e % CH_NB;
-    sd[i][j] = (i < nb && j <= i) ? Lw[(size_t)(k0 + i) * ld + k0 + j] : (i == j ? 1.0 : 0.0);
+__device__ __forceinline__ double ld_cg(const double* p) { return __ldcg(p); }
+
+// Grid barrier: monotonically increasing arrival counter; `target` is this CTA's private copy of
+// the count that completes the next barrier.  Data written before the barrier is visible after it
+// to loads that bypass L1 (ld_cg).
+__device__ __forceinline__ void grid_barrier(unsigned* ctr, unsigned& target, unsigned nblocks) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    target += nblocks;
+    __threadfence();
+    atomicAdd(ctr, 1u);
+    unsigned v;
+    do {
+      asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
+    } while (v < target);
   }
   __syncthreads();
-  for (int k = 0; k < nb; ++k) {
-    if (tid == 0) {
-      double d = sd[k][k];
-      if (!(d > 0.0)) {
-        if (blockIdx.x == 0 && info) atomicCAS(info, 0, k0 + k + 1);
-        d = 1.0;
-      }
-      sd[k][k] = sqrt(d);
-    }
-    __syncthreads();
-    if (tid > k && tid < nb) sd[tid][k] /= sd[k][k];
-    __syncthreads();
-    // trailing update of the block: elements (i,j), k < j <= i < nb
-    for (int e = tid; e < CH_NB * CH_NB; e += 128) {
-      const int i = e / CH_NB, j = e % CH_NB;
-      if (j > k && j <= i && i < nb) sd[i][j] = fma(-sd[i][k], sd[j][k], sd[i][j]);
-    }
-    __syncthreads();
-  }
-  if (blockIdx.x == 0) {
-    double* dst = Ldiag + (size_t)(k0 / CH_NB) * CH_NB * CH_NB;
-    for (int e = tid; e < CH_NB * CH_NB; e += 128) dst[e] = sd[e / CH_NB][e % CH_NB];
-  }
-  // panel rows below the diagonal block (including the rhs row N): one row per thread
-  const int row = k0 + nb + blockIdx.x * 128 + tid;
-  if (row <= N) {
-    double x[CH_NB];
-    double* src = Lw + (size_t)row * ld + k0;
-#pragma unroll
-    for (int j = 0; j < CH_NB; ++j) x[j] = (j < nb) ? src[j] : 0.0;
-#pragma unroll
-    for (int j = 0; j < CH_NB; ++j) {
-      double a = x[j];
-#pragma unroll
-      for (int m = 0; m < j; ++m) a = fma(-x[m], sd[j][m], a);
-      x[j] = a / sd[j][j];
-    }
-#pragma unroll
-    for (int j = 0; j < CH_NB; ++j)
-      if (j < nb) src[j] = x[j];
-  }
 }
 
-__global__ void __launch_bounds__(256) k_chol_update(double* Lw, int N, int ld, int k0) {
-  // tile (ti, tj), tj <= ti, of the trailing matrix starting at r0 = k0 + NB
-  const int r0 = k0 + CH_NB;
-  const int ti = blockIdx.y, tj = blockIdx.x;
-  if (tj > ti) return;
-  __shared__ double pi[CH_NB][CH_NB + 1], pj[CH_NB][CH_NB + 1];
-  const int tid = threadIdx.x;
-  for (int e = tid; e < CH_NB * CH_NB; e += 256) {
-    const int r = e / CH_NB, m = e % CH_NB;
-    const int gi = r0 + ti * CH_NB + r, gj = r0 + tj * CH_NB + r;
-    pi[r][m] = (gi <= N) ? Lw[(size_t)gi * ld + k0 + m] : 0.0;
-    pj[r][m] = (gj < N) ? Lw[(size_t)gj * ld + k0 + m] : 0.0;
+// sqrt and reciprocal-multiply with one fused correction step each
+__device__ __forceinline__ void sqrt_and_rinv(double a, double& d, double& r) {
+  r = rsqrt(a);
+  d = a * r;
+  d = fma(fma(-d, d, a), 0.5 * r, d);   // d = sqrt(a), < 1 ulp
+  r = fma(fma(-d, r, 1.0), r, r);       // r = 1/d
+}
+__device__ __forceinline__ double div_by(double x, double d, double r) {  // x / d given r ~ 1/d
+  const double q = x * r;
+  return fma(fma(-q, d, x), r, q);
+}
+
+__device__ __forceinline__ double rcp_newton(double a) {  // 1/a for normal positive a, ~1 ulp
+  // seed r0 (>= 20 bits), e = 1 - a r0; 1/a = r0 (1 + e + e^2 + O(e^3)): three dependent fp64 ops
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a));
+  const double e = fma(-a, r, 1.0);
+  return fma(r, fma(e, e, e), r);
+}
+
+// Cholesky of the 32x32 block in sd (lower triangle) by the whole CTA.  The 32 dependent steps run
+// the square-root-free elimination a_ij -= a_ik a_jk / a_kk; the columns are scaled by
+// 1/sqrt(pivot) afterwards, which gives exactly the Cholesky factor.  Thread (warp w, lane j) keeps
+// its elements (4w..4w+3, j) in registers for the whole elimination; per step only the pivot
+// column travels through shared memory (double buffered, so one barrier per step), which keeps
+// the step at 4 shared loads per thread.  srd receives 1/L_jj.  Returns the 0-based index of the
+// first non-positive pivot (or -1); failed pivots are replaced by 1 so the work stays finite.
+__device__ __forceinline__ int cta_potrf32(double (*sd)[CH_NB + 1], double* srd, double (*colb)[CH_NB],
+                                           int tid) {
+  static_assert(CH_WARPS == 8, "row ownership below assumes 8 warps x 4 rows");
+  const int j = tid & 31, i0 = (tid >> 5) * 4;
+  double c[4];
+  __syncthreads();  // sd was just filled by other threads
+#pragma unroll
+  for (int rr = 0; rr < 4; ++rr) c[rr] = sd[i0 + rr][j];
+  if (j == 0) {
+#pragma unroll
+    for (int rr = 0; rr < 4; ++rr) colb[0][i0 + rr] = c[rr];
   }
+  int bad = -1;
+#pragma unroll 1
+  for (int k = 0; k < CH_NB - 1; ++k) {
+    __syncthreads();
+    const double* cur = colb[k & 1];
+    double akk = cur[k];
+    const double ajk = cur[j];
+    const double2 a01 = *reinterpret_cast<const double2*>(cur + i0);
+    const double2 a23 = *reinterpret_cast<const double2*>(cur + i0 + 2);
+    if (!(akk > 0.0)) {
+      if (bad < 0) bad = k;
+      akk = 1.0;
+    }
+    // branch-free so that the loads and products are scheduled ahead of the reciprocal chain
+    const double p0 = a01.x * ajk, p1 = a01.y * ajk, p2 = a23.x * ajk, p3 = a23.y * ajk;
+    const double inv = (j > k) ? rcp_newton(akk) : 0.0;   // columns <= k are final
+    c[0] = fma(-p0, inv, c[0]);
+    c[1] = fma(-p1, inv, c[1]);
+    c[2] = fma(-p2, inv, c[2]);
+    c[3] = fma(-p3, inv, c[3]);
+    if (j == k + 1) {
+      double* nxt = colb[(k + 1) & 1];
+      *reinterpret_cast<double2*>(nxt + i0) = make_double2(c[0], c[1]);
+      *reinterpret_cast<double2*>(nxt + i0 + 2) = make_double2(c[2], c[3]);
+    }
+  }
+  // pivots (the diagonal as it stood when its column was eliminated) -> srd, then scale
   __syncthreads();
-  const int c = tid & 31, rb = tid >> 5;  // 8 row groups x 32 columns; 4 rows each
+#pragma unroll
+  for (int rr = 0; rr < 4; ++rr)
+    if (i0 + rr == j) srd[j] = c[rr];
+  __syncthreads();
+  double piv = srd[j];
+  if (!(srd[CH_NB - 1] > 0.0) && bad < 0) bad = CH_NB - 1;
+  if (!(piv > 0.0)) piv = 1.0;
+  double d, r;
+  sqrt_and_rinv(piv, d, r);
 #pragma unroll
   for (int rr = 0; rr < 4; ++rr) {
-    const int r = rb * 4 + rr;
-    const int gi = r0 + ti * CH_NB + r, gj = r0 + tj * CH_NB + c;
-    if (gi <= N && gj < N && gj <= gi) {
-      double a = 0.0;
-#pragma unroll
-      for (int m = 0; m < CH_NB; ++m) a = fma(pi[r][m], pj[c][m], a);
-      Lw[(size_t)gi * ld + gj] -= a;
+    const int i = i0 + rr;
+    sd[i][j] = (i == j) ? d : (i > j ? div_by(c[rr], d, r) : 0.0);
+  }
+  __syncthreads();
+  if (i0 == 0) srd[j] = r;
+  __syncthreads();
+  return bad;
+}
+
+__global__ void __launch_bounds__(CH_THREADS, 1)
+k_chol_fused(const double* __restrict__ A, const double* __restrict__ b, double* Lw,
+             int N, int ld, int* info, unsigned* bar) {
+  __shared__ double sd[CH_NB][CH_NB + 1];      // factored diagonal block
+  __shared__ double srd[CH_NB];                // reciprocals of its diagonal
+  __shared__ __align__(16) double colb[2][CH_NB];  // pivot column exchange of cta_potrf32
+  __shared__ double ss[CH_NB][CH_NB + 1];      // ss[m][j] = L[m][j] / L[j][j] (panel substitution)
+  __shared__ double pi[CH_NB][CH_NB + 1], pj[CH_NB][CH_NB + 1];
+  const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
+  const unsigned nblocks = gridDim.x;
+  unsigned target = 0;
+
+  // ---- phase 0: workspace <- lower triangle of A, row N <- b
+  {
+    const size_t total = (size_t)(N + 1) * N;
+    if (blockIdx.x == 0 && tid == 0 && info) *info = 0;
+    for (size_t e = (size_t)blockIdx.x * CH_THREADS + tid; e < total; e += (size_t)nblocks * CH_THREADS) {
+      const int i = (int)(e / N), j = (int)(e - (size_t)i * N);
+      if (i == N) Lw[(size_t)N * ld + j] = b[j];
+      else if (j <= i) Lw[(size_t)i * ld + j] = A[e];
     }
+  }
+  CH_STAMP(0)
+  grid_barrier(bar, target, nblocks);
+  CH_STAMP(1)
+  int stamp = 2;
+  (void)stamp;
+
+  const int gw = blockIdx.x * CH_WARPS + wrp, ngw = nblocks * CH_WARPS;
+  for (int k0 = 0; k0 < N; k0 += CH_NB) {
+    const int nb = min(CH_NB, N - k0);
+    const int rbelow = k0 + nb;                 // first row below the diagonal block
+    // ---- panel phase: CTAs that own panel rows (and CTA 0) factor the diagonal block
+    const bool has_rows = blockIdx.x * CH_WARPS < (N + 1 - rbelow);
+    if (has_rows || blockIdx.x == 0) {
+      for (int e = tid; e < CH_NB * CH_NB; e += CH_THREADS) {
+        const int i = e >> 5, j = e & 31;
+        sd[i][j] = (i < nb && j <= i) ? ld_cg(Lw + (size_t)(k0 + i) * ld + k0 + j) : (i == j ? 1.0 : 0.0);
+      }
+      const int bad = cta_potrf32(sd, srd, colb, tid);
+      if (bad >= 0 && bad < nb && blockIdx.x == 0 && tid == 0 && info) atomicCAS(info, 0, k0 + bad + 1);
+      for (int e = tid; e < CH_NB * CH_NB; e += CH_THREADS) {
+        const int i = e >> 5, j = e & 31;
+        ss[i][j] = sd[i][j] * srd[j];
+      }
+      if (blockIdx.x == 0) {
+        for (int e = tid; e < CH_NB * CH_NB; e += CH_THREADS) {
+          const int i = e >> 5, j = e & 31;
+          if (i < nb && j <= i) Lw[(size_t)(k0 + i) * ld + k0 + j] = sd[i][j];
+        }
+      }
+      __syncthreads();
+      CH_STAMP(stamp + 0)
+      // rows below (including the rhs row N): one row per warp, lane j holds entry j
+      for (int row = rbelow + gw; row <= N; row += ngw) {
+        double* src = Lw + (size_t)row * ld + k0;
+        double x = (lane < nb) ? ld_cg(src + lane) : 0.0;
+        // x_j = a_j / L_jj, a_m -= x_j L_mj = a_j (L_mj / L_jj): with the column-scaled factor
+        // ss the dependent chain per step is one shuffle and one fma; the division is off it
+#pragma unroll
+        for (int j = 0; j < CH_NB - 1; ++j) {
+          const double aj = __shfl_sync(0xffffffffu, x, j);
+          if (lane > j) x = fma(-aj, ss[lane][j], x);
+        }
+        if (lane < nb) src[lane] = div_by(x, sd[lane][lane], srd[lane]);
+      }
+    }
+    CH_STAMP(stamp + 1)
+    grid_barrier(bar, target, nblocks);
+    CH_STAMP(stamp + 2)
+    // ---- update phase: tiles (ti, tj), tj <= ti, of the trailing matrix starting at r0
+    const int r0 = k0 + CH_NB;
+    if (r0 <= N) {
+      const int T = (N + 1 - r0 + CH_NB - 1) / CH_NB;
+      const int ntile = T * (T + 1) / 2;
+      const int tx = tid & 15, ty = tid >> 4;      // outputs (ty, ty+16) x (tx, tx+16)
+      double gpi[4], gpj[4], cur[4];
+      int ti = 0, tj = 0;
+      auto decode = [&](int t, int& oi, int& oj) {   // t -> (ti, tj): ti(ti+1)/2 <= t
+        int q = (int)((sqrt(8.0 * t + 1.0) - 1.0) * 0.5);
+        while ((q + 1) * (q + 2) / 2 <= t) ++q;
+        while (q * (q + 1) / 2 > t) --q;
+        oi = q; oj = t - q * (q + 1) / 2;
+      };
+      auto fetch = [&](int fi, int fj) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const int e = tid + q * CH_THREADS, r = e >> 5, m = e & 31;
+          const int gi = r0 + fi * CH_NB + r, gj = r0 + fj * CH_NB + r;
+          gpi[q] = (gi <= N) ? ld_cg(Lw + (size_t)gi * ld + k0 + m) : 0.0;
+          gpj[q] = (gj < N) ? ld_cg(Lw + (size_t)gj * ld + k0 + m) : 0.0;
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const int gi = r0 + fi * CH_NB + ty + 16 * (q >> 1), gj = r0 + fj * CH_NB + tx + 16 * (q & 1);
+          cur[q] = (gi <= N && gj < N && gj <= gi) ? ld_cg(Lw + (size_t)gi * ld + gj) : 0.0;
+        }
+      };
+      int t = blockIdx.x;
+      if (t < ntile) { decode(t, ti, tj); fetch(ti, tj); }
+      while (t < ntile) {
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const int e = tid + q * CH_THREADS, r = e >> 5, m = e & 31;
+          pi[r][m] = gpi[q];
+          pj[r][m] = gpj[q];
+        }
+        double c0[4] = {cur[0], cur[1], cur[2], cur[3]};
+        const int ci = ti, cj = tj;
+        __syncthreads();
+        t += nblocks;
+        if (t < ntile) { decode(t, ti, tj); fetch(ti, tj); }
+        double acc[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+        for (int m = 0; m < CH_NB; ++m) {
+          const double a0 = pi[ty][m], a1 = pi[ty + 16][m], b0 = pj[tx][m], b1 = pj[tx + 16][m];
+          acc[0] = fma(a0, b0, acc[0]);
+          acc[1] = fma(a0, b1, acc[1]);
+          acc[2] = fma(a1, b0, acc[2]);
+          acc[3] = fma(a1, b1, acc[3]);
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const int gi = r0 + ci * CH_NB + ty + 16 * (q >> 1), gj = r0 + cj * CH_NB + tx + 16 * (q & 1);
+          if (gi <= N && gj < N && gj <= gi) Lw[(size_t)gi * ld + gj] = c0[q] - acc[q];
+        }
+      }
+      CH_STAMP(stamp + 3)
+      grid_barrier(bar, target, nblocks);
+      CH_STAMP(stamp + 4)
+    }
+    stamp += 5;
+  }
+
+  // last CTA out resets the barrier counter for the next launch
+  __syncthreads();
+  if (tid == 0) {
+    unsigned* done = bar + 1;
+    const unsigned old = atomicInc(done, nblocks - 1);
+    if (old == nblocks - 1) { __threadfence(); *bar = 0u; }
   }
 }
 
-__global__ void __launch_bounds__(1024) k_chol_back(const double* __restrict__ Lw,
-                                                     const double* __restrict__ Ldiag, double* c,
-                                                     int N, int ld) {
+// Back substitution Lc^T c = z; z is row N of the workspace.  Per 32-block (last to first): the
+// block's triangular system is solved by warp 0 (lane m holds r_m), then every thread j < k0
+// updates r_j -= sum_i L[k0+i][j] x_i with its 32 loads issued together (coalesced along j).
+__global__ void __launch_bounds__(1024, 1) k_chol_back(const double* __restrict__ Lw, double* c, int N, int ld) {
   extern __shared__ double sm[];
-  double* r = sm;             // N running right-hand side
-  double* ld_s = sm + N;      // 32 x 33 diagonal factor
-  double* cb = ld_s + CH_NB * (CH_NB + 1);  // 32 solved values of the current block
-  const int tid = threadIdx.x;
+  double* r = sm;                           // N running right-hand side
+  double* ls = sm + N;                      // 32 x 33 diagonal factor
+  double* rd = ls + CH_NB * (CH_NB + 1);    // reciprocals of its diagonal
+  double* cb = rd + CH_NB;                  // 32 solved values of the current block
+  const int tid = threadIdx.x, lane = tid & 31;
   for (int j = tid; j < N; j += 1024) r[j] = Lw[(size_t)N * ld + j];
   const int nblk = (N + CH_NB - 1) / CH_NB;
+  {
+    const int k0 = (nblk - 1) * CH_NB, nb = N - k0;
+    const int i = tid >> 5, j = tid & 31;
+    ls[i * (CH_NB + 1) + j] = (i < nb && j <= i) ? Lw[(size_t)(k0 + i) * ld + k0 + j] : (i == j ? 1.0 : 0.0);
+  }
+  __syncthreads();
   for (int kb = nblk - 1; kb >= 0; --kb) {
     const int k0 = kb * CH_NB;
     const int nb = min(CH_NB, N - k0);
-    __syncthreads();
-    for (int e = tid; e < CH_NB * CH_NB; e += 1024)
-      ld_s[(e / CH_NB) * (CH_NB + 1) + (e % CH_NB)] = Ldiag[(size_t)kb * CH_NB * CH_NB + e];
-    __syncthreads();
     if (tid < 32) {
-      // Lkk^T x = r_k: lane m holds r_m; columns solved from the last to the first
-      double rm = (tid < nb) ? r[k0 + tid] : 0.0;
-      for (int j = nb - 1; j >= 0; --j) {
+      rd[lane] = 1.0 / ls[lane * (CH_NB + 1) + lane];
+      __syncwarp();
+      double rm = (lane < nb) ? r[k0 + lane] : 0.0;
+#pragma unroll
+      for (int j = CH_NB - 1; j >= 0; --j) {
         const double rj = __shfl_sync(0xffffffffu, rm, j);
-        const double xj = rj / ld_s[j * (CH_NB + 1) + j];
-        if (tid == j) rm = xj;
-        else if (tid < j) rm = fma(-ld_s[j * (CH_NB + 1) + tid], xj, rm);
+        const double xj = div_by(rj, ls[j * (CH_NB + 1) + j], rd[j]);
+        if (lane == j) rm = xj;
+        else if (lane < j) rm = fma(-ls[j * (CH_NB + 1) + lane], xj, rm);
       }
-      if (tid < nb) {
-        cb[tid] = rm;
-        c[k0 + tid] = rm;
+      if (lane < nb) {
+        cb[lane] = rm;
+        c[k0 + lane] = rm;
+      } else {
+        cb[lane] = 0.0;
       }
+    }
+    // prefetch the next diagonal block while warp 0 solves
+    double nxt = 0.0;
+    if (kb > 0) {
+      const int i = tid >> 5, j = tid & 31;
+      nxt = (j <= i) ? Lw[(size_t)(k0 - CH_NB + i) * ld + k0 - CH_NB + j] : 0.0;
     }
     __syncthreads();
-    // r[j] -= sum_i L[k0+i][j] x_i for all j < k0 (coalesced along j)
+    if (kb > 0) ls[(tid >> 5) * (CH_NB + 1) + (tid & 31)] = nxt;
     for (int j = tid; j < k0; j += 1024) {
-      double a = r[j];
-#pragma unroll 8
-      for (int i = 0; i < nb; ++i) a = fma(-Lw[(size_t)(k0 + i) * ld + j], cb[i], a);
-      r[j] = a;
+      double v[CH_NB];
+#pragma unroll
+      for (int i = 0; i < CH_NB; ++i) v[i] = (i < nb) ? Lw[(size_t)(k0 + i) * ld + j] : 0.0;
+      double a0 = r[j], a1 = 0.0;
+#pragma unroll
+      for (int i = 0; i < CH_NB; i += 2) {
+        a0 = fma(-v[i], cb[i], a0);
+        a1 = fma(-v[i + 1], cb[i + 1], a1);
+      }
+      r[j] = a0 + a1;
     }
+    __syncthreads();
   }
 }
 
 sfft_status sfft_launch_solve(sfft_plan* p, const double* A, const double* b, double* c, int* info,
                               cudaStream_t st, int* nl) {
-  const int N = p->N, ld = p->ldL;
-  k_chol_load<<<148 * 4, 256, 0, st>>>(A, b, p->Lw, N, ld, info);
-  SFFT_LAUNCH_CHECK();
+  int N = p->N, ld = p->ldL;
+  double* Lw = p->Lw;
+  unsigned* bar = p->cholBar;
+  void* args[] = {(void*)&A, (void*)&b, (void*)&Lw, (void*)&N, (void*)&ld, (void*)&info, (void*)&bar};
+  // every CTA must be resident for the grid barrier: cooperative launch, one CTA per SM at most
+  int grid = p->num_sms;
+  const int rows = N + 1, maxUseful = (rows + CH_WARPS - 1) / CH_WARPS;
+  const int T = (N + CH_NB - 1) / CH_NB, tiles = T * (T + 1) / 2;
+  int want = maxUseful > tiles ? maxUseful : tiles;
+  if (want < 1) want = 1;
+  if (grid > want) grid = want;
+  SFFT_CUDA_TRY(cudaLaunchCooperativeKernel((const void*)k_chol_fused, dim3(grid), dim3(CH_THREADS), args, 0, st));
   ++*nl;
-  for (int k0 = 0; k0 < N; k0 += CH_NB) {
-    const int nb = (N - k0) < CH_NB ? (N - k0) : CH_NB;
-    const int rows_below = N + 1 - (k0 + nb);  // includes the rhs row
-    const int gp = rows_below > 0 ? (rows_below + 127) / 128 : 1;
-    k_chol_panel<<<gp, 128, 0, st>>>(p->Lw, p->Ldiag, N, ld, k0, info);
-    SFFT_LAUNCH_CHECK();
-    ++*nl;
-    if (k0 + CH_NB < N) {
-      const int nt = (N + 1 - (k0 + CH_NB) + CH_NB - 1) / CH_NB;
-      dim3 g(nt, nt);
-      k_chol_update<<<g, 256, 0, st>>>(p->Lw, N, ld, k0);
-      SFFT_LAUNCH_CHECK();
-      ++*nl;
-    } else if (k0 + nb < N + 1 && k0 + CH_NB >= N) {
-      // last panel: nothing but the rhs row's own (unused) diagonal entry remains
-    }
-  }
-  const size_t smem = ((size_t)N + CH_NB * (CH_NB + 1) + CH_NB) * sizeof(double);
-  SFFT_CUDA_TRY(cudaFuncSetAttribute(k_chol_back, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  k_chol_back<<<1, 1024, smem, st>>>(p->Lw, p->Ldiag, c, N, ld);
+  const size_t smem = ((size_t)N + CH_NB * (CH_NB + 1) + 2 * CH_NB) * sizeof(double);
+  k_chol_back<<<1, 1024, smem, st>>>(Lw, c, N, ld);
   SFFT_LAUNCH_CHECK();
   ++*nl;
   return SFFT_OK;

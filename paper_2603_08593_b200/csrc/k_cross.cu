@@ -181,18 +181,21 @@ struct LagParams {
   const cplx* twW;
 };
 
-__global__ void __launch_bounds__(256) k_lag_idft(LagParams P) {
+#define LAG_SLICES 8
+
+__global__ void __launch_bounds__(32 * LAG_SLICES) k_lag_idft(LagParams P) {
   const int pair = blockIdx.x, dyi = blockIdx.y;
   const int D = P.pairs[pair].D;
   if (dyi > 2 * D) return;
-  const int lane = threadIdx.x & 31, slice = threadIdx.x >> 5;  // 8 slices over kx
+  const int lane = threadIdx.x & 31, slice = threadIdx.x >> 5;  // slices interleave over kx
   const cplx* Yr = P.Y + ((size_t)pair * P.nLag + dyi) * P.pitch;
-  __shared__ double red[2][8][32];
+  __shared__ double red[2][LAG_SLICES][33];
   double ap[2] = {0.0, 0.0}, am[2] = {0.0, 0.0};
   const int dx = lane;
   if (dx <= D) {
     int it = 0;
-    for (int kx = 1 + slice; kx < P.NC; kx += 8, ++it) {
+#pragma unroll 4
+    for (int kx = 1 + slice; kx < P.NC; kx += LAG_SLICES, ++it) {
       const cplx y = Yr[kx];
       const cplx t = ldg2(P.twW + ((kx * dx) & (P.W - 1)));  // (c, -s)
       const double pc = y.x * t.x, qs = y.y * (-t.y);
@@ -205,7 +208,7 @@ __global__ void __launch_bounds__(256) k_lag_idft(LagParams P) {
   __syncthreads();
   if (slice == 0 && dx <= D) {
     double sp = 0.0, sm = 0.0;
-    for (int k = 0; k < 8; k += 2) {
+    for (int k = 0; k < LAG_SLICES; k += 2) {
       sp += red[0][k][lane] + red[0][k + 1][lane];
       sm += red[1][k][lane] + red[1][k + 1][lane];
     }
@@ -316,7 +319,7 @@ sfft_status sfft_launch_lag_gather(sfft_plan* p, double* A, double* b, cudaStrea
   LP.pitch = p->pitch; LP.nLag = p->nLag; LP.invP = 1.0 / ((double)p->H * (double)p->W);
   LP.twW = p->twW;
   dim3 g1(p->nPair, p->nLag);
-  k_lag_idft<<<g1, 256, 0, st>>>(LP);
+  k_lag_idft<<<g1, 32 * LAG_SLICES, 0, st>>>(LP);
   SFFT_LAUNCH_CHECK();
   ++*nl;
   MomParams MP;

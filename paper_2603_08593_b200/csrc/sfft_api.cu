@@ -40,7 +40,7 @@ static void plan_free(sfft_plan* p) {
   if (!p) return;
   cudaFree(p->twNC); cudaFree(p->twW); cudaFree(p->twH); cudaFree(p->d_pairs); cudaFree(p->d_groups);
   cudaFree(p->T); cudaFree(p->F); cudaFree(p->Y); cudaFree(p->Cmap); cudaFree(p->rowMom);
-  cudaFree(p->mom); cudaFree(p->Lw); cudaFree(p->Ldiag); cudaFree(p->Etab); cudaFree(p->Mhat);
+  cudaFree(p->mom); cudaFree(p->Lw); cudaFree(p->cholBar); cudaFree(p->Etab); cudaFree(p->Mhat);
   free(p->h_pairs);
   for (int i = 0; i < 2 * SFFT_PROF_MAX; ++i) if (p->prof_ev[i]) cudaEventDestroy(p->prof_ev[i]);
   delete p;
@@ -142,7 +142,7 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   dalloc((void**)&p->rowMom, sizeof(double) * (size_t)(p->nMomA + p->nMomS) * H);
   dalloc((void**)&p->mom, sizeof(double) * (size_t)(p->nMomA * p->nMomA + p->TB));
   dalloc((void**)&p->Lw, sizeof(double) * (size_t)(p->N + 1) * p->ldL);
-  dalloc((void**)&p->Ldiag, sizeof(double) * (size_t)((p->N + 31) / 32) * 32 * 32);
+  dalloc((void**)&p->cholBar, 2 * sizeof(unsigned));
   dalloc((void**)&p->Etab, sizeof(cplx) * (size_t)p->TK * (2 * w + 1) * p->NC);
   dalloc((void**)&p->Mhat, sizeof(cplx) * HN);
   dalloc((void**)&p->d_pairs, sizeof(PairDesc) * p->nPair);
@@ -152,6 +152,7 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
       upload_twiddles(&p->twH, H) != cudaSuccess ||
       cudaMemcpy(p->d_pairs, p->h_pairs, sizeof(PairDesc) * p->nPair, cudaMemcpyHostToDevice) != cudaSuccess ||
       cudaMemcpy(p->d_groups, groups.data(), sizeof(CrossGroup) * groups.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemset(p->cholBar, 0, 2 * sizeof(unsigned)) != cudaSuccess ||
       cudaMemset(p->F, 0, sizeof(cplx) * HP * p->nSpec) != cudaSuccess ||
       cudaMemset(p->Y, 0, sizeof(cplx) * (size_t)p->nPair * p->nLag * p->pitch) != cudaSuccess ||
       cudaMemset(p->Cmap, 0, sizeof(double) * (size_t)p->nPair * p->nLag * p->nLag) != cudaSuccess) {

@@ -111,7 +111,7 @@ struct sfft_plan {
   double* rowMom;   // [nMomA + nMomS][H]
   double* mom;      // [(2DB+1)^2 + TB] reduced moments
   double* Lw;       // Cholesky workspace (N+1) x ldL
-  double* Ldiag;    // factored diagonal blocks
+  unsigned* cholBar; // grid-barrier counters of k_chol_fused (arrivals, finished CTAs)
   cplx* Etab;       // subtract: E[TK][2w+1][NC]
   cplx* Mhat;       // subtract: mixed row spectra [H][NC]
   int ldL;
