@@ -11,8 +11,17 @@
 // EPT complex values in registers per pass, so every pass is: load all -> barrier -> twiddle +
 // register butterfly -> store all -> barrier (in place, no ping-pong buffer).
 //
-// Twiddles come from a table tw[m] = exp(-2 pi i m / N) built on the host in long double
-// (correctly rounded), read through the read-only path; the inverse conjugates them.
+// Twiddles come from per-pass tables built on the host in long double (correctly rounded): the
+// pass with radix R and sub-transform stride NS reads tab[(r-1)*NS + k] = exp(-2 pi i r k/(NS R)),
+// so the lanes of a warp (consecutive k) read one contiguous segment per r through the
+// read-only path; the inverse conjugates them.  The passes of one length are concatenated in
+// pass order (fft_pass_table_size / fft_fill_pass_tables on the host, FftCfg<N>::tw_off on the
+// device).
+//
+// The first pass can take its inputs straight from registers (fft_first_from_regs) and the last
+// pass can leave its outputs in registers (fft_last_to_regs), so a kernel that loads from / stores
+// to global memory in the butterfly's own access pattern never stages those elements in shared
+// memory.
 #pragma once
 #include "sfft_common.cuh"
 
@@ -124,17 +133,98 @@ struct Dft<16, DIR> {
   }
 };
 
+
+// Radix plan per length (first radix = elements per thread).  Kept in one place for host and device.
+__host__ __device__ constexpr int fft_num_passes(int N) {
+  return (N == 8 || N == 16) ? 1 : (N <= 256 ? 2 : 3);
+}
+__host__ __device__ constexpr int fft_radix(int N, int pass) {
+  switch (N) {
+    case 8: return 8;
+    case 16: return 16;
+    case 32: return pass == 0 ? 8 : 4;
+    case 64: return 8;
+    case 128: return pass == 0 ? 16 : 8;
+    case 256: return 16;
+    case 512: return 8;
+    case 1024: return pass == 0 ? 16 : 8;
+    case 2048: return pass == 2 ? 8 : 16;
+    case 4096: return 16;
+    default: return 0;
+  }
+}
+// stride NS of pass `pass` = product of the earlier radices
+__host__ __device__ constexpr int fft_pass_ns(int N, int pass) {
+  int ns = 1;
+  for (int i = 0; i < pass; ++i) ns *= fft_radix(N, i);
+  return ns;
+}
+// offset of a pass's twiddle block inside the concatenated table (pass 0 has none)
+__host__ __device__ constexpr int fft_tw_off(int N, int pass) {
+  int off = 0;
+  for (int i = 1; i < pass; ++i) off += (fft_radix(N, i) - 1) * fft_pass_ns(N, i);
+  return off;
+}
+__host__ __device__ constexpr int fft_pass_table_size(int N) {
+  return fft_tw_off(N, fft_num_passes(N)) > 0 ? fft_tw_off(N, fft_num_passes(N)) : 1;
+}
+
 template <int N>
 struct FftCfg {
-  // first radix = elements per thread
-  static constexpr int EPT = (N == 8 || N == 32 || N == 64 || N == 512) ? 8 : 16;
+  static constexpr int EPT = fft_radix(N, 0);   // first radix = elements per thread
+  static constexpr int NPASS = fft_num_passes(N);
   static constexpr int PADSHIFT = (EPT == 8) ? 3 : 4;
   static constexpr int SEQ_STRIDE = N + (N >> PADSHIFT);
   static __host__ __device__ constexpr int phys(int n) { return n + (n >> PADSHIFT); }
 };
 
+// Butterfly index i -> (sequence, butterfly j).  SEQ_FAST: adjacent threads work on adjacent
+// sequences (the column kernels, where adjacent sequences are adjacent in global memory).
+template <int NB, bool SEQ_FAST>
+__device__ __forceinline__ void fft_map(int i, int nseq, int& seq, int& j) {
+  if (SEQ_FAST) { seq = i % nseq; j = i / nseq; }
+  else { seq = i / NB; j = i & (NB - 1); }
+}
+
+// twiddle + butterfly + Stockham store of one radix-R butterfly held in v[]
 template <int N, int R, int NS, int DIR>
-__device__ __forceinline__ void fft_pass(cplx* s, int tid, int nth, const cplx* __restrict__ tw,
+__device__ __forceinline__ void fft_twiddle_bfly(cplx* v, int j, const cplx* __restrict__ tw) {
+  if constexpr (NS > 1) {
+    const int k = j & (NS - 1);
+    cplx t[R];
+#pragma unroll
+    for (int r = 1; r < R; ++r) t[r] = ldg2(tw + (r - 1) * NS + k);
+#pragma unroll
+    for (int r = 1; r < R; ++r) {
+      if (DIR > 0) t[r].y = -t[r].y;
+      v[r] = cmul(v[r], t[r]);
+    }
+  }
+  Dft<R, DIR>::run(v);
+}
+template <int N, int R, int NS>
+__device__ __forceinline__ void fft_store(const cplx* v, cplx* base, int j) {
+  using C = FftCfg<N>;
+  const int k = j & (NS - 1);
+  const int o = (j - k) * R + k;
+#pragma unroll
+  for (int r = 0; r < R; ++r) base[C::phys(o + r * NS)] = v[r];
+}
+
+// Pass 0 from registers: the calling thread supplies v[r] = x[seq][j + r*N/EPT], r < EPT, for the
+// butterfly (seq, j) it chose (any one-to-one assignment of threads to butterflies).  Ends with a
+// barrier unless the transform has a single pass and NOSYNC is set.
+template <int N, int DIR>
+__device__ __forceinline__ void fft_first_from_regs(cplx* v, cplx* s, int seq, int j, int seq_stride) {
+  using C = FftCfg<N>;
+  Dft<C::EPT, DIR>::run(v);
+  fft_store<N, C::EPT, 1>(v, s + seq * seq_stride, j);
+  __syncthreads();
+}
+
+// One in-place pass shared memory -> shared memory.
+template <int N, int R, int NS, int DIR, bool SEQ_FAST>
+__device__ __forceinline__ void fft_pass(cplx* s, int tid, int nth, int nseq, const cplx* __restrict__ tw,
                                          const int seq_stride) {
   using C = FftCfg<N>;
   constexpr int NB = N / R;        // butterflies per sequence
@@ -142,8 +232,8 @@ __device__ __forceinline__ void fft_pass(cplx* s, int tid, int nth, const cplx* 
   cplx v[IT][R];
 #pragma unroll
   for (int m = 0; m < IT; ++m) {
-    const int i = tid + m * nth;
-    const int seq = i / NB, j = i & (NB - 1);
+    int seq, j;
+    fft_map<NB, SEQ_FAST>(tid + m * nth, nseq, seq, j);
     const cplx* base = s + seq * seq_stride;
 #pragma unroll
     for (int r = 0; r < R; ++r) v[m][r] = base[C::phys(j + r * NB)];
@@ -151,66 +241,34 @@ __device__ __forceinline__ void fft_pass(cplx* s, int tid, int nth, const cplx* 
   __syncthreads();
 #pragma unroll
   for (int m = 0; m < IT; ++m) {
-    const int i = tid + m * nth;
-    const int seq = i / NB, j = i & (NB - 1);
-    const int k = j & (NS - 1);
-    if constexpr (NS > 1) {
-#pragma unroll
-      for (int r = 1; r < R; ++r) {
-        cplx t = ldg2(tw + r * k * (N / (NS * R)));
-        if (DIR > 0) t.y = -t.y;
-        v[m][r] = cmul(v[m][r], t);
-      }
-    }
-    Dft<R, DIR>::run(v[m]);
-    cplx* base = s + seq * seq_stride;
-    const int o = (j - k) * R + k;
-#pragma unroll
-    for (int r = 0; r < R; ++r) base[C::phys(o + r * NS)] = v[m][r];
+    int seq, j;
+    fft_map<NB, SEQ_FAST>(tid + m * nth, nseq, seq, j);
+    fft_twiddle_bfly<N, R, NS, DIR>(v[m], j, tw);
+    fft_store<N, R, NS>(v[m], s + seq * seq_stride, j);
   }
   __syncthreads();
 }
 
-// In-place FFT of every sequence the CTA holds.  All nth = nseq*N/EPT threads must call it.
-// On entry the data must be visible (a __syncthreads after the producer's stores); on exit the
-// results are visible to every thread.  DIR = -1: X[k] = sum x[n] e^{-2 pi i nk/N}; +1: e^{+...},
-// unnormalised.
-template <int N, int DIR>
-__device__ __forceinline__ void fft_smem(cplx* s, int tid, int nth, const cplx* __restrict__ tw,
-                                         const int seq_stride = FftCfg<N>::SEQ_STRIDE) {
-  if constexpr (N == 8) {
-    fft_pass<N, 8, 1, DIR>(s, tid, nth, tw, seq_stride);
-  } else if constexpr (N == 16) {
-    fft_pass<N, 16, 1, DIR>(s, tid, nth, tw, seq_stride);
-  } else if constexpr (N == 32) {
-    fft_pass<N, 8, 1, DIR>(s, tid, nth, tw, seq_stride);
-    fft_pass<N, 4, 8, DIR>(s, tid, nth, tw, seq_stride);
-  } else if constexpr (N == 64) {
-    fft_pass<N, 8, 1, DIR>(s, tid, nth, tw, seq_stride);
-    fft_pass<N, 8, 8, DIR>(s, tid, nth, tw, seq_stride);
-  } else if constexpr (N == 128) {
-    fft_pass<N, 16, 1, DIR>(s, tid, nth, tw, seq_stride);
-    fft_pass<N, 8, 16, DIR>(s, tid, nth, tw, seq_stride);
-  } else if constexpr (N == 256) {
-    fft_pass<N, 16, 1, DIR>(s, tid, nth, tw, seq_stride);
-    fft_pass<N, 16, 16, DIR>(s, tid, nth, tw, seq_stride);
-  } else if constexpr (N == 512) {
-    fft_pass<N, 8, 1, DIR>(s, tid, nth, tw, seq_stride);
-    fft_pass<N, 8, 8, DIR>(s, tid, nth, tw, seq_stride);
-    fft_pass<N, 8, 64, DIR>(s, tid, nth, tw, seq_stride);
-  } else if constexpr (N == 1024) {
-    fft_pass<N, 16, 1, DIR>(s, tid, nth, tw, seq_stride);
-    fft_pass<N, 8, 16, DIR>(s, tid, nth, tw, seq_stride);
-    fft_pass<N, 8, 128, DIR>(s, tid, nth, tw, seq_stride);
-  } else if constexpr (N == 2048) {
-    fft_pass<N, 16, 1, DIR>(s, tid, nth, tw, seq_stride);
-    fft_pass<N, 16, 16, DIR>(s, tid, nth, tw, seq_stride);
-    fft_pass<N, 8, 256, DIR>(s, tid, nth, tw, seq_stride);
-  } else if constexpr (N == 4096) {
-    fft_pass<N, 16, 1, DIR>(s, tid, nth, tw, seq_stride);
-    fft_pass<N, 16, 16, DIR>(s, tid, nth, tw, seq_stride);
-    fft_pass<N, 16, 256, DIR>(s, tid, nth, tw, seq_stride);
-  } else {
-    static_assert(N == 8, "unsupported FFT length");
+// Last pass, outputs left in registers: butterfly m of the thread is (seq[m], j[m]) from fft_map
+// and holds X[seq][j + r*N/R] in v[m*R + r].  No trailing barrier (nothing is written to smem).
+template <int N, int R, int NS, int DIR, bool SEQ_FAST>
+__device__ __forceinline__ void fft_pass_to_regs(const cplx* s, cplx* v, int tid, int nth, int nseq,
+                                                 const cplx* __restrict__ tw, const int seq_stride) {
+  using C = FftCfg<N>;
+  constexpr int NB = N / R;
+  constexpr int IT = C::EPT / R;
+#pragma unroll
+  for (int m = 0; m < IT; ++m) {
+    int seq, j;
+    fft_map<NB, SEQ_FAST>(tid + m * nth, nseq, seq, j);
+    const cplx* base = s + seq * seq_stride;
+#pragma unroll
+    for (int r = 0; r < R; ++r) v[m * R + r] = base[C::phys(j + r * NB)];
+  }
+#pragma unroll
+  for (int m = 0; m < IT; ++m) {
+    int seq, j;
+    fft_map<NB, SEQ_FAST>(tid + m * nth, nseq, seq, j);
+    fft_twiddle_bfly<N, R, NS, DIR>(v + m * R, j, tw);
   }
 }

@@ -181,37 +181,51 @@ struct LagParams {
   const cplx* twW;
 };
 
-#define LAG_SLICES 8
+#define LAG_TH 256
+#define LAG_MAXD 10
 
-__global__ void __launch_bounds__(32 * LAG_SLICES) k_lag_idft(LagParams P) {
+// One CTA per (pair, lag row): lanes run along kx (coalesced reads of the lag row), every thread
+// keeps the 2D+1 partial sums of its kx values in registers, then a fixed-order reduction
+// (warp shuffle tree, then the warps in order) so the result is reproducible.
+__global__ void __launch_bounds__(LAG_TH) k_lag_idft(LagParams P) {
   const int pair = blockIdx.x, dyi = blockIdx.y;
   const int D = P.pairs[pair].D;
   if (dyi > 2 * D) return;
-  const int lane = threadIdx.x & 31, slice = threadIdx.x >> 5;  // slices interleave over kx
+  const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
   const cplx* Yr = P.Y + ((size_t)pair * P.nLag + dyi) * P.pitch;
-  __shared__ double red[2][LAG_SLICES][33];
-  double ap[2] = {0.0, 0.0}, am[2] = {0.0, 0.0};
-  const int dx = lane;
-  if (dx <= D) {
-    int it = 0;
-#pragma unroll 4
-    for (int kx = 1 + slice; kx < P.NC; kx += LAG_SLICES, ++it) {
-      const cplx y = Yr[kx];
-      const cplx t = ldg2(P.twW + ((kx * dx) & (P.W - 1)));  // (c, -s)
-      const double pc = y.x * t.x, qs = y.y * (-t.y);
-      ap[it & 1] += pc - qs;  // Re(y e^{+i th})
-      am[it & 1] += pc + qs;  // Re(y e^{-i th})
+  double ap[LAG_MAXD + 1], am[LAG_MAXD + 1];
+#pragma unroll
+  for (int dx = 0; dx <= LAG_MAXD; ++dx) { ap[dx] = 0.0; am[dx] = 0.0; }
+  for (int kx = 1 + tid; kx < P.NC; kx += LAG_TH) {
+    const cplx y = Yr[kx];
+    ap[0] += y.x;
+#pragma unroll
+    for (int dx = 1; dx <= LAG_MAXD; ++dx) {
+      if (dx <= D) {
+        const cplx t = ldg2(P.twW + ((kx * dx) & (P.W - 1)));  // (c, -s)
+        const double pc = y.x * t.x, qs = y.y * (-t.y);
+        ap[dx] += pc - qs;  // Re(y e^{+i th})
+        am[dx] += pc + qs;  // Re(y e^{-i th})
+      }
     }
   }
-  red[0][slice][lane] = ap[0] + ap[1];
-  red[1][slice][lane] = am[0] + am[1];
-  __syncthreads();
-  if (slice == 0 && dx <= D) {
-    double sp = 0.0, sm = 0.0;
-    for (int k = 0; k < LAG_SLICES; k += 2) {
-      sp += red[0][k][lane] + red[0][k + 1][lane];
-      sm += red[1][k][lane] + red[1][k + 1][lane];
+  __shared__ double red[2][LAG_MAXD + 1][LAG_TH / 32];
+#pragma unroll
+  for (int dx = 0; dx <= LAG_MAXD; ++dx) {
+    double a = ap[dx], b = am[dx];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+      a += __shfl_xor_sync(0xffffffffu, a, off);
+      b += __shfl_xor_sync(0xffffffffu, b, off);
     }
+    if (lane == 0) { red[0][dx][wrp] = a; red[1][dx][wrp] = b; }
+  }
+  __syncthreads();
+  if (tid <= D) {
+    const int dx = tid;
+    double sp = 0.0, sm = 0.0;
+    for (int k = 0; k < LAG_TH / 32; ++k) { sp += red[0][dx][k]; sm += red[1][dx][k]; }
+    if (dx == 0) sm = sp;
     const double y0 = Yr[0].x, yn = Yr[P.NC].x;
     const double sgn = (dx & 1) ? -1.0 : 1.0;
     double* out = P.Cmap + ((size_t)pair * P.nLag + dyi) * P.nLag;
@@ -319,7 +333,7 @@ sfft_status sfft_launch_lag_gather(sfft_plan* p, double* A, double* b, cudaStrea
   LP.pitch = p->pitch; LP.nLag = p->nLag; LP.invP = 1.0 / ((double)p->H * (double)p->W);
   LP.twW = p->twW;
   dim3 g1(p->nPair, p->nLag);
-  k_lag_idft<<<g1, 32 * LAG_SLICES, 0, st>>>(LP);
+  k_lag_idft<<<g1, LAG_TH, 0, st>>>(LP);
   SFFT_LAUNCH_CHECK();
   ++*nl;
   MomParams MP;

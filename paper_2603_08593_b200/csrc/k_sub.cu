@@ -46,61 +46,101 @@ struct MixParams {
   const cplx* G;   // [DK+1][H][NC] row spectra of xi^p R
   const cplx* E;   // [TK][2w+1][NC]
   cplx* Mhat;      // [H][NC]
-  int H, NC, w, DK, TK, KT;
+  int H, NC, DK, TK, KT;
+  int monoK[SFFT_MAX_T][2];
 };
 
-#define MIX_YT 32
+#define MIX_RY 8   // output rows per thread
+#define MIX_TH 128 // threads per block
 
-__global__ void __launch_bounds__(256) k_mix(MixParams P) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int KT = P.KT, w = P.w, S1 = 2 * w + 1, H = P.H, NC = P.NC;
-  const int nrow = MIX_YT + 2 * w;
-  cplx* Gs = reinterpret_cast<cplx*>(smem_raw);           // [DK+1][nrow][KT]
-  cplx* Es = Gs + (size_t)(P.DK + 1) * nrow * KT;         // [TK][S1][KT]
-  const int kx0 = blockIdx.x * KT, y0 = blockIdx.y * MIX_YT;
+// Register-tiled y-mixing.  A thread owns one kx and MIX_RY consecutive output rows; per xi power p
+// it loads the MIX_RY + 2w source rows of G_p once into registers, scales them by eta^q in place
+// for q = 0..DK-p, and for every (q, v) applies one E value to all MIX_RY accumulators: one global
+// (L1-resident) load per MIX_RY complex FMAs instead of two shared loads per FMA.  Lanes run
+// along kx, so every load and store is a contiguous 512-byte segment.
+// The packed column kx = 0 holds (X[0], X[W/2]), both real with real factors, and is combined
+// component-wise by the extra x-block (four threads per row, fixed-order shuffle reduction).
+template <int WK>
+__global__ void __launch_bounds__(MIX_TH, 3) k_mix(MixParams P) {
+  constexpr int RY = MIX_RY, S1 = 2 * WK + 1, WIN = RY + 2 * WK;
+  const int H = P.H, NC = P.NC, KT = P.KT;
   const int tid = threadIdx.x;
-  for (int e = tid; e < (P.DK + 1) * nrow * KT; e += 256) {
-    const int kl = e % KT, ri = (e / KT) % nrow, p = e / (KT * nrow);
-    const int yy = (y0 - w + ri + H) & (H - 1);
-    Gs[e] = P.G[((size_t)p * H + yy) * NC + kx0 + kl];
-  }
-  for (int e = tid; e < P.TK * S1 * KT; e += 256) {
-    const int kl = e % KT, r = e / KT;
-    Es[e] = P.E[(size_t)r * NC + kx0 + kl];
-  }
-  __syncthreads();
-  const int kl = tid % KT, rg = tid / KT;
-  const int nrg = 256 / KT;                 // row groups
-  const int rows_per = MIX_YT / nrg;        // rows per thread
+  const int rowsPerBlock = (MIX_TH / KT) * RY;
   const double invH = 1.0 / (double)H;
-  const bool packed = (kx0 + kl) == 0;
-  for (int rr = 0; rr < rows_per; ++rr) {
-    const int yi = rg * rows_per + rr;
-    cplx acc = cmake(0.0, 0.0);
-    for (int vi = 0; vi < S1; ++vi) {
-      const int ri = yi + 2 * w - vi;  // source row y - v, v = vi - w, as an index into the tile
-      const int yy = (y0 - w + ri + H) & (H - 1);
-      const double eta = (double)(2 * yy + 1 - H) * invH;
-      for (int p = 0; p <= P.DK; ++p) {
-        // c_p = sum_q E_(p,q)[v] eta^q (Horner, highest q first); t(p,q) = d(d+1)/2 + q, d = p+q
-        cplx c = cmake(0.0, 0.0);
-        for (int q = P.DK - p; q >= 0; --q) {
-          const int d = p + q;
-          const cplx e = Es[((d * (d + 1) / 2 + q) * S1 + vi) * KT + kl];
-          c.x = fma(c.x, eta, e.x);
-          c.y = fma(c.y, eta, e.y);
-        }
-        const cplx g = Gs[((size_t)p * nrow + ri) * KT + kl];
-        if (packed) {
-          acc.x = fma(c.x, g.x, acc.x);
-          acc.y = fma(c.y, g.y, acc.y);
-        } else {
-          cfma(acc, c, g);
+  if (blockIdx.x == gridDim.x - 1) {
+    // ---- packed column (rowsPerBlock is a multiple of MIX_TH / 4, so the trip count is uniform)
+    for (int r = tid >> 2; r < rowsPerBlock; r += MIX_TH / 4) {
+      const int y = blockIdx.y * rowsPerBlock + r, part = tid & 3;
+      const bool live = y < H;
+      double ax = 0.0, ay = 0.0;
+      if (live) {
+        for (int idx = part; idx < P.TK * S1; idx += 4) {
+          const int t = idx / S1, vi = idx - t * S1;
+          const int p = P.monoK[t][0], q = P.monoK[t][1];
+          const int yy = (y - vi + WK + H) & (H - 1);
+          const double eq = ipow((double)(2 * yy + 1 - H) * invH, q);
+          const cplx e = P.E[(size_t)idx * NC];
+          const cplx g = P.G[((size_t)p * H + yy) * NC];
+          ax = fma(e.x * eq, g.x, ax);
+          ay = fma(e.y * eq, g.y, ay);
         }
       }
+      ax += __shfl_xor_sync(0xffffffffu, ax, 1);
+      ay += __shfl_xor_sync(0xffffffffu, ay, 1);
+      ax += __shfl_xor_sync(0xffffffffu, ax, 2);
+      ay += __shfl_xor_sync(0xffffffffu, ay, 2);
+      if (live && part == 0) P.Mhat[(size_t)y * NC] = cmake(ax, ay);
     }
-    P.Mhat[(size_t)(y0 + yi) * NC + kx0 + kl] = acc;
+    return;
   }
+  const int kl = tid % KT, rg = tid / KT;
+  const int kx = blockIdx.x * KT + kl;
+  const int y0 = blockIdx.y * rowsPerBlock + rg * RY;
+  if (y0 >= H) return;
+  cplx acc[RY];
+#pragma unroll
+  for (int i = 0; i < RY; ++i) acc[i] = cmake(0.0, 0.0);
+  for (int p = 0; p <= P.DK; ++p) {
+    cplx g[WIN];
+    const cplx* Gp = P.G + (size_t)p * H * NC + kx;
+#pragma unroll
+    for (int i = 0; i < WIN; ++i) {
+      const int yy = (y0 - WK + i + H) & (H - 1);
+      g[i] = Gp[(size_t)yy * NC];
+    }
+    for (int q = 0; q <= P.DK - p; ++q) {
+      if (q > 0) {
+#pragma unroll
+        for (int i = 0; i < WIN; ++i) {
+          const int yy = (y0 - WK + i + H) & (H - 1);
+          const double eta = (double)(2 * yy + 1 - H) * invH;
+          g[i].x *= eta;
+          g[i].y *= eta;
+        }
+      }
+      const int d = p + q;
+      const cplx* Et = P.E + (size_t)(d * (d + 1) / 2 + q) * S1 * NC + kx;
+#pragma unroll
+      for (int vi = 0; vi < S1; ++vi) {
+        const cplx e = Et[(size_t)vi * NC];
+#pragma unroll
+        for (int i = 0; i < RY; ++i) cfma(acc[i], e, g[i + 2 * WK - vi]);
+      }
+    }
+  }
+  if (kx != 0) {
+#pragma unroll
+    for (int i = 0; i < RY; ++i) P.Mhat[(size_t)(y0 + i) * NC + kx] = acc[i];
+  }
+}
+
+template <int WK>
+static sfft_status launch_mix_t(const MixParams& MP, cudaStream_t st) {
+  const int rowsPerBlock = (MIX_TH / MP.KT) * MIX_RY;
+  dim3 gm(MP.NC / MP.KT + 1, (MP.H + rowsPerBlock - 1) / rowsPerBlock);
+  k_mix<WK><<<gm, MIX_TH, 0, st>>>(MP);
+  SFFT_LAUNCH_CHECK();
+  return SFFT_OK;
 }
 
 sfft_status sfft_launch_row_inv_sub(sfft_plan* p, const double* S, const double* c, double* D,
@@ -124,23 +164,21 @@ sfft_status sfft_launch_subtract(sfft_plan* p, const double* R, const double* S,
   ++*nl;
   // 3. y-mixing
   MixParams MP;
-  MP.G = p->T; MP.E = p->Etab; MP.Mhat = p->Mhat; MP.H = p->H; MP.NC = p->NC; MP.w = p->w;
+  MP.G = p->T; MP.E = p->Etab; MP.Mhat = p->Mhat; MP.H = p->H; MP.NC = p->NC;
   MP.DK = p->DK; MP.TK = p->TK;
-  int KT = 32;
-  if (KT > p->NC) KT = p->NC;
-  auto need = [&](int kt) {
-    return ((size_t)(p->DK + 1) * (MIX_YT + 2 * p->w) + (size_t)p->TK * (2 * p->w + 1)) * kt * sizeof(cplx);
-  };
-  while (KT > 8 && need(KT) > 200 * 1024) KT >>= 1;
-  MP.KT = KT;
-  const size_t smem = need(KT);
-  SFFT_CUDA_TRY(cudaFuncSetAttribute(k_mix, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  const int yt = p->H < MIX_YT ? p->H : MIX_YT;
-  if (yt != MIX_YT) return SFFT_ERR_UNSUPPORTED;
-  dim3 gm(p->NC / KT, p->H / MIX_YT);
-  k_mix<<<gm, 256, smem, st>>>(MP);
+  MP.KT = p->NC < 32 ? p->NC : 32;
+  for (int t = 0; t < p->TK; ++t) { MP.monoK[t][0] = p->monoK[t][0]; MP.monoK[t][1] = p->monoK[t][1]; }
+  switch (p->w) {
+    case 0: s = launch_mix_t<0>(MP, st); break;
+    case 1: s = launch_mix_t<1>(MP, st); break;
+    case 2: s = launch_mix_t<2>(MP, st); break;
+    case 3: s = launch_mix_t<3>(MP, st); break;
+    case 4: s = launch_mix_t<4>(MP, st); break;
+    case 5: s = launch_mix_t<5>(MP, st); break;
+    default: s = SFFT_ERR_UNSUPPORTED; break;
+  }
   delete pmix;
-  SFFT_LAUNCH_CHECK();
+  if (s != SFFT_OK) return s;
   ++*nl;
   // 4. inverse rows + subtraction
   { ProfScope ps(p, 8, st); s = sfft_launch_row_inv_sub(p, S, c, D, st, nl); }
