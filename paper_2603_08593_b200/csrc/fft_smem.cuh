@@ -272,3 +272,54 @@ __device__ __forceinline__ void fft_pass_to_regs(const cplx* s, cplx* v, int tid
     fft_twiddle_bfly<N, R, NS, DIR>(v + m * R, j, tw);
   }
 }
+
+template <int N, int PASS, int DIR, bool SEQ_FAST>
+__device__ __forceinline__ void fft_run_pass(cplx* s, int tid, int nth, int nseq, const cplx* __restrict__ tw,
+                                             int seq_stride) {
+  fft_pass<N, fft_radix(N, PASS), fft_pass_ns(N, PASS), DIR, SEQ_FAST>(s, tid, nth, nseq,
+                                                                       tw + fft_tw_off(N, PASS), seq_stride);
+}
+template <int N, int PASS, int DIR, bool SEQ_FAST>
+__device__ __forceinline__ void fft_run_pass_to_regs(const cplx* s, cplx* v, int tid, int nth, int nseq,
+                                                     const cplx* __restrict__ tw, int seq_stride) {
+  fft_pass_to_regs<N, fft_radix(N, PASS), fft_pass_ns(N, PASS), DIR, SEQ_FAST>(
+      s, v, tid, nth, nseq, tw + fft_tw_off(N, PASS), seq_stride);
+}
+
+// Whole transform with the inputs in registers and the outputs left in shared memory
+// (s[seq*seq_stride + phys(k)] = X[seq][k], visible to every thread on return).
+// v[r] = x[seq][j + r*N/EPT] for the caller's butterfly (seq, j) = fft_map<N/EPT, SEQ_FAST>(tid).
+// The CTA must have exactly nseq*N/EPT threads.  DIR = -1: X[k] = sum x[n] e^{-2 pi i nk/N};
+// +1: e^{+...}; unnormalised.  A barrier must separate earlier readers of s from this call.
+template <int N, int DIR, bool SEQ_FAST>
+__device__ __forceinline__ void fft_regs_to_smem(cplx* v, cplx* s, int tid, int nth, int nseq,
+                                                 const cplx* __restrict__ tw, int seq_stride) {
+  using C = FftCfg<N>;
+  int seq, j;
+  fft_map<N / C::EPT, SEQ_FAST>(tid, nseq, seq, j);
+  fft_first_from_regs<N, DIR>(v, s, seq, j, seq_stride);
+  if constexpr (C::NPASS >= 2) fft_run_pass<N, 1, DIR, SEQ_FAST>(s, tid, nth, nseq, tw, seq_stride);
+  if constexpr (C::NPASS >= 3) fft_run_pass<N, 2, DIR, SEQ_FAST>(s, tid, nth, nseq, tw, seq_stride);
+}
+
+// Whole transform registers -> registers.  On return, with RL = fft_radix(N, NPASS-1) and
+// (seq_m, j_m) = fft_map<N/RL, SEQ_FAST>(tid + m*nth), v[m*RL + r] = X[seq_m][j_m + r*N/RL].
+// No trailing barrier: a barrier must separate this call from the next writer of s.
+template <int N, int DIR, bool SEQ_FAST>
+__device__ __forceinline__ void fft_regs_to_regs(cplx* v, cplx* s, int tid, int nth, int nseq,
+                                                 const cplx* __restrict__ tw, int seq_stride) {
+  using C = FftCfg<N>;
+  if constexpr (C::NPASS == 1) {
+    Dft<C::EPT, DIR>::run(v);
+  } else {
+    int seq, j;
+    fft_map<N / C::EPT, SEQ_FAST>(tid, nseq, seq, j);
+    fft_first_from_regs<N, DIR>(v, s, seq, j, seq_stride);
+    if constexpr (C::NPASS == 2) {
+      fft_run_pass_to_regs<N, 1, DIR, SEQ_FAST>(s, v, tid, nth, nseq, tw, seq_stride);
+    } else {
+      fft_run_pass<N, 1, DIR, SEQ_FAST>(s, tid, nth, nseq, tw, seq_stride);
+      fft_run_pass_to_regs<N, 2, DIR, SEQ_FAST>(s, v, tid, nth, nseq, tw, seq_stride);
+    }
+  }
+}

@@ -21,14 +21,21 @@ struct RowFwdParams {
   int H, W, nimg;
   RowImage img[8];
   cplx* T;  // [nimg][H][NC]
-  const cplx* twNC;
+  const cplx* twP;   // per-pass twiddle tables for length NC
   const cplx* twW;
   int moments, nMomA, nMomS;
   double* rowMom;  // [nMomA + nMomS][H]
 };
 
-template <int NC>
-__global__ void __launch_bounds__(256) k_row_fwd(RowFwdParams P) {
+#define ROW_NMOM (2 * SFFT_MAX_DEG + 1 + SFFT_MAX_DEG + 1)
+
+// One CTA = RB rows, NC/EPT threads per row.  A thread's EPT input elements j = tr + e*TPR are
+// exactly the inputs of its first-pass butterfly, so they go from global memory through the
+// weighting (mask, xi^p) into the butterfly without being staged in shared memory; the inputs of
+// the next image are requested before the split/store phase of the current one.  The mask is
+// read once and kept as two bits per element.
+template <int NC, int MINB>
+__global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
   using C = FftCfg<NC>;
   constexpr int EPT = C::EPT;
   constexpr int TPR = NC / EPT;  // threads per row
@@ -42,66 +49,104 @@ __global__ void __launch_bounds__(256) k_row_fwd(RowFwdParams P) {
   const double invW = 1.0 / (double)W;
   const size_t rowoff = (size_t)y * W;
 
-  if (P.moments) {
-    // fused reductions (tree order: per-thread partial -> binary tree over the row's threads)
-    double acc[2 * SFFT_MAX_DEG + 1 + SFFT_MAX_DEG + 1];
-    const int nq = P.nMomA + P.nMomS;
+  // mask bits: bit 2e = element 2j masked, bit 2e+1 = element 2j+1 masked, j = tr + e*TPR
+  unsigned mbits = 0u;
+  if (P.mask) {
+    uchar2 mk[EPT];
 #pragma unroll
-    for (int q = 0; q < 2 * SFFT_MAX_DEG + 2 + SFFT_MAX_DEG; ++q) acc[q] = 0.0;
+    for (int e = 0; e < EPT; ++e) mk[e] = *reinterpret_cast<const uchar2*>(P.mask + rowoff + 2 * (tr + e * TPR));
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) mbits |= (mk[e].x ? 1u : 0u) << (2 * e) | (mk[e].y ? 1u : 0u) << (2 * e + 1);
+  }
+
+  if (P.moments) {
+    // fused reductions sum_x m xi^a and sum_x m xi^p S: per-thread partials, shuffle tree inside
+    // the row's lanes, then the row's warps in order (fixed order, reproducible)
+    double acc[ROW_NMOM];
+#pragma unroll
+    for (int q = 0; q < ROW_NMOM; ++q) acc[q] = 0.0;
+    double2 sv[EPT];
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) sv[e] = *reinterpret_cast<const double2*>(P.S + rowoff + 2 * (tr + e * TPR));
+#pragma unroll
     for (int e = 0; e < EPT; ++e) {
       const int j = tr + e * TPR;
-      const double2 sv = *reinterpret_cast<const double2*>(P.S + rowoff + 2 * j);
-      double m0 = 1.0, m1 = 1.0;
-      if (P.mask) {
-        const uchar2 mk = *reinterpret_cast<const uchar2*>(P.mask + rowoff + 2 * j);
-        m0 = mk.x ? 0.0 : 1.0;
-        m1 = mk.y ? 0.0 : 1.0;
-      }
       const double x0 = (double)(4 * j + 1 - W) * invW, x1 = (double)(4 * j + 3 - W) * invW;
-      double p0 = m0, p1 = m1;
-      for (int a = 0; a < P.nMomA; ++a) {
-        acc[a] += p0 + p1;
-        if (a < P.nMomS) acc[P.nMomA + a] += p0 * sv.x + p1 * sv.y;
-        p0 *= x0;
-        p1 *= x1;
+      double p0 = ((mbits >> (2 * e)) & 1u) ? 0.0 : 1.0, p1 = ((mbits >> (2 * e + 1)) & 1u) ? 0.0 : 1.0;
+#pragma unroll
+      for (int a = 0; a < 2 * SFFT_MAX_DEG + 1; ++a) {
+        if (a < P.nMomA) {
+          acc[a] += p0 + p1;
+          if (a < P.nMomS) acc[2 * SFFT_MAX_DEG + 1 + a] += p0 * sv[e].x + p1 * sv[e].y;
+          p0 *= x0;
+          p1 *= x1;
+        }
       }
     }
-    double* red = reinterpret_cast<double*>(smem_raw);
-    for (int q = 0; q < nq; ++q) red[q * nth + tid] = acc[q];
-    __syncthreads();
-    for (int off = TPR / 2; off > 0; off >>= 1) {
-      if (tr < off)
-        for (int q = 0; q < nq; ++q) red[q * nth + tid] += red[q * nth + tid + off];
+    constexpr int LW = TPR < 32 ? TPR : 32;   // lanes of one row inside a warp
+#pragma unroll
+    for (int q = 0; q < ROW_NMOM; ++q) {
+#pragma unroll
+      for (int off = LW / 2; off > 0; off >>= 1) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], off);
+    }
+    double* red = reinterpret_cast<double*>(smem_raw);   // [ROW_NMOM][warps]
+    constexpr int WPR = TPR / 32 > 0 ? TPR / 32 : 1;      // warps per row
+    if (TPR > 32) {
+      if ((tid & 31) == 0)
+#pragma unroll
+        for (int q = 0; q < ROW_NMOM; ++q) red[q * (nth / 32) + (tid >> 5)] = acc[q];
       __syncthreads();
     }
-    if (tr == 0)
-      for (int q = 0; q < nq; ++q) P.rowMom[(size_t)q * H + y] = red[q * nth + tid];
-    __syncthreads();
+    if (tr == 0) {
+#pragma unroll
+      for (int q = 0; q < ROW_NMOM; ++q) {
+        double v = acc[q];
+        if (TPR > 32) {
+          v = 0.0;
+          for (int k = 0; k < WPR; ++k) v += red[q * (nth / 32) + (tid >> 5) + k];
+        }
+        const int a = q < 2 * SFFT_MAX_DEG + 1 ? q : q - (2 * SFFT_MAX_DEG + 1);
+        const bool isS = q >= 2 * SFFT_MAX_DEG + 1;
+        if (!isS && a < P.nMomA) P.rowMom[(size_t)a * H + y] = v;
+        if (isS && a < P.nMomS) P.rowMom[(size_t)(P.nMomA + a) * H + y] = v;
+      }
+    }
+    if (TPR > 32) __syncthreads();
   }
 
   cplx* srow = s + r * C::SEQ_STRIDE;
+  double2 raw[EPT];
+  auto fetch = [&](int im) {   // always defines raw[], so nothing of it stays live across the FFT
+    const int src_id = im < P.nimg ? P.img[im].src : 2;
+    if (src_id != 2) {
+      const double* src = (src_id == 0 ? P.R : P.S) + rowoff;
+#pragma unroll
+      for (int e = 0; e < EPT; ++e) raw[e] = *reinterpret_cast<const double2*>(src + 2 * (tr + e * TPR));
+    } else {
+#pragma unroll
+      for (int e = 0; e < EPT; ++e) raw[e] = make_double2(1.0, 1.0);
+    }
+  };
+  fetch(0);
   for (int im = 0; im < P.nimg; ++im) {
     const RowImage d = P.img[im];
-    const double* src = d.src == 0 ? P.R : P.S;
-#pragma unroll 4
+    const unsigned mb = d.masked ? mbits : 0u;
+    cplx v[EPT];
+#pragma unroll
     for (int e = 0; e < EPT; ++e) {
       const int j = tr + e * TPR;
-      double2 v = make_double2(1.0, 1.0);
-      if (d.src != 2) v = *reinterpret_cast<const double2*>(src + rowoff + 2 * j);
-      if (d.masked && P.mask) {
-        const uchar2 mk = *reinterpret_cast<const uchar2*>(P.mask + rowoff + 2 * j);
-        if (mk.x) v.x = 0.0;
-        if (mk.y) v.y = 0.0;
-      }
+      double2 t = raw[e];
+      if ((mb >> (2 * e)) & 1u) t.x = 0.0;
+      if ((mb >> (2 * e + 1)) & 1u) t.y = 0.0;
       if (d.pxi > 0) {
         const double x0 = (double)(4 * j + 1 - W) * invW, x1 = (double)(4 * j + 3 - W) * invW;
-        v.x *= ipow(x0, d.pxi);
-        v.y *= ipow(x1, d.pxi);
+        t.x *= ipow(x0, d.pxi);
+        t.y *= ipow(x1, d.pxi);
       }
-      srow[C::phys(j)] = v;
+      v[e] = t;
     }
-    __syncthreads();
-    fft_smem<NC, -1>(s, tid, nth, P.twNC);
+    fft_regs_to_smem<NC, -1, false>(v, s, tid, nth, RB, P.twP, C::SEQ_STRIDE);
+    fetch(im + 1);
     // split: X[k] = Xe + w^k Xo, X[NC-k] = conj(Xe - w^k Xo), w = e^{-2 pi i / W}
     cplx* out = P.T + ((size_t)im * H + y) * NC;
     for (int k = tr; k <= NC / 2; k += TPR) {
@@ -129,91 +174,116 @@ struct RowInvParams {
   const double* coeffs;  // device, length N; background part at offB
   double* D;
   int H, W, offB, DB;
-  const cplx* twNC;
+  const cplx* twP;
   const cplx* twW;
 };
 
-template <int NC>
-__global__ void __launch_bounds__(256) k_row_inv_sub(RowInvParams P) {
+// C2R row transform fused with D = S - M - B.  The merge (half spectrum -> packed complex
+// sequence) is evaluated per element straight from global memory into the first butterfly, and
+// the last pass leaves the row in registers for the subtraction, so shared memory carries only the
+// exchanges between passes.
+template <int NC, int MINB>
+__global__ void __launch_bounds__(128, MINB) k_row_inv_sub(RowInvParams P) {
   using C = FftCfg<NC>;
   constexpr int EPT = C::EPT;
   constexpr int TPR = NC / EPT;
+  constexpr int RL = fft_radix(NC, C::NPASS - 1);
+  constexpr int NBL = NC / RL, ITL = EPT / RL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx* s = reinterpret_cast<cplx*>(smem_raw);
   const int tid = threadIdx.x, nth = blockDim.x;
   const int RB = nth / TPR;
   const int r = tid / TPR, tr = tid - r * TPR;
-  const int y = blockIdx.x * RB + r;
+  const int y0 = blockIdx.x * RB;
   const int W = P.W, H = P.H;
-  cplx* srow = s + r * C::SEQ_STRIDE;
-  const cplx* in = P.Mhat + (size_t)y * NC;
-  // merge: Z[k] = Xe + i Xo, Z[NC-k] = conj(Xe) + i conj(Xo),
-  //        Xe = (X[k] + conj(X[NC-k]))/2, Xo = (X[k] - conj(X[NC-k]))/2 * e^{+2 pi i k/W}
-  for (int k = tr; k <= NC / 2; k += TPR) {
-    if (k == 0) {
-      const cplx x0 = in[0];  // (X[0], X[NC]) both real
-      srow[C::phys(0)] = cmake(0.5 * (x0.x + x0.y), 0.5 * (x0.x - x0.y));
-    } else {
-      const cplx xk = in[k];
-      const cplx xm = cconj(in[NC - k]);
-      const cplx xe = cscale(cadd(xk, xm), 0.5);
-      const cplx xo = cmul(cconj(ldg2(P.twW + k)), cscale(csub(xk, xm), 0.5));
-      srow[C::phys(k)] = cadd(xe, cmul_pi(xo));
-      if (k != NC - k) srow[C::phys(NC - k)] = cadd(cconj(xe), cmul_pi(cconj(xo)));
+  const cplx* in = P.Mhat + (size_t)(y0 + r) * NC;
+  // merge: Z[k] = Xe + i Xo,  Xe = (X[k] + conj(X[NC-k]))/2,  Xo = (X[k] - conj(X[NC-k]))/2 * e^{+2 pi i k/W}
+  cplx v[EPT];
+  {
+    cplx xk[EPT], xm[EPT], tw[EPT];
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+      const int k = tr + e * TPR;
+      xk[e] = in[k];
+      xm[e] = in[(NC - k) & (NC - 1)];
+      tw[e] = ldg2(P.twW + k);
+    }
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+      const int k = tr + e * TPR;
+      if (k == 0) {
+        v[e] = cmake(0.5 * (xk[e].x + xk[e].y), 0.5 * (xk[e].x - xk[e].y));  // (X[0], X[NC]) both real
+      } else {
+        const cplx m = cconj(xm[e]);
+        const cplx xe = cscale(cadd(xk[e], m), 0.5);
+        const cplx xo = cmul(cconj(tw[e]), cscale(csub(xk[e], m), 0.5));
+        v[e] = cadd(xe, cmul_pi(xo));
+      }
     }
   }
-  __syncthreads();
-  fft_smem<NC, +1>(s, tid, nth, P.twNC);
-  // background polynomial coefficients
-  double beta[SFFT_MAX_T];
-  int nb = 0;
-  for (int d = 0; d <= P.DB; ++d)
-    for (int q = 0; q <= d; ++q) { beta[nb] = P.coeffs[P.offB + nb]; ++nb; }
+  fft_regs_to_regs<NC, +1, false>(v, s, tid, nth, RB, P.twP, C::SEQ_STRIDE);
   const double invW = 1.0 / (double)W, invNC = 1.0 / (double)NC;
-  const double eta = (double)(2 * y + 1 - H) / (double)H;
-  const size_t rowoff = (size_t)y * W;
-#pragma unroll 4
-  for (int e = 0; e < EPT; ++e) {
-    const int j = tr + e * TPR;
-    const cplx z = srow[C::phys(j)];
-    const double2 sv = *reinterpret_cast<const double2*>(P.S + rowoff + 2 * j);
-    const double x0 = (double)(4 * j + 1 - W) * invW, x1 = (double)(4 * j + 3 - W) * invW;
-    double b0 = 0.0, b1 = 0.0;
-    int t = 0;
-    for (int d = 0; d <= P.DB; ++d)
-      for (int q = 0; q <= d; ++q) {
-        const double eq = ipow(eta, q);
-        b0 += beta[t] * ipow(x0, d - q) * eq;
-        b1 += beta[t] * ipow(x1, d - q) * eq;
-        ++t;
+#pragma unroll
+  for (int m = 0; m < ITL; ++m) {
+    int sq, j;
+    fft_map<NBL, false>(tid + m * nth, RB, sq, j);
+    const int y = y0 + sq;
+    // background: B = sum_p cp[p] xi^p,  cp[p] = sum_q beta_(p,q) eta^q
+    const double eta = (double)(2 * y + 1 - H) / (double)H;
+    double cp[SFFT_MAX_DEG + 1];
+#pragma unroll
+    for (int p = 0; p <= SFFT_MAX_DEG; ++p) cp[p] = 0.0;
+    for (int d = 0, t = 0; d <= P.DB; ++d)
+      for (int q = 0; q <= d; ++q, ++t) {
+        const double term = P.coeffs[P.offB + t] * ipow(eta, q);
+#pragma unroll
+        for (int p = 0; p <= SFFT_MAX_DEG; ++p)
+          if (p == d - q) cp[p] += term;
       }
-    double2 o;
-    o.x = sv.x - z.x * invNC - b0;
-    o.y = sv.y - z.y * invNC - b1;
-    *reinterpret_cast<double2*>(P.D + rowoff + 2 * j) = o;
+    const size_t rowoff = (size_t)y * W;
+    double2 sv[RL];
+#pragma unroll
+    for (int rr = 0; rr < RL; ++rr) sv[rr] = *reinterpret_cast<const double2*>(P.S + rowoff + 2 * (j + rr * NBL));
+#pragma unroll
+    for (int rr = 0; rr < RL; ++rr) {
+      const int n = j + rr * NBL;
+      const cplx z = v[m * RL + rr];
+      const double x0 = (double)(4 * n + 1 - W) * invW, x1 = (double)(4 * n + 3 - W) * invW;
+      double b0 = cp[SFFT_MAX_DEG], b1 = cp[SFFT_MAX_DEG];
+#pragma unroll
+      for (int p = SFFT_MAX_DEG - 1; p >= 0; --p) {
+        b0 = fma(b0, x0, cp[p]);
+        b1 = fma(b1, x1, cp[p]);
+      }
+      double2 o;
+      o.x = sv[rr].x - z.x * invNC - b0;
+      o.y = sv[rr].y - z.y * invNC - b1;
+      *reinterpret_cast<double2*>(P.D + rowoff + 2 * n) = o;
+    }
   }
 }
 
 // ------------------------------------------------------------------------------------------------
 
-static int rows_per_cta(int NC, int H) {
-  const int EPT = (NC == 8 || NC == 32 || NC == 64 || NC == 512) ? 8 : 16;
+static int row_threads(int NC, int H, int EPT) {
   const int TPR = NC / EPT;
-  int RB = 256 / TPR;
+  int RB = 128 / TPR;
   if (RB < 1) RB = 1;
-  if (NC >= 2048) RB = 2;
   if (RB > H) RB = H;
-  return RB;
+  return RB * TPR;
 }
 
 template <int NC>
 static sfft_status launch_row_fwd_t(const RowFwdParams& P, cudaStream_t st) {
   using C = FftCfg<NC>;
-  const int RB = rows_per_cta(NC, P.H);
-  const int nth = RB * (NC / C::EPT);
-  const size_t smem = (size_t)RB * C::SEQ_STRIDE * sizeof(cplx);
-  SFFT_CUDA_TRY(cudaFuncSetAttribute(k_row_fwd<NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  k_row_fwd<NC><<<P.H / RB, nth, smem, st>>>(P);
+  const int nth = row_threads(NC, P.H, C::EPT);
+  const int RB = nth / (NC / C::EPT);
+  size_t smem = (size_t)RB * C::SEQ_STRIDE * sizeof(cplx);
+  const size_t red = (size_t)ROW_NMOM * (nth / 32 + 1) * sizeof(double);
+  if (smem < red) smem = red;
+  constexpr int MINB = 3;
+  SFFT_CUDA_TRY(cudaFuncSetAttribute(k_row_fwd<NC, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  k_row_fwd<NC, MINB><<<P.H / RB, nth, smem, st>>>(P);
   SFFT_LAUNCH_CHECK();
   return SFFT_OK;
 }
@@ -221,18 +291,18 @@ static sfft_status launch_row_fwd_t(const RowFwdParams& P, cudaStream_t st) {
 template <int NC>
 static sfft_status launch_row_inv_t(const RowInvParams& P, cudaStream_t st) {
   using C = FftCfg<NC>;
-  const int RB = rows_per_cta(NC, P.H);
-  const int nth = RB * (NC / C::EPT);
+  const int nth = row_threads(NC, P.H, C::EPT);
+  const int RB = nth / (NC / C::EPT);
   const size_t smem = (size_t)RB * C::SEQ_STRIDE * sizeof(cplx);
-  SFFT_CUDA_TRY(cudaFuncSetAttribute(k_row_inv_sub<NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  k_row_inv_sub<NC><<<P.H / RB, nth, smem, st>>>(P);
+  constexpr int MINB = 3;
+  SFFT_CUDA_TRY(cudaFuncSetAttribute(k_row_inv_sub<NC, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  k_row_inv_sub<NC, MINB><<<P.H / RB, nth, smem, st>>>(P);
   SFFT_LAUNCH_CHECK();
   return SFFT_OK;
 }
 
 #define SFFT_DISPATCH_NC(NCV, CALL)                       \
   switch (NCV) {                                          \
-    case 8: return CALL<8>(P, st);                        \
     case 16: return CALL<16>(P, st);                      \
     case 32: return CALL<32>(P, st);                      \
     case 64: return CALL<64>(P, st);                      \
@@ -250,7 +320,7 @@ sfft_status sfft_launch_row_fwd(sfft_plan* p, const double* R, const double* S,
   RowFwdParams P;
   P.R = R; P.S = S; P.mask = mask; P.H = p->H; P.W = p->W; P.nimg = nimg;
   for (int i = 0; i < nimg; ++i) P.img[i] = imgs[i];
-  P.T = Tout; P.twNC = p->twNC; P.twW = p->twW;
+  P.T = Tout; P.twP = p->twPNC; P.twW = p->twW;
   P.moments = moments ? 1 : 0; P.nMomA = p->nMomA; P.nMomS = p->nMomS; P.rowMom = p->rowMom;
   ++*nl;
   SFFT_DISPATCH_NC(p->NC, launch_row_fwd_t)
@@ -260,7 +330,7 @@ sfft_status sfft_launch_row_inv_sub(sfft_plan* p, const double* S, const double*
                                     cudaStream_t st, int* nl) {
   RowInvParams P;
   P.Mhat = p->Mhat; P.S = S; P.coeffs = c; P.D = D; P.H = p->H; P.W = p->W;
-  P.offB = p->L * p->TK; P.DB = p->DB; P.twNC = p->twNC; P.twW = p->twW;
+  P.offB = p->L * p->TK; P.DB = p->DB; P.twP = p->twPNC; P.twW = p->twW;
   ++*nl;
   SFFT_DISPATCH_NC(p->NC, launch_row_inv_t)
 }

@@ -5,7 +5,7 @@
 #include <new>
 #include <vector>
 
-#include "sfft_common.cuh"
+#include "fft_smem.cuh"
 
 static bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 static int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
@@ -36,9 +36,35 @@ static cudaError_t upload_twiddles(cplx** dst, int n) {
   return cudaMemcpy(*dst, h.data(), sizeof(cplx) * (size_t)n, cudaMemcpyHostToDevice);
 }
 
+// long-double e^{-2 pi i num/den}, exact on the axes, rounded once to double
+static cplx unit_root(long long num, long long den) {
+  const long double twopi = 6.283185307179586476925286766559005768L;
+  num %= den;
+  if ((4 * num) % den == 0) {
+    const int quad = (int)((4 * num) / den);
+    return cmake(quad == 0 ? 1.0 : (quad == 2 ? -1.0 : 0.0), quad == 1 ? -1.0 : (quad == 3 ? 1.0 : 0.0));
+  }
+  const long double ang = -twopi * (long double)num / (long double)den;
+  return cmake((double)cosl(ang), (double)sinl(ang));
+}
+
+// Per-pass twiddle tables of the length-n FFT (layout: fft_smem.cuh): pass i >= 1 with radix R and
+// stride NS stores exp(-2 pi i r k/(NS R)) at off_i + (r-1)*NS + k.
+static cudaError_t upload_pass_tables(cplx** dst, int n) {
+  std::vector<cplx> h(fft_pass_table_size(n), cmake(1.0, 0.0));
+  for (int pass = 1; pass < fft_num_passes(n); ++pass) {
+    const int R = fft_radix(n, pass), NS = fft_pass_ns(n, pass), off = fft_tw_off(n, pass);
+    for (int r = 1; r < R; ++r)
+      for (int k = 0; k < NS; ++k) h[off + (r - 1) * NS + k] = unit_root((long long)r * k, (long long)NS * R);
+  }
+  cudaError_t e = cudaMalloc((void**)dst, sizeof(cplx) * h.size());
+  if (e != cudaSuccess) return e;
+  return cudaMemcpy(*dst, h.data(), sizeof(cplx) * h.size(), cudaMemcpyHostToDevice);
+}
+
 static void plan_free(sfft_plan* p) {
   if (!p) return;
-  cudaFree(p->twNC); cudaFree(p->twW); cudaFree(p->twH); cudaFree(p->d_pairs); cudaFree(p->d_groups);
+  cudaFree(p->twPNC); cudaFree(p->twPH); cudaFree(p->twW); cudaFree(p->twH); cudaFree(p->d_pairs); cudaFree(p->d_groups);
   cudaFree(p->T); cudaFree(p->F); cudaFree(p->Y); cudaFree(p->Cmap); cudaFree(p->rowMom);
   cudaFree(p->mom); cudaFree(p->Lw); cudaFree(p->cholBar); cudaFree(p->Etab); cudaFree(p->Mhat);
   free(p->h_pairs);
@@ -148,7 +174,7 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   dalloc((void**)&p->d_pairs, sizeof(PairDesc) * p->nPair);
   dalloc((void**)&p->d_groups, sizeof(CrossGroup) * groups.size());
   if (!ok) { plan_free(p); return SFFT_ERR_ALLOC; }
-  if (upload_twiddles(&p->twNC, p->NC) != cudaSuccess || upload_twiddles(&p->twW, W) != cudaSuccess ||
+  if (upload_pass_tables(&p->twPNC, p->NC) != cudaSuccess || upload_pass_tables(&p->twPH, H) != cudaSuccess || upload_twiddles(&p->twW, W) != cudaSuccess ||
       upload_twiddles(&p->twH, H) != cudaSuccess ||
       cudaMemcpy(p->d_pairs, p->h_pairs, sizeof(PairDesc) * p->nPair, cudaMemcpyHostToDevice) != cudaSuccess ||
       cudaMemcpy(p->d_groups, groups.data(), sizeof(CrossGroup) * groups.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
@@ -160,7 +186,7 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
     plan_free(p);
     return SFFT_ERR_CUDA;
   }
-  ws += sizeof(cplx) * (size_t)(p->NC + W + H);
+  ws += sizeof(cplx) * (size_t)(fft_pass_table_size(p->NC) + fft_pass_table_size(H) + W + H);
   p->ws_bytes = ws;
   if (cudaDeviceSynchronize() != cudaSuccess) { cudaGetLastError(); plan_free(p); return SFFT_ERR_CUDA; }
   *out = p;

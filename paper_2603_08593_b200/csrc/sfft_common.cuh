@@ -95,7 +95,8 @@ struct sfft_plan {
   int nMomS;     // DB+1 row moments     sum_x m xi^p S
 
   // device tables
-  cplx* twNC;    // e^{-2 pi i m / NC}, m in [0, NC)
+  cplx* twPNC;   // per-pass FFT twiddle tables for length NC (fft_smem.cuh)
+  cplx* twPH;    // per-pass FFT twiddle tables for length H
   cplx* twW;     // e^{-2 pi i m / W},  m in [0, W)
   cplx* twH;     // e^{-2 pi i m / H},  m in [0, H)
   PairDesc* d_pairs;
