@@ -155,7 +155,7 @@ def stage_models(plan_dims, peaks, alu_peak):
     TK, TB = (DK + 1) * (DK + 2) // 2, (DB + 1) * (DB + 2) // 2
     L = (2 * w + 1) ** 2
     N = L * TK + TB
-    nRow, nSpec = DK + 1 + 1 + DB + 1, TK + 1 + TB
+    nRow, nSpec = DK + 1 + 1, TK + 1   # lean plan: the kernel-background block needs no transform
 
     def fft_instr(n):  # Stockham radix-16/8/4 passes as implemented (fft_smem.cuh)
         plans = {8: [8], 16: [16], 32: [8, 4], 64: [8, 8], 128: [16, 8], 256: [16, 16], 512: [8, 8, 8],
@@ -167,14 +167,16 @@ def stage_models(plan_dims, peaks, alu_peak):
         return tot
 
     rowfft = fft_instr(NC) + 8.0 * NC
-    nKK, nKO = TK * (TK + 1) // 2, TK * (1 + TB)
+    nKK, nKS = TK * (TK + 1) // 2, TK
     col_pair = lambda D: H * 4.0 + (H / 8.0) * (58.0 + 8.0 * D)
     m = {}
     m["build.row_fwd"] = (nRow * H * rowfft, 2 * P * 8 + P + nRow * P * 8)
     m["build.col_fwd"] = (nSpec * NC * fft_instr(H), (nRow + nSpec) * P * 8)
     m["build.cross_KK"] = ((NC + 1) * nKK * col_pair(2 * w), TK * P * 8)
-    m["build.cross_KO"] = ((NC + 1) * nKO * col_pair(w), nSpec * P * 8)
-    m["build.lag_gather"] = ((nKK * (4 * w + 1) * (2 * w + 1) + nKO * (2 * w + 1) * (w + 1)) * NC * 4.0, N * N * 8.0)
+    m["build.cross_KS"] = ((NC + 1) * nKS * col_pair(w), nSpec * P * 8)
+    # sparse kernel-background part: ~1% special pixels (border), L shifts, TK*TB products; reads the mask twice
+    m["build.kb_sparse"] = (0.01 * P * L * TK * TB, 2.0 * P)
+    m["build.lag_gather"] = ((nKK * (4 * w + 1) * (2 * w + 1) + nKS * (2 * w + 1) * (w + 1)) * NC * 4.0, N * N * 8.0)
     m["solve"] = (N ** 3 / 6.0 + 2.0 * N * N, 2.0 * N * N * 8)
     m["subtract.row_fwd"] = ((DK + 1) * H * rowfft, P * 8 + (DK + 1) * P * 8)
     per_v = sum(2 * (DK - p) + 4 for p in range(DK + 1))

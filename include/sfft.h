@@ -67,7 +67,7 @@ const char* sfft_status_string(sfft_status s);
 /* Build the normal equations (north_star subsystems (1)-(4)):
  * weighted masked images -> batched fp64 2-D real FFTs -> Fourier-domain cross products and
  * inverse transforms restricted to the lag window -> gather into A and b.
- *   R, S  in : H*W fp64 (device).      mask in: H*W uint8 (device), nonzero = excluded; NULL = none.
+ *   R, S  in : H*W fp64 (device).      mask in: H*W uint8 (device, 16-byte aligned), nonzero = excluded; NULL = none.
  *   A    out : N*N fp64 row-major, FULL symmetric matrix (both triangles written).
  *   b    out : N fp64.
  * Errors: INVALID_ARG on NULL p/R/S/A/b or misalignment; CUDA on a launch failure. */
@@ -102,9 +102,10 @@ sfft_status sfft_probe_fp64(int kind, int iters, double* tflops, double* elapsed
  * pairs between reads).  sfft_profile_read synchronises on the pending events, folds them into
  * per-stage totals and returns the accumulated milliseconds and pair count of `stage`:
  *   0 build: row pass (k_row_fwd)          1 build: column pass (k_col_fwd)
- *   2 build: cross+pruned inverse, K-K     3 build: cross+pruned inverse, K-S and K-Psi
+ *   2 build: cross+pruned inverse, K-K     3 build: cross+pruned inverse, K-S
  *   4 build: lag-row inverse + moments + gather      5 solve (all kernels)
  *   6 subtract: row pass   7 subtract: phase table + y-mixing   8 subtract: inverse rows + D
+ *   9 build: sparse part of the kernel-background block (special-pixel list + correction sums)
  * reset != 0 clears that stage's totals after reading. */
 sfft_status sfft_profile_enable(sfft_plan* p, int on);
 sfft_status sfft_profile_read(sfft_plan* p, int stage, double* total_ms, int* count, int reset);

@@ -21,8 +21,9 @@ EXPORTED_SYMBOLS = [
     "sfft_profile_enable", "sfft_profile_read",
 ]
 
-STAGE_NAMES = ["build.row_fwd", "build.col_fwd", "build.cross_KK", "build.cross_KO",
-               "build.lag_gather", "solve", "subtract.row_fwd", "subtract.mix", "subtract.row_inv"]
+STAGE_NAMES = ["build.row_fwd", "build.col_fwd", "build.cross_KK", "build.cross_KS",
+               "build.lag_gather", "solve", "subtract.row_fwd", "subtract.mix", "subtract.row_inv",
+               "build.kb_sparse"]
 
 
 class SfftError(RuntimeError):

@@ -124,8 +124,8 @@ static sfft_status launch_col_fwd_t(ColFwdParams& P, cudaStream_t st) {
 sfft_status sfft_launch_col_fwd(sfft_plan* p, cudaStream_t st, int* nl) {
   ColFwdParams P;
   P.T = p->T; P.F = p->F; P.H = p->H; P.NC = p->NC; P.pitch = p->pitch; P.twP = p->twPH;
-  // spectra order: R~ monomials (TK), S~, Psi monomials (TB); row-pass images: R~ xi^p (DK+1),
-  // S~, Psi xi^p (DB+1).  Groups are listed heaviest first (most eta powers per source).
+  // spectra order: R~ monomials (TK), S~; row-pass images: R~ xi^p (DK+1), S~.
+  // Groups are listed heaviest first (most eta powers per source).
   int n = 0;
   auto add_group = [&](int src, int pxi, int deg, int spec0, const int (*mono)[2], int nmono) {
     int k = 0;
@@ -134,10 +134,8 @@ sfft_status sfft_launch_col_fwd(sfft_plan* p, cudaStream_t st, int* nl) {
     (void)deg;
     P.grp_src[n] = src; P.grp_n[n] = k; ++n;
   };
-  const int maxdeg = p->DK > p->DB ? p->DK : p->DB;
-  for (int pxi = 0; pxi <= maxdeg; ++pxi) {
-    if (pxi <= p->DK) add_group(pxi, pxi, p->DK, 0, p->monoK, p->TK);
-    if (pxi <= p->DB) add_group(p->DK + 2 + pxi, pxi, p->DB, p->TK + 1, p->monoB, p->TB);
+  for (int pxi = 0; pxi <= p->DK; ++pxi) {
+    add_group(pxi, pxi, p->DK, 0, p->monoK, p->TK);
     if (pxi == 0) { P.grp_src[n] = p->DK + 1; P.grp_n[n] = 1; P.grp_spec[n][0] = p->TK; P.grp_q[n][0] = 0; ++n; }
   }
   P.ngrp = n;

@@ -235,24 +235,28 @@ __global__ void __launch_bounds__(LAG_TH) k_lag_idft(LagParams P) {
 }
 
 struct MomParams {
-  const double* rowMom;  // [nMomA + nMomS][H]
-  double* mom;           // [nMomA*nMomA] then [TB]
-  int H, nMomA, nMomS, TB;
+  const double* rowMom;  // [nMomA + nMomS + nMomR][H]
+  double* mom;           // [nMomA*nMomA] then [TB] then [nMomR*nMomR]
+  int H, nMomA, nMomS, nMomR, TB;
   int monoB[SFFT_MAX_T][2];
 };
 
 __global__ void __launch_bounds__(256) k_mom_final(MomParams P) {
   // block q < nMomA^2: (a,b) = (q / nMomA, q % nMomA) -> sum_y eta^b rowMom[a][y]
-  // block q >= nMomA^2: background rhs t' -> sum_y eta^q rowMomS[p][y]
+  // next TB blocks: background rhs t' -> sum_y eta^q rowMomS[p][y]; then nMomR^2 blocks: mu_ab
   const int q = blockIdx.x;
   int row, pw;
   if (q < P.nMomA * P.nMomA) {
     row = q / P.nMomA;
     pw = q % P.nMomA;
-  } else {
+  } else if (q < P.nMomA * P.nMomA + P.TB) {
     const int t = q - P.nMomA * P.nMomA;
     row = P.nMomA + P.monoB[t][0];
     pw = P.monoB[t][1];
+  } else {   // mu_ab = sum m R xi^a eta^b
+    const int e = q - P.nMomA * P.nMomA - P.TB;
+    row = P.nMomA + P.nMomS + e / P.nMomR;
+    pw = e % P.nMomR;
   }
   const double* src = P.rowMom + (size_t)row * P.H;
   const double invH = 1.0 / (double)P.H;
@@ -272,11 +276,18 @@ __global__ void __launch_bounds__(256) k_mom_final(MomParams P) {
 struct GatherParams {
   const double* Cmap;
   const double* mom;
+  const double* kbCorr;   // [(t*L + s)*TB + t'] sparse part of the kernel-background block (k_kb.cu)
   double* A;
   double* b;
-  int w, L, TK, TB, N, nLag, nMomA;
-  int monoB[SFFT_MAX_T][2];
+  int w, L, TK, TB, N, nLag, nMomA, nMomR, H, W;
+  int monoK[SFFT_MAX_T][2], monoB[SFFT_MAX_T][2];
 };
+
+__device__ __forceinline__ double binom(int n, int k) {
+  double r = 1.0;
+  for (int i = 1; i <= k; ++i) r = r * (double)(n - k + i) / (double)i;
+  return r;
+}
 
 __global__ void __launch_bounds__(256) k_gather(GatherParams P) {
   const int N = P.N, L = P.L, w = P.w, S1 = 2 * w + 1;
@@ -292,7 +303,7 @@ __global__ void __launch_bounds__(256) k_gather(GatherParams P) {
       if (i < nK) {
         const int t = i / L, s = i - t * L;
         const int u = s % S1 - w, vv = s / S1 - w;
-        const int pair = nKK + t * (1 + P.TB);  // (t, S)
+        const int pair = nKK + t;  // (t, S)
         v = P.Cmap[pair * lag2 + (size_t)(vv + w) * P.nLag + (u + w)];
       } else {
         v = P.mom[P.nMomA * P.nMomA + (i - nK)];
@@ -316,8 +327,17 @@ __global__ void __launch_bounds__(256) k_gather(GatherParams P) {
       const int ik = i < nK ? i : j, ib = (i < nK ? j : i) - nK;
       const int t = ik / L, s = ik - t * L;
       const int u = s % S1 - w, vv = s / S1 - w;
-      const int pair = nKK + t * (1 + P.TB) + 1 + ib;  // (t, Psi_ib)
-      v = P.Cmap[pair * lag2 + (size_t)(vv + w) * P.nLag + (u + w)];
+      // moments part: sum_x' R~_t(x') P_t'(x' + (u,v)), the polynomial expanded about x'
+      const int pk = P.monoK[t][0], qk = P.monoK[t][1], pb = P.monoB[ib][0], qb = P.monoB[ib][1];
+      const double dx = 2.0 * (double)u / (double)P.W, dy = 2.0 * (double)vv / (double)P.H;
+      const double* mu = P.mom + P.nMomA * P.nMomA + P.TB;
+      double acc = 0.0;
+      for (int ii = 0; ii <= pb; ++ii) {
+        const double cx = binom(pb, ii) * ipow(dx, pb - ii);
+        for (int jj = 0; jj <= qb; ++jj)
+          acc += cx * binom(qb, jj) * ipow(dy, qb - jj) * mu[(pk + ii) * P.nMomR + (qk + jj)];
+      }
+      v = acc + P.kbCorr[((size_t)t * L + s) * P.TB + ib];
     } else {
       const int a = i - nK, c = j - nK;
       const int pa = P.monoB[a][0] + P.monoB[c][0], qa = P.monoB[a][1] + P.monoB[c][1];
@@ -337,16 +357,18 @@ sfft_status sfft_launch_lag_gather(sfft_plan* p, double* A, double* b, cudaStrea
   SFFT_LAUNCH_CHECK();
   ++*nl;
   MomParams MP;
-  MP.rowMom = p->rowMom; MP.mom = p->mom; MP.H = p->H; MP.nMomA = p->nMomA; MP.nMomS = p->nMomS;
+  MP.rowMom = p->rowMom; MP.mom = p->mom; MP.H = p->H; MP.nMomA = p->nMomA; MP.nMomS = p->nMomS; MP.nMomR = p->nMomR;
   MP.TB = p->TB;
   for (int t = 0; t < p->TB; ++t) { MP.monoB[t][0] = p->monoB[t][0]; MP.monoB[t][1] = p->monoB[t][1]; }
-  k_mom_final<<<p->nMomA * p->nMomA + p->TB, 256, 0, st>>>(MP);
+  k_mom_final<<<p->nMomA * p->nMomA + p->TB + p->nMomR * p->nMomR, 256, 0, st>>>(MP);
   SFFT_LAUNCH_CHECK();
   ++*nl;
   GatherParams GP;
   GP.Cmap = p->Cmap; GP.mom = p->mom; GP.A = A; GP.b = b; GP.w = p->w; GP.L = p->L; GP.TK = p->TK;
-  GP.TB = p->TB; GP.N = p->N; GP.nLag = p->nLag; GP.nMomA = p->nMomA;
+  GP.TB = p->TB; GP.N = p->N; GP.nLag = p->nLag; GP.nMomA = p->nMomA; GP.nMomR = p->nMomR;
+  GP.H = p->H; GP.W = p->W; GP.kbCorr = p->kbCorr;
   for (int t = 0; t < p->TB; ++t) { GP.monoB[t][0] = p->monoB[t][0]; GP.monoB[t][1] = p->monoB[t][1]; }
+  for (int t = 0; t < p->TK; ++t) { GP.monoK[t][0] = p->monoK[t][0]; GP.monoK[t][1] = p->monoK[t][1]; }
   const size_t total = (size_t)p->N * p->N + p->N;
   int blocks = (int)((total + 255) / 256);
   if (blocks > 148 * 16) blocks = 148 * 16;

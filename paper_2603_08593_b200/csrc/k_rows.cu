@@ -23,11 +23,11 @@ struct RowFwdParams {
   cplx* T;  // [nimg][H][NC]
   const cplx* twP;   // per-pass twiddle tables for length NC
   const cplx* twW;
-  int moments, nMomA, nMomS;
-  double* rowMom;  // [nMomA + nMomS][H]
+  int moments, nMomA, nMomS, nMomR;
+  double* rowMom;  // [nMomA + nMomS + nMomR][H]
 };
 
-#define ROW_NMOM (2 * SFFT_MAX_DEG + 1 + SFFT_MAX_DEG + 1)
+#define ROW_NMA (2 * SFFT_MAX_DEG + 1)   // most moments of one family (mask, S or R)
 
 // One CTA = RB rows, NC/EPT threads per row.  A thread's EPT input elements j = tr + e*TPR are
 // exactly the inputs of its first-pass butterfly, so they go from global memory through the
@@ -57,61 +57,6 @@ __global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
     for (int e = 0; e < EPT; ++e) mk[e] = *reinterpret_cast<const uchar2*>(P.mask + rowoff + 2 * (tr + e * TPR));
 #pragma unroll
     for (int e = 0; e < EPT; ++e) mbits |= (mk[e].x ? 1u : 0u) << (2 * e) | (mk[e].y ? 1u : 0u) << (2 * e + 1);
-  }
-
-  if (P.moments) {
-    // fused reductions sum_x m xi^a and sum_x m xi^p S: per-thread partials, shuffle tree inside
-    // the row's lanes, then the row's warps in order (fixed order, reproducible)
-    double acc[ROW_NMOM];
-#pragma unroll
-    for (int q = 0; q < ROW_NMOM; ++q) acc[q] = 0.0;
-    double2 sv[EPT];
-#pragma unroll
-    for (int e = 0; e < EPT; ++e) sv[e] = *reinterpret_cast<const double2*>(P.S + rowoff + 2 * (tr + e * TPR));
-#pragma unroll
-    for (int e = 0; e < EPT; ++e) {
-      const int j = tr + e * TPR;
-      const double x0 = (double)(4 * j + 1 - W) * invW, x1 = (double)(4 * j + 3 - W) * invW;
-      double p0 = ((mbits >> (2 * e)) & 1u) ? 0.0 : 1.0, p1 = ((mbits >> (2 * e + 1)) & 1u) ? 0.0 : 1.0;
-#pragma unroll
-      for (int a = 0; a < 2 * SFFT_MAX_DEG + 1; ++a) {
-        if (a < P.nMomA) {
-          acc[a] += p0 + p1;
-          if (a < P.nMomS) acc[2 * SFFT_MAX_DEG + 1 + a] += p0 * sv[e].x + p1 * sv[e].y;
-          p0 *= x0;
-          p1 *= x1;
-        }
-      }
-    }
-    constexpr int LW = TPR < 32 ? TPR : 32;   // lanes of one row inside a warp
-#pragma unroll
-    for (int q = 0; q < ROW_NMOM; ++q) {
-#pragma unroll
-      for (int off = LW / 2; off > 0; off >>= 1) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], off);
-    }
-    double* red = reinterpret_cast<double*>(smem_raw);   // [ROW_NMOM][warps]
-    constexpr int WPR = TPR / 32 > 0 ? TPR / 32 : 1;      // warps per row
-    if (TPR > 32) {
-      if ((tid & 31) == 0)
-#pragma unroll
-        for (int q = 0; q < ROW_NMOM; ++q) red[q * (nth / 32) + (tid >> 5)] = acc[q];
-      __syncthreads();
-    }
-    if (tr == 0) {
-#pragma unroll
-      for (int q = 0; q < ROW_NMOM; ++q) {
-        double v = acc[q];
-        if (TPR > 32) {
-          v = 0.0;
-          for (int k = 0; k < WPR; ++k) v += red[q * (nth / 32) + (tid >> 5) + k];
-        }
-        const int a = q < 2 * SFFT_MAX_DEG + 1 ? q : q - (2 * SFFT_MAX_DEG + 1);
-        const bool isS = q >= 2 * SFFT_MAX_DEG + 1;
-        if (!isS && a < P.nMomA) P.rowMom[(size_t)a * H + y] = v;
-        if (isS && a < P.nMomS) P.rowMom[(size_t)(P.nMomA + a) * H + y] = v;
-      }
-    }
-    if (TPR > 32) __syncthreads();
   }
 
   cplx* srow = s + r * C::SEQ_STRIDE;
@@ -144,6 +89,58 @@ __global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
         t.y *= ipow(x1, d.pxi);
       }
       v[e] = t;
+    }
+    if (P.moments && d.pxi == 0 && d.src != 2) {
+      // fused reductions on the masked, unweighted image just formed (fixed order: per-thread
+      // partials, shuffle tree inside the row's lanes, then the row's warps in order):
+      //   src R: acc[a] = sum_x m R xi^a, a < nMomR
+      //   src S: acc[a] = sum_x m S xi^a, a < nMomS;  acc[ROW_NMA + a] = sum_x m xi^a, a < nMomA
+      double acc[2 * ROW_NMA];
+#pragma unroll
+      for (int q = 0; q < 2 * ROW_NMA; ++q) acc[q] = 0.0;
+      const bool isS = d.src == 1;
+      const int n0 = isS ? P.nMomS : P.nMomR, n1 = isS ? P.nMomA : 0;
+#pragma unroll
+      for (int e = 0; e < EPT; ++e) {
+        const int j = tr + e * TPR;
+        const double x0 = (double)(4 * j + 1 - W) * invW, x1 = (double)(4 * j + 3 - W) * invW;
+        double f0 = v[e].x, f1 = v[e].y;
+        double p0 = ((mb >> (2 * e)) & 1u) ? 0.0 : 1.0, p1 = ((mb >> (2 * e + 1)) & 1u) ? 0.0 : 1.0;
+#pragma unroll
+        for (int a = 0; a < ROW_NMA; ++a) {
+          if (a < n0) { acc[a] += f0 + f1; f0 *= x0; f1 *= x1; }
+          if (a < n1) { acc[ROW_NMA + a] += p0 + p1; p0 *= x0; p1 *= x1; }
+        }
+      }
+      constexpr int LW = TPR < 32 ? TPR : 32;        // lanes of one row inside a warp
+      constexpr int WPR = TPR / 32 > 0 ? TPR / 32 : 1;  // warps per row
+#pragma unroll
+      for (int q = 0; q < 2 * ROW_NMA; ++q) {
+#pragma unroll
+        for (int off = LW / 2; off > 0; off >>= 1) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], off);
+      }
+      double* red = reinterpret_cast<double*>(smem_raw);   // [2*ROW_NMA][warps]; s is idle here
+      if (TPR > 32) {
+        if ((tid & 31) == 0) {
+#pragma unroll
+          for (int q = 0; q < 2 * ROW_NMA; ++q) red[q * (nth / 32) + (tid >> 5)] = acc[q];
+        }
+        __syncthreads();
+      }
+      if (tr == 0) {
+        const int base0 = isS ? P.nMomA : P.nMomA + P.nMomS;   // rowMom rows: mask, S, R families
+#pragma unroll
+        for (int q = 0; q < 2 * ROW_NMA; ++q) {
+          double t = acc[q];
+          if (TPR > 32) {
+            t = 0.0;
+            for (int k = 0; k < WPR; ++k) t += red[q * (nth / 32) + (tid >> 5) + k];
+          }
+          if (q < ROW_NMA) { if (q < n0) P.rowMom[(size_t)(base0 + q) * H + y] = t; }
+          else if (q - ROW_NMA < n1) P.rowMom[(size_t)(q - ROW_NMA) * H + y] = t;
+        }
+      }
+      if (TPR > 32) __syncthreads();
     }
     fft_regs_to_smem<NC, -1, false>(v, s, tid, nth, RB, P.twP, C::SEQ_STRIDE);
     fetch(im + 1);
@@ -279,7 +276,7 @@ static sfft_status launch_row_fwd_t(const RowFwdParams& P, cudaStream_t st) {
   const int nth = row_threads(NC, P.H, C::EPT);
   const int RB = nth / (NC / C::EPT);
   size_t smem = (size_t)RB * C::SEQ_STRIDE * sizeof(cplx);
-  const size_t red = (size_t)ROW_NMOM * (nth / 32 + 1) * sizeof(double);
+  const size_t red = (size_t)2 * ROW_NMA * (nth / 32 + 1) * sizeof(double);
   if (smem < red) smem = red;
   constexpr int MINB = 3;
   SFFT_CUDA_TRY(cudaFuncSetAttribute(k_row_fwd<NC, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -321,7 +318,7 @@ sfft_status sfft_launch_row_fwd(sfft_plan* p, const double* R, const double* S,
   P.R = R; P.S = S; P.mask = mask; P.H = p->H; P.W = p->W; P.nimg = nimg;
   for (int i = 0; i < nimg; ++i) P.img[i] = imgs[i];
   P.T = Tout; P.twP = p->twPNC; P.twW = p->twW;
-  P.moments = moments ? 1 : 0; P.nMomA = p->nMomA; P.nMomS = p->nMomS; P.rowMom = p->rowMom;
+  P.moments = moments ? 1 : 0; P.nMomA = p->nMomA; P.nMomS = p->nMomS; P.nMomR = p->nMomR; P.rowMom = p->rowMom;
   ++*nl;
   SFFT_DISPATCH_NC(p->NC, launch_row_fwd_t)
 }

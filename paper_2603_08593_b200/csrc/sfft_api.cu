@@ -66,7 +66,7 @@ static void plan_free(sfft_plan* p) {
   if (!p) return;
   cudaFree(p->twPNC); cudaFree(p->twPH); cudaFree(p->twW); cudaFree(p->twH); cudaFree(p->d_pairs); cudaFree(p->d_groups);
   cudaFree(p->T); cudaFree(p->F); cudaFree(p->Y); cudaFree(p->Cmap); cudaFree(p->rowMom);
-  cudaFree(p->mom); cudaFree(p->Lw); cudaFree(p->cholBar); cudaFree(p->Etab); cudaFree(p->Mhat);
+  cudaFree(p->mom); cudaFree(p->spCount); cudaFree(p->spOff); cudaFree(p->spList); cudaFree(p->kbPart); cudaFree(p->kbCorr); cudaFree(p->Lw); cudaFree(p->cholBar); cudaFree(p->Etab); cudaFree(p->Mhat);
   free(p->h_pairs);
   for (int i = 0; i < 2 * SFFT_PROF_MAX; ++i) if (p->prof_ev[i]) cudaEventDestroy(p->prof_ev[i]);
   delete p;
@@ -108,19 +108,20 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   p->NC = W / 2;
   p->pitch = p->NC + SFFT_PITCH_PAD;
   p->log2H = ilog2(H); p->log2NC = ilog2(p->NC);
-  p->nRowImg = (DK + 1) + 1 + (DB + 1);
-  p->nSpec = p->TK + 1 + p->TB;
-  p->nPair = p->TK * (p->TK + 1) / 2 + p->TK * (1 + p->TB);
+  p->nRowImg = (DK + 1) + 1;
+  p->nSpec = p->TK + 1;
+  p->nPair = p->TK * (p->TK + 1) / 2 + p->TK;
   p->Dmax = 2 * w;
   p->nLag = 2 * p->Dmax + 1;
   p->nMomA = 2 * DB + 1;
   p->nMomS = DB + 1;
+  p->nMomR = DK + DB + 1;
   p->ldL = (p->N + 1 + 3) & ~3;
   int dev = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, dev);
 
-  // pair list: kernel-kernel pairs (t <= t2) first, then for each t: (t,S), (t,Psi_0..)
+  // pair list: kernel-kernel pairs (t <= t2) first, then (t,S) for each t
   p->h_pairs = (PairDesc*)malloc(sizeof(PairDesc) * p->nPair);
   if (!p->h_pairs) { plan_free(p); return SFFT_ERR_ALLOC; }
   int n = 0;
@@ -128,7 +129,6 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
     for (int t2 = t; t2 < p->TK; ++t2) { p->h_pairs[n].fa = t; p->h_pairs[n].fb = t2; p->h_pairs[n].D = 2 * w; ++n; }
   for (int t = 0; t < p->TK; ++t) {
     p->h_pairs[n].fa = t; p->h_pairs[n].fb = p->TK; p->h_pairs[n].D = w; ++n;
-    for (int t2 = 0; t2 < p->TB; ++t2) { p->h_pairs[n].fa = t; p->h_pairs[n].fb = p->TK + 1 + t2; p->h_pairs[n].D = w; ++n; }
   }
 
   // k_cross groups: consecutive pairs (same D class) packed while the group holds <= SFFT_CR_GP
@@ -165,8 +165,16 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   dalloc((void**)&p->F, sizeof(cplx) * HP * p->nSpec);
   dalloc((void**)&p->Y, sizeof(cplx) * (size_t)p->nPair * p->nLag * p->pitch);
   dalloc((void**)&p->Cmap, sizeof(double) * (size_t)p->nPair * p->nLag * p->nLag);
-  dalloc((void**)&p->rowMom, sizeof(double) * (size_t)(p->nMomA + p->nMomS) * H);
-  dalloc((void**)&p->mom, sizeof(double) * (size_t)(p->nMomA * p->nMomA + p->TB));
+  dalloc((void**)&p->rowMom, sizeof(double) * (size_t)(p->nMomA + p->nMomS + p->nMomR) * H);
+  dalloc((void**)&p->mom, sizeof(double) * (size_t)(p->nMomA * p->nMomA + p->TB + p->nMomR * p->nMomR));
+  {
+    const int nsub = 128 / p->L > 0 ? 128 / p->L : 1;
+    dalloc((void**)&p->spCount, sizeof(int) * (size_t)H);
+    dalloc((void**)&p->spOff, sizeof(int) * (size_t)(H + 1));
+    dalloc((void**)&p->spList, sizeof(int) * (size_t)H * W);
+    dalloc((void**)&p->kbPart, sizeof(double) * (size_t)SFFT_KB_NBLK * nsub * p->TK * p->L * p->TB);
+    dalloc((void**)&p->kbCorr, sizeof(double) * (size_t)p->TK * p->L * p->TB);
+  }
   dalloc((void**)&p->Lw, sizeof(double) * (size_t)(p->N + 1) * p->ldL);
   dalloc((void**)&p->cholBar, 2 * sizeof(unsigned));
   dalloc((void**)&p->Etab, sizeof(cplx) * (size_t)p->TK * (2 * w + 1) * p->NC);
@@ -207,22 +215,24 @@ static bool aligned16(const void* q) { return (((uintptr_t)q) & 15) == 0; }
 sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
                               double* A, double* b, void* stream) {
   if (!p || !R || !S || !A || !b) return SFFT_ERR_INVALID_ARG;
-  if (!aligned16(R) || !aligned16(S) || !aligned16(A) || !aligned16(b) || (mask && (((uintptr_t)mask) & 1)))
+  if (!aligned16(R) || !aligned16(S) || !aligned16(A) || !aligned16(b) || (mask && !aligned16(mask)))
     return SFFT_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   int nl = 0;
-  // a1 + a2 (row pass): m xi^p R (p<=DK), m S, m xi^p (p<=DB), with the fused moment reductions
+  // a1 + a2 (row pass): m xi^p R (p<=DK), m S, with the fused moment reductions
+  // (sum m xi^a, sum m S xi^p, sum m R xi^a)
   RowImage imgs[8];
   int n = 0;
   for (int q = 0; q <= p->DK; ++q) { imgs[n].src = 0; imgs[n].pxi = q; imgs[n].masked = 1; ++n; }
   imgs[n].src = 1; imgs[n].pxi = 0; imgs[n].masked = 1; ++n;
-  for (int q = 0; q <= p->DB; ++q) { imgs[n].src = 2; imgs[n].pxi = q; imgs[n].masked = 1; ++n; }
   sfft_status s;
   { ProfScope ps(p, 0, st); s = sfft_launch_row_fwd(p, R, S, mask, imgs, n, p->T, true, st, &nl); }
   if (s != SFFT_OK) return s;
   { ProfScope ps(p, 1, st); s = sfft_launch_col_fwd(p, st, &nl); }  // a2 (column pass, applies eta^q)
   if (s != SFFT_OK) return s;
   s = sfft_launch_cross(p, st, &nl);         // a3 (cross products + lag-pruned inverse along ky)
+  if (s != SFFT_OK) return s;
+  { ProfScope ps(p, 9, st); s = sfft_launch_kb(p, R, mask, st, &nl); }  // kernel-background block, sparse part
   if (s != SFFT_OK) return s;
   { ProfScope ps(p, 4, st); s = sfft_launch_lag_gather(p, A, b, st, &nl); }  // a3 (kx inverse on lag rows) + a4
   if (s != SFFT_OK) return s;

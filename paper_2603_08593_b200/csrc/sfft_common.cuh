@@ -12,7 +12,8 @@
 #define SFFT_CR_CT 16        // k_cross: columns per CTA
 #define SFFT_CR_GP 21        // k_cross: pairs per CTA (threads = SFFT_CR_GP * SFFT_CR_CT)
 #define SFFT_CR_MAXSPEC 24   // k_cross: spectra a group may stage
-#define SFFT_NSTAGE 9      // see sfft_profile_read in include/sfft.h
+#define SFFT_KB_NBLK 296     // x-CTAs of the kernel-background correction kernel (2 per SM)
+#define SFFT_NSTAGE 10     // see sfft_profile_read in include/sfft.h
 #define SFFT_PROF_MAX 512
 
 typedef double2 cplx;
@@ -85,14 +86,15 @@ struct sfft_plan {
   int NC;        // W/2
   int pitch;     // spectrum row pitch (complex elements) = NC + SFFT_PITCH_PAD
   int log2H, log2NC;
-  int nRowImg;   // forward row-pass images in build: R~ xi^p (DK+1), S~ (1), Psi xi^p (DB+1)
-  int nSpec;     // spectra: TK + 1 + TB
-  int nPair;     // TK(TK+1)/2 + TK + TK*TB
+  int nRowImg;   // forward row-pass images in build: R~ xi^p (DK+1), S~ (1)
+  int nSpec;     // spectra: TK + 1  (the kernel-background block needs none, see k_kb.cu)
+  int nPair;     // TK(TK+1)/2 + TK
   int Dmax;      // 2w
   int nLag;      // 2*Dmax+1
   int monoK[SFFT_MAX_T][2], monoB[SFFT_MAX_T][2];
   int nMomA;     // 2*DB+1 row moments  sum_x m xi^a
   int nMomS;     // DB+1 row moments     sum_x m xi^p S
+  int nMomR;     // DK+DB+1 row moments  sum_x m xi^a R
 
   // device tables
   cplx* twPNC;   // per-pass FFT twiddle tables for length NC (fft_smem.cuh)
@@ -109,8 +111,15 @@ struct sfft_plan {
   cplx* F;       // spectra          [nSpec][H][pitch]  (column NC = Nyquist)
   cplx* Y;       // lag rows         [nPair][nLag][pitch]
   double* Cmap;  // lag windows      [nPair][nLag][nLag]
-  double* rowMom;   // [nMomA + nMomS][H]
-  double* mom;      // [(2DB+1)^2 + TB] reduced moments
+  double* rowMom;   // [nMomA + nMomS + nMomR][H]
+  double* mom;      // [nMomA^2] mask moments, [TB] background rhs, [nMomR^2] moments of m R
+  // kernel-background block without transforms (k_kb.cu): special target pixels (masked, or within
+  // w of an edge), their per-row counts/offsets, per-CTA partial corrections and the reduced ones
+  int* spCount;     // [H]
+  int* spOff;       // [H + 1]   exclusive scan; spOff[H] = number of special pixels
+  int* spList;      // [H*W]     y*W + x, bit 31 set when the pixel is masked
+  double* kbPart;   // [KB_NBLK][L*TK*TB]
+  double* kbCorr;   // [L*TK*TB]
   double* Lw;       // Cholesky workspace (N+1) x ldL
   unsigned* cholBar; // grid-barrier counters of k_chol_fused (arrivals, finished CTAs)
   cplx* Etab;       // subtract: E[TK][2w+1][NC]
@@ -161,6 +170,7 @@ sfft_status sfft_launch_row_fwd(sfft_plan* p, const double* R, const double* S,
                                 cplx* Tout, bool moments, cudaStream_t st, int* nl);
 sfft_status sfft_launch_col_fwd(sfft_plan* p, cudaStream_t st, int* nl);
 sfft_status sfft_launch_cross(sfft_plan* p, cudaStream_t st, int* nl);
+sfft_status sfft_launch_kb(sfft_plan* p, const double* R, const unsigned char* mask, cudaStream_t st, int* nl);
 sfft_status sfft_launch_lag_gather(sfft_plan* p, double* A, double* b, cudaStream_t st, int* nl);
 sfft_status sfft_launch_solve(sfft_plan* p, const double* A, const double* b, double* c, int* info,
                               cudaStream_t st, int* nl);
