@@ -1,8 +1,8 @@
 // Row-direction kernels.
 //
 //  k_row_fwd   : (a1)+(a2 first pass) -- generation of the polynomial-weighted, masked images
-//                m xi^p R, m S, m xi^p fused into the first (row, R2C) pass of the 2-D FFT, plus
-//                the fused fp64 reductions sum_x m xi^a and sum_x m xi^p S per row
+//                m xi^p R, m S fused into the first (row, R2C) pass of the 2-D FFT, plus the fused
+//                fp64 row reductions sum_x m xi^a, sum_x m xi^a S and sum_x m xi^a R
 //                (north_star subsystems (1),(2)).  The eta^q factor of a
 //                monomial is a function of y only, so it commutes with the row transform and is
 //                applied by the column pass: only DK+1 (not T_K) row transforms of R are needed.
@@ -17,29 +17,76 @@
 struct RowFwdParams {
   const double* R;
   const double* S;
-  const unsigned char* mask;
-  int H, W, nimg;
-  RowImage img[8];
-  cplx* T;  // [nimg][H][NC]
+  const unsigned char* mask;   // applied when non-NULL
+  int H, W;
+  int nR;        // images 0..nR-1 are xi^p R, p = image index
+  int withS;     // image nR is S (weight 1)
+  cplx* T;       // [nimg][H][pitchT]
+  int pitchT;    // row pitch of T in complex elements
+  int packed;    // 1: T[y][0] = X[0] + i X[W/2];  0: T[y][0] = X[0], T[y][NC] = X[W/2]
   const cplx* twP;   // per-pass twiddle tables for length NC
   const cplx* twW;
-  int moments, nMomA, nMomS, nMomR;
+  int moments, DB, nMomA, nMomS, nMomR;
+  double fullA[2 * SFFT_MAX_DEG + 1];   // sum over a whole row of xi^a
   double* rowMom;  // [nMomA + nMomS + nMomR][H]
 };
 
-#define ROW_NMA (2 * SFFT_MAX_DEG + 1)   // most moments of one family (mask, S or R)
+#define ROW_NMA (2 * SFFT_MAX_DEG + 1)   // most mask moments
+
+// v[e] = raw[e] * (x0^PW, x1^PW): x0 = xi(2j), x1 = xi(2j+1), j = tr + e*TPR; xi(2j) = xb + e*step
+// (all values are multiples of 1/W, so the affine form is exact).
+template <int EPT, int PW>
+__device__ __forceinline__ void row_weight(const double2* raw, cplx* v, double xb, double step, double dx1) {
+#pragma unroll
+  for (int e = 0; e < EPT; ++e) {
+    const double x0 = fma((double)e, step, xb), x1 = x0 + dx1;
+    double w0 = x0, w1 = x1;
+    if (PW >= 2) { w0 *= x0; w1 *= x1; }
+    if (PW >= 3) { w0 *= x0; w1 *= x1; }
+    v[e] = cmake(raw[e].x * w0, raw[e].y * w1);
+  }
+}
+
+// hi[i] = sum_e v[e].x x0^(i+1) + v[e].y x1^(i+1), i < NDB (per-thread partial, sequential in e)
+template <int EPT, int NDB>
+__device__ __forceinline__ void row_extra_moments(const cplx* v, double xb, double step, double dx1, double* hi) {
+#pragma unroll
+  for (int i = 0; i < SFFT_MAX_DEG; ++i) hi[i] = 0.0;
+#pragma unroll
+  for (int e = 0; e < EPT; ++e) {
+    const double x0 = fma((double)e, step, xb), x1 = x0 + dx1;
+    double f0 = v[e].x, f1 = v[e].y;
+#pragma unroll
+    for (int i = 0; i < NDB; ++i) {
+      f0 *= x0;
+      f1 *= x1;
+      hi[i] += f0 + f1;
+    }
+  }
+}
 
 // One CTA = RB rows, NC/EPT threads per row.  A thread's EPT input elements j = tr + e*TPR are
 // exactly the inputs of its first-pass butterfly, so they go from global memory through the
 // weighting (mask, xi^p) into the butterfly without being staged in shared memory; the inputs of
 // the next image are requested before the split/store phase of the current one.  The mask is
 // read once and kept as two bits per element.
+//
+// Fused reductions (moments != 0), all in a fixed order:
+//   sum_x m xi^p R, p <= DK and sum_x m S : the DC bin of the image's own row transform;
+//   sum_x m xi^a R, DK < a <= DK+DB and sum_x m xi^a S, 0 < a <= DB: DB extra sums on the
+//     weighted values of the last R image and of the S image (shuffle tree, then warps in order);
+//   sum_x m xi^a, a <= 2 DB: the closed-form whole-row sum minus the (rare) masked pixels.
 template <int NC, int MINB>
 __global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
   using C = FftCfg<NC>;
   constexpr int EPT = C::EPT;
   constexpr int TPR = NC / EPT;  // threads per row
+  constexpr int LW = TPR < 32 ? TPR : 32;           // lanes of one row inside a warp
+  constexpr int WPR = TPR / 32 > 0 ? TPR / 32 : 1;  // warps per row
+  constexpr int NSLOT = 128 / LW;                   // (row, warp-of-row) slots of a CTA
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ double redM[ROW_NMA][NSLOT];
+  __shared__ double redX[SFFT_MAX_DEG][NSLOT];
   cplx* s = reinterpret_cast<cplx*>(smem_raw);
   const int tid = threadIdx.x, nth = blockDim.x;
   const int RB = nth / TPR;
@@ -47,7 +94,10 @@ __global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
   const int y = blockIdx.x * RB + r;
   const int W = P.W, H = P.H;
   const double invW = 1.0 / (double)W;
+  const double xb = (double)(4 * tr + 1 - W) * invW, step = (double)(4 * TPR) * invW, dx1 = 2.0 * invW;
   const size_t rowoff = (size_t)y * W;
+  const int slot = tid / LW;
+  const int nimg = P.nR + P.withS;
 
   // mask bits: bit 2e = element 2j masked, bit 2e+1 = element 2j+1 masked, j = tr + e*TPR
   unsigned mbits = 0u;
@@ -61,98 +111,121 @@ __global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
 
   cplx* srow = s + r * C::SEQ_STRIDE;
   double2 raw[EPT];
-  auto fetch = [&](int im) {   // always defines raw[], so nothing of it stays live across the FFT
-    const int src_id = im < P.nimg ? P.img[im].src : 2;
-    if (src_id != 2) {
-      const double* src = (src_id == 0 ? P.R : P.S) + rowoff;
+  auto fetch = [&](int im) {
+    if (im < nimg) {
+      const double* src = (im < P.nR ? P.R : P.S) + rowoff;
 #pragma unroll
       for (int e = 0; e < EPT; ++e) raw[e] = *reinterpret_cast<const double2*>(src + 2 * (tr + e * TPR));
     } else {
 #pragma unroll
-      for (int e = 0; e < EPT; ++e) raw[e] = make_double2(1.0, 1.0);
+      for (int e = 0; e < EPT; ++e) raw[e] = make_double2(0.0, 0.0);
     }
   };
   fetch(0);
-  for (int im = 0; im < P.nimg; ++im) {
-    const RowImage d = P.img[im];
-    const unsigned mb = d.masked ? mbits : 0u;
-    cplx v[EPT];
+
+  if (P.moments) {
+    // masked part of sum_x m xi^a: only warps that hold a masked pixel do any work
+    double ms[ROW_NMA];
 #pragma unroll
-    for (int e = 0; e < EPT; ++e) {
-      const int j = tr + e * TPR;
-      double2 t = raw[e];
-      if ((mb >> (2 * e)) & 1u) t.x = 0.0;
-      if ((mb >> (2 * e + 1)) & 1u) t.y = 0.0;
-      if (d.pxi > 0) {
-        const double x0 = (double)(4 * j + 1 - W) * invW, x1 = (double)(4 * j + 3 - W) * invW;
-        t.x *= ipow(x0, d.pxi);
-        t.y *= ipow(x1, d.pxi);
+    for (int a = 0; a < ROW_NMA; ++a) ms[a] = 0.0;
+    if (__any_sync(0xffffffffu, mbits != 0u)) {
+      unsigned mm = mbits;
+      while (mm) {
+        const int bit = __ffs(mm) - 1;
+        mm &= mm - 1;
+        const int j = tr + (bit >> 1) * TPR;
+        const double x = (double)(4 * j + 1 + 2 * (bit & 1) - W) * invW;
+        double pw = 1.0;
+#pragma unroll
+        for (int a = 0; a < ROW_NMA; ++a) { ms[a] += pw; pw *= x; }
       }
-      v[e] = t;
-    }
-    if (P.moments && d.pxi == 0 && d.src != 2) {
-      // fused reductions on the masked, unweighted image just formed (fixed order: per-thread
-      // partials, shuffle tree inside the row's lanes, then the row's warps in order):
-      //   src R: acc[a] = sum_x m R xi^a, a < nMomR
-      //   src S: acc[a] = sum_x m S xi^a, a < nMomS;  acc[ROW_NMA + a] = sum_x m xi^a, a < nMomA
-      double acc[2 * ROW_NMA];
 #pragma unroll
-      for (int q = 0; q < 2 * ROW_NMA; ++q) acc[q] = 0.0;
-      const bool isS = d.src == 1;
-      const int n0 = isS ? P.nMomS : P.nMomR, n1 = isS ? P.nMomA : 0;
+      for (int a = 0; a < ROW_NMA; ++a) {
+#pragma unroll
+        for (int off = LW / 2; off > 0; off >>= 1) ms[a] += __shfl_xor_sync(0xffffffffu, ms[a], off);
+      }
+    }
+    if ((tid & (LW - 1)) == 0) {
+#pragma unroll
+      for (int a = 0; a < ROW_NMA; ++a) redM[a][slot] = ms[a];
+    }
+  }
+
+  for (int im = 0; im < nimg; ++im) {
+    const int pw = im < P.nR ? im : 0;
+    if (mbits) {
 #pragma unroll
       for (int e = 0; e < EPT; ++e) {
-        const int j = tr + e * TPR;
-        const double x0 = (double)(4 * j + 1 - W) * invW, x1 = (double)(4 * j + 3 - W) * invW;
-        double f0 = v[e].x, f1 = v[e].y;
-        double p0 = ((mb >> (2 * e)) & 1u) ? 0.0 : 1.0, p1 = ((mb >> (2 * e + 1)) & 1u) ? 0.0 : 1.0;
-#pragma unroll
-        for (int a = 0; a < ROW_NMA; ++a) {
-          if (a < n0) { acc[a] += f0 + f1; f0 *= x0; f1 *= x1; }
-          if (a < n1) { acc[ROW_NMA + a] += p0 + p1; p0 *= x0; p1 *= x1; }
-        }
+        if ((mbits >> (2 * e)) & 1u) raw[e].x = 0.0;
+        if ((mbits >> (2 * e + 1)) & 1u) raw[e].y = 0.0;
       }
-      constexpr int LW = TPR < 32 ? TPR : 32;        // lanes of one row inside a warp
-      constexpr int WPR = TPR / 32 > 0 ? TPR / 32 : 1;  // warps per row
+    }
+    cplx v[EPT];
+    switch (pw) {
+      case 0:
 #pragma unroll
-      for (int q = 0; q < 2 * ROW_NMA; ++q) {
-#pragma unroll
-        for (int off = LW / 2; off > 0; off >>= 1) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], off);
+        for (int e = 0; e < EPT; ++e) v[e] = raw[e];
+        break;
+      case 1: row_weight<EPT, 1>(raw, v, xb, step, dx1); break;
+      case 2: row_weight<EPT, 2>(raw, v, xb, step, dx1); break;
+      default: row_weight<EPT, 3>(raw, v, xb, step, dx1); break;
+    }
+    const bool extra = P.moments && P.DB > 0 && im >= P.nR - 1;
+    if (extra) {
+      double hi[SFFT_MAX_DEG];
+      switch (P.DB) {
+        case 1: row_extra_moments<EPT, 1>(v, xb, step, dx1, hi); break;
+        case 2: row_extra_moments<EPT, 2>(v, xb, step, dx1, hi); break;
+        default: row_extra_moments<EPT, 3>(v, xb, step, dx1, hi); break;
       }
-      double* red = reinterpret_cast<double*>(smem_raw);   // [2*ROW_NMA][warps]; s is idle here
-      if (TPR > 32) {
-        if ((tid & 31) == 0) {
 #pragma unroll
-          for (int q = 0; q < 2 * ROW_NMA; ++q) red[q * (nth / 32) + (tid >> 5)] = acc[q];
-        }
-        __syncthreads();
-      }
-      if (tr == 0) {
-        const int base0 = isS ? P.nMomA : P.nMomA + P.nMomS;   // rowMom rows: mask, S, R families
+      for (int i = 0; i < SFFT_MAX_DEG; ++i) {
 #pragma unroll
-        for (int q = 0; q < 2 * ROW_NMA; ++q) {
-          double t = acc[q];
-          if (TPR > 32) {
-            t = 0.0;
-            for (int k = 0; k < WPR; ++k) t += red[q * (nth / 32) + (tid >> 5) + k];
-          }
-          if (q < ROW_NMA) { if (q < n0) P.rowMom[(size_t)(base0 + q) * H + y] = t; }
-          else if (q - ROW_NMA < n1) P.rowMom[(size_t)(q - ROW_NMA) * H + y] = t;
-        }
+        for (int off = LW / 2; off > 0; off >>= 1) hi[i] += __shfl_xor_sync(0xffffffffu, hi[i], off);
       }
-      if (TPR > 32) __syncthreads();
+      if ((tid & (LW - 1)) == 0) {
+#pragma unroll
+        for (int i = 0; i < SFFT_MAX_DEG; ++i) redX[i][slot] = hi[i];
+      }
     }
     fft_regs_to_smem<NC, -1, false>(v, s, tid, nth, RB, P.twP, C::SEQ_STRIDE);
     fetch(im + 1);
     // split: X[k] = Xe + w^k Xo, X[NC-k] = conj(Xe - w^k Xo), w = e^{-2 pi i / W}
-    cplx* out = P.T + ((size_t)im * H + y) * NC;
+    cplx* out = P.T + ((size_t)im * H + y) * P.pitchT;
     for (int k = tr; k <= NC / 2; k += TPR) {
       const cplx zk = srow[C::phys(k)];
       const cplx zm = cconj(srow[C::phys((NC - k) & (NC - 1))]);
       const cplx xe = cscale(cadd(zk, zm), 0.5);
       const cplx xo = cmul_mi(cscale(csub(zk, zm), 0.5));
       if (k == 0) {
-        out[0] = cmake(xe.x + xo.x, xe.x - xo.x);
+        const double dc = xe.x + xo.x, ny = xe.x - xo.x;
+        if (P.packed) {
+          out[0] = cmake(dc, ny);
+        } else {
+          out[0] = cmake(dc, 0.0);
+          out[NC] = cmake(ny, 0.0);
+        }
+        if (P.moments) {   // tr == 0 here: the row's moment writer
+          double* momS = P.rowMom + (size_t)P.nMomA * H + y;
+          double* momR = momS + (size_t)P.nMomS * H;
+          const int s0 = r * WPR;
+          if (im < P.nR) momR[(size_t)im * H] = dc; else momS[0] = dc;
+          if (extra) {
+            double* dst = im < P.nR ? momR + (size_t)P.nR * H : momS + H;
+            for (int i = 0; i < P.DB; ++i) {
+              double t = 0.0;
+              for (int k2 = 0; k2 < WPR; ++k2) t += redX[i][s0 + k2];
+              dst[(size_t)i * H] = t;
+            }
+          }
+          if (im == 0) {
+            for (int a = 0; a < P.nMomA; ++a) {
+              double t = 0.0;
+              for (int k2 = 0; k2 < WPR; ++k2) t += redM[a][s0 + k2];
+              P.rowMom[(size_t)a * H + y] = P.fullA[a] - t;
+            }
+          }
+        }
       } else {
         const cplx t = cmul(ldg2(P.twW + k), xo);
         out[k] = cadd(xe, t);
@@ -276,8 +349,6 @@ static sfft_status launch_row_fwd_t(const RowFwdParams& P, cudaStream_t st) {
   const int nth = row_threads(NC, P.H, C::EPT);
   const int RB = nth / (NC / C::EPT);
   size_t smem = (size_t)RB * C::SEQ_STRIDE * sizeof(cplx);
-  const size_t red = (size_t)2 * ROW_NMA * (nth / 32 + 1) * sizeof(double);
-  if (smem < red) smem = red;
   constexpr int MINB = 3;
   SFFT_CUDA_TRY(cudaFuncSetAttribute(k_row_fwd<NC, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   k_row_fwd<NC, MINB><<<P.H / RB, nth, smem, st>>>(P);
@@ -312,13 +383,15 @@ static sfft_status launch_row_inv_t(const RowInvParams& P, cudaStream_t st) {
   }
 
 sfft_status sfft_launch_row_fwd(sfft_plan* p, const double* R, const double* S,
-                                const unsigned char* mask, const RowImage* imgs, int nimg,
-                                cplx* Tout, bool moments, cudaStream_t st, int* nl) {
+                                const unsigned char* mask, bool build, cplx* Tout, int pitchT, bool packed,
+                                cudaStream_t st, int* nl) {
   RowFwdParams P;
-  P.R = R; P.S = S; P.mask = mask; P.H = p->H; P.W = p->W; P.nimg = nimg;
-  for (int i = 0; i < nimg; ++i) P.img[i] = imgs[i];
-  P.T = Tout; P.twP = p->twPNC; P.twW = p->twW;
-  P.moments = moments ? 1 : 0; P.nMomA = p->nMomA; P.nMomS = p->nMomS; P.nMomR = p->nMomR; P.rowMom = p->rowMom;
+  P.R = R; P.S = S; P.mask = mask; P.H = p->H; P.W = p->W;
+  P.nR = p->DK + 1; P.withS = build ? 1 : 0;
+  P.T = Tout; P.pitchT = pitchT; P.packed = packed ? 1 : 0; P.twP = p->twPNC; P.twW = p->twW;
+  P.moments = build ? 1 : 0; P.DB = p->DB; P.nMomA = p->nMomA; P.nMomS = p->nMomS; P.nMomR = p->nMomR;
+  P.rowMom = p->rowMom;
+  for (int a = 0; a < ROW_NMA; ++a) P.fullA[a] = p->fullA[a];
   ++*nl;
   SFFT_DISPATCH_NC(p->NC, launch_row_fwd_t)
 }

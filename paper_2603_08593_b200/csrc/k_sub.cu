@@ -149,10 +149,8 @@ sfft_status sfft_launch_row_inv_sub(sfft_plan* p, const double* S, const double*
 sfft_status sfft_launch_subtract(sfft_plan* p, const double* R, const double* S, const double* c,
                                  double* D, cudaStream_t st, int* nl) {
   // 1. row spectra of xi^p R (unmasked), p = 0..DK, into the row-pass scratch
-  RowImage imgs[SFFT_MAX_DEG + 1];
-  for (int q = 0; q <= p->DK; ++q) { imgs[q].src = 0; imgs[q].pxi = q; imgs[q].masked = 0; }
   sfft_status s;
-  { ProfScope ps(p, 6, st); s = sfft_launch_row_fwd(p, R, S, nullptr, imgs, p->DK + 1, p->T, false, st, nl); }
+  { ProfScope ps(p, 6, st); s = sfft_launch_row_fwd(p, R, S, nullptr, false, p->T, p->NC, true, st, nl); }
   if (s != SFFT_OK) return s;
   ProfScope* pmix = new ProfScope(p, 7, st);
   // 2. x-phase table of the kernel coefficients

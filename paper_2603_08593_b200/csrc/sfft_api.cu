@@ -68,6 +68,9 @@ static void plan_free(sfft_plan* p) {
   cudaFree(p->T); cudaFree(p->F); cudaFree(p->Y); cudaFree(p->Cmap); cudaFree(p->rowMom);
   cudaFree(p->mom); cudaFree(p->spCount); cudaFree(p->spOff); cudaFree(p->spList); cudaFree(p->kbPart); cudaFree(p->kbCorr); cudaFree(p->Lw); cudaFree(p->cholBar); cudaFree(p->Etab); cudaFree(p->Mhat);
   free(p->h_pairs);
+  if (p->side) cudaStreamDestroy(p->side);
+  if (p->evFork) cudaEventDestroy(p->evFork);
+  if (p->evJoin) cudaEventDestroy(p->evJoin);
   for (int i = 0; i < 2 * SFFT_PROF_MAX; ++i) if (p->prof_ev[i]) cudaEventDestroy(p->prof_ev[i]);
   delete p;
 }
@@ -117,6 +120,12 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   p->nMomS = DB + 1;
   p->nMomR = DK + DB + 1;
   p->ldL = (p->N + 1 + 3) & ~3;
+  for (int a = 0; a <= 2 * SFFT_MAX_DEG; ++a) {   // whole-row sums of xi^a (odd powers cancel exactly)
+    long double acc = 0.0L;
+    if ((a & 1) == 0)
+      for (int x = 0; x < W; ++x) acc += powl((long double)(2 * x + 1 - W) / (long double)W, (long double)a);
+    p->fullA[a] = (double)acc;
+  }
   int dev = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, dev);
@@ -153,6 +162,13 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
     if (cls == 0) { p->nGroupKK = ng; p->maxnsKK = maxns; } else { p->nGroupKO = ng; p->maxnsKO = maxns; }
   }
 
+  if (cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreateWithFlags(&p->evFork, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&p->evJoin, cudaEventDisableTiming) != cudaSuccess) {
+    cudaGetLastError();
+    plan_free(p);
+    return SFFT_ERR_CUDA;
+  }
   size_t ws = 0;
   bool ok = true;
   auto dalloc = [&](void** ptr, size_t bytes) {
@@ -221,19 +237,21 @@ sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S, co
   int nl = 0;
   // a1 + a2 (row pass): m xi^p R (p<=DK), m S, with the fused moment reductions
   // (sum m xi^a, sum m S xi^p, sum m R xi^a)
-  RowImage imgs[8];
-  int n = 0;
-  for (int q = 0; q <= p->DK; ++q) { imgs[n].src = 0; imgs[n].pxi = q; imgs[n].masked = 1; ++n; }
-  imgs[n].src = 1; imgs[n].pxi = 0; imgs[n].masked = 1; ++n;
   sfft_status s;
-  { ProfScope ps(p, 0, st); s = sfft_launch_row_fwd(p, R, S, mask, imgs, n, p->T, true, st, &nl); }
+  // the sparse part of the kernel-background block reads only R and the mask: it runs on the
+  // plan's side stream, concurrently with the transforms, and is joined before the gather
+  SFFT_CUDA_TRY(cudaEventRecord(p->evFork, st));
+  SFFT_CUDA_TRY(cudaStreamWaitEvent(p->side, p->evFork, 0));
+  { ProfScope ps(p, 9, p->side); s = sfft_launch_kb(p, R, mask, p->side, &nl); }
+  if (s != SFFT_OK) return s;
+  SFFT_CUDA_TRY(cudaEventRecord(p->evJoin, p->side));
+  { ProfScope ps(p, 0, st); s = sfft_launch_row_fwd(p, R, S, mask, true, p->T, p->NC, true, st, &nl); }
   if (s != SFFT_OK) return s;
   { ProfScope ps(p, 1, st); s = sfft_launch_col_fwd(p, st, &nl); }  // a2 (column pass, applies eta^q)
   if (s != SFFT_OK) return s;
   s = sfft_launch_cross(p, st, &nl);         // a3 (cross products + lag-pruned inverse along ky)
   if (s != SFFT_OK) return s;
-  { ProfScope ps(p, 9, st); s = sfft_launch_kb(p, R, mask, st, &nl); }  // kernel-background block, sparse part
-  if (s != SFFT_OK) return s;
+  SFFT_CUDA_TRY(cudaStreamWaitEvent(st, p->evJoin, 0));
   { ProfScope ps(p, 4, st); s = sfft_launch_lag_gather(p, A, b, st, &nl); }  // a3 (kx inverse on lag rows) + a4
   if (s != SFFT_OK) return s;
   p->launches[0] = nl;

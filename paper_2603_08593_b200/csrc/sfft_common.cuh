@@ -57,13 +57,6 @@ __device__ __forceinline__ double ipow(double x, int n) {
   return r;
 }
 
-// One image produced by the forward row pass: src (0 = R, 1 = S, 2 = all-ones), xi power, masked.
-struct RowImage {
-  int src;
-  int pxi;
-  int masked;
-};
-
 // A cross-correlation pair: spectra indices into the plan's spectrum array and its lag half-range.
 struct PairDesc {
   int fa;   // spectrum index of f  (conj side)
@@ -95,6 +88,7 @@ struct sfft_plan {
   int nMomA;     // 2*DB+1 row moments  sum_x m xi^a
   int nMomS;     // DB+1 row moments     sum_x m xi^p S
   int nMomR;     // DK+DB+1 row moments  sum_x m xi^a R
+  double fullA[2 * SFFT_MAX_DEG + 1];   // sum_x xi(x)^a over one whole row (long double on the host)
 
   // device tables
   cplx* twPNC;   // per-pass FFT twiddle tables for length NC (fft_smem.cuh)
@@ -128,6 +122,10 @@ struct sfft_plan {
   size_t ws_bytes;
   int launches[3];
   int num_sms;
+  // plan-owned side stream: stages of one call that do not depend on each other run concurrently
+  // (forked from and joined back into the caller stream with events; no host synchronisation)
+  cudaStream_t side;
+  cudaEvent_t evFork, evJoin;
   // optional per-stage CUDA-event timing (sfft_profile_*): events are recorded on the caller
   // stream around each stage; nothing synchronises until sfft_profile_read.
   int prof_on;
@@ -165,9 +163,10 @@ struct ProfScope {  // RAII: record an event pair around one stage when profilin
   } while (0)
 
 // ---- stage entry points implemented in the k_*.cu files (host functions) ----------------------
+// build = true: images m xi^p R (p <= DK) and m S with the fused row moments; false: xi^p R only
 sfft_status sfft_launch_row_fwd(sfft_plan* p, const double* R, const double* S,
-                                const unsigned char* mask, const RowImage* imgs, int nimg,
-                                cplx* Tout, bool moments, cudaStream_t st, int* nl);
+                                const unsigned char* mask, bool build, cplx* Tout, int pitchT, bool packed,
+                                cudaStream_t st, int* nl);
 sfft_status sfft_launch_col_fwd(sfft_plan* p, cudaStream_t st, int* nl);
 sfft_status sfft_launch_cross(sfft_plan* p, cudaStream_t st, int* nl);
 sfft_status sfft_launch_kb(sfft_plan* p, const double* R, const unsigned char* mask, cudaStream_t st, int* nl);
