@@ -177,6 +177,8 @@ struct LagParams {
   double* Cmap;  // [nPair][nLag][nLag]; pair with half-range D uses rows/cols [0, 2D]
   const PairDesc* pairs;
   int NC, W, pitch, nLag;
+  int nPart;            // partial lag-row sets (residue classes of k_colx), added in order
+  size_t partStride;    // elements between two sets
   double invP;
   const cplx* twW;
 };
@@ -197,7 +199,8 @@ __global__ void __launch_bounds__(LAG_TH) k_lag_idft(LagParams P) {
 #pragma unroll
   for (int dx = 0; dx <= LAG_MAXD; ++dx) { ap[dx] = 0.0; am[dx] = 0.0; }
   for (int kx = 1 + tid; kx < P.NC; kx += LAG_TH) {
-    const cplx y = Yr[kx];
+    cplx y = Yr[kx];
+    for (int q = 1; q < P.nPart; ++q) y = cadd(y, Yr[kx + q * P.partStride]);
     ap[0] += y.x;
 #pragma unroll
     for (int dx = 1; dx <= LAG_MAXD; ++dx) {
@@ -226,7 +229,8 @@ __global__ void __launch_bounds__(LAG_TH) k_lag_idft(LagParams P) {
     double sp = 0.0, sm = 0.0;
     for (int k = 0; k < LAG_TH / 32; ++k) { sp += red[0][dx][k]; sm += red[1][dx][k]; }
     if (dx == 0) sm = sp;
-    const double y0 = Yr[0].x, yn = Yr[P.NC].x;
+    double y0 = Yr[0].x, yn = Yr[P.NC].x;
+    for (int q = 1; q < P.nPart; ++q) { y0 += Yr[q * P.partStride].x; yn += Yr[P.NC + q * P.partStride].x; }
     const double sgn = (dx & 1) ? -1.0 : 1.0;
     double* out = P.Cmap + ((size_t)pair * P.nLag + dyi) * P.nLag;
     out[D + dx] = (y0 + sgn * yn + 2.0 * sp) * P.invP;
@@ -352,6 +356,7 @@ sfft_status sfft_launch_lag_gather(sfft_plan* p, double* A, double* b, cudaStrea
   LP.Y = p->Y; LP.Cmap = p->Cmap; LP.pairs = p->d_pairs; LP.NC = p->NC; LP.W = p->W;
   LP.pitch = p->pitch; LP.nLag = p->nLag; LP.invP = 1.0 / ((double)p->H * (double)p->W);
   LP.twW = p->twW;
+  LP.nPart = p->nPart; LP.partStride = (size_t)p->nPair * p->nLag * p->pitch;
   dim3 g1(p->nPair, p->nLag);
   k_lag_idft<<<g1, LAG_TH, 0, st>>>(LP);
   SFFT_LAUNCH_CHECK();

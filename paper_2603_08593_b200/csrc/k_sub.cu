@@ -150,7 +150,7 @@ sfft_status sfft_launch_subtract(sfft_plan* p, const double* R, const double* S,
                                  double* D, cudaStream_t st, int* nl) {
   // 1. row spectra of xi^p R (unmasked), p = 0..DK, into the row-pass scratch
   sfft_status s;
-  { ProfScope ps(p, 6, st); s = sfft_launch_row_fwd(p, R, S, nullptr, false, p->T, p->NC, true, st, nl); }
+  { ProfScope ps(p, 6, st); s = sfft_launch_row_fwd(p, R, S, nullptr, false, p->T, p->NC, true, false, st, nl); }
   if (s != SFFT_OK) return s;
   ProfScope* pmix = new ProfScope(p, 7, st);
   // 2. x-phase table of the kernel coefficients

@@ -64,6 +64,7 @@ static cudaError_t upload_pass_tables(cplx** dst, int n) {
 
 static void plan_free(sfft_plan* p) {
   if (!p) return;
+  cudaFree(p->twP512);
   cudaFree(p->twPNC); cudaFree(p->twPH); cudaFree(p->twW); cudaFree(p->twH); cudaFree(p->d_pairs); cudaFree(p->d_groups);
   cudaFree(p->T); cudaFree(p->F); cudaFree(p->Y); cudaFree(p->Cmap); cudaFree(p->rowMom);
   cudaFree(p->mom); cudaFree(p->spCount); cudaFree(p->spOff); cudaFree(p->spList); cudaFree(p->kbPart); cudaFree(p->kbCorr); cudaFree(p->Lw); cudaFree(p->cholBar); cudaFree(p->Etab); cudaFree(p->Mhat);
@@ -120,6 +121,9 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   p->nMomS = DB + 1;
   p->nMomR = DK + DB + 1;
   p->ldL = (p->N + 1 + 3) & ~3;
+  p->fused = sfft_colx_supported(H, p->nPair) ? 1 : 0;
+  p->nPart = p->fused ? H / 512 : 1;
+  p->pitchT = p->fused ? p->NC + 8 : p->NC;
   for (int a = 0; a <= 2 * SFFT_MAX_DEG; ++a) {   // whole-row sums of xi^a (odd powers cancel exactly)
     long double acc = 0.0L;
     if ((a & 1) == 0)
@@ -177,9 +181,14 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
     ws += bytes;
   };
   const size_t HN = (size_t)H * p->NC, HP = (size_t)H * p->pitch;
-  dalloc((void**)&p->T, sizeof(cplx) * HN * p->nRowImg);
-  dalloc((void**)&p->F, sizeof(cplx) * HP * p->nSpec);
-  dalloc((void**)&p->Y, sizeof(cplx) * (size_t)p->nPair * p->nLag * p->pitch);
+  // fused path: pair-major T[img][NC/2+1][H][2]; subtract always uses row-major packed [DK+1][H][NC]
+  size_t Tbytes = sizeof(cplx) * (size_t)H * p->pitchT * p->nRowImg;
+  if (p->fused) Tbytes = sizeof(cplx) * (size_t)H * 2 * (p->NC / 2 + 1) * p->nRowImg;
+  const size_t Fbytes = p->fused ? 256 : sizeof(cplx) * HP * p->nSpec;   // no spectra in HBM on the fused path
+  const size_t Ybytes = sizeof(cplx) * (size_t)p->nPart * p->nPair * p->nLag * p->pitch;
+  dalloc((void**)&p->T, Tbytes);
+  dalloc((void**)&p->F, Fbytes);
+  dalloc((void**)&p->Y, Ybytes);
   dalloc((void**)&p->Cmap, sizeof(double) * (size_t)p->nPair * p->nLag * p->nLag);
   dalloc((void**)&p->rowMom, sizeof(double) * (size_t)(p->nMomA + p->nMomS + p->nMomR) * H);
   dalloc((void**)&p->mom, sizeof(double) * (size_t)(p->nMomA * p->nMomA + p->TB + p->nMomR * p->nMomR));
@@ -198,13 +207,19 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   dalloc((void**)&p->d_pairs, sizeof(PairDesc) * p->nPair);
   dalloc((void**)&p->d_groups, sizeof(CrossGroup) * groups.size());
   if (!ok) { plan_free(p); return SFFT_ERR_ALLOC; }
+  if (p->fused && (upload_pass_tables(&p->twP512, 512) != cudaSuccess || sfft_colx_init() != SFFT_OK)) {
+    cudaGetLastError();
+    plan_free(p);
+    return SFFT_ERR_CUDA;
+  }
   if (upload_pass_tables(&p->twPNC, p->NC) != cudaSuccess || upload_pass_tables(&p->twPH, H) != cudaSuccess || upload_twiddles(&p->twW, W) != cudaSuccess ||
       upload_twiddles(&p->twH, H) != cudaSuccess ||
       cudaMemcpy(p->d_pairs, p->h_pairs, sizeof(PairDesc) * p->nPair, cudaMemcpyHostToDevice) != cudaSuccess ||
       cudaMemcpy(p->d_groups, groups.data(), sizeof(CrossGroup) * groups.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
       cudaMemset(p->cholBar, 0, 2 * sizeof(unsigned)) != cudaSuccess ||
-      cudaMemset(p->F, 0, sizeof(cplx) * HP * p->nSpec) != cudaSuccess ||
-      cudaMemset(p->Y, 0, sizeof(cplx) * (size_t)p->nPair * p->nLag * p->pitch) != cudaSuccess ||
+      cudaMemset(p->T, 0, Tbytes) != cudaSuccess ||
+      cudaMemset(p->F, 0, Fbytes) != cudaSuccess ||
+      cudaMemset(p->Y, 0, Ybytes) != cudaSuccess ||
       cudaMemset(p->Cmap, 0, sizeof(double) * (size_t)p->nPair * p->nLag * p->nLag) != cudaSuccess) {
     cudaGetLastError();
     plan_free(p);
@@ -245,11 +260,17 @@ sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S, co
   { ProfScope ps(p, 9, p->side); s = sfft_launch_kb(p, R, mask, p->side, &nl); }
   if (s != SFFT_OK) return s;
   SFFT_CUDA_TRY(cudaEventRecord(p->evJoin, p->side));
-  { ProfScope ps(p, 0, st); s = sfft_launch_row_fwd(p, R, S, mask, true, p->T, p->NC, true, st, &nl); }
+  { ProfScope ps(p, 0, st); s = sfft_launch_row_fwd(p, R, S, mask, true, p->T, p->pitchT, !p->fused, p->fused != 0, st, &nl); }
   if (s != SFFT_OK) return s;
-  { ProfScope ps(p, 1, st); s = sfft_launch_col_fwd(p, st, &nl); }  // a2 (column pass, applies eta^q)
-  if (s != SFFT_OK) return s;
-  s = sfft_launch_cross(p, st, &nl);         // a3 (cross products + lag-pruned inverse along ky)
+  if (p->fused) {
+    // a2 (column pass, applies eta^q) + a3 (cross products + lag-pruned inverse along ky), fused
+    ProfScope ps(p, 1, st);
+    s = sfft_launch_colx(p, st, &nl);
+  } else {
+    { ProfScope ps(p, 1, st); s = sfft_launch_col_fwd(p, st, &nl); }
+    if (s != SFFT_OK) return s;
+    s = sfft_launch_cross(p, st, &nl);
+  }
   if (s != SFFT_OK) return s;
   SFFT_CUDA_TRY(cudaStreamWaitEvent(st, p->evJoin, 0));
   { ProfScope ps(p, 4, st); s = sfft_launch_lag_gather(p, A, b, st, &nl); }  // a3 (kx inverse on lag rows) + a4
