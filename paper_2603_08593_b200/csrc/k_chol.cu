@@ -75,21 +75,23 @@ __device__ __forceinline__ double rcp_newton(double a) {  // 1/a for normal posi
   return fma(r, fma(e, e, e), r);
 }
 
-// Cholesky of the 32x32 block in sd (lower triangle) by the whole CTA.  The 32 dependent steps run
-// the square-root-free elimination a_ij -= a_ik a_jk / a_kk; the columns are scaled by
-// 1/sqrt(pivot) afterwards, which gives exactly the Cholesky factor.  Thread (warp w, lane j) keeps
-// its elements (4w..4w+3, j) in registers for the whole elimination; per step only the pivot
-// column travels through shared memory (double buffered, so one barrier per step), which keeps
-// the step at 4 shared loads per thread.  srd receives 1/L_jj.  Returns the 0-based index of the
-// first non-positive pivot (or -1); failed pivots are replaced by 1 so the work stays finite.
-__device__ __forceinline__ int cta_potrf32(double (*sd)[CH_NB + 1], double* srd, double (*colb)[CH_NB],
-                                           int tid) {
+#define CH_PB 64              // panel width (two 32-blocks factored inside the CTA)
+#define CH_LDS (CH_PB + 1)    // row pitch of the 64x64 shared arrays
+
+// Cholesky of a 32x32 block (lower triangle, row pitch CH_LDS) in shared memory by the whole CTA.
+// The 32 dependent steps run the square-root-free elimination a_ij -= a_ik a_jk / a_kk; the
+// columns are scaled by 1/sqrt(pivot) afterwards, which gives exactly the Cholesky factor.
+// Thread (warp w, lane j) keeps its elements (4w..4w+3, j) in registers for the whole elimination;
+// per step only the pivot column travels through shared memory (double buffered, so one barrier
+// per step).  srd receives 1/L_jj.  Returns the 0-based index of the first non-positive pivot (or
+// -1); failed pivots are replaced by 1 so the work stays finite.
+__device__ __forceinline__ int cta_potrf32(double* sd, double* srd, double (*colb)[CH_NB], int tid) {
   static_assert(CH_WARPS == 8, "row ownership below assumes 8 warps x 4 rows");
   const int j = tid & 31, i0 = (tid >> 5) * 4;
   double c[4];
   __syncthreads();  // sd was just filled by other threads
 #pragma unroll
-  for (int rr = 0; rr < 4; ++rr) c[rr] = sd[i0 + rr][j];
+  for (int rr = 0; rr < 4; ++rr) c[rr] = sd[(i0 + rr) * CH_LDS + j];
   if (j == 0) {
 #pragma unroll
     for (int rr = 0; rr < 4; ++rr) colb[0][i0 + rr] = c[rr];
@@ -134,7 +136,7 @@ __device__ __forceinline__ int cta_potrf32(double (*sd)[CH_NB + 1], double* srd,
 #pragma unroll
   for (int rr = 0; rr < 4; ++rr) {
     const int i = i0 + rr;
-    sd[i][j] = (i == j) ? d : (i > j ? div_by(c[rr], d, r) : 0.0);
+    sd[i * CH_LDS + j] = (i == j) ? d : (i > j ? div_by(c[rr], d, r) : 0.0);
   }
   __syncthreads();
   if (i0 == 0) srd[j] = r;
@@ -142,14 +144,84 @@ __device__ __forceinline__ int cta_potrf32(double (*sd)[CH_NB + 1], double* srd,
   return bad;
 }
 
+// Cholesky of the 64x64 block sd (row pitch CH_LDS) by the whole CTA as a 2x2 recursion on
+// 32-blocks: potrf(A11); X = A21 L11^-T by row substitution (4 rows per warp, interleaved chains);
+// A22 -= X X^T; potrf(A22).  ss receives the column-scaled factor ss[i][j] = L[i][j] / L[j][j] and
+// srd the reciprocals 1/L_jj of all 64 columns.  Returns the first bad pivot (or -1).
+__device__ __forceinline__ int cta_potrf64(double* sd, double* ss, double* srd, double (*colb)[CH_NB], int tid) {
+  const int lane = tid & 31, wrp = tid >> 5;
+  CH_STAMP(200)
+  int bad = cta_potrf32(sd, srd, colb, tid);
+  CH_STAMP(201)
+  // ss11 (needed by the substitution below)
+  for (int e = tid; e < CH_NB * CH_NB; e += CH_THREADS) {
+    const int i = e >> 5, j = e & 31;
+    ss[i * CH_LDS + j] = sd[i * CH_LDS + j] * srd[j];
+  }
+  __syncthreads();
+  {  // rows 32 + 4 wrp .. +3: x_j = a_j / L_jj, a_m -= a_j ss[m][j]
+    double x[4];
+#pragma unroll
+    for (int rr = 0; rr < 4; ++rr) x[rr] = sd[(CH_NB + 4 * wrp + rr) * CH_LDS + lane];
+#pragma unroll
+    for (int j = 0; j < CH_NB - 1; ++j) {
+      const double sj = ss[lane * CH_LDS + j];
+#pragma unroll
+      for (int rr = 0; rr < 4; ++rr) {
+        const double aj = __shfl_sync(0xffffffffu, x[rr], j);
+        if (lane > j) x[rr] = fma(-aj, sj, x[rr]);
+      }
+    }
+    const double d = sd[lane * CH_LDS + lane], r = srd[lane];
+#pragma unroll
+    for (int rr = 0; rr < 4; ++rr) sd[(CH_NB + 4 * wrp + rr) * CH_LDS + lane] = div_by(x[rr], d, r);
+  }
+  __syncthreads();
+  CH_STAMP(202)
+  {  // A22 -= L21 L21^T on the lower triangle (outputs (ty, ty+16) x (tx, tx+16))
+    const int tx = tid & 15, ty = tid >> 4;
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    const double* ri0 = sd + (CH_NB + ty) * CH_LDS, *ri1 = sd + (CH_NB + ty + 16) * CH_LDS;
+    const double* rj0 = sd + (CH_NB + tx) * CH_LDS, *rj1 = sd + (CH_NB + tx + 16) * CH_LDS;
+#pragma unroll
+    for (int m = 0; m < CH_NB; ++m) {
+      const double a0 = ri0[m], a1 = ri1[m], b0 = rj0[m], b1 = rj1[m];
+      acc[0] = fma(a0, b0, acc[0]);
+      acc[1] = fma(a0, b1, acc[1]);
+      acc[2] = fma(a1, b0, acc[2]);
+      acc[3] = fma(a1, b1, acc[3]);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const int i = ty + 16 * (q >> 1), j = tx + 16 * (q & 1);
+      if (j <= i) sd[(CH_NB + i) * CH_LDS + CH_NB + j] -= acc[q];
+    }
+  }
+  CH_STAMP(203)
+  const int bad2 = cta_potrf32(sd + CH_NB * CH_LDS + CH_NB, srd + CH_NB, colb, tid);
+  CH_STAMP(204)
+  if (bad < 0 && bad2 >= 0) bad = CH_NB + bad2;
+  for (int e = tid; e < CH_PB * CH_PB; e += CH_THREADS) {
+    const int i = e >> 6, j = e & 63;
+    if (i >= CH_NB || j >= CH_NB) ss[i * CH_LDS + j] = (j <= i) ? sd[i * CH_LDS + j] * srd[j] : 0.0;
+  }
+  __syncthreads();
+  return bad;
+}
+
 __global__ void __launch_bounds__(CH_THREADS, 1)
 k_chol_fused(const double* __restrict__ A, const double* __restrict__ b, double* Lw,
              int N, int ld, int* info, unsigned* bar) {
-  __shared__ double sd[CH_NB][CH_NB + 1];      // factored diagonal block
-  __shared__ double srd[CH_NB];                // reciprocals of its diagonal
+  // shared memory: panel phase  sd[64][65] (factored diagonal block), ss[64][65] (column-scaled);
+  //                update phase pi[32][65], pj[32][65] (aliasing sd / ss)
+  extern __shared__ __align__(16) double ch_smem[];
+  double* sd = ch_smem;
+  double* ss = sd + CH_PB * CH_LDS;
+  double* pi = sd;
+  double* pj = ss;
+  __shared__ double srd[CH_PB];                    // reciprocals of the diagonal
   __shared__ __align__(16) double colb[2][CH_NB];  // pivot column exchange of cta_potrf32
-  __shared__ double ss[CH_NB][CH_NB + 1];      // ss[m][j] = L[m][j] / L[j][j] (panel substitution)
-  __shared__ double pi[CH_NB][CH_NB + 1], pj[CH_NB][CH_NB + 1];
   const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
   const unsigned nblocks = gridDim.x;
   unsigned target = 0;
@@ -171,54 +243,60 @@ k_chol_fused(const double* __restrict__ A, const double* __restrict__ b, double*
   (void)stamp;
 
   const int gw = blockIdx.x * CH_WARPS + wrp, ngw = nblocks * CH_WARPS;
-  for (int k0 = 0; k0 < N; k0 += CH_NB) {
-    const int nb = min(CH_NB, N - k0);
+  for (int k0 = 0; k0 < N; k0 += CH_PB) {
+    const int nb = min(CH_PB, N - k0);
     const int rbelow = k0 + nb;                 // first row below the diagonal block
     // ---- panel phase: CTAs that own panel rows (and CTA 0) factor the diagonal block
     const bool has_rows = blockIdx.x * CH_WARPS < (N + 1 - rbelow);
     if (has_rows || blockIdx.x == 0) {
-      for (int e = tid; e < CH_NB * CH_NB; e += CH_THREADS) {
-        const int i = e >> 5, j = e & 31;
-        sd[i][j] = (i < nb && j <= i) ? ld_cg(Lw + (size_t)(k0 + i) * ld + k0 + j) : (i == j ? 1.0 : 0.0);
+      for (int e = tid; e < CH_PB * CH_PB; e += CH_THREADS) {
+        const int i = e >> 6, j = e & 63;
+        sd[i * CH_LDS + j] = (i < nb && j <= i) ? ld_cg(Lw + (size_t)(k0 + i) * ld + k0 + j) : (i == j ? 1.0 : 0.0);
       }
-      const int bad = cta_potrf32(sd, srd, colb, tid);
+      const int bad = cta_potrf64(sd, ss, srd, colb, tid);
       if (bad >= 0 && bad < nb && blockIdx.x == 0 && tid == 0 && info) atomicCAS(info, 0, k0 + bad + 1);
-      for (int e = tid; e < CH_NB * CH_NB; e += CH_THREADS) {
-        const int i = e >> 5, j = e & 31;
-        ss[i][j] = sd[i][j] * srd[j];
-      }
       if (blockIdx.x == 0) {
-        for (int e = tid; e < CH_NB * CH_NB; e += CH_THREADS) {
-          const int i = e >> 5, j = e & 31;
-          if (i < nb && j <= i) Lw[(size_t)(k0 + i) * ld + k0 + j] = sd[i][j];
+        for (int e = tid; e < CH_PB * CH_PB; e += CH_THREADS) {
+          const int i = e >> 6, j = e & 63;
+          if (i < nb && j <= i) Lw[(size_t)(k0 + i) * ld + k0 + j] = sd[i * CH_LDS + j];
         }
       }
-      __syncthreads();
       CH_STAMP(stamp + 0)
-      // rows below (including the rhs row N): one row per warp, lane j holds entry j
+      // rows below (including the rhs row N): one row per warp, lane holds entries lane and lane+32.
+      // x_j = a_j / L_jj, a_m -= x_j L_mj = a_j ss[m][j]: per step one shuffle and one fma on the
+      // dependent chain; the divisions are off it
       for (int row = rbelow + gw; row <= N; row += ngw) {
         double* src = Lw + (size_t)row * ld + k0;
-        double x = (lane < nb) ? ld_cg(src + lane) : 0.0;
-        // x_j = a_j / L_jj, a_m -= x_j L_mj = a_j (L_mj / L_jj): with the column-scaled factor
-        // ss the dependent chain per step is one shuffle and one fma; the division is off it
+        double x0 = (lane < nb) ? ld_cg(src + lane) : 0.0;
+        double x1 = (lane + CH_NB < nb) ? ld_cg(src + lane + CH_NB) : 0.0;
+        const double* s0 = ss + lane * CH_LDS, *s1 = ss + (lane + CH_NB) * CH_LDS;
+#pragma unroll
+        for (int j = 0; j < CH_NB; ++j) {
+          const double aj = __shfl_sync(0xffffffffu, x0, j);
+          if (lane > j) x0 = fma(-aj, s0[j], x0);
+          x1 = fma(-aj, s1[j], x1);
+        }
 #pragma unroll
         for (int j = 0; j < CH_NB - 1; ++j) {
-          const double aj = __shfl_sync(0xffffffffu, x, j);
-          if (lane > j) x = fma(-aj, ss[lane][j], x);
+          const double aj = __shfl_sync(0xffffffffu, x1, j);
+          if (lane > j) x1 = fma(-aj, s1[CH_NB + j], x1);
         }
-        if (lane < nb) src[lane] = div_by(x, sd[lane][lane], srd[lane]);
+        if (lane < nb) src[lane] = div_by(x0, sd[lane * CH_LDS + lane], srd[lane]);
+        if (lane + CH_NB < nb)
+          src[lane + CH_NB] = div_by(x1, sd[(lane + CH_NB) * CH_LDS + lane + CH_NB], srd[lane + CH_NB]);
       }
     }
     CH_STAMP(stamp + 1)
     grid_barrier(bar, target, nblocks);
     CH_STAMP(stamp + 2)
-    // ---- update phase: tiles (ti, tj), tj <= ti, of the trailing matrix starting at r0
-    const int r0 = k0 + CH_NB;
+    // ---- update phase: 32x32 tiles (ti, tj), tj <= ti, of the trailing matrix starting at r0,
+    //      A22 -= L21 L21^T with the panel's 64 columns
+    const int r0 = k0 + CH_PB;
     if (r0 <= N) {
       const int T = (N + 1 - r0 + CH_NB - 1) / CH_NB;
       const int ntile = T * (T + 1) / 2;
       const int tx = tid & 15, ty = tid >> 4;      // outputs (ty, ty+16) x (tx, tx+16)
-      double gpi[4], gpj[4], cur[4];
+      double gpi[8], gpj[8], cur[4];
       int ti = 0, tj = 0;
       auto decode = [&](int t, int& oi, int& oj) {   // t -> (ti, tj): ti(ti+1)/2 <= t
         int q = (int)((sqrt(8.0 * t + 1.0) - 1.0) * 0.5);
@@ -228,8 +306,8 @@ k_chol_fused(const double* __restrict__ A, const double* __restrict__ b, double*
       };
       auto fetch = [&](int fi, int fj) {
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const int e = tid + q * CH_THREADS, r = e >> 5, m = e & 31;
+        for (int q = 0; q < 8; ++q) {
+          const int e = tid + q * CH_THREADS, r = e >> 6, m = e & 63;
           const int gi = r0 + fi * CH_NB + r, gj = r0 + fj * CH_NB + r;
           gpi[q] = (gi <= N) ? ld_cg(Lw + (size_t)gi * ld + k0 + m) : 0.0;
           gpj[q] = (gj < N) ? ld_cg(Lw + (size_t)gj * ld + k0 + m) : 0.0;
@@ -245,10 +323,10 @@ k_chol_fused(const double* __restrict__ A, const double* __restrict__ b, double*
       while (t < ntile) {
         __syncthreads();
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const int e = tid + q * CH_THREADS, r = e >> 5, m = e & 31;
-          pi[r][m] = gpi[q];
-          pj[r][m] = gpj[q];
+        for (int q = 0; q < 8; ++q) {
+          const int e = tid + q * CH_THREADS, r = e >> 6, m = e & 63;
+          pi[r * CH_LDS + m] = gpi[q];
+          pj[r * CH_LDS + m] = gpj[q];
         }
         double c0[4] = {cur[0], cur[1], cur[2], cur[3]};
         const int ci = ti, cj = tj;
@@ -256,9 +334,11 @@ k_chol_fused(const double* __restrict__ A, const double* __restrict__ b, double*
         t += nblocks;
         if (t < ntile) { decode(t, ti, tj); fetch(ti, tj); }
         double acc[4] = {0.0, 0.0, 0.0, 0.0};
+        const double* a0p = pi + ty * CH_LDS, *a1p = pi + (ty + 16) * CH_LDS;
+        const double* b0p = pj + tx * CH_LDS, *b1p = pj + (tx + 16) * CH_LDS;
 #pragma unroll
-        for (int m = 0; m < CH_NB; ++m) {
-          const double a0 = pi[ty][m], a1 = pi[ty + 16][m], b0 = pj[tx][m], b1 = pj[tx + 16][m];
+        for (int m = 0; m < CH_PB; ++m) {
+          const double a0 = a0p[m], a1 = a1p[m], b0 = b0p[m], b1 = b1p[m];
           acc[0] = fma(a0, b0, acc[0]);
           acc[1] = fma(a0, b1, acc[1]);
           acc[2] = fma(a1, b0, acc[2]);
@@ -362,7 +442,9 @@ sfft_status sfft_launch_solve(sfft_plan* p, const double* A, const double* b, do
   int want = maxUseful > tiles ? maxUseful : tiles;
   if (want < 1) want = 1;
   if (grid > want) grid = want;
-  SFFT_CUDA_TRY(cudaLaunchCooperativeKernel((const void*)k_chol_fused, dim3(grid), dim3(CH_THREADS), args, 0, st));
+  const size_t smemF = (size_t)2 * CH_PB * CH_LDS * sizeof(double);
+  SFFT_CUDA_TRY(cudaFuncSetAttribute(k_chol_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smemF));
+  SFFT_CUDA_TRY(cudaLaunchCooperativeKernel((const void*)k_chol_fused, dim3(grid), dim3(CH_THREADS), args, smemF, st));
   ++*nl;
   const size_t smem = ((size_t)N + CH_NB * (CH_NB + 1) + 2 * CH_NB) * sizeof(double);
   k_chol_back<<<1, 1024, smem, st>>>(Lw, c, N, ld);

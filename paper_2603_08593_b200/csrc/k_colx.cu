@@ -48,9 +48,17 @@ struct ColxParams {
 // (fixed by the 512-point split, so one table serves every plan; written by sfft_colx_init).
 // Held in constant memory: with the b loop unrolled they are immediate operands of the DFMAs.
 #define CX_TWD 10
+#ifndef CX_UNROLL
+#define CX_UNROLL 4
+#endif
+constexpr int CXU = CX_UNROLL;   // unroll factor of the b loop in phase C
 __constant__ cplx cx_twlag[16][CX_TWD];
 
 __device__ __forceinline__ int cx_swz(int n) { return n ^ ((n >> 3) & 7); }
+__host__ __device__ __forceinline__ int cx_col_stride(int nSpec) {
+  const int n = nSpec * CX_PITCH;
+  return n + ((4 - (n & 7)) & 7);
+}
 
 // sum_m w_DR^{c m} x[m]: the residue-c output of a DR-point forward DFT (c is CTA-uniform)
 template <int DR>
@@ -170,6 +178,9 @@ __global__ void __launch_bounds__(CX_TH, 2) k_colx(ColxParams P) {
   const int kx0 = (blockIdx.x / DR) * 2;
   const int H = P.H, nSpec = P.nSpec;
   const double invH = 1.0 / (double)H;
+  // column 1's sequences start 4 (mod 8) elements after column 0's: the two columns of phase A's
+  // quarter-warp stores fall into disjoint bank groups
+  const int colStride = cx_col_stride(nSpec);
 
   // ---- phase A: load the two columns of every row image, decimate to the class, twiddle -------
   constexpr int KB = 16 / DR > 4 ? 4 : 16 / DR;    // items per thread and batch (KB*DR loads in flight)
@@ -191,7 +202,7 @@ __global__ void __launch_bounds__(CX_TH, 2) k_colx(ColxParams P) {
         const int i = tid + CX_TH * (k0 + k), col = i & 1, yp = i >> 1;
         const cplx tw = ldg2(P.twH + c * yp);       // e^{-2 pi i c y'/H}; c*yp < H
         const double eta0 = (double)(2 * yp + 1 - H) * invH;
-        cplx* dst = sq + (size_t)(col * nSpec) * CX_PITCH + cx_swz(yp);
+        cplx* dst = sq + (size_t)col * colStride + cx_swz(yp);
         for (int q = 0; q < nq; ++q) {
           if (q > 0) {
 #pragma unroll
@@ -207,7 +218,8 @@ __global__ void __launch_bounds__(CX_TH, 2) k_colx(ColxParams P) {
   __syncthreads();
 
   // ---- phase B: one warp per sequence ---------------------------------------------------------
-  for (int sidx = wrp; sidx < 2 * nSpec; sidx += CX_NW) cx_warp_fft512(sq + (size_t)sidx * CX_PITCH, lane, P.twP);
+  for (int sidx = wrp; sidx < 2 * nSpec; sidx += CX_NW)
+    cx_warp_fft512(sq + (size_t)(sidx / nSpec) * colStride + (size_t)(sidx % nSpec) * CX_PITCH, lane, P.twP);
   __syncthreads();
 
   // ---- phase C: cross products + pruned inverse; lanes = pairs, warps = (column, b quarter) ----
@@ -219,12 +231,12 @@ __global__ void __launch_bounds__(CX_TH, 2) k_colx(ColxParams P) {
     const int pair = pg + lane;
     const bool has_pair = pair < P.nPair;
     const PairDesc pd = P.pairs[has_pair ? pair : 0];
-    const cplx* pa = sq + (size_t)(col * nSpec + pd.fa) * CX_PITCH;
-    const cplx* pb = sq + (size_t)(col * nSpec + pd.fb) * CX_PITCH;
+    const cplx* pa = sq + (size_t)col * colStride + (size_t)pd.fa * CX_PITCH;
+    const cplx* pb = sq + (size_t)col * colStride + (size_t)pd.fb * CX_PITCH;
     cplx acc[2 * D + 1];
 #pragma unroll
     for (int i = 0; i < 2 * D + 1; ++i) acc[i] = cmake(0.0, 0.0);
-#pragma unroll
+#pragma unroll CXU
     for (int bb = 0; bb < NBW; ++bb) {
       const int pbv = cx_swz(bq * NBW + bb);
       cplx x[8];
@@ -267,7 +279,7 @@ __global__ void __launch_bounds__(CX_TH, 2) k_colx(ColxParams P) {
 
 template <int DR, int D>
 static sfft_status launch_colx_t(const ColxParams& P, cudaStream_t st) {
-  size_t smem = (size_t)2 * P.nSpec * CX_PITCH * sizeof(cplx);
+  size_t smem = (size_t)2 * cx_col_stride(P.nSpec) * sizeof(cplx);
   const size_t red = (size_t)2 * CX_NBQ * (2 * D + 1) * 32 * sizeof(cplx);
   if (smem < red) smem = red;
   SFFT_CUDA_TRY(cudaFuncSetAttribute(k_colx<DR, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

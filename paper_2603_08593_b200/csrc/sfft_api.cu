@@ -166,7 +166,9 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
     if (cls == 0) { p->nGroupKK = ng; p->maxnsKK = maxns; } else { p->nGroupKO = ng; p->maxnsKO = maxns; }
   }
 
-  if (cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking) != cudaSuccess ||
+  int prLo = 0, prHi = 0;   // the side stream's small kernels take free slots ahead of the big grids
+  cudaDeviceGetStreamPriorityRange(&prLo, &prHi);
+  if (cudaStreamCreateWithPriority(&p->side, cudaStreamNonBlocking, prHi) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->evFork, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->evJoin, cudaEventDisableTiming) != cudaSuccess) {
     cudaGetLastError();
