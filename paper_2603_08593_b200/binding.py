@@ -17,7 +17,7 @@ _LIB_NAME = "libsfft.so"
 EXPORTED_SYMBOLS = [
     "sfft_plan_create", "sfft_plan_destroy", "sfft_num_coeffs", "sfft_workspace_bytes",
     "sfft_status_string", "sfft_build_system", "sfft_solve", "sfft_subtract",
-    "sfft_probe_fp64", "sfft_last_launch_count", "sfft_version",
+    "sfft_probe_fp64", "sfft_last_launch_count", "sfft_plan_fused", "sfft_version",
     "sfft_profile_enable", "sfft_profile_read",
 ]
 
@@ -71,6 +71,8 @@ def load_library():
     lib.sfft_probe_fp64.restype = i32
     lib.sfft_last_launch_count.argtypes = [vp, i32]
     lib.sfft_last_launch_count.restype = i32
+    lib.sfft_plan_fused.argtypes = [vp]
+    lib.sfft_plan_fused.restype = i32
     lib.sfft_profile_enable.argtypes = [vp, i32]
     lib.sfft_profile_enable.restype = i32
     lib.sfft_profile_read.argtypes = [vp, i32, dbl_p, ctypes.POINTER(i32), i32]
@@ -198,6 +200,11 @@ class SfftPlan:
     # -- diagnostics
     def last_launch_count(self, which: int) -> int:
         return int(self._lib.sfft_last_launch_count(self._p, which))
+
+    @property
+    def fused(self) -> bool:
+        """True if the plan runs the fused column-FFT + cross-spectra kernel (sfft_plan_fused)."""
+        return int(self._lib.sfft_plan_fused(self._p)) == 1
 
     def profile_enable(self, on: bool = True):
         _check(self._lib, self._lib.sfft_profile_enable(self._p, 1 if on else 0), "sfft_profile_enable")

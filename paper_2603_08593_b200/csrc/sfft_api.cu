@@ -342,6 +342,8 @@ sfft_status sfft_profile_read(sfft_plan* p, int stage, double* total_ms, int* co
   return SFFT_OK;
 }
 
+int sfft_plan_fused(const sfft_plan* p) { return p ? p->fused : -1; }
+
 int sfft_last_launch_count(const sfft_plan* p, int which) {
   if (!p || which < 0 || which > 2) return -1;
   return p->launches[which];
