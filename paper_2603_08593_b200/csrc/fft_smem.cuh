@@ -187,13 +187,17 @@ __device__ __forceinline__ void fft_map(int i, int nseq, int& seq, int& j) {
 }
 
 // twiddle + butterfly + Stockham store of one radix-R butterfly held in v[]
-template <int N, int R, int NS, int DIR>
-__device__ __forceinline__ void fft_twiddle_bfly(cplx* v, int j, const cplx* __restrict__ tw) {
+template <int N, int R, int NS>
+__device__ __forceinline__ void fft_twiddle_load(cplx* t, int j, const cplx* __restrict__ tw) {
   if constexpr (NS > 1) {
     const int k = j & (NS - 1);
-    cplx t[R];
 #pragma unroll
     for (int r = 1; r < R; ++r) t[r] = ldg2(tw + (r - 1) * NS + k);
+  }
+}
+template <int N, int R, int NS, int DIR>
+__device__ __forceinline__ void fft_twiddle_apply(cplx* v, cplx* t) {
+  if constexpr (NS > 1) {
 #pragma unroll
     for (int r = 1; r < R; ++r) {
       if (DIR > 0) t[r].y = -t[r].y;
@@ -201,6 +205,12 @@ __device__ __forceinline__ void fft_twiddle_bfly(cplx* v, int j, const cplx* __r
     }
   }
   Dft<R, DIR>::run(v);
+}
+template <int N, int R, int NS, int DIR>
+__device__ __forceinline__ void fft_twiddle_bfly(cplx* v, int j, const cplx* __restrict__ tw) {
+  cplx t[R];
+  fft_twiddle_load<N, R, NS>(t, j, tw);
+  fft_twiddle_apply<N, R, NS, DIR>(v, t);
 }
 template <int N, int R, int NS>
 __device__ __forceinline__ void fft_store(const cplx* v, cplx* base, int j) {
@@ -229,7 +239,15 @@ __device__ __forceinline__ void fft_pass(cplx* s, int tid, int nth, int nseq, co
   using C = FftCfg<N>;
   constexpr int NB = N / R;        // butterflies per sequence
   constexpr int IT = C::EPT / R;   // butterflies per thread
-  cplx v[IT][R];
+  cplx v[IT][R], t[IT][R];
+  // the twiddles do not depend on the data: their (global, L1/L2) loads are issued first so that
+  // their latency hides under the shared-memory reads and the barrier
+#pragma unroll
+  for (int m = 0; m < IT; ++m) {
+    int seq, j;
+    fft_map<NB, SEQ_FAST>(tid + m * nth, nseq, seq, j);
+    fft_twiddle_load<N, R, NS>(t[m], j, tw);
+  }
 #pragma unroll
   for (int m = 0; m < IT; ++m) {
     int seq, j;
@@ -243,7 +261,7 @@ __device__ __forceinline__ void fft_pass(cplx* s, int tid, int nth, int nseq, co
   for (int m = 0; m < IT; ++m) {
     int seq, j;
     fft_map<NB, SEQ_FAST>(tid + m * nth, nseq, seq, j);
-    fft_twiddle_bfly<N, R, NS, DIR>(v[m], j, tw);
+    fft_twiddle_apply<N, R, NS, DIR>(v[m], t[m]);
     fft_store<N, R, NS>(v[m], s + seq * seq_stride, j);
   }
   __syncthreads();
@@ -257,6 +275,13 @@ __device__ __forceinline__ void fft_pass_to_regs(const cplx* s, cplx* v, int tid
   using C = FftCfg<N>;
   constexpr int NB = N / R;
   constexpr int IT = C::EPT / R;
+  cplx t[IT][R];
+#pragma unroll
+  for (int m = 0; m < IT; ++m) {
+    int seq, j;
+    fft_map<NB, SEQ_FAST>(tid + m * nth, nseq, seq, j);
+    fft_twiddle_load<N, R, NS>(t[m], j, tw);
+  }
 #pragma unroll
   for (int m = 0; m < IT; ++m) {
     int seq, j;
@@ -266,11 +291,7 @@ __device__ __forceinline__ void fft_pass_to_regs(const cplx* s, cplx* v, int tid
     for (int r = 0; r < R; ++r) v[m * R + r] = base[C::phys(j + r * NB)];
   }
 #pragma unroll
-  for (int m = 0; m < IT; ++m) {
-    int seq, j;
-    fft_map<NB, SEQ_FAST>(tid + m * nth, nseq, seq, j);
-    fft_twiddle_bfly<N, R, NS, DIR>(v + m * R, j, tw);
-  }
+  for (int m = 0; m < IT; ++m) fft_twiddle_apply<N, R, NS, DIR>(v + m * R, t[m]);
 }
 
 template <int N, int PASS, int DIR, bool SEQ_FAST>

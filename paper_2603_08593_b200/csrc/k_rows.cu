@@ -33,6 +33,21 @@ struct RowFwdParams {
 };
 
 #define ROW_NMA (2 * SFFT_MAX_DEG + 1)   // most mask moments
+// streaming (evict-first) accesses for the bulk data keep the twiddle tables resident in L1
+#define SFFT_ROW_STREAM 1
+#ifdef SFFT_ROW_STREAM
+#define ROW_LD(p) __ldcs(p)
+#define ROW_ST(p, v) __stcs(p, v)
+#else
+#define ROW_LD(p) (*(p))
+#define ROW_ST(p, v) (*(p) = (v))
+#endif
+#ifndef SFFT_ROW_NBT
+#define SFFT_ROW_NBT 2    // bins of the split step loaded per batch
+#endif
+#ifndef SFFT_ROW_MINB
+#define SFFT_ROW_MINB 3   // CTAs per SM the row kernels are compiled for
+#endif
 
 // v[e] = raw[e] * (x0^PW, x1^PW): x0 = xi(2j), x1 = xi(2j+1), j = tr + e*TPR; xi(2j) = xb + e*step
 // (all values are multiples of 1/W, so the affine form is exact).
@@ -116,7 +131,7 @@ __global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
     if (im < nimg) {
       const double* src = (im < P.nR ? P.R : P.S) + rowoff;
 #pragma unroll
-      for (int e = 0; e < EPT; ++e) raw[e] = *reinterpret_cast<const double2*>(src + 2 * (tr + e * TPR));
+      for (int e = 0; e < EPT; ++e) raw[e] = ROW_LD(reinterpret_cast<const double2*>(src + 2 * (tr + e * TPR)));
     } else {
 #pragma unroll
       for (int e = 0; e < EPT; ++e) raw[e] = make_double2(0.0, 0.0);
@@ -195,19 +210,34 @@ __global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
     // element k of this row: row-major out[k], or pair-major ((im*NP + k/2)*H + y)*2 + k%2
     cplx* out = P.pairT ? P.T + ((size_t)im * (NC / 2 + 1) * H + y) * 2 : P.T + ((size_t)im * H + y) * P.pitchT;
     const size_t kmul = P.pairT ? (size_t)H * 2 : 2;   // offset of column pair k/2
-    auto at = [&](int k) -> cplx& { return out[(size_t)(k >> 1) * kmul + (k & 1)]; };
-    for (int k = tr; k <= NC / 2; k += TPR) {
-      const cplx zk = srow[C::phys(k)];
-      const cplx zm = cconj(srow[C::phys((NC - k) & (NC - 1))]);
-      const cplx xe = cscale(cadd(zk, zm), 0.5);
-      const cplx xo = cmul_mi(cscale(csub(zk, zm), 0.5));
-      if (k == 0) {
+    auto at = [&](int k) -> cplx* { return out + (size_t)(k >> 1) * kmul + (k & 1); };
+    // all twiddles and sequence elements of the thread's NIT bins are requested up front (the loop
+    // is latency bound otherwise: one shared and one global load chain per bin)
+    constexpr int NIT = (NC / 2) / TPR;
+    constexpr int NBT = NIT >= SFFT_ROW_NBT ? SFFT_ROW_NBT : NIT;   // bins per batch (register budget: raw[] is live here)
+#pragma unroll 1
+    for (int i0 = 0; i0 < NIT; i0 += NBT) {
+    cplx tws[NBT], zks[NBT], zms[NBT];
+#pragma unroll
+    for (int i = 0; i < NBT; ++i) tws[i] = ldg2(P.twW + tr + (i0 + i) * TPR);
+#pragma unroll
+    for (int i = 0; i < NBT; ++i) {
+      const int k = tr + (i0 + i) * TPR;
+      zks[i] = srow[C::phys(k)];
+      zms[i] = cconj(srow[C::phys((NC - k) & (NC - 1))]);
+    }
+#pragma unroll
+    for (int i = 0; i < NBT; ++i) {
+      const int k = tr + (i0 + i) * TPR;
+      const cplx xe = cscale(cadd(zks[i], zms[i]), 0.5);
+      const cplx xo = cmul_mi(cscale(csub(zks[i], zms[i]), 0.5));
+      if (i0 + i == 0 && tr == 0) {
         const double dc = xe.x + xo.x, ny = xe.x - xo.x;
         if (P.packed) {
           out[0] = cmake(dc, ny);
         } else {
-          at(0) = cmake(dc, 0.0);
-          at(NC) = cmake(ny, 0.0);
+          ROW_ST(at(0), cmake(dc, 0.0));
+          ROW_ST(at(NC), cmake(ny, 0.0));
         }
         if (P.moments) {   // tr == 0 here: the row's moment writer
           double* momS = P.rowMom + (size_t)P.nMomA * H + y;
@@ -216,10 +246,10 @@ __global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
           if (im < P.nR) momR[(size_t)im * H] = dc; else momS[0] = dc;
           if (extra) {
             double* dst = im < P.nR ? momR + (size_t)P.nR * H : momS + H;
-            for (int i = 0; i < P.DB; ++i) {
+            for (int ii = 0; ii < P.DB; ++ii) {
               double t = 0.0;
-              for (int k2 = 0; k2 < WPR; ++k2) t += redX[i][s0 + k2];
-              dst[(size_t)i * H] = t;
+              for (int k2 = 0; k2 < WPR; ++k2) t += redX[ii][s0 + k2];
+              dst[(size_t)ii * H] = t;
             }
           }
           if (im == 0) {
@@ -231,10 +261,18 @@ __global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
           }
         }
       } else {
-        const cplx t = cmul(ldg2(P.twW + k), xo);
-        at(k) = cadd(xe, t);
-        if (k != NC - k) at(NC - k) = cconj(csub(xe, t));
+        const cplx t = cmul(tws[i], xo);
+        ROW_ST(at(k), cadd(xe, t));
+        ROW_ST(at(NC - k), cconj(csub(xe, t)));
       }
+    }
+    }
+    if (tr == 0) {   // the middle bin k = NC/2 pairs with itself
+      const cplx z = srow[C::phys(NC / 2)];
+      const cplx zc = cconj(z);
+      const cplx xe = cscale(cadd(z, zc), 0.5);
+      const cplx xo = cmul_mi(cscale(csub(z, zc), 0.5));
+      ROW_ST(at(NC / 2), cadd(xe, cmul(ldg2(P.twW + NC / 2), xo)));
     }
     __syncthreads();
   }
@@ -353,7 +391,7 @@ static sfft_status launch_row_fwd_t(const RowFwdParams& P, cudaStream_t st) {
   const int nth = row_threads(NC, P.H, C::EPT);
   const int RB = nth / (NC / C::EPT);
   size_t smem = (size_t)RB * C::SEQ_STRIDE * sizeof(cplx);
-  constexpr int MINB = 3;
+  constexpr int MINB = SFFT_ROW_MINB;
   SFFT_CUDA_TRY(cudaFuncSetAttribute(k_row_fwd<NC, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   k_row_fwd<NC, MINB><<<P.H / RB, nth, smem, st>>>(P);
   SFFT_LAUNCH_CHECK();
@@ -366,7 +404,7 @@ static sfft_status launch_row_inv_t(const RowInvParams& P, cudaStream_t st) {
   const int nth = row_threads(NC, P.H, C::EPT);
   const int RB = nth / (NC / C::EPT);
   const size_t smem = (size_t)RB * C::SEQ_STRIDE * sizeof(cplx);
-  constexpr int MINB = 3;
+  constexpr int MINB = SFFT_ROW_MINB;
   SFFT_CUDA_TRY(cudaFuncSetAttribute(k_row_inv_sub<NC, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   k_row_inv_sub<NC, MINB><<<P.H / RB, nth, smem, st>>>(P);
   SFFT_LAUNCH_CHECK();
