@@ -50,10 +50,15 @@ struct MixParams {
   int monoK[SFFT_MAX_T][2];
 };
 
+#ifndef MIX_RY
 #define MIX_RY 8   // output rows per thread
+#endif
+#ifndef MIX_MINB
+#define MIX_MINB 3
+#endif
 #define MIX_TH 128 // threads per block
 
-// Register-tiled y-mixing.  A thread owns one kx and MIX_RY consecutive output rows; per xi power p
+// Register-tiled y-mixing (the eta^q factors of one xi power are folded by Horner's rule).  A thread owns one kx and MIX_RY consecutive output rows; per xi power p
 // it loads the MIX_RY + 2w source rows of G_p once into registers, scales them by eta^q in place
 // for q = 0..DK-p, and for every (q, v) applies one E value to all MIX_RY accumulators: one global
 // (L1-resident) load per MIX_RY complex FMAs instead of two shared loads per FMA.  Lanes run
@@ -61,7 +66,7 @@ struct MixParams {
 // The packed column kx = 0 holds (X[0], X[W/2]), both real with real factors, and is combined
 // component-wise by the extra x-block (four threads per row, fixed-order shuffle reduction).
 template <int WK>
-__global__ void __launch_bounds__(MIX_TH, 3) k_mix(MixParams P) {
+__global__ void __launch_bounds__(MIX_TH, MIX_MINB) k_mix(MixParams P) {
   constexpr int RY = MIX_RY, S1 = 2 * WK + 1, WIN = RY + 2 * WK;
   const int H = P.H, NC = P.NC, KT = P.KT;
   const int tid = threadIdx.x;
@@ -100,6 +105,14 @@ __global__ void __launch_bounds__(MIX_TH, 3) k_mix(MixParams P) {
   cplx acc[RY];
 #pragma unroll
   for (int i = 0; i < RY; ++i) acc[i] = cmake(0.0, 0.0);
+  double eta[WIN];   // eta of the window's source rows (each row's own coordinate, also when wrapped)
+#pragma unroll
+  for (int i = 0; i < WIN; ++i) {
+    const int yy = (y0 - WK + i + H) & (H - 1);
+    eta[i] = (double)(2 * yy + 1 - H) * invH;
+  }
+  // per xi power p: M += sum_v W_p(v, y - v) G_p[y - v],  W_p(v, y') = sum_q E_(p,q)[v] eta(y')^q
+  // evaluated by Horner in eta, so a (v, row) pair costs one complex fma plus 2 (DK - p) real fmas
   for (int p = 0; p <= P.DK; ++p) {
     cplx g[WIN];
     const cplx* Gp = P.G + (size_t)p * H * NC + kx;
@@ -108,23 +121,50 @@ __global__ void __launch_bounds__(MIX_TH, 3) k_mix(MixParams P) {
       const int yy = (y0 - WK + i + H) & (H - 1);
       g[i] = Gp[(size_t)yy * NC];
     }
-    for (int q = 0; q <= P.DK - p; ++q) {
-      if (q > 0) {
-#pragma unroll
-        for (int i = 0; i < WIN; ++i) {
-          const int yy = (y0 - WK + i + H) & (H - 1);
-          const double eta = (double)(2 * yy + 1 - H) * invH;
-          g[i].x *= eta;
-          g[i].y *= eta;
-        }
-      }
-      const int d = p + q;
-      const cplx* Et = P.E + (size_t)(d * (d + 1) / 2 + q) * S1 * NC + kx;
+    const int nq = P.DK - p + 1;
+    // E_(p,q) = monomial index d(d+1)/2 + q with d = p + q
+    const cplx* E0 = P.E + (size_t)(p * (p + 1) / 2) * S1 * NC + kx;
+    const cplx* E1 = P.E + (size_t)((p + 1) * (p + 2) / 2 + 1) * S1 * NC + kx;
+    const cplx* E2 = P.E + (size_t)((p + 2) * (p + 3) / 2 + 2) * S1 * NC + kx;
+    const cplx* E3 = P.E + (size_t)((p + 3) * (p + 4) / 2 + 3) * S1 * NC + kx;
+    if (nq == 1) {
 #pragma unroll
       for (int vi = 0; vi < S1; ++vi) {
-        const cplx e = Et[(size_t)vi * NC];
+        const cplx e0 = E0[(size_t)vi * NC];
 #pragma unroll
-        for (int i = 0; i < RY; ++i) cfma(acc[i], e, g[i + 2 * WK - vi]);
+        for (int i = 0; i < RY; ++i) cfma(acc[i], e0, g[i + 2 * WK - vi]);
+      }
+    } else if (nq == 2) {
+#pragma unroll
+      for (int vi = 0; vi < S1; ++vi) {
+        const cplx e0 = E0[(size_t)vi * NC], e1 = E1[(size_t)vi * NC];
+#pragma unroll
+        for (int i = 0; i < RY; ++i) {
+          const double h = eta[i + 2 * WK - vi];
+          cfma(acc[i], cmake(fma(h, e1.x, e0.x), fma(h, e1.y, e0.y)), g[i + 2 * WK - vi]);
+        }
+      }
+    } else if (nq == 3) {
+#pragma unroll
+      for (int vi = 0; vi < S1; ++vi) {
+        const cplx e0 = E0[(size_t)vi * NC], e1 = E1[(size_t)vi * NC], e2 = E2[(size_t)vi * NC];
+#pragma unroll
+        for (int i = 0; i < RY; ++i) {
+          const double h = eta[i + 2 * WK - vi];
+          const cplx w = cmake(fma(h, fma(h, e2.x, e1.x), e0.x), fma(h, fma(h, e2.y, e1.y), e0.y));
+          cfma(acc[i], w, g[i + 2 * WK - vi]);
+        }
+      }
+    } else {
+#pragma unroll
+      for (int vi = 0; vi < S1; ++vi) {
+        const cplx e0 = E0[(size_t)vi * NC], e1 = E1[(size_t)vi * NC], e2 = E2[(size_t)vi * NC], e3 = E3[(size_t)vi * NC];
+#pragma unroll
+        for (int i = 0; i < RY; ++i) {
+          const double h = eta[i + 2 * WK - vi];
+          const cplx w = cmake(fma(h, fma(h, fma(h, e3.x, e2.x), e1.x), e0.x), fma(h, fma(h, fma(h, e3.y, e2.y), e1.y), e0.y));
+          cfma(acc[i], w, g[i + 2 * WK - vi]);
+        }
       }
     }
   }
