@@ -86,38 +86,62 @@ __device__ __forceinline__ double rcp_newton(double a) {  // 1/a for normal posi
 // per step).  srd receives 1/L_jj.  Returns the 0-based index of the first non-positive pivot (or
 // -1); failed pivots are replaced by 1 so the work stays finite.
 __device__ __forceinline__ int cta_potrf32(double* sd, double* srd, double (*colb)[CH_NB], int tid) {
+  // TWO pivots per exchange step: columns k, k+1 travel through shared memory together and the
+  // trailing elements are eliminated with the inverse of the 2x2 pivot block (one reciprocal of its
+  // determinant on the dependent chain); column k+1 itself receives the single-pivot update, so the
+  // stored values are exactly those of the column-by-column elimination.
   static_assert(CH_WARPS == 8, "row ownership below assumes 8 warps x 4 rows");
   const int j = tid & 31, i0 = (tid >> 5) * 4;
   double c[4];
   __syncthreads();  // sd was just filled by other threads
 #pragma unroll
   for (int rr = 0; rr < 4; ++rr) c[rr] = sd[(i0 + rr) * CH_LDS + j];
-  if (j == 0) {
+  if (j < 2) {
 #pragma unroll
-    for (int rr = 0; rr < 4; ++rr) colb[0][i0 + rr] = c[rr];
+    for (int rr = 0; rr < 4; ++rr) colb[j][i0 + rr] = c[rr];
   }
   int bad = -1;
 #pragma unroll 1
-  for (int k = 0; k < CH_NB - 1; ++k) {
+  for (int k = 0; k < CH_NB; k += 2) {
     __syncthreads();
-    const double* cur = colb[k & 1];
-    double akk = cur[k];
-    const double ajk = cur[j];
-    const double2 a01 = *reinterpret_cast<const double2*>(cur + i0);
-    const double2 a23 = *reinterpret_cast<const double2*>(cur + i0 + 2);
-    if (!(akk > 0.0)) {
+    const double* col0 = colb[(k & 2)];       // column k   (buffers 0,1 / 2,3 alternate)
+    const double* col1 = colb[(k & 2) + 1];   // column k+1, not yet eliminated by column k
+    double d00 = col0[k];
+    const double d10 = col0[k + 1], d11 = col1[k + 1];
+    const double aj0 = col0[j], aj1 = col1[j];
+    const double2 p01 = *reinterpret_cast<const double2*>(col0 + i0);
+    const double2 p23 = *reinterpret_cast<const double2*>(col0 + i0 + 2);
+    const double2 q01 = *reinterpret_cast<const double2*>(col1 + i0);
+    const double2 q23 = *reinterpret_cast<const double2*>(col1 + i0 + 2);
+    if (!(d00 > 0.0)) {
       if (bad < 0) bad = k;
-      akk = 1.0;
+      d00 = 1.0;
     }
-    // branch-free so that the loads and products are scheduled ahead of the reciprocal chain
-    const double p0 = a01.x * ajk, p1 = a01.y * ajk, p2 = a23.x * ajk, p3 = a23.y * ajk;
-    const double inv = (j > k) ? rcp_newton(akk) : 0.0;   // columns <= k are final
-    c[0] = fma(-p0, inv, c[0]);
-    c[1] = fma(-p1, inv, c[1]);
-    c[2] = fma(-p2, inv, c[2]);
-    c[3] = fma(-p3, inv, c[3]);
-    if (j == k + 1) {
-      double* nxt = colb[(k + 1) & 1];
+    double det = fma(d00, d11, -(d10 * d10));
+    const double inv00 = rcp_newton(d00);
+    if (!(det > 0.0)) {           // second pivot det/d00 not positive
+      if (bad < 0) bad = k + 1;
+      det = d00;
+    }
+    // numerators of D^-1 [aj0 aj1]^T, then the products with the thread's rows: all ahead of the
+    // reciprocal of det
+    const double n0 = fma(d11, aj0, -(d10 * aj1)), n1 = fma(d00, aj1, -(d10 * aj0));
+    const double t0 = fma(p01.x, n0, q01.x * n1), t1 = fma(p01.y, n0, q01.y * n1);
+    const double t2 = fma(p23.x, n0, q23.x * n1), t3 = fma(p23.y, n0, q23.y * n1);
+    const double f = (j > k + 1) ? rcp_newton(det) : 0.0;   // columns <= k+1 take no 2x2 update
+    c[0] = fma(-t0, f, c[0]);
+    c[1] = fma(-t1, f, c[1]);
+    c[2] = fma(-t2, f, c[2]);
+    c[3] = fma(-t3, f, c[3]);
+    if (j == k + 1) {             // column k+1: eliminated by column k alone
+      const double g = d10 * inv00;
+      c[0] = fma(-p01.x, g, c[0]);
+      c[1] = fma(-p01.y, g, c[1]);
+      c[2] = fma(-p23.x, g, c[2]);
+      c[3] = fma(-p23.y, g, c[3]);
+    }
+    if ((j == k + 2 || j == k + 3) && k + 2 < CH_NB) {
+      double* nxt = colb[((k + 2) & 2) + (j - k - 2)];
       *reinterpret_cast<double2*>(nxt + i0) = make_double2(c[0], c[1]);
       *reinterpret_cast<double2*>(nxt + i0 + 2) = make_double2(c[2], c[3]);
     }
@@ -129,7 +153,6 @@ __device__ __forceinline__ int cta_potrf32(double* sd, double* srd, double (*col
     if (i0 + rr == j) srd[j] = c[rr];
   __syncthreads();
   double piv = srd[j];
-  if (!(srd[CH_NB - 1] > 0.0) && bad < 0) bad = CH_NB - 1;
   if (!(piv > 0.0)) piv = 1.0;
   double d, r;
   sqrt_and_rinv(piv, d, r);
@@ -221,7 +244,7 @@ k_chol_fused(const double* __restrict__ A, const double* __restrict__ b, double*
   double* pi = sd;
   double* pj = ss;
   __shared__ double srd[CH_PB];                    // reciprocals of the diagonal
-  __shared__ __align__(16) double colb[2][CH_NB];  // pivot column exchange of cta_potrf32
+  __shared__ __align__(16) double colb[4][CH_NB];  // pivot column exchange of cta_potrf32 (2 x 2 columns)
   const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
   const unsigned nblocks = gridDim.x;
   unsigned target = 0;
