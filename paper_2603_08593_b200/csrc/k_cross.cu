@@ -198,17 +198,37 @@ __global__ void __launch_bounds__(LAG_TH) k_lag_idft(LagParams P) {
   double ap[LAG_MAXD + 1], am[LAG_MAXD + 1];
 #pragma unroll
   for (int dx = 0; dx <= LAG_MAXD; ++dx) { ap[dx] = 0.0; am[dx] = 0.0; }
-  for (int kx = 1 + tid; kx < P.NC; kx += LAG_TH) {
-    cplx y = Yr[kx];
-    for (int q = 1; q < P.nPart; ++q) y = cadd(y, Yr[kx + q * P.partStride]);
-    ap[0] += y.x;
+  // four kx per step: their class partials and first twiddles are requested together; the twiddles
+  // of the higher lags follow by the recurrence t_dx = t_{dx-1} t_1 (<= 10 products, error ~1e-15)
+  for (int kx0 = 1 + tid; kx0 < P.NC; kx0 += 4 * LAG_TH) {
+    cplx ys[4], t1[4];
 #pragma unroll
-    for (int dx = 1; dx <= LAG_MAXD; ++dx) {
-      if (dx <= D) {
-        const cplx t = ldg2(P.twW + ((kx * dx) & (P.W - 1)));  // (c, -s)
-        const double pc = y.x * t.x, qs = y.y * (-t.y);
-        ap[dx] += pc - qs;  // Re(y e^{+i th})
-        am[dx] += pc + qs;  // Re(y e^{-i th})
+    for (int u = 0; u < 4; ++u) {
+      const int kx = kx0 + u * LAG_TH;
+      const bool in = kx < P.NC;
+      ys[u] = in ? Yr[kx] : cmake(0.0, 0.0);
+      t1[u] = in ? ldg2(P.twW + kx) : cmake(1.0, 0.0);   // (c, -s) of angle 2 pi kx / W
+    }
+    for (int q = 1; q < P.nPart; ++q) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int kx = kx0 + u * LAG_TH;
+        if (kx < P.NC) ys[u] = cadd(ys[u], Yr[kx + q * P.partStride]);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const cplx y = ys[u];
+      ap[0] += y.x;
+      cplx t = t1[u];
+#pragma unroll
+      for (int dx = 1; dx <= LAG_MAXD; ++dx) {
+        if (dx <= D) {
+          const double pc = y.x * t.x, qs = y.y * (-t.y);
+          ap[dx] += pc - qs;  // Re(y e^{+i th})
+          am[dx] += pc + qs;  // Re(y e^{-i th})
+          t = cmul(t, t1[u]);
+        }
       }
     }
   }
@@ -351,6 +371,18 @@ __global__ void __launch_bounds__(256) k_gather(GatherParams P) {
   }
 }
 
+// final reduction of the row moments (depends on the row pass only)
+sfft_status sfft_launch_moments(sfft_plan* p, cudaStream_t st, int* nl) {
+  MomParams MP;
+  MP.rowMom = p->rowMom; MP.mom = p->mom; MP.H = p->H; MP.nMomA = p->nMomA; MP.nMomS = p->nMomS; MP.nMomR = p->nMomR;
+  MP.TB = p->TB;
+  for (int t = 0; t < p->TB; ++t) { MP.monoB[t][0] = p->monoB[t][0]; MP.monoB[t][1] = p->monoB[t][1]; }
+  k_mom_final<<<p->nMomA * p->nMomA + p->TB + p->nMomR * p->nMomR, 256, 0, st>>>(MP);
+  SFFT_LAUNCH_CHECK();
+  ++*nl;
+  return SFFT_OK;
+}
+
 sfft_status sfft_launch_lag_gather(sfft_plan* p, double* A, double* b, cudaStream_t st, int* nl) {
   LagParams LP;
   LP.Y = p->Y; LP.Cmap = p->Cmap; LP.pairs = p->d_pairs; LP.NC = p->NC; LP.W = p->W;
@@ -359,13 +391,6 @@ sfft_status sfft_launch_lag_gather(sfft_plan* p, double* A, double* b, cudaStrea
   LP.nPart = p->nPart; LP.partStride = (size_t)p->nPair * p->nLag * p->pitch;
   dim3 g1(p->nPair, p->nLag);
   k_lag_idft<<<g1, LAG_TH, 0, st>>>(LP);
-  SFFT_LAUNCH_CHECK();
-  ++*nl;
-  MomParams MP;
-  MP.rowMom = p->rowMom; MP.mom = p->mom; MP.H = p->H; MP.nMomA = p->nMomA; MP.nMomS = p->nMomS; MP.nMomR = p->nMomR;
-  MP.TB = p->TB;
-  for (int t = 0; t < p->TB; ++t) { MP.monoB[t][0] = p->monoB[t][0]; MP.monoB[t][1] = p->monoB[t][1]; }
-  k_mom_final<<<p->nMomA * p->nMomA + p->TB + p->nMomR * p->nMomR, 256, 0, st>>>(MP);
   SFFT_LAUNCH_CHECK();
   ++*nl;
   GatherParams GP;

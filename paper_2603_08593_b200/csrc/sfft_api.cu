@@ -72,6 +72,7 @@ static void plan_free(sfft_plan* p) {
   if (p->side) cudaStreamDestroy(p->side);
   if (p->evFork) cudaEventDestroy(p->evFork);
   if (p->evJoin) cudaEventDestroy(p->evJoin);
+  if (p->evRow) cudaEventDestroy(p->evRow);
   for (int i = 0; i < 2 * SFFT_PROF_MAX; ++i) if (p->prof_ev[i]) cudaEventDestroy(p->prof_ev[i]);
   delete p;
 }
@@ -170,7 +171,8 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   cudaDeviceGetStreamPriorityRange(&prLo, &prHi);
   if (cudaStreamCreateWithPriority(&p->side, cudaStreamNonBlocking, prHi) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->evFork, cudaEventDisableTiming) != cudaSuccess ||
-      cudaEventCreateWithFlags(&p->evJoin, cudaEventDisableTiming) != cudaSuccess) {
+      cudaEventCreateWithFlags(&p->evJoin, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&p->evRow, cudaEventDisableTiming) != cudaSuccess) {
     cudaGetLastError();
     plan_free(p);
     return SFFT_ERR_CUDA;
@@ -261,9 +263,14 @@ sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S, co
   SFFT_CUDA_TRY(cudaStreamWaitEvent(p->side, p->evFork, 0));
   { ProfScope ps(p, 9, p->side); s = sfft_launch_kb(p, R, mask, p->side, &nl); }
   if (s != SFFT_OK) return s;
-  SFFT_CUDA_TRY(cudaEventRecord(p->evJoin, p->side));
   { ProfScope ps(p, 0, st); s = sfft_launch_row_fwd(p, R, S, mask, true, p->T, p->pitchT, !p->fused, p->fused != 0, st, &nl); }
   if (s != SFFT_OK) return s;
+  // the final moment reduction needs only the row pass: it follows the sparse chain on the side stream
+  SFFT_CUDA_TRY(cudaEventRecord(p->evRow, st));
+  SFFT_CUDA_TRY(cudaStreamWaitEvent(p->side, p->evRow, 0));
+  s = sfft_launch_moments(p, p->side, &nl);
+  if (s != SFFT_OK) return s;
+  SFFT_CUDA_TRY(cudaEventRecord(p->evJoin, p->side));
   if (p->fused) {
     // a2 (column pass, applies eta^q) + a3 (cross products + lag-pruned inverse along ky), fused
     ProfScope ps(p, 1, st);

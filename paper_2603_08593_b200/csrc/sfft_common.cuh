@@ -129,7 +129,7 @@ struct sfft_plan {
   // plan-owned side stream: stages of one call that do not depend on each other run concurrently
   // (forked from and joined back into the caller stream with events; no host synchronisation)
   cudaStream_t side;
-  cudaEvent_t evFork, evJoin;
+  cudaEvent_t evFork, evJoin, evRow;
   // optional per-stage CUDA-event timing (sfft_profile_*): events are recorded on the caller
   // stream around each stage; nothing synchronises until sfft_profile_read.
   int prof_on;
@@ -178,6 +178,7 @@ int sfft_colx_dinst(int w);
 sfft_status sfft_colx_init();
 bool sfft_colx_supported(int H, int nPair);
 sfft_status sfft_launch_kb(sfft_plan* p, const double* R, const unsigned char* mask, cudaStream_t st, int* nl);
+sfft_status sfft_launch_moments(sfft_plan* p, cudaStream_t st, int* nl);
 sfft_status sfft_launch_lag_gather(sfft_plan* p, double* A, double* b, cudaStream_t st, int* nl);
 sfft_status sfft_launch_solve(sfft_plan* p, const double* A, const double* b, double* c, int* info,
                               cudaStream_t st, int* nl);
