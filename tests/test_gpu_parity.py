@@ -102,6 +102,23 @@ def test_ragged_shapes_and_degrees(H, W, w, DK, DB, masked):
     run_case(R, S, mask, w, DK, DB, 30.0)
 
 
+@pytest.mark.parametrize("H,W,w,DK,DB,masked", [
+    (1024, 32, 0, 0, 0, True), (1024, 64, 1, 1, 3, True), (1024, 32, 2, 2, 1, False),
+    (2048, 32, 3, 2, 2, True), (1024, 128, 5, 1, 0, True), (4096, 32, 2, 2, 2, True),
+    (1024, 64, 4, 3, 1, True)])
+def test_fused_column_cross_path(H, W, w, DK, DB, masked):
+    """H in {1024, 2048, 4096}: the fused column-FFT + cross-spectra kernel (every residue-class
+    count DR = 2, 4, 8, every instantiated lag range) against the oracle; DK = 3 (> 32 map pairs)
+    must fall back to the separate kernels at the same sizes."""
+    rng = np.random.default_rng(H + 13 * W + w)
+    R = 50.0 * rng.standard_normal((H, W)) + 500.0 * (rng.random((H, W)) > 0.98)
+    S = 0.7 * np.roll(R, (1 if w else 0, -1 if w else 0), (0, 1)) + 30.0 * rng.standard_normal((H, W)) + 200.0
+    mask = (rng.random((H, W)) < 0.03).astype(np.uint8) if masked else None
+    with SfftPlan(H, W, w, DK, DB) as plan:
+        assert plan.fused == (DK <= 2)
+    run_case(R, S, mask, w, DK, DB, 30.0, full_D=False)
+
+
 def test_mid_config():
     pr = synth.make_pair("mid")
     run_case(pr.R, pr.S, pr.mask, pr.cfg.w, pr.cfg.DK, pr.cfg.DB, pr.sky_rms, full_D=False)
