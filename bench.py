@@ -453,8 +453,9 @@ def run_cuda(args, rank, world, local_rank):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full captures
 # summarised under profiles/ (filled in when a capture of that kernel exists; else null).
-NCU_TRAFFIC = {"build.colx": 322.9e6,      # profiles/r01d_ncu_full.md (k_colx<4,10>)
-               "build.row_fwd": 364.1e6}
+NCU_TRAFFIC = {"build.colx": 323.5e6,        # profiles/r01e_ncu_full.md (k_colx<4,10>)
+               "build.row_fwd": 359.0e6, "subtract.row_fwd": 210.2e6, "subtract.mix": 263.1e6,
+               "subtract.row_inv": 171.8e6, "solve": 4.6e6}
 
 
 def main():
