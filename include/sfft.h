@@ -121,6 +121,12 @@ int sfft_last_launch_count(const sfft_plan* p, int which);
  * holds the fused kernel and stages 2, 3 stay empty. */
 int sfft_plan_fused(const sfft_plan* p);
 
+/* Throughput knob for pipelines that keep several plans in flight on different streams: caps the
+ * number of CTAs of the cooperative Cholesky kernel (default 0 = one per SM, the lowest latency for
+ * a single pair).  A smaller grid leaves whole SMs to the other plans' transform kernels while this
+ * plan's latency-bound solve runs.  Results are bitwise independent of the setting. */
+sfft_status sfft_plan_set_solve_ctas(sfft_plan* p, int max_ctas);
+
 /* Library version string, e.g. "sfft-b200 0.1 (sm_100a)". */
 const char* sfft_version(void);
 

@@ -17,7 +17,7 @@ _LIB_NAME = "libsfft.so"
 EXPORTED_SYMBOLS = [
     "sfft_plan_create", "sfft_plan_destroy", "sfft_num_coeffs", "sfft_workspace_bytes",
     "sfft_status_string", "sfft_build_system", "sfft_solve", "sfft_subtract",
-    "sfft_probe_fp64", "sfft_last_launch_count", "sfft_plan_fused", "sfft_version",
+    "sfft_probe_fp64", "sfft_last_launch_count", "sfft_plan_fused", "sfft_plan_set_solve_ctas", "sfft_version",
     "sfft_profile_enable", "sfft_profile_read",
 ]
 
@@ -73,6 +73,8 @@ def load_library():
     lib.sfft_last_launch_count.restype = i32
     lib.sfft_plan_fused.argtypes = [vp]
     lib.sfft_plan_fused.restype = i32
+    lib.sfft_plan_set_solve_ctas.argtypes = [vp, i32]
+    lib.sfft_plan_set_solve_ctas.restype = i32
     lib.sfft_profile_enable.argtypes = [vp, i32]
     lib.sfft_profile_enable.restype = i32
     lib.sfft_profile_read.argtypes = [vp, i32, dbl_p, ctypes.POINTER(i32), i32]
@@ -200,6 +202,10 @@ class SfftPlan:
     # -- diagnostics
     def last_launch_count(self, which: int) -> int:
         return int(self._lib.sfft_last_launch_count(self._p, which))
+
+    def set_solve_ctas(self, max_ctas: int) -> None:
+        """sfft_plan_set_solve_ctas: cap the Cholesky kernel's grid (0 = one CTA per SM)."""
+        _check(self._lib, self._lib.sfft_plan_set_solve_ctas(self._p, int(max_ctas)), "sfft_plan_set_solve_ctas")
 
     @property
     def fused(self) -> bool:

@@ -465,6 +465,7 @@ sfft_status sfft_launch_solve(sfft_plan* p, const double* A, const double* b, do
   int want = maxUseful > tiles ? maxUseful : tiles;
   if (want < 1) want = 1;
   if (grid > want) grid = want;
+  if (p->cholMaxCtas > 0 && grid > p->cholMaxCtas) grid = p->cholMaxCtas;
   const size_t smemF = (size_t)2 * CH_PB * CH_LDS * sizeof(double);
   SFFT_CUDA_TRY(cudaFuncSetAttribute(k_chol_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smemF));
   SFFT_CUDA_TRY(cudaLaunchCooperativeKernel((const void*)k_chol_fused, dim3(grid), dim3(CH_THREADS), args, smemF, st));

@@ -351,6 +351,12 @@ sfft_status sfft_profile_read(sfft_plan* p, int stage, double* total_ms, int* co
 
 int sfft_plan_fused(const sfft_plan* p) { return p ? p->fused : -1; }
 
+sfft_status sfft_plan_set_solve_ctas(sfft_plan* p, int max_ctas) {
+  if (!p || max_ctas < 0) return SFFT_ERR_INVALID_ARG;
+  p->cholMaxCtas = max_ctas;
+  return SFFT_OK;
+}
+
 int sfft_last_launch_count(const sfft_plan* p, int which) {
   if (!p || which < 0 || which > 2) return -1;
   return p->launches[which];

@@ -119,6 +119,7 @@ struct sfft_plan {
   double* kbPart;   // [KB_NBLK][L*TK*TB]
   double* kbCorr;   // [L*TK*TB]
   double* Lw;       // Cholesky workspace (N+1) x ldL
+  int cholMaxCtas;   // cap on the CTAs of k_chol_fused (0 = one per SM); see sfft_plan_set_solve_ctas
   unsigned* cholBar; // grid-barrier counters of k_chol_fused (arrivals, finished CTAs)
   cplx* Etab;       // subtract: E[TK][2w+1][NC]
   cplx* Mhat;       // subtract: mixed row spectra [H][NC]
