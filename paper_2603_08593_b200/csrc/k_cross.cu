@@ -301,6 +301,7 @@ struct GatherParams {
   const double* Cmap;
   const double* mom;
   const double* kbCorr;   // [(t*L + s)*TB + t'] sparse part of the kernel-background block (k_kb.cu)
+  const double* kbStrip;  // [(t*L + s)*TB + t'] part of the fully masked target rows (k_kb_strip)
   double* A;
   double* b;
   int w, L, TK, TB, N, nLag, nMomA, nMomR, H, W;
@@ -361,7 +362,7 @@ __global__ void __launch_bounds__(256) k_gather(GatherParams P) {
         for (int jj = 0; jj <= qb; ++jj)
           acc += cx * binom(qb, jj) * ipow(dy, qb - jj) * mu[(pk + ii) * P.nMomR + (qk + jj)];
       }
-      v = acc + P.kbCorr[((size_t)t * L + s) * P.TB + ib];
+      v = acc - P.kbStrip[((size_t)t * L + s) * P.TB + ib] + P.kbCorr[((size_t)t * L + s) * P.TB + ib];
     } else {
       const int a = i - nK, c = j - nK;
       const int pa = P.monoB[a][0] + P.monoB[c][0], qa = P.monoB[a][1] + P.monoB[c][1];
@@ -371,6 +372,38 @@ __global__ void __launch_bounds__(256) k_gather(GatherParams P) {
   }
 }
 
+struct StripParams {
+  const int* fmList;      // fully masked target rows: count, then the rows in ascending order
+  const double* rowMomR;  // [nMomR][H] sum_x m R xi^a per row
+  double* kbStrip;        // [(t*L + s)*TB + t']
+  int w, L, TK, TB, H, W;
+  int monoK[SFFT_MAX_T][2], monoB[SFFT_MAX_T][2];
+};
+
+// Part of the kernel-background block that belongs to fully masked target rows y (k_kb.cu):
+//   sum_y eta'^qk (eta' + dy)^qb sum_ii C(pb,ii) dx^(pb-ii) rowMomR[pk+ii][y'],  y' = wrap(y - v) the source
+// row and eta' its own coordinate; one thread per entry, rows in ascending order.
+__global__ void __launch_bounds__(128) k_kb_strip(StripParams P) {
+  const int e = blockIdx.x * 128 + threadIdx.x;
+  if (e >= P.TK * P.L * P.TB) return;
+  const int ib = e % P.TB, ik = e / P.TB, t = ik / P.L, s = ik - t * P.L, S1 = 2 * P.w + 1;
+  const int u = s % S1 - P.w, vv = s / S1 - P.w;
+  const int pk = P.monoK[t][0], qk = P.monoK[t][1], pb = P.monoB[ib][0], qb = P.monoB[ib][1];
+  const double dx = 2.0 * (double)u / (double)P.W, dy = 2.0 * (double)vv / (double)P.H;
+  double cx[SFFT_MAX_DEG + 1];
+  for (int ii = 0; ii <= pb; ++ii) cx[ii] = binom(pb, ii) * ipow(dx, pb - ii);
+  double strip = 0.0;
+  const int nfm = P.fmList[0];
+  for (int f = 0; f < nfm; ++f) {
+    const int ys = (P.fmList[1 + f] - vv + P.H) & (P.H - 1);
+    const double etas = (double)(2 * ys + 1 - P.H) / (double)P.H;
+    double rsum = 0.0;
+    for (int ii = 0; ii <= pb; ++ii) rsum += cx[ii] * P.rowMomR[(size_t)(pk + ii) * P.H + ys];
+    strip += ipow(etas, qk) * ipow(etas + dy, qb) * rsum;
+  }
+  P.kbStrip[e] = strip;
+}
+
 // final reduction of the row moments (depends on the row pass only)
 sfft_status sfft_launch_moments(sfft_plan* p, cudaStream_t st, int* nl) {
   MomParams MP;
@@ -378,6 +411,14 @@ sfft_status sfft_launch_moments(sfft_plan* p, cudaStream_t st, int* nl) {
   MP.TB = p->TB;
   for (int t = 0; t < p->TB; ++t) { MP.monoB[t][0] = p->monoB[t][0]; MP.monoB[t][1] = p->monoB[t][1]; }
   k_mom_final<<<p->nMomA * p->nMomA + p->TB + p->nMomR * p->nMomR, 256, 0, st>>>(MP);
+  SFFT_LAUNCH_CHECK();
+  ++*nl;
+  StripParams SP;
+  SP.fmList = p->fmList; SP.rowMomR = p->rowMom + (size_t)(p->nMomA + p->nMomS) * p->H; SP.kbStrip = p->kbStrip;
+  SP.w = p->w; SP.L = p->L; SP.TK = p->TK; SP.TB = p->TB; SP.H = p->H; SP.W = p->W;
+  for (int t = 0; t < p->TB; ++t) { SP.monoB[t][0] = p->monoB[t][0]; SP.monoB[t][1] = p->monoB[t][1]; }
+  for (int t = 0; t < p->TK; ++t) { SP.monoK[t][0] = p->monoK[t][0]; SP.monoK[t][1] = p->monoK[t][1]; }
+  k_kb_strip<<<(p->TK * p->L * p->TB + 127) / 128, 128, 0, st>>>(SP);
   SFFT_LAUNCH_CHECK();
   ++*nl;
   return SFFT_OK;
@@ -397,6 +438,7 @@ sfft_status sfft_launch_lag_gather(sfft_plan* p, double* A, double* b, cudaStrea
   GP.Cmap = p->Cmap; GP.mom = p->mom; GP.A = A; GP.b = b; GP.w = p->w; GP.L = p->L; GP.TK = p->TK;
   GP.TB = p->TB; GP.N = p->N; GP.nLag = p->nLag; GP.nMomA = p->nMomA; GP.nMomR = p->nMomR;
   GP.H = p->H; GP.W = p->W; GP.kbCorr = p->kbCorr;
+  GP.kbStrip = p->kbStrip;
   for (int t = 0; t < p->TB; ++t) { GP.monoB[t][0] = p->monoB[t][0]; GP.monoB[t][1] = p->monoB[t][1]; }
   for (int t = 0; t < p->TK; ++t) { GP.monoK[t][0] = p->monoK[t][0]; GP.monoK[t][1] = p->monoK[t][1]; }
   const size_t total = (size_t)p->N * p->N + p->N;

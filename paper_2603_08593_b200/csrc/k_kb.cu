@@ -12,6 +12,10 @@
 // wrapping the bracket vanishes identically.  (I) is a combination of the moments
 // mu_ab = sum m R xi^a eta^b, a+b <= DK+DB (fused into the row pass, k_rows.cu), expanded in
 // k_gather with delta_x = 2u/W, delta_y = 2v/H; (II) is the sparse sum evaluated here.
+// Fully masked target rows (a CCD's top and bottom border) are taken out of the sparse sum: all W
+// targets of such a row y are masked, so their part of (II) is -sum_x' R~_t(x', y') P_t'(x'+u, y'+v)
+// over the WHOLE source row y' = wrap(y - v), a combination of the row moments sum_x m R xi^a that
+// the row pass already delivers (evaluated in k_gather).
 // Every sum has a fixed order (per-row ordered compaction, per-thread sequential partials, ordered
 // final reduction), so the block is reproducible run to run.
 #include "sfft_common.cuh"
@@ -37,13 +41,18 @@ __device__ __forceinline__ bool sp_strip(int x, int y, int W, int H, int w) {
 
 // One warp per row, 16 pixels per lane and step.  FILL = false: count the row's special pixels.
 // FILL = true: write them, in x order, at spOff[y].
+// A row whose W pixels are all masked is not listed: its whole contribution is a combination of
+// the source rows' moments (k_gather), see the header of this file; fmFlag[y] marks such rows.
 template <bool FILL>
 __global__ void __launch_bounds__(256) k_sp_rows(const unsigned char* __restrict__ mask, int H, int W, int w,
-                                                 int* spCount, const int* __restrict__ spOff, int* spList) {
+                                                 int* spCount, const int* __restrict__ spOff, int* spList,
+                                                 int* fmFlag) {
   const int lane = threadIdx.x & 31;
   const int y = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (y >= H) return;
+  if (FILL && fmFlag[y]) return;
   const int base = FILL ? spOff[y] : 0;
+  int nmasked = 0;
   const bool edge_row = y < w || y >= H - w;
   int total = 0;
   for (int k = 0; k < (W + 511) / 512; ++k) {   // uniform trip count for the shuffles
@@ -60,6 +69,7 @@ __global__ void __launch_bounds__(256) k_sp_rows(const unsigned char* __restrict
             if ((wd[q] >> (8 * i)) & 0xffu) mk |= 1u << (4 * q + i);
       }
       flags = mk;
+      nmasked += __popc(mk);
       if (edge_row) flags = 0xffffu;
       else if (x0 < w || x0 + 16 > W - w) {
 #pragma unroll
@@ -88,18 +98,48 @@ __global__ void __launch_bounds__(256) k_sp_rows(const unsigned char* __restrict
   }
   if (!FILL) {
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1) total += __shfl_xor_sync(0xffffffffu, total, off);
-    if (lane == 0) spCount[y] = total;
+    for (int off = 16; off > 0; off >>= 1) {
+      total += __shfl_xor_sync(0xffffffffu, total, off);
+      nmasked += __shfl_xor_sync(0xffffffffu, nmasked, off);
+    }
+    if (lane == 0) {
+      const int full = nmasked == W;
+      fmFlag[y] = full;
+      spCount[y] = full ? 0 : total;
+    }
   }
 }
 
 // Exclusive scan of the per-row counts (H <= 4096) by one CTA.
-__global__ void __launch_bounds__(1024) k_sp_scan(const int* __restrict__ spCount, int* spOff, int H) {
+// Also compacts the fully masked rows, in ascending order, into fmList[1..], fmList[0] = their number.
+__global__ void __launch_bounds__(1024) k_sp_scan(const int* __restrict__ spCount, int* spOff, int H,
+                                                  const int* __restrict__ fmFlag, int* fmList) {
   __shared__ int part[1024];
   const int tid = threadIdx.x;
   const int per = (H + 1023) / 1024;
   int loc[4] = {0, 0, 0, 0};
   int sum = 0;
+  {
+    int fl[4] = {0, 0, 0, 0}, fsum = 0;
+    for (int i = 0; i < per; ++i) {
+      const int y = tid * per + i;
+      fl[i] = y < H ? fmFlag[y] : 0;
+      fsum += fl[i];
+    }
+    part[tid] = fsum;
+    __syncthreads();
+    for (int off = 1; off < 1024; off <<= 1) {
+      const int t = tid >= off ? part[tid - off] : 0;
+      __syncthreads();
+      part[tid] += t;
+      __syncthreads();
+    }
+    int run = part[tid] - fsum;
+    for (int i = 0; i < per; ++i)
+      if (fl[i]) fmList[1 + run++] = tid * per + i;
+    if (tid == 1023) fmList[0] = part[1023];
+    __syncthreads();
+  }
   for (int i = 0; i < per; ++i) {
     const int y = tid * per + i;
     loc[i] = y < H ? spCount[y] : 0;
@@ -278,11 +318,11 @@ static sfft_status launch_kb_corr_tb(const KbParams& P, cudaStream_t st) {
 sfft_status sfft_launch_kb(sfft_plan* p, const double* R, const unsigned char* mask, cudaStream_t st, int* nl) {
   const int H = p->H, W = p->W;
   const int rowsPerBlock = 8;
-  k_sp_rows<false><<<(H + rowsPerBlock - 1) / rowsPerBlock, 32 * rowsPerBlock, 0, st>>>(mask, H, W, p->w, p->spCount, nullptr, nullptr);
+  k_sp_rows<false><<<(H + rowsPerBlock - 1) / rowsPerBlock, 32 * rowsPerBlock, 0, st>>>(mask, H, W, p->w, p->spCount, nullptr, nullptr, p->fmFlag);
   SFFT_LAUNCH_CHECK();
-  k_sp_scan<<<1, 1024, 0, st>>>(p->spCount, p->spOff, H);
+  k_sp_scan<<<1, 1024, 0, st>>>(p->spCount, p->spOff, H, p->fmFlag, p->fmList);
   SFFT_LAUNCH_CHECK();
-  k_sp_rows<true><<<(H + rowsPerBlock - 1) / rowsPerBlock, 32 * rowsPerBlock, 0, st>>>(mask, H, W, p->w, p->spCount, p->spOff, p->spList);
+  k_sp_rows<true><<<(H + rowsPerBlock - 1) / rowsPerBlock, 32 * rowsPerBlock, 0, st>>>(mask, H, W, p->w, p->spCount, p->spOff, p->spList, p->fmFlag);
   SFFT_LAUNCH_CHECK();
   KbParams P;
   P.R = R; P.mask = mask; P.spOff = p->spOff; P.spList = p->spList; P.part = p->kbPart;

@@ -67,7 +67,7 @@ static void plan_free(sfft_plan* p) {
   cudaFree(p->twP512);
   cudaFree(p->twPNC); cudaFree(p->twPH); cudaFree(p->twW); cudaFree(p->twH); cudaFree(p->d_pairs); cudaFree(p->d_groups);
   cudaFree(p->T); cudaFree(p->F); cudaFree(p->Y); cudaFree(p->Cmap); cudaFree(p->rowMom);
-  cudaFree(p->mom); cudaFree(p->spCount); cudaFree(p->spOff); cudaFree(p->spList); cudaFree(p->kbPart); cudaFree(p->kbCorr); cudaFree(p->Lw); cudaFree(p->cholBar); cudaFree(p->Etab); cudaFree(p->Mhat);
+  cudaFree(p->mom); cudaFree(p->spCount); cudaFree(p->spOff); cudaFree(p->spList); cudaFree(p->fmFlag); cudaFree(p->fmList); cudaFree(p->kbPart); cudaFree(p->kbCorr); cudaFree(p->kbStrip); cudaFree(p->Lw); cudaFree(p->cholBar); cudaFree(p->Etab); cudaFree(p->Mhat);
   free(p->h_pairs);
   if (p->side) cudaStreamDestroy(p->side);
   if (p->evFork) cudaEventDestroy(p->evFork);
@@ -201,8 +201,11 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
     dalloc((void**)&p->spCount, sizeof(int) * (size_t)H);
     dalloc((void**)&p->spOff, sizeof(int) * (size_t)(H + 1));
     dalloc((void**)&p->spList, sizeof(int) * (size_t)H * W);
+    dalloc((void**)&p->fmFlag, sizeof(int) * (size_t)H);
+    dalloc((void**)&p->fmList, sizeof(int) * (size_t)(H + 1));
     dalloc((void**)&p->kbPart, sizeof(double) * (size_t)SFFT_KB_NBLK * nsub * p->TK * p->L * p->TB);
     dalloc((void**)&p->kbCorr, sizeof(double) * (size_t)p->TK * p->L * p->TB);
+    dalloc((void**)&p->kbStrip, sizeof(double) * (size_t)p->TK * p->L * p->TB);
   }
   dalloc((void**)&p->Lw, sizeof(double) * (size_t)(p->N + 1) * p->ldL);
   dalloc((void**)&p->cholBar, 2 * sizeof(unsigned));

@@ -116,8 +116,11 @@ struct sfft_plan {
   int* spCount;     // [H]
   int* spOff;       // [H + 1]   exclusive scan; spOff[H] = number of special pixels
   int* spList;      // [H*W]     y*W + x, bit 31 set when the pixel is masked
+  int* fmFlag;      // [H]       1 if every pixel of the row is masked (such rows are not listed)
+  int* fmList;      // [H + 1]   number of fully masked rows, then the rows in ascending order
   double* kbPart;   // [KB_NBLK][L*TK*TB]
   double* kbCorr;   // [L*TK*TB]
+  double* kbStrip;  // [L*TK*TB] part of the fully masked target rows (from row moments)
   double* Lw;       // Cholesky workspace (N+1) x ldL
   int cholMaxCtas;   // cap on the CTAs of k_chol_fused (0 = one per SM); see sfft_plan_set_solve_ctas
   unsigned* cholBar; // grid-barrier counters of k_chol_fused (arrivals, finished CTAs)
