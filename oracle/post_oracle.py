@@ -1,0 +1,82 @@
+"""CPU ORACLE for the two steps that follow SFFT differencing -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s cpu_baseline legs may import this module.
+It shares no code with the CUDA path and does not import the package.  Plain numpy loops, float64.
+
+(1) Multi-template combination -- PAPER.md:158 (§2.3.2): "For multi-exposure templates, the science
+    image is differenced against each individual template exposure, producing N_TEMP difference
+    images per science exposure.  All difference images are subsequently normalized to a common
+    photometric zero point (Section 2.3.1) and median-combined to produce a single final difference
+    image"; N_TEMP "a tunable parameter with a default of 5" (§2.1.1).
+    Definition written out: out[y,x] = median_k( scale_k * D_k[y,x] ), scale_k the flux factor that
+    brings image k to the common zero point (scale_k = 10^(0.4 (zp_ref - zp_k))).
+    Reading M1 (paper silent): for an even number of images the median is the mean of the two
+    middle values (the usual convention; the default N_TEMP = 5 is odd).
+
+(2) Monte-Carlo limiting flux -- PAPER.md:164 (§2.3.3): "We measure aperture fluxes at 1024 randomly
+    selected background positions using the same aperture definition, and deriving the 5 sigma
+    threshold from their standard deviation, converted to magnitudes with the corresponding zero
+    point"; aperture "0.6731 x FWHM" (§2.3.1).
+    Readings (paper silent): L1 the aperture is the hard-edged disc of pixels whose centres lie within
+    `radius` of the (real-valued) position, pixel (y,x) centred at integer coordinates; L2 a position
+    is a "background position" when its disc lies inside the frame and touches no masked pixel --
+    other positions are dropped (flux NaN); L3 the standard deviation is the population one
+    (divide by the number of kept apertures); L4 the positions are inputs (the random draw is the
+    caller's), so both sides see the same ones; L5 m_lim = zp - 2.5 log10(5 sigma).
+
+Pins (tests/test_post_pins.py): statistics.median on small stacks, permutation and scale
+invariance, known order statistics; Gauss circle lattice counts N(r) for the disc, a constant image
+(flux = c N(r), sigma = 0), a linear ramp (flux = N(r) * value at the centre for integer centres),
+white noise (sigma ~ sigma_pix sqrt N(r)), masked / out-of-frame positions dropped.
+"""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+
+
+def median_combine(Ds, scales):
+    """out = median over k of scales[k] * Ds[k], element by element (sort, take the middle)."""
+    stack = np.stack([np.asarray(D, dtype=np.float64) * float(s) for D, s in zip(Ds, scales)], axis=0)
+    n = stack.shape[0]
+    srt = np.sort(stack, axis=0)
+    if n % 2 == 1:
+        return srt[n // 2].copy()
+    return 0.5 * (srt[n // 2 - 1] + srt[n // 2])
+
+
+def aperture_flux(D, mask, x0, y0, radius):
+    """Sum of D over the pixels whose centres lie within `radius` of (x0, y0); NaN if the disc
+    leaves the frame or touches a masked pixel (readings L1, L2).  Explicit loops."""
+    H, W = D.shape
+    r2 = radius * radius
+    ylo, yhi = int(math.ceil(y0 - radius)), int(math.floor(y0 + radius))
+    xlo, xhi = int(math.ceil(x0 - radius)), int(math.floor(x0 + radius))
+    if ylo < 0 or xlo < 0 or yhi > H - 1 or xhi > W - 1:
+        return float("nan")
+    tot = 0.0
+    for y in range(ylo, yhi + 1):
+        for x in range(xlo, xhi + 1):
+            if (x - x0) ** 2 + (y - y0) ** 2 <= r2:
+                if mask is not None and mask[y, x]:
+                    return float("nan")
+                tot += float(D[y, x])
+    return tot
+
+
+def aperture_stats(D, mask, xs, ys, radius):
+    """Fluxes at the given positions and (count, mean, population sigma) of the kept ones."""
+    flux = np.array([aperture_flux(D, mask, float(x), float(y), radius) for x, y in zip(xs, ys)])
+    kept = flux[~np.isnan(flux)]
+    n = kept.size
+    if n == 0:
+        return flux, (0, float("nan"), float("nan"))
+    mean = float(np.sum(kept) / n)
+    sigma = float(math.sqrt(np.sum((kept - mean) ** 2) / n))
+    return flux, (n, mean, sigma)
+
+
+def limiting_magnitude(sigma, zero_point):
+    """m_lim = zp - 2.5 log10(5 sigma)  (reading L5)."""
+    return zero_point - 2.5 * math.log10(5.0 * sigma)
