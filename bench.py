@@ -367,6 +367,40 @@ def run_cuda(args, rank, world, local_rank):
     e2e_value = shard.aggregate_rate(args.steps, world, ms_e2e)
     assert all(int(B["info"].item()) == 0 for B in bufs)
 
+    # ---- the two steps after the differencing, timed alone on the device
+    post = None
+    if world == 1:
+        from paper_2603_08593_b200 import aperture_stats, median_combine
+        nT = 5   # N_TEMP default
+        Dt = [torch.randn((cfg.H, cfg.W), dtype=torch.float64, device="cuda") * 40 for _ in range(nT)]
+        sc = [1.0, 0.93, 1.1, 0.8, 1.25]
+        outm = torch.empty_like(Dt[0])
+        gq = torch.Generator(device="cuda").manual_seed(7)
+        xs = torch.rand(1024, dtype=torch.float64, device="cuda", generator=gq) * cfg.W
+        ys = torch.rand(1024, dtype=torch.float64, device="cuda", generator=gq) * cfg.H
+        for _ in range(3):
+            median_combine(Dt, sc, out=outm)
+            aperture_stats(D, devp[0][2], xs, ys, 0.6731 * 5.0)
+        g0, g1, g2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        reps = 10
+        g0.record()
+        for _ in range(reps):
+            median_combine(Dt, sc, out=outm)
+        g1.record()
+        for _ in range(reps):
+            aperture_stats(D, devp[0][2], xs, ys, 0.6731 * 5.0)
+        g2.record()
+        torch.cuda.synchronize()
+        t_med, t_ap = g0.elapsed_time(g1) / reps, g1.elapsed_time(g2) / reps
+        med_bytes = (nT + 1) * cfg.H * cfg.W * 8
+        post = {"median_combine": {"templates": nT, "ms": round(t_med, 4), "hbm_gbs": round(med_bytes / t_med / 1e6, 1),
+                                   "frac_of_hbm_peak": round(med_bytes / t_med / 1e6 / peaks["hbm_gbs"], 4),
+                                   "bytes": med_bytes},
+                "aperture_stats": {"positions": 1024, "radius_px": round(0.6731 * 5.0, 3), "ms": round(t_ap, 4),
+                                   "bound": "latency (two small kernels)"}}
+        del Dt, outm
+        torch.cuda.empty_cache()
+
     exposure = None
     if world == 1 and args.exposure_ccds > 0:
         del bufs
@@ -448,6 +482,7 @@ def run_cuda(args, rank, world, local_rank):
         "stages": table,
         "cpu_baseline": cpu,
         "exposure": exposure,
+        "post_differencing": post,
     }
     print(json.dumps(out), flush=True)
     if world > 1:

@@ -88,6 +88,35 @@ sfft_status sfft_solve(sfft_plan* p, const double* A, const double* b, double* c
 sfft_status sfft_subtract(sfft_plan* p, const double* R, const double* S, const double* coeffs,
                           double* D, void* stream);
 
+/* ---- steps that follow the differencing of one CCD ---------- */
+
+#define SFFT_MAX_TEMPLATES 9
+
+/* Multi-template combination (§2.3.2: the N_TEMP difference images of one science
+ * exposure are "normalized to a common photometric zero point ... and median-combined"; N_TEMP
+ * defaults to 5):  out[i] = median over k of scale[k] * D[k][i],  i < npix.
+ * For even n the median is the mean of the two middle values (reading M1).
+ *   D     in : HOST array of n DEVICE pointers, each npix fp64, 16-byte aligned, none aliasing out.
+ *   scale in : HOST array of n flux factors (10^(0.4 (zp_ref - zp_k))).
+ *   out  out : npix fp64 (device, 16-byte aligned).      1 <= n <= SFFT_MAX_TEMPLATES.
+ * Enqueues one kernel on `stream`; never synchronises.  Needs no plan. */
+sfft_status sfft_median_combine(const double* const* D, const double* scale, int n, size_t npix,
+                                double* out, void* stream);
+
+/* Monte-Carlo limiting flux of a difference image (§2.3.3: "aperture fluxes at 1024
+ * randomly selected background positions ... deriving the 5 sigma threshold from their standard
+ * deviation").  The positions are INPUTS (the random draw is the caller's).
+ *   D in: H*W fp64 (device);  mask in: H*W uint8 (device), nonzero = not background, NULL = none.
+ *   xs, ys in: n real-valued pixel positions (device; pixel (y,x) is centred at integer coordinates).
+ *   flux out: n fp64 (device): sum of D over the pixels whose centres lie within `radius` of the
+ *     position; NaN when that disc leaves the frame or touches a masked pixel (readings L1, L2).
+ *   stats out: 3 fp64 (device): number of kept positions, their mean flux, their population
+ *     standard deviation sigma.  The limiting magnitude is zp - 2.5 log10(5 sigma) (host arithmetic).
+ * 0 < radius <= 64.  Enqueues two kernels on `stream`; never synchronises.  Needs no plan. */
+sfft_status sfft_aperture_stats(const double* D, const unsigned char* mask, int H, int W,
+                                const double* xs, const double* ys, int n, double radius,
+                                double* flux, double* stats, void* stream);
+
 /* ---- diagnostics (not on the hot path) ------------------------------------------------------ */
 
 /* Per-stage device times of the most recent build/solve/subtract calls are NOT recorded by the

@@ -11,6 +11,9 @@ from .binding import (  # noqa: F401
     lib_path,
     load_library,
     EXPORTED_SYMBOLS,
+    median_combine,
+    aperture_stats,
 )
 
-__all__ = ["synth", "SfftPlan", "SfftError", "lib_path", "load_library", "EXPORTED_SYMBOLS"]
+__all__ = ["synth", "SfftPlan", "SfftError", "lib_path", "load_library", "EXPORTED_SYMBOLS",
+           "median_combine", "aperture_stats"]

@@ -18,7 +18,7 @@ EXPORTED_SYMBOLS = [
     "sfft_plan_create", "sfft_plan_destroy", "sfft_num_coeffs", "sfft_workspace_bytes",
     "sfft_status_string", "sfft_build_system", "sfft_solve", "sfft_subtract",
     "sfft_probe_fp64", "sfft_last_launch_count", "sfft_plan_fused", "sfft_plan_set_solve_ctas", "sfft_version",
-    "sfft_profile_enable", "sfft_profile_read",
+    "sfft_profile_enable", "sfft_profile_read", "sfft_median_combine", "sfft_aperture_stats",
 ]
 
 STAGE_NAMES = ["build.row_fwd", "build.col_fwd", "build.cross_KK", "build.cross_KS",
@@ -75,6 +75,10 @@ def load_library():
     lib.sfft_plan_fused.restype = i32
     lib.sfft_plan_set_solve_ctas.argtypes = [vp, i32]
     lib.sfft_plan_set_solve_ctas.restype = i32
+    lib.sfft_median_combine.argtypes = [vp, vp, i32, ctypes.c_size_t, vp, vp]
+    lib.sfft_median_combine.restype = i32
+    lib.sfft_aperture_stats.argtypes = [vp, vp, i32, i32, vp, vp, i32, ctypes.c_double, vp, vp, vp]
+    lib.sfft_aperture_stats.restype = i32
     lib.sfft_profile_enable.argtypes = [vp, i32]
     lib.sfft_profile_enable.restype = i32
     lib.sfft_profile_read.argtypes = [vp, i32, dbl_p, ctypes.POINTER(i32), i32]
@@ -233,3 +237,39 @@ def probe_fp64(kind: int = 0, iters: int = 4096, stream=None):
     _check(lib, lib.sfft_probe_fp64(kind, iters, ctypes.byref(tf), ctypes.byref(ms),
                                     _stream_handle(stream)), "sfft_probe_fp64")
     return tf.value, ms.value
+
+
+def median_combine(Ds, scales, out=None, stream=None):
+    """sfft_median_combine: out = median_k(scales[k] * Ds[k]) per pixel.  Ds: CUDA
+    float64 tensors of one shape.  Argument marshalling only."""
+    import torch
+    lib = load_library()
+    n = len(Ds)
+    assert n == len(scales) and n >= 1
+    for D in Ds:
+        assert D.is_cuda and D.dtype == torch.float64 and D.is_contiguous() and D.shape == Ds[0].shape
+    if out is None:
+        out = torch.empty_like(Ds[0])
+    ptrs = (ctypes.c_void_p * n)(*[D.data_ptr() for D in Ds])
+    sc = (ctypes.c_double * n)(*[float(s) for s in scales])
+    st = torch.cuda.current_stream() if stream is None else stream
+    _check(lib, lib.sfft_median_combine(ptrs, sc, n, Ds[0].numel(), out.data_ptr(), st.cuda_stream), "sfft_median_combine")
+    return out
+
+
+def aperture_stats(D, mask, xs, ys, radius, stream=None):
+    """sfft_aperture_stats: fluxes at the given positions and (count, mean, sigma) of the kept ones
+    (PAPER.md:164).  D: CUDA float64 [H,W]; mask: CUDA uint8 or None; xs, ys: CUDA float64 [n]."""
+    import torch
+    lib = load_library()
+    H, W = D.shape
+    n = xs.numel()
+    assert D.is_cuda and D.dtype == torch.float64 and D.is_contiguous()
+    assert xs.is_cuda and ys.is_cuda and xs.dtype == torch.float64 and ys.dtype == torch.float64 and ys.numel() == n
+    flux = torch.empty(n, dtype=torch.float64, device=D.device)
+    stats = torch.empty(3, dtype=torch.float64, device=D.device)
+    st = torch.cuda.current_stream() if stream is None else stream
+    _check(lib, lib.sfft_aperture_stats(D.data_ptr(), 0 if mask is None else mask.data_ptr(), H, W, xs.data_ptr(),
+                                        ys.data_ptr(), n, float(radius), flux.data_ptr(), stats.data_ptr(),
+                                        st.cuda_stream), "sfft_aperture_stats")
+    return flux, stats

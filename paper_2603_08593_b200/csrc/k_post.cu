@@ -1,0 +1,182 @@
+// The two steps that follow the differencing of one CCD:
+//
+//  k_median<N>      : multi-template combination, out = median_k(scale_k * D_k) per pixel
+//                     (§2.3.2: the N_TEMP difference images are "normalized to a common
+//                     photometric zero point ... and median-combined"; N_TEMP default 5).
+//                     HBM-bound: N reads + 1 write of 8 bytes per pixel, 128-bit accesses, values
+//                     sorted in registers by a fully unrolled insertion network.
+//  k_aperture_flux  : Monte-Carlo limiting flux (§2.3.3: "aperture fluxes at 1024 randomly
+//                     selected background positions ... deriving the 5 sigma threshold from their
+//                     standard deviation"): one warp per position sums the hard-edged disc of pixels
+//                     whose centres lie within `radius`; NaN if the disc leaves the frame or touches
+//                     a masked pixel (readings L1, L2).  The positions are inputs.
+//  k_aperture_stats : count, mean and population sigma of the kept fluxes, fixed-order tree sums.
+#include <math.h>
+#include "sfft_common.cuh"
+
+#define POST_MAXN SFFT_MAX_TEMPLATES
+
+struct MedianParams {
+  const double* D[POST_MAXN];
+  double scale[POST_MAXN];
+  double* out;
+  size_t npix;
+};
+
+template <int N>
+__device__ __forceinline__ double median_of(double* v) {
+  // insertion sort with compile-time indices (stays in registers)
+#pragma unroll
+  for (int i = 1; i < N; ++i) {
+#pragma unroll
+    for (int j = i; j > 0; --j) {
+      const double a = v[j - 1], b = v[j];
+      v[j - 1] = fmin(a, b);
+      v[j] = fmax(a, b);
+    }
+  }
+  if (N & 1) return v[N / 2];
+  return 0.5 * (v[(N - 1) / 2] + v[N / 2]);
+}
+
+template <int N>
+__global__ void __launch_bounds__(256) k_median(MedianParams P) {
+  const size_t npair = P.npix >> 1;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < npair; i += (size_t)gridDim.x * blockDim.x) {
+    double a[N], b[N];
+#pragma unroll
+    for (int k = 0; k < N; ++k) {
+      const double2 t = __ldcs(reinterpret_cast<const double2*>(P.D[k]) + i);
+      a[k] = t.x * P.scale[k];
+      b[k] = t.y * P.scale[k];
+    }
+    __stcs(reinterpret_cast<double2*>(P.out) + i, make_double2(median_of<N>(a), median_of<N>(b)));
+  }
+  if ((P.npix & 1) && blockIdx.x == 0 && threadIdx.x == 0) {   // odd tail
+    double a[N];
+#pragma unroll
+    for (int k = 0; k < N; ++k) a[k] = P.D[k][P.npix - 1] * P.scale[k];
+    P.out[P.npix - 1] = median_of<N>(a);
+  }
+}
+
+template <int N>
+static sfft_status launch_median_t(const MedianParams& P, cudaStream_t st) {
+  size_t blocks = ((P.npix >> 1) + 255) / 256;
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  if (blocks < 1) blocks = 1;
+  k_median<N><<<(unsigned)blocks, 256, 0, st>>>(P);
+  SFFT_LAUNCH_CHECK();
+  return SFFT_OK;
+}
+
+__global__ void __launch_bounds__(256) k_aperture_flux(const double* __restrict__ D, const unsigned char* __restrict__ mask,
+                                                       int H, int W, const double* __restrict__ xs,
+                                                       const double* __restrict__ ys, int n, double radius,
+                                                       double* flux) {
+  const int a = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (a >= n) return;
+  const double x0 = xs[a], y0 = ys[a], r2 = radius * radius;
+  const int ylo = (int)ceil(y0 - radius), yhi = (int)floor(y0 + radius);
+  const int xlo = (int)ceil(x0 - radius), xhi = (int)floor(x0 + radius);
+  const bool inside = ylo >= 0 && xlo >= 0 && yhi <= H - 1 && xhi <= W - 1;   // warp-uniform
+  double acc = 0.0;
+  int bad = 0;
+  if (inside) {
+    const int bw = xhi - xlo + 1, npx = bw * (yhi - ylo + 1);
+    for (int e = lane; e < npx; e += 32) {
+      const int y = ylo + e / bw, x = xlo + e % bw;
+      const double dx = (double)x - x0, dy = (double)y - y0;
+      if (dx * dx + dy * dy <= r2) {
+        if (mask && mask[(size_t)y * W + x]) bad = 1;
+        acc += D[(size_t)y * W + x];
+      }
+    }
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    acc += __shfl_xor_sync(0xffffffffu, acc, off);
+    bad |= __shfl_xor_sync(0xffffffffu, bad, off);
+  }
+  if (lane == 0) flux[a] = (inside && !bad) ? acc : nan("");
+}
+
+// stats[0] = number of kept (non-NaN) fluxes, stats[1] = their mean, stats[2] = population sigma
+__global__ void __launch_bounds__(1024) k_aperture_stats(const double* __restrict__ flux, int n, double* stats) {
+  __shared__ double red[1024];
+  __shared__ double s_mean;
+  const int tid = threadIdx.x;
+  auto block_sum = [&](double v) {
+    red[tid] = v;
+    __syncthreads();
+    for (int off = 512; off > 0; off >>= 1) {
+      if (tid < off) red[tid] += red[tid + off];
+      __syncthreads();
+    }
+    const double r = red[0];
+    __syncthreads();
+    return r;
+  };
+  double cnt = 0.0, sum = 0.0;
+  for (int i = tid; i < n; i += 1024) {
+    const double f = flux[i];
+    if (f == f) { cnt += 1.0; sum += f; }
+  }
+  const double N = block_sum(cnt), S = block_sum(sum);
+  if (tid == 0) s_mean = N > 0.0 ? S / N : nan("");
+  __syncthreads();
+  const double mean = s_mean;
+  double sq = 0.0;
+  for (int i = tid; i < n; i += 1024) {
+    const double f = flux[i];
+    if (f == f) sq += (f - mean) * (f - mean);
+  }
+  const double Q = block_sum(sq);
+  if (tid == 0) {
+    stats[0] = N;
+    stats[1] = mean;
+    stats[2] = N > 0.0 ? sqrt(Q / N) : nan("");
+  }
+}
+
+extern "C" {
+
+sfft_status sfft_median_combine(const double* const* D, const double* scale, int n, size_t npix, double* out,
+                                void* stream) {
+  if (!D || !scale || !out || n < 1 || n > POST_MAXN || npix == 0) return SFFT_ERR_INVALID_ARG;
+  MedianParams P;
+  for (int k = 0; k < n; ++k) {
+    if (!D[k] || (((uintptr_t)D[k]) & 15) || D[k] == out) return SFFT_ERR_INVALID_ARG;
+    P.D[k] = D[k];
+    P.scale[k] = scale[k];
+  }
+  if (((uintptr_t)out) & 15) return SFFT_ERR_INVALID_ARG;
+  P.out = out; P.npix = npix;
+  cudaStream_t st = (cudaStream_t)stream;
+  switch (n) {
+    case 1: return launch_median_t<1>(P, st);
+    case 2: return launch_median_t<2>(P, st);
+    case 3: return launch_median_t<3>(P, st);
+    case 4: return launch_median_t<4>(P, st);
+    case 5: return launch_median_t<5>(P, st);
+    case 6: return launch_median_t<6>(P, st);
+    case 7: return launch_median_t<7>(P, st);
+    case 8: return launch_median_t<8>(P, st);
+    default: return launch_median_t<9>(P, st);
+  }
+}
+
+sfft_status sfft_aperture_stats(const double* D, const unsigned char* mask, int H, int W, const double* xs,
+                                const double* ys, int n, double radius, double* flux, double* stats,
+                                void* stream) {
+  if (!D || !xs || !ys || !flux || !stats || H < 1 || W < 1 || n < 1 || !(radius > 0.0) || radius > 64.0)
+    return SFFT_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  k_aperture_flux<<<(n + 7) / 8, 256, 0, st>>>(D, mask, H, W, xs, ys, n, radius, flux);
+  SFFT_LAUNCH_CHECK();
+  k_aperture_stats<<<1, 1024, 0, st>>>(flux, n, stats);
+  SFFT_LAUNCH_CHECK();
+  return SFFT_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,75 @@
+"""Parity of the two post-differencing kernels (sfft_median_combine, sfft_aperture_stats) against
+oracle/post_oracle.py, through the C ABI.  Median: bit-exact (it selects values, or averages two).
+Aperture fluxes: 1e-12 of sum|D| over the disc (the summation order differs); dropped positions
+must agree exactly; sigma to 1e-10 relative."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import post_oracle as po
+from paper_2603_08593_b200 import aperture_stats, median_combine
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 6, 7, 8, 9])
+@pytest.mark.parametrize("shape", [(37, 53), (64, 128), (1, 1), (3, 333)])
+def test_median_combine_bit_exact(n, shape):
+    rng = np.random.default_rng(n * 100 + shape[0])
+    Ds = [40.0 * rng.standard_normal(shape) for _ in range(n)]
+    for D in Ds[:2]:   # ties and repeated values
+        D[rng.random(shape) < 0.2] = 1.5
+    sc = rng.uniform(0.7, 1.4, n)
+    out = median_combine([torch.from_numpy(D).cuda() for D in Ds], sc).cpu().numpy()
+    assert np.array_equal(out, po.median_combine(Ds, sc))
+
+
+def test_median_combine_full_ccd_sampled():
+    """5 templates at the full CCD size (the launch bench.py times): sampled pixels against the
+    definition, and the order-statistic property min <= median <= max everywhere."""
+    H, W, n = 2048, 4096, 5
+    g = torch.Generator(device="cuda").manual_seed(5)
+    Ds = [torch.randn((H, W), dtype=torch.float64, device="cuda", generator=g) * 40 for _ in range(n)]
+    sc = [1.0, 0.93, 1.1, 0.8, 1.25]
+    out = median_combine(Ds, sc)
+    stack = torch.stack([D * s for D, s in zip(Ds, sc)])
+    assert bool((out >= stack.min(0).values).all()) and bool((out <= stack.max(0).values).all())
+    assert int(((stack < out).sum(0) == 2).sum()) == H * W      # exactly two values below the median (no ties)
+    rng = np.random.default_rng(0)
+    ys, xs = rng.integers(0, H, 200), rng.integers(0, W, 200)
+    host = [D.cpu().numpy() for D in Ds]
+    for y, x in zip(ys, xs):
+        assert out[y, x].item() == sorted(sc[k] * host[k][y, x] for k in range(n))[2]
+
+
+@pytest.mark.parametrize("radius", [1.0, 2.7, 4.2, 9.5])
+def test_aperture_stats_parity(radius):
+    rng = np.random.default_rng(int(radius * 10))
+    H, W, n = 300, 420, 1024
+    D = 40.0 * rng.standard_normal((H, W)) + 3.0
+    mask = (rng.random((H, W)) < 0.002).astype(np.uint8)
+    xs, ys = rng.uniform(-2, W + 2, n), rng.uniform(-2, H + 2, n)   # some positions leave the frame
+    fo, (cnt, mean, sigma) = po.aperture_stats(D, mask, xs, ys, radius)
+    dev = lambda a: torch.from_numpy(a).cuda()
+    fg, st = aperture_stats(dev(D), dev(mask), dev(xs), dev(ys), radius)
+    fg, st = fg.cpu().numpy(), st.cpu().numpy()
+    assert np.array_equal(np.isnan(fg), np.isnan(fo))
+    assert 0 < cnt < n
+    keep = ~np.isnan(fo)
+    scale = 40.0 * 4 * radius * radius + 10
+    assert np.max(np.abs(fg[keep] - fo[keep])) <= 1e-12 * scale
+    assert st[0] == cnt
+    assert abs(st[1] - mean) <= 1e-10 * abs(sigma)
+    assert abs(st[2] - sigma) <= 1e-10 * sigma
+    # no mask: nothing but the frame edge drops a position
+    fg2, st2 = aperture_stats(dev(D), None, dev(xs), dev(ys), radius)
+    fo2, (c2, m2, s2) = po.aperture_stats(D, None, xs, ys, radius)
+    assert int(st2[0].item()) == c2 and abs(st2[2].item() - s2) <= 1e-10 * s2
+
+
+def test_aperture_all_dropped_gives_nan_stats():
+    D = torch.ones((32, 32), dtype=torch.float64, device="cuda")
+    xs = torch.tensor([0.0, 31.0], dtype=torch.float64, device="cuda")
+    ys = torch.tensor([0.0, 31.0], dtype=torch.float64, device="cuda")
+    flux, st = aperture_stats(D, None, xs, ys, 3.0)
+    assert bool(torch.isnan(flux).all()) and st[0].item() == 0 and bool(torch.isnan(st[1:]).all())
