@@ -167,6 +167,30 @@ def test_exact_recovery_on_gpu():
         assert float(D.abs().max()) <= 1e-9 * np.max(np.abs(S))
 
 
+def test_maximum_size_integer_shift_property():
+    """Largest supported frame (4096 x 4096, w = 5, DK = DB = 2, N = 732; fused path with 8 residue
+    classes): no oracle at this size, so a property that holds at any size is checked -- with
+    mask = NULL and S = roll(R, (v0, u0)) + beta0 the fit is the single delta at (u0, v0) plus the
+    constant background, and D vanishes."""
+    H = W = 4096
+    w, DK, DB = 5, 2, 2
+    g = torch.Generator(device="cuda").manual_seed(11)
+    R = torch.randn((H, W), dtype=torch.float64, device="cuda", generator=g) * 50.0
+    u0, v0, beta0 = -3, 2, 100.0
+    S = torch.roll(R, shifts=(v0, u0), dims=(0, 1)) + beta0
+    with SfftPlan(H, W, w, DK, DB) as plan:
+        assert plan.fused
+        A, b, c, info, D = plan.difference(R, S, None)
+        assert int(info.item()) == 0
+        L = (2 * w + 1) ** 2
+        c0 = torch.zeros_like(c)
+        c0[(v0 + w) * (2 * w + 1) + (u0 + w)] = 1.0
+        c0[L * 6] = beta0
+        assert float((c - c0).abs().max()) <= 1e-9 * beta0
+        assert float(D.abs().max()) <= 1e-8 * beta0
+        assert torch.equal(A, A.T)
+
+
 def test_not_positive_definite_reports_info():
     H = W = 64
     with SfftPlan(H, W, 1, 0, 0) as plan:
