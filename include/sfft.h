@@ -88,6 +88,16 @@ sfft_status sfft_solve(sfft_plan* p, const double* A, const double* b, double* c
 sfft_status sfft_subtract(sfft_plan* p, const double* R, const double* S, const double* coeffs,
                           double* D, void* stream);
 
+/* Optional overlap hint.  The first stage of sfft_subtract (row transforms of xi^p R) does not need
+ * the coefficients: this call enqueues it on the plan's side stream, ordered after everything already
+ * enqueued on `stream` and concurrent with what the caller enqueues next -- typically sfft_solve,
+ * which is latency-bound and leaves most SMs idle.  The next sfft_subtract on this plan with the SAME
+ * R pointer waits for it and skips that stage; any other R, or an intervening sfft_build_system,
+ * discards the prepared data.  Contract: R is not modified between this call and that sfft_subtract.
+ * Results are bitwise those of sfft_subtract alone.  Call order: build_system, subtract_prepare,
+ * solve, subtract. */
+sfft_status sfft_subtract_prepare(sfft_plan* p, const double* R, void* stream);
+
 /* ---- steps that follow the differencing of one CCD ---------- */
 
 #define SFFT_MAX_TEMPLATES 9

@@ -16,7 +16,7 @@ _LIB_NAME = "libsfft.so"
 # every symbol include/sfft.h declares (tests check the built library exports all of them)
 EXPORTED_SYMBOLS = [
     "sfft_plan_create", "sfft_plan_destroy", "sfft_num_coeffs", "sfft_workspace_bytes",
-    "sfft_status_string", "sfft_build_system", "sfft_solve", "sfft_subtract",
+    "sfft_status_string", "sfft_build_system", "sfft_solve", "sfft_subtract", "sfft_subtract_prepare",
     "sfft_probe_fp64", "sfft_last_launch_count", "sfft_plan_fused", "sfft_plan_set_solve_ctas", "sfft_version",
     "sfft_profile_enable", "sfft_profile_read", "sfft_median_combine", "sfft_aperture_stats",
 ]
@@ -71,6 +71,8 @@ def load_library():
     lib.sfft_probe_fp64.restype = i32
     lib.sfft_last_launch_count.argtypes = [vp, i32]
     lib.sfft_last_launch_count.restype = i32
+    lib.sfft_subtract_prepare.argtypes = [vp, vp, vp]
+    lib.sfft_subtract_prepare.restype = i32
     lib.sfft_plan_fused.argtypes = [vp]
     lib.sfft_plan_fused.restype = i32
     lib.sfft_plan_set_solve_ctas.argtypes = [vp, i32]
@@ -186,9 +188,17 @@ class SfftPlan:
             _stream_handle(stream)), "sfft_subtract")
         return D
 
+    def subtract_prepare(self, R, stream=None):
+        """sfft_subtract_prepare: start the coefficient-independent stage of the next subtract(R, ...)
+        on the plan's side stream (overlaps the solve).  R must stay unmodified until that subtract."""
+        import torch
+        _check(self._lib, self._lib.sfft_subtract_prepare(
+            self._p, _dev_ptr(R, torch.float64, self.H * self.W, "R"), _stream_handle(stream)), "sfft_subtract_prepare")
+
     def difference(self, R, S, mask, stream=None):
-        """One pass of the whole hot path: build -> solve -> subtract (device tensors in/out)."""
+        """One pass of the whole hot path: build -> (subtract_prepare) -> solve -> subtract."""
         A, b = self.build_system(R, S, mask, stream=stream)
+        self.subtract_prepare(R, stream=stream)
         c, info = self.solve(A, b, stream=stream)
         D = self.subtract(R, S, c, stream=stream)
         return A, b, c, info, D

@@ -466,6 +466,9 @@ sfft_status sfft_launch_solve(sfft_plan* p, const double* A, const double* b, do
   if (want < 1) want = 1;
   if (grid > want) grid = want;
   if (p->cholMaxCtas > 0 && grid > p->cholMaxCtas) grid = p->cholMaxCtas;
+  // a prepared subtract stage is running on the side stream: leave about a third of the SMs to it
+  // (the solve is latency-bound: 96 instead of 148 CTAs cost it ~2 %)
+  if (p->cholMaxCtas == 0 && p->prepValid && grid > (p->num_sms * 13) / 20) grid = (p->num_sms * 13) / 20;
   const size_t smemF = (size_t)2 * CH_PB * CH_LDS * sizeof(double);
   SFFT_CUDA_TRY(cudaFuncSetAttribute(k_chol_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smemF));
   SFFT_CUDA_TRY(cudaLaunchCooperativeKernel((const void*)k_chol_fused, dim3(grid), dim3(CH_THREADS), args, smemF, st));

@@ -186,12 +186,23 @@ static sfft_status launch_mix_t(const MixParams& MP, cudaStream_t st) {
 sfft_status sfft_launch_row_inv_sub(sfft_plan* p, const double* S, const double* c, double* D,
                                     cudaStream_t st, int* nl);
 
+// row spectra of xi^p R (unmasked), p = 0..DK, into the row-pass scratch
+sfft_status sfft_launch_subtract_rows(sfft_plan* p, const double* R, cudaStream_t st, int* nl) {
+  ProfScope ps(p, 6, st);
+  return sfft_launch_row_fwd(p, R, R, nullptr, false, p->T, p->NC, true, false, st, nl);
+}
+
 sfft_status sfft_launch_subtract(sfft_plan* p, const double* R, const double* S, const double* c,
                                  double* D, cudaStream_t st, int* nl) {
-  // 1. row spectra of xi^p R (unmasked), p = 0..DK, into the row-pass scratch
+  // 1. row spectra of xi^p R: already there if sfft_subtract_prepare ran for this R
   sfft_status s;
-  { ProfScope ps(p, 6, st); s = sfft_launch_row_fwd(p, R, S, nullptr, false, p->T, p->NC, true, false, st, nl); }
-  if (s != SFFT_OK) return s;
+  if (p->prepValid && p->prepR == R) {
+    SFFT_CUDA_TRY(cudaStreamWaitEvent(st, p->evPrep, 0));
+  } else {
+    s = sfft_launch_subtract_rows(p, R, st, nl);
+    if (s != SFFT_OK) return s;
+  }
+  p->prepValid = 0;
   ProfScope* pmix = new ProfScope(p, 7, st);
   // 2. x-phase table of the kernel coefficients
   ETabParams EP;

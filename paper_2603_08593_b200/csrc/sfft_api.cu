@@ -73,6 +73,7 @@ static void plan_free(sfft_plan* p) {
   if (p->evFork) cudaEventDestroy(p->evFork);
   if (p->evJoin) cudaEventDestroy(p->evJoin);
   if (p->evRow) cudaEventDestroy(p->evRow);
+  if (p->evPrep) cudaEventDestroy(p->evPrep);
   for (int i = 0; i < 2 * SFFT_PROF_MAX; ++i) if (p->prof_ev[i]) cudaEventDestroy(p->prof_ev[i]);
   delete p;
 }
@@ -172,7 +173,8 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   if (cudaStreamCreateWithPriority(&p->side, cudaStreamNonBlocking, prHi) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->evFork, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->evJoin, cudaEventDisableTiming) != cudaSuccess ||
-      cudaEventCreateWithFlags(&p->evRow, cudaEventDisableTiming) != cudaSuccess) {
+      cudaEventCreateWithFlags(&p->evRow, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&p->evPrep, cudaEventDisableTiming) != cudaSuccess) {
     cudaGetLastError();
     plan_free(p);
     return SFFT_ERR_CUDA;
@@ -257,6 +259,7 @@ sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S, co
     return SFFT_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   int nl = 0;
+  p->prepValid = 0;   // the row-pass scratch is about to be overwritten
   // a1 + a2 (row pass): m xi^p R (p<=DK), m S, with the fused moment reductions
   // (sum m xi^a, sum m S xi^p, sum m R xi^a)
   sfft_status s;
@@ -305,10 +308,27 @@ sfft_status sfft_subtract(sfft_plan* p, const double* R, const double* S, const 
                           void* stream) {
   if (!p || !R || !S || !coeffs || !D) return SFFT_ERR_INVALID_ARG;
   if (!aligned16(R) || !aligned16(S) || !aligned16(D) || D == R || D == S) return SFFT_ERR_INVALID_ARG;
-  int nl = 0;
+  int nl = (p->prepValid && p->prepR == R) ? p->launches[2] : 0;
   sfft_status s = sfft_launch_subtract(p, R, S, coeffs, D, (cudaStream_t)stream, &nl);
   if (s != SFFT_OK) return s;
   p->launches[2] = nl;
+  return SFFT_OK;
+}
+
+sfft_status sfft_subtract_prepare(sfft_plan* p, const double* R, void* stream) {
+  if (!p || !R || !aligned16(R)) return SFFT_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  int nl = 0;
+  // ordered after everything already enqueued on `stream` (the build that used the scratch before),
+  // then concurrent with whatever the caller enqueues next (typically sfft_solve)
+  SFFT_CUDA_TRY(cudaEventRecord(p->evFork, st));
+  SFFT_CUDA_TRY(cudaStreamWaitEvent(p->side, p->evFork, 0));
+  sfft_status s = sfft_launch_subtract_rows(p, R, p->side, &nl);
+  if (s != SFFT_OK) return s;
+  SFFT_CUDA_TRY(cudaEventRecord(p->evPrep, p->side));
+  p->prepR = R;
+  p->prepValid = 1;
+  p->launches[2] = nl;   // counted with the subtract call it belongs to
   return SFFT_OK;
 }
 

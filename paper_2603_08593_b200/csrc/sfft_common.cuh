@@ -133,7 +133,10 @@ struct sfft_plan {
   // plan-owned side stream: stages of one call that do not depend on each other run concurrently
   // (forked from and joined back into the caller stream with events; no host synchronisation)
   cudaStream_t side;
-  cudaEvent_t evFork, evJoin, evRow;
+  cudaEvent_t evFork, evJoin, evRow, evPrep;
+  // sfft_subtract_prepare: the row spectra of xi^p R for the next sfft_subtract are already in T
+  const double* prepR;
+  int prepValid;
   // optional per-stage CUDA-event timing (sfft_profile_*): events are recorded on the caller
   // stream around each stage; nothing synchronises until sfft_profile_read.
   int prof_on;
@@ -188,4 +191,5 @@ sfft_status sfft_launch_solve(sfft_plan* p, const double* A, const double* b, do
                               cudaStream_t st, int* nl);
 sfft_status sfft_launch_subtract(sfft_plan* p, const double* R, const double* S, const double* c,
                                  double* D, cudaStream_t st, int* nl);
+sfft_status sfft_launch_subtract_rows(sfft_plan* p, const double* R, cudaStream_t st, int* nl);
 sfft_status sfft_run_probe(int kind, int iters, double* tflops, double* ms, cudaStream_t st);
