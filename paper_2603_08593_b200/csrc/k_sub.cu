@@ -196,9 +196,9 @@ sfft_status sfft_launch_subtract(sfft_plan* p, const double* R, const double* S,
                                  double* D, cudaStream_t st, int* nl) {
   // 1. row spectra of xi^p R: already there if sfft_subtract_prepare ran for this R
   sfft_status s;
-  if (p->prepValid && p->prepR == R) {
-    SFFT_CUDA_TRY(cudaStreamWaitEvent(st, p->evPrep, 0));
-  } else {
+  // (a pending prepare always has to finish first: it writes the same scratch)
+  if (p->prepValid) SFFT_CUDA_TRY(cudaStreamWaitEvent(st, p->evPrep, 0));
+  if (!(p->prepValid && p->prepR == R)) {
     s = sfft_launch_subtract_rows(p, R, st, nl);
     if (s != SFFT_OK) return s;
   }

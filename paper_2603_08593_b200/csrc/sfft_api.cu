@@ -259,7 +259,9 @@ sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S, co
     return SFFT_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   int nl = 0;
-  p->prepValid = 0;   // the row-pass scratch is about to be overwritten
+  // the row-pass scratch is about to be overwritten: an unconsumed prepare finishes first, then is dropped
+  if (p->prepValid) SFFT_CUDA_TRY(cudaStreamWaitEvent(st, p->evPrep, 0));
+  p->prepValid = 0;
   // a1 + a2 (row pass): m xi^p R (p<=DK), m S, with the fused moment reductions
   // (sum m xi^a, sum m S xi^p, sum m R xi^a)
   sfft_status s;

@@ -228,3 +228,32 @@ def test_non_default_stream():
         A0, b0, c0, info0, D0 = plan.difference(Rd, Sd, Md)
         torch.cuda.synchronize()
         assert torch.equal(D, D0) and torch.equal(c, c0)
+
+
+def test_subtract_prepare_is_bitwise_neutral_and_safe():
+    """sfft_subtract_prepare only moves work: D is bitwise the same with and without it; a prepare for
+    another R, or one followed by a new build_system, is discarded."""
+    pr = synth.make_pair("small")
+    cfg = pr.cfg
+    with SfftPlan(cfg.H, cfg.W, cfg.w, cfg.DK, cfg.DB) as plan:
+        R, S, M = dev(pr.R), dev(pr.S), dev(pr.mask)
+        A, b = plan.build_system(R, S, M)
+        c, info = plan.solve(A, b)
+        D0 = plan.subtract(R, S, c).clone()
+        # prepared for the same R
+        plan.subtract_prepare(R)
+        c1, _ = plan.solve(A, b)
+        assert torch.equal(plan.subtract(R, S, c1), D0)
+        # prepared for ANOTHER image: must not be used
+        R2 = (R * 1.5).contiguous()
+        plan.subtract_prepare(R2)
+        assert torch.equal(plan.subtract(R, S, c), D0)
+        # prepared, then the scratch is reused by a build: must not be used either
+        plan.subtract_prepare(R)
+        plan.build_system(R, S, M)
+        assert torch.equal(plan.subtract(R, S, c), D0)
+        # a prepare is consumed by one subtract only
+        plan.subtract_prepare(R)
+        assert torch.equal(plan.subtract(R, S, c), D0)
+        assert torch.equal(plan.subtract(R, S, c), D0)
+        torch.cuda.synchronize()
