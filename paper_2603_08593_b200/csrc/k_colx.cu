@@ -301,7 +301,7 @@ static sfft_status launch_colx_d(const ColxParams& P, cudaStream_t st) {
   }
 }
 
-// lag half-range the kernel is instantiated with for kernel half-width w (= stride of twLag)
+// lag half-range the kernel is instantiated with for kernel half-width w
 int sfft_colx_dinst(int w) { return w == 0 ? 1 : 2 * w; }
 
 bool sfft_colx_supported(int H, int nPair) { return (H == 1024 || H == 2048 || H == 4096) && nPair <= 32; }
