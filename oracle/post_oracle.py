@@ -80,3 +80,64 @@ def aperture_stats(D, mask, xs, ys, radius):
 def limiting_magnitude(sigma, zero_point):
     """m_lim = zp - 2.5 log10(5 sigma)  (reading L5)."""
     return zero_point - 2.5 * math.log10(5.0 * sigma)
+
+
+# --------------------------------------------------------------------------- resampling (NEXT-4)
+# PAPER.md:156 (§2.3.2): "We first reproject the new science image onto the WCS of the corresponding
+# template image(s) using SWARP ... ensuring pixel-level alignment"; PAPER.md:96, 118 (§2.1.1): archival
+# exposures and their data-quality masks are "resampled onto the expected WCS of the target CCD";
+# "the resampled ood images are discretized using an empirical threshold of 0.3: pixels with values
+# above 0.3 are flagged as bad (set to 2^1), and others are flagged as good (set to 2^0)".
+# The paper gives neither the interpolant nor a WCS; readings (DESIGN.md):
+#   R1 the pixel map is an affine one, x_in = M0 + M1 x_out + M2 y_out, y_in = M3 + M4 x_out + M5 y_out
+#      (a synthetic stand-in for the WCS pair; pixel centres at integer coordinates);
+#   R2 the interpolant is the separable Lanczos kernel of order a (SWarp's default resampling is
+#      LANCZOS3): L(t) = sinc(t) sinc(t/a) for |t| < a, else 0, taps at floor(x_in) - a + 1 .. + a;
+#   R3 the 2a x 2a weights are divided by their sum (a constant image stays constant); no Jacobian
+#      flux factor is applied;
+#   R4 an output pixel whose taps leave the input frame is set to 0 and reported as outside;
+#   R5 masks: the 0/1 bad indicator is interpolated with the same weights, value > 0.3 -> 2 (bad),
+#      else 1 (good); outside pixels are bad.
+
+
+def _lanczos(t, a):
+    t = abs(t)
+    if t >= a:
+        return 0.0
+    if t == 0.0:
+        return 1.0
+    if t == math.floor(t):
+        return 0.0          # sinc vanishes at the non-zero integers (exactly, not to rounding)
+    pt = math.pi * t
+    return a * math.sin(pt) * math.sin(pt / a) / (pt * pt)
+
+
+def resample_affine(img, M, Hout, Wout, a=3):
+    """(out, outside): Lanczos-a resampling of `img` through the affine map M (readings R1-R4)."""
+    Hin, Win = img.shape
+    out = np.zeros((Hout, Wout))
+    outside = np.zeros((Hout, Wout), dtype=np.uint8)
+    for yo in range(Hout):
+        for xo in range(Wout):
+            xi = M[0] + M[1] * xo + M[2] * yo
+            yi = M[3] + M[4] * xo + M[5] * yo
+            x0, y0 = math.floor(xi), math.floor(yi)
+            if x0 - a + 1 < 0 or y0 - a + 1 < 0 or x0 + a > Win - 1 or y0 + a > Hin - 1:
+                outside[yo, xo] = 1
+                continue
+            wx = [_lanczos(xi - (x0 - a + 1 + k), a) for k in range(2 * a)]
+            wy = [_lanczos(yi - (y0 - a + 1 + k), a) for k in range(2 * a)]
+            acc = 0.0
+            for j in range(2 * a):
+                row = 0.0
+                for k in range(2 * a):
+                    row += wx[k] * float(img[y0 - a + 1 + j, x0 - a + 1 + k])
+                acc += wy[j] * row
+            out[yo, xo] = acc / (sum(wx) * sum(wy))
+    return out, outside
+
+
+def resample_mask_affine(mask, M, Hout, Wout, a=3, threshold=0.3):
+    """Resampled data-quality mask: 2 = bad, 1 = good (readings R4, R5)."""
+    val, outside = resample_affine((np.asarray(mask) != 0).astype(np.float64), M, Hout, Wout, a)
+    return np.where((val > threshold) | (outside != 0), 2, 1).astype(np.uint8)

@@ -85,3 +85,56 @@ def test_stats_constant_and_white_noise():
     assert s2 == pytest.approx(5.0 * math.sqrt(57), rel=0.12)
     assert po.limiting_magnitude(s2, 30.0) == pytest.approx(30.0 - 2.5 * math.log10(5 * s2))
     assert po.limiting_magnitude(1.0, 25.0) == pytest.approx(25.0 - 2.5 * math.log10(5.0))
+
+
+# --------------------------------------------------------------------------- resampling pins
+IDENT = [0.0, 1.0, 0.0, 0.0, 0.0, 1.0]
+
+
+def test_resample_identity_and_integer_shift_are_exact():
+    rng = np.random.default_rng(8)
+    img = rng.standard_normal((24, 30))
+    out, outside = po.resample_affine(img, IDENT, 24, 30, a=3)
+    inner = outside == 0
+    assert inner[2:21, 2:27].all() and not inner[0].any() and not inner[:, -1].any()   # taps need a-1 / a pixels of margin
+    assert np.array_equal(out[inner], img[inner])            # L(0) = 1, L(k) = 0: exact
+    M = [4.0, 1.0, 0.0, -3.0, 0.0, 1.0]                      # x_in = x_out + 4, y_in = y_out - 3
+    out, outside = po.resample_affine(img, M, 24, 30, a=3)
+    for yo, xo in [(10, 10), (8, 3), (20, 20)]:
+        assert outside[yo, xo] == 0 and out[yo, xo] == img[yo - 3, xo + 4]
+    assert outside[0, 0] == 1 and out[0, 0] == 0.0           # y_in = -3 leaves the frame
+
+
+@pytest.mark.parametrize("a", [2, 3, 4])
+def test_resample_constant_and_lanczos_kernel_values(a):
+    M = [0.37, 1.01, 0.02, -0.21, -0.015, 0.99]
+    out, outside = po.resample_affine(np.full((40, 40), 7.25), M, 36, 36, a=a)
+    assert np.allclose(out[outside == 0], 7.25, rtol=1e-14)
+    # textbook values of the kernel: L(1/2) = 2a sin(pi/(2a)) / (pi^2/2 ...) written out for a = 3: 0.6079271
+    assert po._lanczos(0.0, a) == 1.0 and po._lanczos(float(a), a) == 0.0 and po._lanczos(1.0, a) == 0.0
+    assert po._lanczos(0.5, 3) == pytest.approx(3 * 1.0 * math.sin(math.pi / 6) / (math.pi ** 2 / 4), rel=1e-15)
+    assert po._lanczos(0.5, 3) == pytest.approx(0.6079271018540267, rel=1e-12)
+
+
+def test_resample_band_limited_wave_subpixel_shift():
+    """A slowly varying sinusoid sampled off-grid: Lanczos-3 reproduces the analytic value to a few 1e-3."""
+    y, x = np.mgrid[0:64, 0:64].astype(np.float64)
+    f = lambda xx, yy: np.sin(2 * np.pi * xx / 23.0) * np.cos(2 * np.pi * yy / 31.0)
+    M = [0.3, 1.0, 0.0, 0.45, 0.0, 1.0]
+    out, outside = po.resample_affine(f(x, y), M, 60, 60, a=3)
+    ok = outside == 0
+    exact = f(x[:60, :60] + 0.3, y[:60, :60] + 0.45)
+    assert np.max(np.abs(out[ok] - exact[ok])) < 6e-3
+    assert np.max(np.abs(out[ok] - f(x[:60, :60], y[:60, :60])[ok])) > 0.05     # and it is not the unshifted image
+
+
+def test_resample_mask_threshold():
+    mask = np.zeros((20, 20), dtype=np.uint8)
+    mask[10, 10] = 1
+    out = po.resample_mask_affine(mask, IDENT, 20, 20)
+    assert out[10, 10] == 2 and out[10, 11] == 1 and out[9, 10] == 1
+    assert out[0, 0] == 2 and out[5, 5] == 1                  # outside -> bad, clean interior -> good
+    # half-pixel shift in x: the bad pixel spreads L(0.5) = 0.608 > 0.3 onto both neighbours, the next ones get
+    # L(1.5) = -0.135 < 0.3
+    out = po.resample_mask_affine(mask, [0.5, 1.0, 0.0, 0.0, 0.0, 1.0], 20, 20)
+    assert out[10, 9] == 2 and out[10, 10] == 2 and out[10, 8] == 1 and out[10, 11] == 1
