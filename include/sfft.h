@@ -127,6 +127,29 @@ sfft_status sfft_aperture_stats(const double* D, const unsigned char* mask, int 
                                 const double* xs, const double* ys, int n, double radius,
                                 double* flux, double* stats, void* stream);
 
+/* Resampling onto another pixel grid, the step before the differencing (§2.3.2: the
+ * science image is reprojected "onto the WCS of the corresponding template image(s) using SWARP";
+ * archival exposures are "resampled onto the expected WCS of the target CCD").  The
+ * paper fixes neither the interpolant nor a WCS; readings R1-R4: the pixel map is affine,
+ *   x_in = M[0] + M[1] x_out + M[2] y_out,   y_in = M[3] + M[4] x_out + M[5] y_out
+ * (pixel centres at integer coordinates; M is a HOST array of 6), the interpolant is the separable
+ * Lanczos kernel of order a (1..4; SWarp's default is 3) with the 2a x 2a weights divided by their
+ * sum and no Jacobian flux factor; an output pixel whose taps leave the input frame is 0.
+ *   in: Hin*Win fp64 (device); out: Hout*Wout fp64 (device, not aliasing in);
+ *   outside (nullable): Hout*Wout uint8 (device), 1 where the taps left the frame, else 0.
+ * Enqueues one kernel on `stream`; needs no plan. */
+sfft_status sfft_resample_affine(const double* in, int Hin, int Win, const double* M, int a, double* out,
+                                 int Hout, int Wout, unsigned char* outside, void* stream);
+
+/* The same resampling for a data-quality mask ("the resampled ood images are discretized
+ * using an empirical threshold of 0.3: pixels with values above 0.3 are flagged as bad (set to 2^1),
+ * and others are flagged as good (set to 2^0)").  in: uint8, nonzero = bad; the 0/1 indicator is
+ * interpolated with the weights above; out: 2 where the value exceeds `threshold` or the taps leave
+ * the frame, else 1 (reading R5).  To use the result as the `mask` of sfft_build_system map 1 -> 0. */
+sfft_status sfft_resample_mask_affine(const unsigned char* in, int Hin, int Win, const double* M, int a,
+                                      double threshold, unsigned char* out, int Hout, int Wout,
+                                      void* stream);
+
 /* ---- diagnostics (not on the hot path) ------------------------------------------------------ */
 
 /* Per-stage device times of the most recent build/solve/subtract calls are NOT recorded by the

@@ -13,7 +13,9 @@ from .binding import (  # noqa: F401
     EXPORTED_SYMBOLS,
     median_combine,
     aperture_stats,
+    resample_affine,
+    resample_mask_affine,
 )
 
 __all__ = ["synth", "SfftPlan", "SfftError", "lib_path", "load_library", "EXPORTED_SYMBOLS",
-           "median_combine", "aperture_stats"]
+           "median_combine", "aperture_stats", "resample_affine", "resample_mask_affine"]

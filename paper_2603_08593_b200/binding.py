@@ -18,7 +18,7 @@ EXPORTED_SYMBOLS = [
     "sfft_plan_create", "sfft_plan_destroy", "sfft_num_coeffs", "sfft_workspace_bytes",
     "sfft_status_string", "sfft_build_system", "sfft_solve", "sfft_subtract", "sfft_subtract_prepare",
     "sfft_probe_fp64", "sfft_last_launch_count", "sfft_plan_fused", "sfft_plan_set_solve_ctas", "sfft_version",
-    "sfft_profile_enable", "sfft_profile_read", "sfft_median_combine", "sfft_aperture_stats",
+    "sfft_profile_enable", "sfft_profile_read", "sfft_median_combine", "sfft_aperture_stats", "sfft_resample_affine", "sfft_resample_mask_affine",
 ]
 
 STAGE_NAMES = ["build.row_fwd", "build.col_fwd", "build.cross_KK", "build.cross_KS",
@@ -81,6 +81,10 @@ def load_library():
     lib.sfft_median_combine.restype = i32
     lib.sfft_aperture_stats.argtypes = [vp, vp, i32, i32, vp, vp, i32, ctypes.c_double, vp, vp, vp]
     lib.sfft_aperture_stats.restype = i32
+    lib.sfft_resample_affine.argtypes = [vp, i32, i32, vp, i32, vp, i32, i32, vp, vp]
+    lib.sfft_resample_affine.restype = i32
+    lib.sfft_resample_mask_affine.argtypes = [vp, i32, i32, vp, i32, ctypes.c_double, vp, i32, i32, vp]
+    lib.sfft_resample_mask_affine.restype = i32
     lib.sfft_profile_enable.argtypes = [vp, i32]
     lib.sfft_profile_enable.restype = i32
     lib.sfft_profile_read.argtypes = [vp, i32, dbl_p, ctypes.POINTER(i32), i32]
@@ -283,3 +287,31 @@ def aperture_stats(D, mask, xs, ys, radius, stream=None):
                                         ys.data_ptr(), n, float(radius), flux.data_ptr(), stats.data_ptr(),
                                         st.cuda_stream), "sfft_aperture_stats")
     return flux, stats
+
+
+def resample_affine(img, M, Hout, Wout, a=3, stream=None):
+    """sfft_resample_affine: (out, outside) of a CUDA float64 image through the affine map M (6 floats)."""
+    import torch
+    lib = load_library()
+    assert img.is_cuda and img.dtype == torch.float64 and img.is_contiguous() and img.dim() == 2
+    out = torch.empty((Hout, Wout), dtype=torch.float64, device=img.device)
+    outside = torch.empty((Hout, Wout), dtype=torch.uint8, device=img.device)
+    Mc = (ctypes.c_double * 6)(*[float(v) for v in M])
+    st = torch.cuda.current_stream() if stream is None else stream
+    _check(lib, lib.sfft_resample_affine(img.data_ptr(), img.shape[0], img.shape[1], Mc, int(a), out.data_ptr(),
+                                         Hout, Wout, outside.data_ptr(), st.cuda_stream), "sfft_resample_affine")
+    return out, outside
+
+
+def resample_mask_affine(mask, M, Hout, Wout, a=3, threshold=0.3, stream=None):
+    """sfft_resample_mask_affine: resampled data-quality mask, 2 = bad, 1 = good."""
+    import torch
+    lib = load_library()
+    assert mask.is_cuda and mask.dtype == torch.uint8 and mask.is_contiguous() and mask.dim() == 2
+    out = torch.empty((Hout, Wout), dtype=torch.uint8, device=mask.device)
+    Mc = (ctypes.c_double * 6)(*[float(v) for v in M])
+    st = torch.cuda.current_stream() if stream is None else stream
+    _check(lib, lib.sfft_resample_mask_affine(mask.data_ptr(), mask.shape[0], mask.shape[1], Mc, int(a),
+                                              float(threshold), out.data_ptr(), Hout, Wout, st.cuda_stream),
+           "sfft_resample_mask_affine")
+    return out

@@ -11,6 +11,8 @@
 //                     whose centres lie within `radius`; NaN if the disc leaves the frame or touches
 //                     a masked pixel (readings L1, L2).  The positions are inputs.
 //  k_aperture_stats : count, mean and population sigma of the kept fluxes, fixed-order tree sums.
+//  k_resample<A>    : the step BEFORE the differencing (NEXT-4): Lanczos-A resampling of an image or a
+//                     data-quality mask through an affine pixel map.
 #include <math.h>
 #include "sfft_common.cuh"
 
@@ -139,6 +141,120 @@ __global__ void __launch_bounds__(1024) k_aperture_stats(const double* __restric
   }
 }
 
+// ---- resampling onto another pixel grid --------------
+// One thread per output pixel: affine map to the input frame, separable Lanczos-A weights
+// L(t) = sinc(t) sinc(t/A) (exact zeros at the non-zero integers), normalised by their sum, 2A x 2A
+// taps; outside the frame -> 0 and flagged.  MASK = true interpolates the 0/1 bad indicator and
+// thresholds it (> thr -> 2, else 1; outside -> 2).
+struct ResampleParams {
+  const void* in;
+  void* out;
+  unsigned char* outside;   // nullable
+  int Hin, Win, Hout, Wout;
+  double M[6];
+  double thr;
+};
+
+// The 2A Lanczos weights of one axis for the fractional offset f = x_in - floor(x_in) in [0, 1):
+// tap k sits at t_k = f + (A - 1 - k).  sin(pi t_k) = (-1)^(A-1-k) sin(pi f) and
+// sin(pi t_k / A) = sin(pi f / A) cos(pi m / A) + cos(pi f / A) sin(pi m / A), m = A - 1 - k, so one
+// sinpi and one sincospi serve all taps; f = 0 gives exact zeros except the tap at t = 0.
+__device__ __forceinline__ double rcp_fast(double a) {   // 1/a for normal a, ~1 ulp: seed + two fused Newton steps
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a));
+  const double e = fma(-a, r, 1.0);
+  r = fma(r, fma(e, e, e), r);
+  return fma(r, fma(-a, r, 1.0), r);
+}
+
+// cos(pi m / A) and sin(pi m / A) for A <= 4, |m| <= A, as compile-time constants
+__host__ __device__ constexpr double lz_unit(int A, int num) {   // cos(pi num / A), num in [0, A]
+  return num == 0 ? 1.0 : num == A ? -1.0 : 2 * num == A ? 0.0
+       : A == 3 ? (num == 1 ? 0.5 : -0.5)
+       : (num == 1 ? 0.70710678118654752440 : -0.70710678118654752440);   // A == 4, num = 1 or 3
+}
+__host__ __device__ constexpr double lz_cos(int A, int m) { return lz_unit(A, m < 0 ? -m : m); }
+__host__ __device__ constexpr double lz_sin(int A, int m) {   // sin(x) = cos(pi/2 - x); here via the table
+  const int am = m < 0 ? -m : m;
+  const double v = am == 0 || am == A ? 0.0 : 2 * am == A ? 1.0
+                 : A == 3 ? 0.86602540378443864676 : 0.70710678118654752440;
+  return m < 0 ? -v : v;
+}
+
+template <int A>
+__device__ __forceinline__ void lanczos_weights(double f, double* w) {
+  const double s1 = sinpi(f);
+  double sa, ca;
+  sincospi(f / (double)A, &sa, &ca);
+  const double pi2 = 9.86960440108935861883;   // pi^2
+#pragma unroll
+  for (int k = 0; k < 2 * A; ++k) {
+    const int m = A - 1 - k;                    // t_k = f + m, m = A-1 .. -A
+    const double t = f + (double)m;
+    const double cm = lz_cos(A, m), sm = lz_sin(A, m);   // compile-time constants after unrolling
+    const double sgn = (m & 1) ? -1.0 : 1.0;
+    const double st = sgn * s1, sta = sa * cm + ca * sm;
+    w[k] = (t == 0.0) ? 1.0 : (double)A * st * sta * rcp_fast(pi2 * t * t);
+  }
+}
+
+template <int A, bool MASK>
+__global__ void __launch_bounds__(256) k_resample(ResampleParams P) {
+  const int xo = blockIdx.x * 32 + (threadIdx.x & 31), yo = blockIdx.y * 8 + (threadIdx.x >> 5);
+  if (xo >= P.Wout || yo >= P.Hout) return;
+  const double xi = P.M[0] + P.M[1] * (double)xo + P.M[2] * (double)yo;
+  const double yi = P.M[3] + P.M[4] * (double)xo + P.M[5] * (double)yo;
+  const double fx = floor(xi), fy = floor(yi);
+  const size_t oidx = (size_t)yo * P.Wout + xo;
+  const bool inside = fx - A + 1 >= 0.0 && fy - A + 1 >= 0.0 && fx + A <= (double)(P.Win - 1) && fy + A <= (double)(P.Hin - 1);
+  if (!inside) {
+    if (MASK) reinterpret_cast<unsigned char*>(P.out)[oidx] = 2;
+    else reinterpret_cast<double*>(P.out)[oidx] = 0.0;
+    if (P.outside) P.outside[oidx] = 1;
+    return;
+  }
+  const int x0 = (int)fx - A + 1, y0 = (int)fy - A + 1;
+  double wx[2 * A], wy[2 * A], sx = 0.0, sy = 0.0;
+  lanczos_weights<A>(xi - fx, wx);
+  lanczos_weights<A>(yi - fy, wy);
+#pragma unroll
+  for (int k = 0; k < 2 * A; ++k) {
+    sx += wx[k];
+    sy += wy[k];
+  }
+  double acc = 0.0;
+#pragma unroll
+  for (int j = 0; j < 2 * A; ++j) {
+    double row = 0.0;
+    const size_t base = (size_t)(y0 + j) * P.Win + x0;
+#pragma unroll
+    for (int k = 0; k < 2 * A; ++k) {
+      const double v = MASK ? (reinterpret_cast<const unsigned char*>(P.in)[base + k] ? 1.0 : 0.0)
+                            : reinterpret_cast<const double*>(P.in)[base + k];
+      row += wx[k] * v;
+    }
+    acc += wy[j] * row;
+  }
+  const double val = acc / (sx * sy);
+  if (MASK) reinterpret_cast<unsigned char*>(P.out)[oidx] = val > P.thr ? 2 : 1;
+  else reinterpret_cast<double*>(P.out)[oidx] = val;
+  if (P.outside) P.outside[oidx] = 0;
+}
+
+template <bool MASK>
+static sfft_status launch_resample(const ResampleParams& P, int a, cudaStream_t st) {
+  dim3 grid((P.Wout + 31) / 32, (P.Hout + 7) / 8);
+  switch (a) {
+    case 1: k_resample<1, MASK><<<grid, 256, 0, st>>>(P); break;
+    case 2: k_resample<2, MASK><<<grid, 256, 0, st>>>(P); break;
+    case 3: k_resample<3, MASK><<<grid, 256, 0, st>>>(P); break;
+    case 4: k_resample<4, MASK><<<grid, 256, 0, st>>>(P); break;
+    default: return SFFT_ERR_UNSUPPORTED;
+  }
+  SFFT_LAUNCH_CHECK();
+  return SFFT_OK;
+}
+
 extern "C" {
 
 sfft_status sfft_median_combine(const double* const* D, const double* scale, int n, size_t npix, double* out,
@@ -177,6 +293,25 @@ sfft_status sfft_aperture_stats(const double* D, const unsigned char* mask, int 
   k_aperture_stats<<<1, 1024, 0, st>>>(flux, n, stats);
   SFFT_LAUNCH_CHECK();
   return SFFT_OK;
+}
+
+sfft_status sfft_resample_affine(const double* in, int Hin, int Win, const double* M, int a, double* out,
+                                 int Hout, int Wout, unsigned char* outside, void* stream) {
+  if (!in || !M || !out || Hin < 1 || Win < 1 || Hout < 1 || Wout < 1 || in == out) return SFFT_ERR_INVALID_ARG;
+  ResampleParams P;
+  P.in = in; P.out = out; P.outside = outside; P.Hin = Hin; P.Win = Win; P.Hout = Hout; P.Wout = Wout; P.thr = 0.0;
+  for (int i = 0; i < 6; ++i) P.M[i] = M[i];
+  return launch_resample<false>(P, a, (cudaStream_t)stream);
+}
+
+sfft_status sfft_resample_mask_affine(const unsigned char* in, int Hin, int Win, const double* M, int a,
+                                      double threshold, unsigned char* out, int Hout, int Wout, void* stream) {
+  if (!in || !M || !out || Hin < 1 || Win < 1 || Hout < 1 || Wout < 1 || in == out) return SFFT_ERR_INVALID_ARG;
+  ResampleParams P;
+  P.in = in; P.out = out; P.outside = nullptr; P.Hin = Hin; P.Win = Win; P.Hout = Hout; P.Wout = Wout;
+  P.thr = threshold;
+  for (int i = 0; i < 6; ++i) P.M[i] = M[i];
+  return launch_resample<true>(P, a, (cudaStream_t)stream);
 }
 
 }  // extern "C"
