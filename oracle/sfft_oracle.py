@@ -276,3 +276,58 @@ def sfft_difference(R, S, mask, w, DK, DB, workers=1, fourier_subtract=True):
     else:
         D = subtract_rollsum(R, S, c, w, DK, DB)
     return A, b, c, D
+
+
+# --------------------------------------------------------------------------- exact objective (NEXT-1)
+# BASELINE.json north_star: "the coefficients minimise sum D^2 over unmasked pixels".  Reading A2
+# (input masking) is what the Fourier formulation needs; the LITERAL objective keeps R and S as they
+# are and drops the masked pixels from the sum:
+#     A_ex = sum_{x unmasked} g(x) g(x)^T,   b_ex = sum_{x unmasked} g(x) S(x),
+#     g(x) = row x of the design matrix built from the UNMASKED R (and the unmasked P_t').
+# Equivalently A_ex = A(mask=None) - sum_{x masked} g(x) g(x)^T.  With it a known kernel is
+# recovered exactly under any mask (pinned in tests/test_oracle_pins.py).
+
+
+def build_system_exact_bruteforce(R, S, mask, w, DK, DB):
+    """A_ex, b_ex from the explicit design matrix of the unmasked images, masked rows dropped."""
+    G, St = design_matrix(R, S, None, w, DK, DB)
+    if mask is None:
+        return G.T @ G, G.T @ St
+    keep = (np.asarray(mask).ravel() == 0)
+    Gk = G[keep]
+    return Gk.T @ Gk, Gk.T @ St[keep]
+
+
+def design_rows(R, mask_pixels, w, DK, DB):
+    """Rows g(x) of the unmasked design matrix for the listed pixels [(y, x), ...], by explicit
+    index arithmetic (no G of the whole image): used at sizes where G does not fit."""
+    H, W = R.shape
+    xi, eta = coords(H, W)
+    out = np.zeros((len(mask_pixels), num_coeffs(w, DK, DB)))
+    sh = shifts(w)
+    L = len(sh)
+    for r, (y, x) in enumerate(mask_pixels):
+        for t, (p, q) in enumerate(monomials(DK)):
+            for s, (u, v) in enumerate(sh):
+                ys, xs = (y - v) % H, (x - u) % W
+                out[r, t * L + s] = xi[xs] ** p * eta[ys] ** q * R[ys, xs]
+        for t2, (p, q) in enumerate(monomials(DB)):
+            out[r, L * len(monomials(DK)) + t2] = xi[x] ** p * eta[y] ** q
+    return out
+
+
+def build_system_exact_fft(R, S, mask, w, DK, DB, workers=1):
+    """A_ex, b_ex as the unmasked Fourier-route system minus the masked pixels' rank-one terms."""
+    A, b = build_system_fft(R, S, None, w, DK, DB, workers=workers)
+    if mask is None:
+        return A, b
+    ys, xs = np.nonzero(np.asarray(mask))
+    pix = list(zip(ys.tolist(), xs.tolist()))
+    A = A.copy()
+    b = b.copy()
+    for i0 in range(0, len(pix), 4096):   # chunks keep the row block small
+        Gm = design_rows(R, pix[i0:i0 + 4096], w, DK, DB)
+        Sm = np.array([S[y, x] for (y, x) in pix[i0:i0 + 4096]])
+        A -= Gm.T @ Gm
+        b -= Gm.T @ Sm
+    return A, b

@@ -322,3 +322,40 @@ def test_O5_longdouble_referee_agrees():
     Al, bl = orc.build_system_fft(R, S, mask, 2, 1, 1, dtype=np.longdouble)
     assert np.max(np.abs(A - Al.astype(np.float64))) <= 1e-14 * np.max(np.abs(A))
     assert np.max(np.abs(b - bl.astype(np.float64))) <= 1e-14 * np.max(np.abs(b))
+
+
+# --------------------------------------------------------------------------- exact objective (NEXT-1)
+def test_exact_objective_recovers_a_known_kernel_under_a_mask():
+    """The literal objective (masked pixels dropped from the sum, images unmasked): S = M(R; c0) gives
+    c = c0 to 1e-9 under a random 8 % mask + border -- which the input-masking reading A2 cannot (A2')."""
+    H, W, w, DK, DB = 40, 48, 2, 1, 1
+    R, _, mask = _rand_case(H, W, 21, masked=True, border=3)
+    rng = np.random.default_rng(4)
+    N = orc.num_coeffs(w, DK, DB)
+    c0 = 0.1 * rng.standard_normal(N)
+    c0[12] = 1.0
+    c0[-3:] = [250.0, 10.0, -5.0]
+    S = orc.model_rollsum(R, c0, w, DK, DB)
+    A, b = orc.build_system_exact_bruteforce(R, S, mask, w, DK, DB)
+    c = orc.solve(A, b)
+    assert np.max(np.abs(c - c0)) <= 1e-9 * np.max(np.abs(c0))
+    # the input-masking system does not recover it (reading A2')
+    A2, b2 = orc.build_system_bruteforce(R, S, mask, w, DK, DB)
+    assert np.max(np.abs(orc.solve(A2, b2) - c0)) > 1e-4 * np.max(np.abs(c0))
+
+
+def test_exact_objective_equals_lstsq_on_unmasked_pixels_and_fft_route():
+    H, W, w, DK, DB = 32, 40, 2, 1, 2
+    R, S, mask = _rand_case(H, W, 22, masked=True, border=0)
+    A, b = orc.build_system_exact_bruteforce(R, S, mask, w, DK, DB)
+    G, St = orc.design_matrix(R, S, None, w, DK, DB)
+    keep = mask.ravel() == 0
+    c_ls = np.linalg.lstsq(G[keep], St[keep], rcond=None)[0]      # library QR/SVD on the plain definition
+    assert np.max(np.abs(orc.solve(A, b) - c_ls)) <= 1e-9 * np.max(np.abs(c_ls))
+    A2, b2 = orc.build_system_exact_fft(R, S, mask, w, DK, DB)    # unmasked Fourier route minus rank-one terms
+    assert np.max(np.abs(A2 - A)) <= 1e-12 * np.max(np.abs(A))
+    assert np.max(np.abs(b2 - b)) <= 1e-12 * np.max(np.abs(b))
+    # mask = None: both objectives coincide
+    A3, b3 = orc.build_system_exact_bruteforce(R, S, None, w, DK, DB)
+    A4, b4 = orc.build_system_bruteforce(R, S, None, w, DK, DB)
+    assert np.array_equal(A3, A4) and np.array_equal(b3, b4)
