@@ -74,6 +74,16 @@ const char* sfft_status_string(sfft_status s);
 sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S,
                               const unsigned char* mask, double* A, double* b, void* stream);
 
+/* The same system for the LITERAL objective "minimise sum D^2 over unmasked pixels" (north_star;
+ * SURVEY.md §8(f) NEXT-1): R and S are used as they are and the masked pixels are dropped from the
+ * sum, A = sum_{x unmasked} g(x) g(x)^T, b = sum_{x unmasked} g(x) S(x), g(x) the design-matrix row of
+ * the unmasked images.  Computed as sfft_build_system with mask = NULL minus the masked pixels'
+ * rank-one terms (a symmetric rank-K update, K = number of masked pixels: ~2 ms more at the full CCD
+ * with a 6-pixel border).  Recovers a known kernel exactly under any mask, which the input-masking
+ * system of sfft_build_system cannot (reading A2').  Same arguments and errors. */
+sfft_status sfft_build_system_exact(sfft_plan* p, const double* R, const double* S,
+                                    const unsigned char* mask, double* A, double* b, void* stream);
+
 /* Solve A c = b by blocked fp64 Cholesky + two triangular solves (north_star (5), a5).
  *   A, b in (device, not modified; only the lower triangle of A is read), coeffs out: N fp64.
  *   info out (device int, may be NULL): 0 = ok; k > 0 = the leading minor of order k is not

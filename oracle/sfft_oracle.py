@@ -331,3 +331,28 @@ def build_system_exact_fft(R, S, mask, w, DK, DB, workers=1):
         A -= Gm.T @ Gm
         b -= Gm.T @ Sm
     return A, b
+
+
+def exact_entry(R, S, mask, w, DK, DB, i, j=None):
+    """One entry of A_ex (or of b_ex when j is None) by a direct sum over the unmasked pixels of
+    two columns of the UNMASKED design matrix (full-size sampled checks without forming G)."""
+    keep = _good(mask, R.shape)
+    if j is None:
+        G_i = normal_entry_column(R, w, DK, DB, i)
+        return float(np.sum(keep * G_i * S))
+    return float(np.sum(keep * normal_entry_column(R, w, DK, DB, i) * normal_entry_column(R, w, DK, DB, j)))
+
+
+def normal_entry_column(R, w, DK, DB, idx):
+    """Column idx of the design matrix of the unmasked images, as an H x W image."""
+    H, W = R.shape
+    L = (2 * w + 1) ** 2
+    TK = (DK + 1) * (DK + 2) // 2
+    xi, eta = coords(H, W)
+    if idx < L * TK:
+        t, s = divmod(idx, L)
+        p, q = monomials(DK)[t]
+        u, v = shifts(w)[s]
+        return np.roll(np.multiply.outer(eta ** q, xi ** p) * R, shift=(v, u), axis=(0, 1))
+    p, q = monomials(DB)[idx - L * TK]
+    return np.multiply.outer(eta ** q, xi ** p)

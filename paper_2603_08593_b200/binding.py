@@ -16,7 +16,7 @@ _LIB_NAME = "libsfft.so"
 # every symbol include/sfft.h declares (tests check the built library exports all of them)
 EXPORTED_SYMBOLS = [
     "sfft_plan_create", "sfft_plan_destroy", "sfft_num_coeffs", "sfft_workspace_bytes",
-    "sfft_status_string", "sfft_build_system", "sfft_solve", "sfft_subtract", "sfft_subtract_prepare",
+    "sfft_status_string", "sfft_build_system", "sfft_build_system_exact", "sfft_solve", "sfft_subtract", "sfft_subtract_prepare",
     "sfft_probe_fp64", "sfft_last_launch_count", "sfft_plan_fused", "sfft_plan_set_solve_ctas", "sfft_version",
     "sfft_profile_enable", "sfft_profile_read", "sfft_median_combine", "sfft_aperture_stats", "sfft_resample_affine", "sfft_resample_mask_affine",
 ]
@@ -71,6 +71,8 @@ def load_library():
     lib.sfft_probe_fp64.restype = i32
     lib.sfft_last_launch_count.argtypes = [vp, i32]
     lib.sfft_last_launch_count.restype = i32
+    lib.sfft_build_system_exact.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    lib.sfft_build_system_exact.restype = i32
     lib.sfft_subtract_prepare.argtypes = [vp, vp, vp]
     lib.sfft_subtract_prepare.restype = i32
     lib.sfft_plan_fused.argtypes = [vp]
@@ -167,6 +169,21 @@ class SfftPlan:
             self._p, _dev_ptr(R, torch.float64, P, "R"), _dev_ptr(S, torch.float64, P, "S"),
             _dev_ptr(mask, torch.uint8, P, "mask"), _dev_ptr(A, torch.float64, self.N * self.N, "A"),
             _dev_ptr(b, torch.float64, self.N, "b"), _stream_handle(stream)), "sfft_build_system")
+        return A, b
+
+    def build_system_exact(self, R, S, mask, A=None, b=None, stream=None):
+        """sfft_build_system_exact: the normal equations of the literal objective (masked pixels
+        dropped from the sum, images used unmasked)."""
+        import torch
+        P = self.H * self.W
+        if A is None:
+            A = torch.empty((self.N, self.N), dtype=torch.float64, device=R.device)
+        if b is None:
+            b = torch.empty(self.N, dtype=torch.float64, device=R.device)
+        _check(self._lib, self._lib.sfft_build_system_exact(
+            self._p, _dev_ptr(R, torch.float64, P, "R"), _dev_ptr(S, torch.float64, P, "S"),
+            _dev_ptr(mask, torch.uint8, P, "mask"), _dev_ptr(A, torch.float64, self.N * self.N, "A"),
+            _dev_ptr(b, torch.float64, self.N, "b"), _stream_handle(stream)), "sfft_build_system_exact")
         return A, b
 
     def solve(self, A, b, coeffs=None, info=None, stream=None):

@@ -1,0 +1,287 @@
+// Exact unmasked-pixel objective (BASELINE.json north_star: "the coefficients
+// minimise sum D^2 over unmasked pixels").  With g(x) the row of the design matrix of the UNMASKED
+// images at pixel x,
+//     A_ex = sum_{x unmasked} g g^T = A(mask = NULL) - sum_{x masked} g(x) g(x)^T,
+//     b_ex = b(mask = NULL) - sum_{x masked} g(x) S(x).
+// sfft_build_system_exact runs the ordinary (Fourier) build with no mask and then subtracts the
+// masked pixels' rank-one terms: a symmetric rank-K update (K = number of masked pixels, 74 k at the
+// full CCD) of the N x N matrix, C = Gm^T Gm with the S values riding as column N.
+//
+//  k_mk_rows / k_mk_scan : ordered list of the masked pixels (per-row counts, scan, fill).
+//  k_exact_syrk          : one CTA = one 128 x 128 tile of the lower triangle x one slice of the
+//                          pixel list; the rows of Gm are GENERATED on the fly from the pixel list
+//                          (column descriptors in shared memory, the R values gathered through
+//                          L1/L2) into double-buffered 16 x 128 panels, 8 x 8 register tiles, the
+//                          next panel's gathers in flight under the current panel's 1024 DFMAs.
+//  k_exact_apply         : adds the slices in order and subtracts the tile from A (both triangles), b.
+// Every sum has a fixed order, so the result is reproducible run to run.
+#include "sfft_common.cuh"
+
+#define EX_T 128      // tile edge
+#define EX_KS 16      // pixels per panel
+#define EX_TH 256
+
+// ---- masked-pixel list ---------------------------------------------------------------------------
+template <bool FILL>
+__global__ void __launch_bounds__(256) k_mk_rows(const unsigned char* __restrict__ mask, int H, int W, int* cnt,
+                                                 const int* __restrict__ off, int* list) {
+  const int lane = threadIdx.x & 31;
+  const int y = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (y >= H) return;
+  const int base = FILL ? off[y] : 0;
+  int total = 0;
+  for (int k = 0; k < (W + 511) / 512; ++k) {   // uniform trip count for the shuffles
+    const int x0 = k * 512 + lane * 16;
+    unsigned mk = 0u;
+    if (x0 < W) {   // W is a multiple of 32
+      const uint4 m16 = *reinterpret_cast<const uint4*>(mask + (size_t)y * W + x0);
+      const unsigned wd[4] = {m16.x, m16.y, m16.z, m16.w};
+#pragma unroll
+      for (int q = 0; q < 4; ++q)
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+          if ((wd[q] >> (8 * i)) & 0xffu) mk |= 1u << (4 * q + i);
+    }
+    const int c = __popc(mk);
+    int incl = c;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += t;
+    }
+    if (FILL) {
+      int pos = base + total + incl - c;
+      while (mk) {
+        const int i = __ffs(mk) - 1;
+        mk &= mk - 1;
+        list[pos++] = y * W + x0 + i;
+      }
+    }
+    total += __shfl_sync(0xffffffffu, incl, 31);
+  }
+  if (!FILL && lane == 0) cnt[y] = total;
+}
+
+__global__ void __launch_bounds__(1024) k_mk_scan(const int* __restrict__ cnt, int* off, int H) {
+  __shared__ int part[1024];
+  const int tid = threadIdx.x;
+  const int per = (H + 1023) / 1024;
+  int loc[4] = {0, 0, 0, 0}, sum = 0;
+  for (int i = 0; i < per; ++i) {
+    const int y = tid * per + i;
+    loc[i] = y < H ? cnt[y] : 0;
+    sum += loc[i];
+  }
+  part[tid] = sum;
+  __syncthreads();
+  for (int o = 1; o < 1024; o <<= 1) {
+    const int t = tid >= o ? part[tid - o] : 0;
+    __syncthreads();
+    part[tid] += t;
+    __syncthreads();
+  }
+  int run = part[tid] - sum;
+  for (int i = 0; i < per; ++i) {
+    const int y = tid * per + i;
+    if (y < H) off[y] = run;
+    run += loc[i];
+  }
+  if (tid == 1023) off[H] = part[1023];
+}
+
+// ---- symmetric rank-K update from the masked pixels -----------------------------------------------
+struct ExactParams {
+  const double* R;
+  const double* S;
+  const int* list;    // masked pixels y*W + x, ascending
+  const int* off;     // off[H] = their number
+  double* Cpart;      // [KSplit][ntiles][EX_T*EX_T]
+  int H, W, w, L, TK, TB, N, ntb, KSplit, log2W;
+  int monoK[SFFT_MAX_T][2], monoB[SFFT_MAX_T][2];
+};
+
+// column n of the design matrix: 0 = padding, 1 = kernel column (p, q, u, v), 2 = background (p, q),
+// 3 = the S values (column N)
+struct ExCol { int kind, p, q, u, v; };
+__device__ __forceinline__ ExCol ex_column(const ExactParams& P, int n) {
+  ExCol c = {0, 0, 0, 0, 0};
+  const int nK = P.L * P.TK, S1 = 2 * P.w + 1;
+  if (n < nK) {
+    const int t = n / P.L, s = n - t * P.L;
+    c.kind = 1; c.p = P.monoK[t][0]; c.q = P.monoK[t][1]; c.u = s % S1 - P.w; c.v = s / S1 - P.w;
+  } else if (n < P.N) {
+    c.kind = 2; c.p = P.monoB[n - nK][0]; c.q = P.monoB[n - nK][1];
+  } else if (n == P.N) {
+    c.kind = 3;
+  }
+  return c;
+}
+
+__global__ void __launch_bounds__(EX_TH, 1) k_exact_syrk(ExactParams P) {
+  extern __shared__ __align__(16) double ex_pan[];   // [2 buffers][2 blocks][EX_KS][EX_T]
+  const int tid = threadIdx.x;
+  int ti = 0;
+  {
+    const int t = blockIdx.x;
+    while ((ti + 1) * (ti + 2) / 2 <= t) ++ti;
+  }
+  const int tj = blockIdx.x - ti * (ti + 1) / 2;
+  const int nm = P.off[P.H];
+  const int chunk = (((nm + P.KSplit - 1) / P.KSplit) + EX_KS - 1) / EX_KS * EX_KS;
+  const int kbeg = blockIdx.y * chunk, kend = min(nm, kbeg + chunk);
+  const int W = P.W, H = P.H;
+  const double invW = 1.0 / (double)W, invH = 1.0 / (double)H;
+
+  // generation role: this thread's column (block half = 0: rows of the tile, 1: its columns)
+  const int half = tid >> 7, gc = tid & 127;
+  const ExCol col = ex_column(P, (half == 0 ? ti : tj) * EX_T + gc);
+  double val[EX_KS];
+  int pix[EX_KS];
+  auto gather = [&](int k0) {   // issue the panel's loads (R or S values); nothing consumes them yet
+#pragma unroll
+    for (int kk = 0; kk < EX_KS; ++kk) {
+      const int k = k0 + kk;
+      pix[kk] = k < kend ? P.list[k] : -1;
+    }
+#pragma unroll
+    for (int kk = 0; kk < EX_KS; ++kk) {
+      double v = 0.0;
+      if (pix[kk] >= 0 && col.kind != 0) {
+        const int y = pix[kk] >> P.log2W, x = pix[kk] & (W - 1);   // W is a power of two
+        if (col.kind == 1) v = P.R[(size_t)((y - col.v + H) & (H - 1)) * W + ((x - col.u + W) & (W - 1))];
+        else if (col.kind == 3) v = P.S[(size_t)y * W + x];
+        else v = 1.0;
+      }
+      val[kk] = v;
+    }
+  };
+  auto finish = [&](int buf) {  // polynomial weights (at the SOURCE pixel for kernel columns), store
+    double* dst = ex_pan + ((size_t)(buf * 2 + half) * EX_KS) * EX_T + gc;
+#pragma unroll
+    for (int kk = 0; kk < EX_KS; ++kk) {
+      double v = val[kk];
+      if (pix[kk] >= 0 && (col.kind == 1 || col.kind == 2)) {
+        const int y = pix[kk] >> P.log2W, x = pix[kk] & (W - 1);
+        const int xs = (x - col.u + W) & (W - 1), ys = (y - col.v + H) & (H - 1);
+        v *= ipow((double)(2 * xs + 1 - W) * invW, col.p) * ipow((double)(2 * ys + 1 - H) * invH, col.q);
+      }
+      dst[kk * EX_T] = v;
+    }
+  };
+
+  // product role: rows {32 i + 2 ty, +1}, columns {32 i + 2 tx, +1}, i < 4
+  const int tx = tid & 15, ty = tid >> 4;
+  double acc[8][8];
+#pragma unroll
+  for (int r = 0; r < 8; ++r)
+#pragma unroll
+    for (int c = 0; c < 8; ++c) acc[r][c] = 0.0;
+
+  if (kbeg < kend) {
+    gather(kbeg);
+    finish(0);
+  }
+  __syncthreads();
+  int buf = 0;
+  for (int k0 = kbeg; k0 < kend; k0 += EX_KS, buf ^= 1) {
+    const bool more = k0 + EX_KS < kend;
+    if (more) gather(k0 + EX_KS);
+    const double* pa = ex_pan + ((size_t)(buf * 2 + 0) * EX_KS) * EX_T + 2 * ty;
+    const double* pb = ex_pan + ((size_t)(buf * 2 + 1) * EX_KS) * EX_T + 2 * tx;
+#pragma unroll 4
+    for (int kk = 0; kk < EX_KS; ++kk) {
+      double a[8], b[8];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const double2 ta = *reinterpret_cast<const double2*>(pa + kk * EX_T + 32 * i);
+        const double2 tb = *reinterpret_cast<const double2*>(pb + kk * EX_T + 32 * i);
+        a[2 * i] = ta.x; a[2 * i + 1] = ta.y;
+        b[2 * i] = tb.x; b[2 * i + 1] = tb.y;
+      }
+#pragma unroll
+      for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int c = 0; c < 8; ++c) acc[r][c] = fma(a[r], b[c], acc[r][c]);
+    }
+    if (more) finish(buf ^ 1);
+    __syncthreads();
+  }
+  double* out = P.Cpart + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * EX_T * EX_T;
+#pragma unroll
+  for (int r = 0; r < 8; ++r) {
+    const int row = 32 * (r >> 1) + 2 * ty + (r & 1);
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+      *reinterpret_cast<double2*>(out + (size_t)row * EX_T + 32 * i + 2 * tx) = make_double2(acc[r][2 * i], acc[r][2 * i + 1]);
+  }
+}
+
+// A[i][j] -= sum_ks C[i][j] (both triangles from the same sum), b[i] -= sum_ks C[N][i]
+__global__ void __launch_bounds__(256) k_exact_apply(const double* __restrict__ Cpart, double* A, double* b, int N,
+                                                     int ntiles, int KSplit) {
+  const size_t total = (size_t)N * (N + 1) / 2 + N;
+  for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (size_t)gridDim.x * blockDim.x) {
+    int i, j;
+    bool rhs = false;
+    if (e < (size_t)N * (N + 1) / 2) {   // lower-triangle entry (i >= j)
+      i = (int)((sqrt(8.0 * (double)e + 1.0) - 1.0) * 0.5);
+      while ((size_t)(i + 1) * (i + 2) / 2 <= e) ++i;
+      while ((size_t)i * (i + 1) / 2 > e) --i;
+      j = (int)(e - (size_t)i * (i + 1) / 2);
+    } else {
+      rhs = true;
+      i = N;
+      j = (int)(e - (size_t)N * (N + 1) / 2);
+    }
+    const int ti = i / EX_T, tj = j / EX_T;
+    const size_t loc = ((size_t)(ti * (ti + 1) / 2 + tj) * EX_T + (i % EX_T)) * EX_T + (j % EX_T);
+    double s = 0.0;
+    for (int ks = 0; ks < KSplit; ++ks) s += Cpart[(size_t)ks * ntiles * EX_T * EX_T + loc];
+    if (rhs) {
+      b[j] -= s;
+    } else {
+      A[(size_t)i * N + j] -= s;
+      if (i != j) A[(size_t)j * N + i] -= s;
+    }
+  }
+}
+
+size_t sfft_exact_scratch_bytes(int N) {
+  const int ntb = (N + 1 + EX_T - 1) / EX_T, ntiles = ntb * (ntb + 1) / 2;
+  int ks = (2 * 148) / ntiles;
+  if (ks < 1) ks = 1;
+  if (ks > 16) ks = 16;
+  return (size_t)ks * ntiles * EX_T * EX_T * sizeof(double);
+}
+
+sfft_status sfft_launch_exact_update(sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
+                                     double* A, double* b, cudaStream_t st, int* nl) {
+  const int H = p->H, W = p->W, rowsPerBlock = 8;
+  // the special-pixel arrays of the kernel-background chain are free once the ordinary build has finished
+  k_mk_rows<false><<<(H + rowsPerBlock - 1) / rowsPerBlock, 32 * rowsPerBlock, 0, st>>>(mask, H, W, p->spCount, nullptr, nullptr);
+  SFFT_LAUNCH_CHECK();
+  k_mk_scan<<<1, 1024, 0, st>>>(p->spCount, p->spOff, H);
+  SFFT_LAUNCH_CHECK();
+  k_mk_rows<true><<<(H + rowsPerBlock - 1) / rowsPerBlock, 32 * rowsPerBlock, 0, st>>>(mask, H, W, p->spCount, p->spOff, p->spList);
+  SFFT_LAUNCH_CHECK();
+  ExactParams P;
+  P.R = R; P.S = S; P.list = p->spList; P.off = p->spOff; P.Cpart = p->exScratch;
+  P.H = H; P.W = W; P.w = p->w; P.L = p->L; P.TK = p->TK; P.TB = p->TB; P.N = p->N;
+  P.ntb = (p->N + 1 + EX_T - 1) / EX_T;
+  P.log2W = p->log2NC + 1;
+  const int ntiles = P.ntb * (P.ntb + 1) / 2;
+  int ks = (2 * 148) / ntiles;
+  if (ks < 1) ks = 1;
+  if (ks > 16) ks = 16;
+  P.KSplit = ks;
+  for (int t = 0; t < p->TK; ++t) { P.monoK[t][0] = p->monoK[t][0]; P.monoK[t][1] = p->monoK[t][1]; }
+  for (int t = 0; t < p->TB; ++t) { P.monoB[t][0] = p->monoB[t][0]; P.monoB[t][1] = p->monoB[t][1]; }
+  const size_t smem = (size_t)2 * 2 * EX_KS * EX_T * sizeof(double);
+  SFFT_CUDA_TRY(cudaFuncSetAttribute(k_exact_syrk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  k_exact_syrk<<<dim3(ntiles, ks), EX_TH, smem, st>>>(P);
+  SFFT_LAUNCH_CHECK();
+  k_exact_apply<<<148 * 4, 256, 0, st>>>(p->exScratch, A, b, p->N, ntiles, ks);
+  SFFT_LAUNCH_CHECK();
+  *nl += 5;
+  return SFFT_OK;
+}

@@ -67,7 +67,7 @@ static void plan_free(sfft_plan* p) {
   cudaFree(p->twP512);
   cudaFree(p->twPNC); cudaFree(p->twPH); cudaFree(p->twW); cudaFree(p->twH); cudaFree(p->d_pairs); cudaFree(p->d_groups);
   cudaFree(p->T); cudaFree(p->F); cudaFree(p->Y); cudaFree(p->Cmap); cudaFree(p->rowMom);
-  cudaFree(p->mom); cudaFree(p->spCount); cudaFree(p->spOff); cudaFree(p->spList); cudaFree(p->fmFlag); cudaFree(p->fmList); cudaFree(p->kbPart); cudaFree(p->kbCorr); cudaFree(p->kbStrip); cudaFree(p->Lw); cudaFree(p->cholBar); cudaFree(p->Etab); cudaFree(p->Mhat);
+  cudaFree(p->mom); cudaFree(p->spCount); cudaFree(p->spOff); cudaFree(p->spList); cudaFree(p->fmFlag); cudaFree(p->fmList); cudaFree(p->kbPart); cudaFree(p->kbCorr); cudaFree(p->kbStrip); cudaFree(p->Lw); cudaFree(p->exScratch); cudaFree(p->cholBar); cudaFree(p->Etab); cudaFree(p->Mhat);
   free(p->h_pairs);
   if (p->side) cudaStreamDestroy(p->side);
   if (p->evFork) cudaEventDestroy(p->evFork);
@@ -209,6 +209,7 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
     dalloc((void**)&p->kbCorr, sizeof(double) * (size_t)p->TK * p->L * p->TB);
     dalloc((void**)&p->kbStrip, sizeof(double) * (size_t)p->TK * p->L * p->TB);
   }
+  dalloc((void**)&p->exScratch, sfft_exact_scratch_bytes(p->N));
   dalloc((void**)&p->Lw, sizeof(double) * (size_t)(p->N + 1) * p->ldL);
   dalloc((void**)&p->cholBar, 2 * sizeof(unsigned));
   dalloc((void**)&p->Etab, sizeof(cplx) * (size_t)p->TK * (2 * w + 1) * p->NC);
@@ -291,6 +292,19 @@ sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S, co
   if (s != SFFT_OK) return s;
   SFFT_CUDA_TRY(cudaStreamWaitEvent(st, p->evJoin, 0));
   { ProfScope ps(p, 4, st); s = sfft_launch_lag_gather(p, A, b, st, &nl); }  // a3 (kx inverse on lag rows) + a4
+  if (s != SFFT_OK) return s;
+  p->launches[0] = nl;
+  return SFFT_OK;
+}
+
+sfft_status sfft_build_system_exact(sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
+                                    double* A, double* b, void* stream) {
+  // the ordinary build on the unmasked images, then the masked pixels' rank-one terms are taken out
+  sfft_status s = sfft_build_system(p, R, S, nullptr, A, b, stream);
+  if (s != SFFT_OK || !mask) return s;
+  if (!aligned16(mask)) return SFFT_ERR_INVALID_ARG;
+  int nl = p->launches[0];
+  s = sfft_launch_exact_update(p, R, S, mask, A, b, (cudaStream_t)stream, &nl);
   if (s != SFFT_OK) return s;
   p->launches[0] = nl;
   return SFFT_OK;

@@ -122,6 +122,7 @@ struct sfft_plan {
   double* kbCorr;   // [L*TK*TB]
   double* kbStrip;  // [L*TK*TB] part of the fully masked target rows (from row moments)
   double* Lw;       // Cholesky workspace (N+1) x ldL
+  double* exScratch; // sfft_build_system_exact: partial tiles of the masked pixels' rank-K update
   int cholMaxCtas;   // cap on the CTAs of k_chol_fused (0 = one per SM); see sfft_plan_set_solve_ctas
   unsigned* cholBar; // grid-barrier counters of k_chol_fused (arrivals, finished CTAs)
   cplx* Etab;       // subtract: E[TK][2w+1][NC]
@@ -181,6 +182,9 @@ sfft_status sfft_launch_row_fwd(sfft_plan* p, const double* R, const double* S,
 sfft_status sfft_launch_col_fwd(sfft_plan* p, cudaStream_t st, int* nl);
 sfft_status sfft_launch_cross(sfft_plan* p, cudaStream_t st, int* nl);
 sfft_status sfft_launch_colx(sfft_plan* p, cudaStream_t st, int* nl);
+size_t sfft_exact_scratch_bytes(int N);
+sfft_status sfft_launch_exact_update(sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
+                                     double* A, double* b, cudaStream_t st, int* nl);
 int sfft_colx_dinst(int w);
 sfft_status sfft_colx_init();
 bool sfft_colx_supported(int H, int nPair);

@@ -257,3 +257,80 @@ def test_subtract_prepare_is_bitwise_neutral_and_safe():
         assert torch.equal(plan.subtract(R, S, c), D0)
         assert torch.equal(plan.subtract(R, S, c), D0)
         torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("H,W,w,DK,DB,border", [(64, 64, 2, 0, 0, 2), (128, 64, 2, 1, 1, 0), (64, 256, 3, 2, 2, 3),
+                                                (1024, 64, 1, 1, 2, 4), (32, 32, 5, 1, 1, 0)])
+def test_exact_objective_parity(H, W, w, DK, DB, border):
+    """sfft_build_system_exact (literal objective: masked pixels dropped, images unmasked) against the
+    oracle's Fourier-route system minus the masked pixels' rank-one terms; several tiles and slices of
+    the rank-K update, ragged tile edges (N + 1 not a multiple of 128), fused and generic plans."""
+    rng = np.random.default_rng(H + W + w)
+    R = 50.0 * rng.standard_normal((H, W)) + 500.0 * (rng.random((H, W)) > 0.98)
+    S = 0.7 * np.roll(R, (1, -1), (0, 1)) + 30.0 * rng.standard_normal((H, W)) + 200.0
+    mask = (rng.random((H, W)) < 0.05).astype(np.uint8)
+    if border:
+        mask[:border] = 1; mask[-border:] = 1; mask[:, :border] = 1; mask[:, -border:] = 1
+    Ao, bo = orc.build_system_exact_fft(R, S, mask, w, DK, DB, workers=8)
+    with SfftPlan(H, W, w, DK, DB) as plan:
+        A, b = plan.build_system_exact(dev(R), dev(S), dev(mask))
+        A2, b2 = plan.build_system_exact(dev(R), dev(S), dev(mask))
+        assert torch.equal(A, A2) and torch.equal(b, b2)          # reproducible
+        A, b = A.cpu().numpy(), b.cpu().numpy()
+        L = (2 * w + 1) ** 2
+        TK = (DK + 1) * (DK + 2) // 2
+        check_system(A, b, Ao, bo, L, TK)
+        # mask = None: identical to the ordinary build
+        A0, b0 = plan.build_system_exact(dev(R), dev(S), None)
+        A1, b1 = plan.build_system(dev(R), dev(S), None)
+        assert torch.equal(A0, A1) and torch.equal(b0, b1)
+
+
+def test_exact_objective_recovers_kernel_under_mask_on_gpu():
+    """S = M(R; c0) with a border + random mask: the exact objective returns c0 to 1e-9 and D = 0 on
+    the GPU path alone; the input-masking system does not (reading A2')."""
+    H, W, w, DK, DB = 128, 256, 2, 2, 2
+    R, _ = synth.white_noise_pair(H, W, 78)
+    rng = np.random.default_rng(2)
+    L, TK = 25, 6
+    c0 = np.zeros(L * TK + 6)
+    c0[:L] = rng.random(L)
+    c0[:L] /= c0[:L].sum()
+    c0[L:L * TK] = 0.1 * rng.standard_normal(L * (TK - 1))
+    c0[L * TK:] = [300.0, 20.0, -10.0, 5.0, 3.0, -4.0]
+    S = orc.model_rollsum(R, c0, w, DK, DB)
+    mask = (rng.random((H, W)) < 0.06).astype(np.uint8)
+    mask[:4] = 1; mask[-4:] = 1; mask[:, :4] = 1; mask[:, -4:] = 1
+    with SfftPlan(H, W, w, DK, DB) as plan:
+        A, b = plan.build_system_exact(dev(R), dev(S), dev(mask))
+        c, info = plan.solve(A, b)
+        assert int(info.item()) == 0
+        assert np.max(np.abs(c.cpu().numpy() - c0)) <= 1e-9 * np.max(np.abs(c0))
+        D = plan.subtract(dev(R), dev(S), c)
+        assert float(D.abs().max()) <= 1e-9 * np.max(np.abs(S))
+        A2, b2 = plan.build_system(dev(R), dev(S), dev(mask))
+        c2, _ = plan.solve(A2, b2)
+        assert np.max(np.abs(c2.cpu().numpy() - c0)) > 1e-5 * np.max(np.abs(c0))
+
+
+def test_exact_objective_full_config_sampled():
+    """Full CCD (2048 x 4096, N = 732, ~74 k masked border pixels): sampled entries of A_ex, b_ex
+    against direct sums over the unmasked pixels; symmetry; the update is a small correction of the
+    unmasked system."""
+    pr = synth.make_pair("full")
+    cfg = pr.cfg
+    with SfftPlan(cfg.H, cfg.W, cfg.w, cfg.DK, cfg.DB) as plan:
+        Rd, Sd, Md = dev(pr.R), dev(pr.S), dev(pr.mask)
+        A, b = plan.build_system_exact(Rd, Sd, Md)
+        c, info = plan.solve(A, b)
+        assert int(info.item()) == 0
+        A, b = A.cpu().numpy(), b.cpu().numpy()
+    assert np.array_equal(A, A.T)
+    rng = np.random.default_rng(3)
+    N = cfg.N
+    scale = np.max(np.abs(A))
+    pairs = [tuple(rng.integers(0, N, 2)) for _ in range(8)] + [(N - 1, N - 1), (N - 3, 17), (0, 0)]
+    for i, j in pairs:
+        assert abs(A[i, j] - orc.exact_entry(pr.R, pr.S, pr.mask, cfg.w, cfg.DK, cfg.DB, int(i), int(j))) <= TOL_AB * scale
+    for i in (0, 61, 725, 731):
+        assert abs(b[i] - orc.exact_entry(pr.R, pr.S, pr.mask, cfg.w, cfg.DK, cfg.DB, i)) <= TOL_AB * np.max(np.abs(b))

@@ -355,6 +355,10 @@ def test_exact_objective_equals_lstsq_on_unmasked_pixels_and_fft_route():
     A2, b2 = orc.build_system_exact_fft(R, S, mask, w, DK, DB)    # unmasked Fourier route minus rank-one terms
     assert np.max(np.abs(A2 - A)) <= 1e-12 * np.max(np.abs(A))
     assert np.max(np.abs(b2 - b)) <= 1e-12 * np.max(np.abs(b))
+    # sampled entries by direct sums over the unmasked pixels
+    for (i, j) in [(0, 0), (3, 40), (60, 7), (A.shape[0] - 1, 5), (A.shape[0] - 2, A.shape[0] - 1)]:
+        assert orc.exact_entry(R, S, mask, w, DK, DB, i, j) == pytest.approx(A[i, j], rel=1e-12, abs=1e-9 * np.max(np.abs(A)))
+    assert orc.exact_entry(R, S, mask, w, DK, DB, 11) == pytest.approx(b[11], rel=1e-12)
     # mask = None: both objectives coincide
     A3, b3 = orc.build_system_exact_bruteforce(R, S, None, w, DK, DB)
     A4, b4 = orc.build_system_bruteforce(R, S, None, w, DK, DB)
