@@ -20,6 +20,10 @@
 #define EX_T 128      // tile edge
 #define EX_KS 16      // pixels per panel
 #define EX_TH 256
+#ifndef EX_UNR
+#define EX_UNR 4
+#endif
+constexpr int EXU = EX_UNR;   // unroll factor of the panel loop
 
 // ---- masked-pixel list ---------------------------------------------------------------------------
 template <bool FILL>
@@ -188,7 +192,7 @@ __global__ void __launch_bounds__(EX_TH, 1) k_exact_syrk(ExactParams P) {
     if (more) gather(k0 + EX_KS);
     const double* pa = ex_pan + ((size_t)(buf * 2 + 0) * EX_KS) * EX_T + 2 * ty;
     const double* pb = ex_pan + ((size_t)(buf * 2 + 1) * EX_KS) * EX_T + 2 * tx;
-#pragma unroll 4
+#pragma unroll EXU
     for (int kk = 0; kk < EX_KS; ++kk) {
       double a[8], b[8];
 #pragma unroll
