@@ -8,11 +8,11 @@
 // full CCD) of the N x N matrix, C = Gm^T Gm with the S values riding as column N.
 //
 //  k_mk_rows / k_mk_scan : ordered list of the masked pixels (per-row counts, scan, fill).
-//  k_exact_syrk          : one CTA = one 128 x 128 tile of the lower triangle x one slice of the
-//                          pixel list; the rows of Gm are GENERATED on the fly from the pixel list
-//                          (column descriptors in shared memory, the R values gathered through
-//                          L1/L2) into double-buffered 16 x 128 panels, 8 x 8 register tiles, the
-//                          next panel's gathers in flight under the current panel's 1024 DFMAs.
+//  k_exact_syrk          : cooperative kernel, one CTA = one 128 x 128 tile of the lower triangle x
+//                          one slice of the pixel list.  Per chunk of 16384 masked pixels all CTAs
+//                          first generate the chunk's rows of Gm once (coalesced), then each adds its
+//                          slice to its tile: 8 x 8 register tiles, double-buffered 16 x 128 panels,
+//                          the next panels' loads in flight under the current panel's 1024 DFMAs.
 //  k_exact_apply         : adds the slices in order and subtracts the tile from A (both triangles), b.
 // Every sum has a fixed order, so the result is reproducible run to run.
 #include "sfft_common.cuh"
@@ -20,6 +20,7 @@
 #define EX_T 128      // tile edge
 #define EX_KS 16      // pixels per panel
 #define EX_TH 256
+#define EX_KC 16384  // masked pixels per chunk of the generated rows
 #ifndef EX_UNR
 #define EX_UNR 4
 #endif
@@ -100,6 +101,8 @@ struct ExactParams {
   const int* list;    // masked pixels y*W + x, ascending
   const int* off;     // off[H] = their number
   double* Cpart;      // [KSplit][ntiles][EX_T*EX_T]
+  double* Gm;         // [EX_KC][Npad] rows of the design matrix of the current chunk of masked pixels
+  unsigned* bar;      // grid-barrier counters (arrivals, finished CTAs)
   int H, W, w, L, TK, TB, N, ntb, KSplit, log2W;
   int monoK[SFFT_MAX_T][2], monoB[SFFT_MAX_T][2];
 };
@@ -121,9 +124,45 @@ __device__ __forceinline__ ExCol ex_column(const ExactParams& P, int n) {
   return c;
 }
 
+// software grid barrier (cooperative launch: every CTA is resident); data written before it is
+// visible after it to loads that bypass L1
+__device__ __forceinline__ void ex_grid_barrier(unsigned* ctr, unsigned& target, unsigned nblocks) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    target += nblocks;
+    __threadfence();
+    atomicAdd(ctr, 1u);
+    unsigned v;
+    do {
+      asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
+    } while (v < target);
+  }
+  __syncthreads();
+}
+
+// element (pixel, column n) of the masked rows of the design matrix
+__device__ __forceinline__ double ex_element(const ExactParams& P, int pixel, int n) {
+  const ExCol col = ex_column(P, n);
+  if (col.kind == 0) return 0.0;
+  const int W = P.W, H = P.H;
+  const int y = pixel >> P.log2W, x = pixel & (W - 1);   // W is a power of two
+  if (col.kind == 3) return P.S[(size_t)y * W + x];
+  const int xs = (x - col.u + W) & (W - 1), ys = (y - col.v + H) & (H - 1);   // u = v = 0 for background columns
+  const double pw = ipow((double)(2 * xs + 1 - W) / (double)W, col.p) * ipow((double)(2 * ys + 1 - H) / (double)H, col.q);
+  return col.kind == 1 ? pw * P.R[(size_t)ys * W + xs] : pw;
+}
+
+// Cooperative kernel, grid = (tiles of the lower triangle) x (slices).  The pixel list is walked in
+// chunks of EX_KC pixels: all CTAs first write the chunk's rows Gm[k][Npad] (every element generated
+// once, coalesced along the columns), meet at a grid barrier, then every CTA adds its slice of the
+// chunk to its 128 x 128 tile (8 x 8 register tiles; the next 16-row panels travel global -> registers
+// under the current panel's 1024 DFMAs, then into the other shared buffer), and a second barrier
+// frees the chunk buffer.
 __global__ void __launch_bounds__(EX_TH, 1) k_exact_syrk(ExactParams P) {
   extern __shared__ __align__(16) double ex_pan[];   // [2 buffers][2 blocks][EX_KS][EX_T]
   const int tid = threadIdx.x;
+  const unsigned nblocks = gridDim.x * gridDim.y;
+  unsigned target = 0;
   int ti = 0;
   {
     const int t = blockIdx.x;
@@ -131,84 +170,79 @@ __global__ void __launch_bounds__(EX_TH, 1) k_exact_syrk(ExactParams P) {
   }
   const int tj = blockIdx.x - ti * (ti + 1) / 2;
   const int nm = P.off[P.H];
-  const int chunk = (((nm + P.KSplit - 1) / P.KSplit) + EX_KS - 1) / EX_KS * EX_KS;
-  const int kbeg = blockIdx.y * chunk, kend = min(nm, kbeg + chunk);
-  const int W = P.W, H = P.H;
-  const double invW = 1.0 / (double)W, invH = 1.0 / (double)H;
-
-  // generation role: this thread's column (block half = 0: rows of the tile, 1: its columns)
-  const int half = tid >> 7, gc = tid & 127;
-  const ExCol col = ex_column(P, (half == 0 ? ti : tj) * EX_T + gc);
-  double val[EX_KS];
-  int pix[EX_KS];
-  auto gather = [&](int k0) {   // issue the panel's loads (R or S values); nothing consumes them yet
-#pragma unroll
-    for (int kk = 0; kk < EX_KS; ++kk) {
-      const int k = k0 + kk;
-      pix[kk] = k < kend ? P.list[k] : -1;
-    }
-#pragma unroll
-    for (int kk = 0; kk < EX_KS; ++kk) {
-      double v = 0.0;
-      if (pix[kk] >= 0 && col.kind != 0) {
-        const int y = pix[kk] >> P.log2W, x = pix[kk] & (W - 1);   // W is a power of two
-        if (col.kind == 1) v = P.R[(size_t)((y - col.v + H) & (H - 1)) * W + ((x - col.u + W) & (W - 1))];
-        else if (col.kind == 3) v = P.S[(size_t)y * W + x];
-        else v = 1.0;
-      }
-      val[kk] = v;
-    }
-  };
-  auto finish = [&](int buf) {  // polynomial weights (at the SOURCE pixel for kernel columns), store
-    double* dst = ex_pan + ((size_t)(buf * 2 + half) * EX_KS) * EX_T + gc;
-#pragma unroll
-    for (int kk = 0; kk < EX_KS; ++kk) {
-      double v = val[kk];
-      if (pix[kk] >= 0 && (col.kind == 1 || col.kind == 2)) {
-        const int y = pix[kk] >> P.log2W, x = pix[kk] & (W - 1);
-        const int xs = (x - col.u + W) & (W - 1), ys = (y - col.v + H) & (H - 1);
-        v *= ipow((double)(2 * xs + 1 - W) * invW, col.p) * ipow((double)(2 * ys + 1 - H) * invH, col.q);
-      }
-      dst[kk * EX_T] = v;
-    }
-  };
-
-  // product role: rows {32 i + 2 ty, +1}, columns {32 i + 2 tx, +1}, i < 4
-  const int tx = tid & 15, ty = tid >> 4;
+  const int Npad = P.ntb * EX_T;
+  const int tx = tid & 15, ty = tid >> 4;   // rows {32 i + 2 ty, +1}, columns {32 i + 2 tx, +1}, i < 4
   double acc[8][8];
 #pragma unroll
   for (int r = 0; r < 8; ++r)
 #pragma unroll
     for (int c = 0; c < 8; ++c) acc[r][c] = 0.0;
 
-  if (kbeg < kend) {
-    gather(kbeg);
-    finish(0);
-  }
-  __syncthreads();
-  int buf = 0;
-  for (int k0 = kbeg; k0 < kend; k0 += EX_KS, buf ^= 1) {
-    const bool more = k0 + EX_KS < kend;
-    if (more) gather(k0 + EX_KS);
-    const double* pa = ex_pan + ((size_t)(buf * 2 + 0) * EX_KS) * EX_T + 2 * ty;
-    const double* pb = ex_pan + ((size_t)(buf * 2 + 1) * EX_KS) * EX_T + 2 * tx;
-#pragma unroll EXU
-    for (int kk = 0; kk < EX_KS; ++kk) {
-      double a[8], b[8];
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const double2 ta = *reinterpret_cast<const double2*>(pa + kk * EX_T + 32 * i);
-        const double2 tb = *reinterpret_cast<const double2*>(pb + kk * EX_T + 32 * i);
-        a[2 * i] = ta.x; a[2 * i + 1] = ta.y;
-        b[2 * i] = tb.x; b[2 * i + 1] = tb.y;
+  for (int c0 = 0; c0 < nm; c0 += EX_KC) {
+    const int kc = min(EX_KC, nm - c0);
+    // ---- phase G: the chunk's rows of the design matrix
+    {
+      const size_t total = (size_t)kc * Npad;
+      const size_t gtid = ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * EX_TH + tid;
+      for (size_t e = gtid; e < total; e += (size_t)nblocks * EX_TH) {
+        const int k = (int)(e / Npad), n = (int)(e - (size_t)k * Npad);
+        P.Gm[e] = ex_element(P, P.list[c0 + k], n);
       }
-#pragma unroll
-      for (int r = 0; r < 8; ++r)
-#pragma unroll
-        for (int c = 0; c < 8; ++c) acc[r][c] = fma(a[r], b[c], acc[r][c]);
     }
-    if (more) finish(buf ^ 1);
+    ex_grid_barrier(P.bar, target, nblocks);
+    // ---- phase S: this CTA's slice [kbeg, kend) of the chunk
+    const int slice = (((kc + P.KSplit - 1) / P.KSplit) + EX_KS - 1) / EX_KS * EX_KS;
+    const int kbeg = blockIdx.y * slice, kend = min(kc, kbeg + slice);
+    // staging: 2 blocks x 16 rows x 128 columns = 2048 double2 per panel pair, 8 per thread
+    double2 stg[8];
+    auto fetch = [&](int k0) {
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        const int e = tid + q * EX_TH;                 // 0..2047
+        const int blk = e >> 10, r = (e >> 6) & 15, c2 = e & 63;
+        const int k = k0 + r;
+        stg[q] = k < kend ? __ldcg(reinterpret_cast<const double2*>(P.Gm + (size_t)k * Npad + (blk == 0 ? ti : tj) * EX_T) + c2)
+                          : make_double2(0.0, 0.0);
+      }
+    };
+    auto stash = [&](int buf) {
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        const int e = tid + q * EX_TH;
+        const int blk = e >> 10, r = (e >> 6) & 15, c2 = e & 63;
+        reinterpret_cast<double2*>(ex_pan + ((size_t)(buf * 2 + blk) * EX_KS + r) * EX_T)[c2] = stg[q];
+      }
+    };
+    if (kbeg < kend) {
+      fetch(kbeg);
+      stash(0);
+    }
     __syncthreads();
+    int buf = 0;
+    for (int k0 = kbeg; k0 < kend; k0 += EX_KS, buf ^= 1) {
+      const bool more = k0 + EX_KS < kend;
+      if (more) fetch(k0 + EX_KS);
+      const double* pa = ex_pan + ((size_t)(buf * 2 + 0) * EX_KS) * EX_T + 2 * ty;
+      const double* pb = ex_pan + ((size_t)(buf * 2 + 1) * EX_KS) * EX_T + 2 * tx;
+#pragma unroll EXU
+      for (int kk = 0; kk < EX_KS; ++kk) {
+        double a[8], b[8];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const double2 ta = *reinterpret_cast<const double2*>(pa + kk * EX_T + 32 * i);
+          const double2 tb = *reinterpret_cast<const double2*>(pb + kk * EX_T + 32 * i);
+          a[2 * i] = ta.x; a[2 * i + 1] = ta.y;
+          b[2 * i] = tb.x; b[2 * i + 1] = tb.y;
+        }
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+#pragma unroll
+          for (int c = 0; c < 8; ++c) acc[r][c] = fma(a[r], b[c], acc[r][c]);
+      }
+      if (more) stash(buf ^ 1);
+      __syncthreads();
+    }
+    if (c0 + EX_KC < nm) ex_grid_barrier(P.bar, target, nblocks);   // the chunk buffer is rewritten next
   }
   double* out = P.Cpart + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * EX_T * EX_T;
 #pragma unroll
@@ -217,6 +251,13 @@ __global__ void __launch_bounds__(EX_TH, 1) k_exact_syrk(ExactParams P) {
 #pragma unroll
     for (int i = 0; i < 4; ++i)
       *reinterpret_cast<double2*>(out + (size_t)row * EX_T + 32 * i + 2 * tx) = make_double2(acc[r][2 * i], acc[r][2 * i + 1]);
+  }
+  // last CTA out resets the barrier counter for the next launch
+  __syncthreads();
+  if (tid == 0) {
+    unsigned* done = P.bar + 1;
+    const unsigned old = atomicInc(done, nblocks - 1);
+    if (old == nblocks - 1) { __threadfence(); *P.bar = 0u; }
   }
 }
 
@@ -250,12 +291,21 @@ __global__ void __launch_bounds__(256) k_exact_apply(const double* __restrict__ 
   }
 }
 
-size_t sfft_exact_scratch_bytes(int N) {
-  const int ntb = (N + 1 + EX_T - 1) / EX_T, ntiles = ntb * (ntb + 1) / 2;
-  int ks = (2 * 148) / ntiles;
+static int exact_ksplit(int ntiles, int num_sms) {   // every CTA of the cooperative grid must be resident
+  int ks = num_sms / ntiles;
   if (ks < 1) ks = 1;
   if (ks > 16) ks = 16;
-  return (size_t)ks * ntiles * EX_T * EX_T * sizeof(double);
+  return ks;
+}
+
+size_t sfft_exact_scratch_bytes(int N) {
+  const int ntb = (N + 1 + EX_T - 1) / EX_T, ntiles = ntb * (ntb + 1) / 2;
+  return (size_t)16 * ntiles * EX_T * EX_T * sizeof(double);
+}
+
+size_t sfft_exact_rows_bytes(int N) {
+  const int ntb = (N + 1 + EX_T - 1) / EX_T;
+  return (size_t)EX_KC * ntb * EX_T * sizeof(double);
 }
 
 sfft_status sfft_launch_exact_update(sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
@@ -274,16 +324,16 @@ sfft_status sfft_launch_exact_update(sfft_plan* p, const double* R, const double
   P.ntb = (p->N + 1 + EX_T - 1) / EX_T;
   P.log2W = p->log2NC + 1;
   const int ntiles = P.ntb * (P.ntb + 1) / 2;
-  int ks = (2 * 148) / ntiles;
-  if (ks < 1) ks = 1;
-  if (ks > 16) ks = 16;
+  if (ntiles > p->num_sms) return SFFT_ERR_UNSUPPORTED;
+  const int ks = exact_ksplit(ntiles, p->num_sms);
   P.KSplit = ks;
+  P.Gm = p->exRows; P.bar = p->exBar;
   for (int t = 0; t < p->TK; ++t) { P.monoK[t][0] = p->monoK[t][0]; P.monoK[t][1] = p->monoK[t][1]; }
   for (int t = 0; t < p->TB; ++t) { P.monoB[t][0] = p->monoB[t][0]; P.monoB[t][1] = p->monoB[t][1]; }
   const size_t smem = (size_t)2 * 2 * EX_KS * EX_T * sizeof(double);
   SFFT_CUDA_TRY(cudaFuncSetAttribute(k_exact_syrk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  k_exact_syrk<<<dim3(ntiles, ks), EX_TH, smem, st>>>(P);
-  SFFT_LAUNCH_CHECK();
+  void* args[] = {(void*)&P};
+  SFFT_CUDA_TRY(cudaLaunchCooperativeKernel((const void*)k_exact_syrk, dim3(ntiles, ks), dim3(EX_TH), args, smem, st));
   k_exact_apply<<<148 * 4, 256, 0, st>>>(p->exScratch, A, b, p->N, ntiles, ks);
   SFFT_LAUNCH_CHECK();
   *nl += 5;

@@ -67,7 +67,7 @@ static void plan_free(sfft_plan* p) {
   cudaFree(p->twP512);
   cudaFree(p->twPNC); cudaFree(p->twPH); cudaFree(p->twW); cudaFree(p->twH); cudaFree(p->d_pairs); cudaFree(p->d_groups);
   cudaFree(p->T); cudaFree(p->F); cudaFree(p->Y); cudaFree(p->Cmap); cudaFree(p->rowMom);
-  cudaFree(p->mom); cudaFree(p->spCount); cudaFree(p->spOff); cudaFree(p->spList); cudaFree(p->fmFlag); cudaFree(p->fmList); cudaFree(p->kbPart); cudaFree(p->kbCorr); cudaFree(p->kbStrip); cudaFree(p->Lw); cudaFree(p->exScratch); cudaFree(p->cholBar); cudaFree(p->Etab); cudaFree(p->Mhat);
+  cudaFree(p->mom); cudaFree(p->spCount); cudaFree(p->spOff); cudaFree(p->spList); cudaFree(p->fmFlag); cudaFree(p->fmList); cudaFree(p->kbPart); cudaFree(p->kbCorr); cudaFree(p->kbStrip); cudaFree(p->Lw); cudaFree(p->exScratch); cudaFree(p->exRows); cudaFree(p->exBar); cudaFree(p->cholBar); cudaFree(p->Etab); cudaFree(p->Mhat);
   free(p->h_pairs);
   if (p->side) cudaStreamDestroy(p->side);
   if (p->evFork) cudaEventDestroy(p->evFork);
@@ -210,6 +210,7 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
     dalloc((void**)&p->kbStrip, sizeof(double) * (size_t)p->TK * p->L * p->TB);
   }
   dalloc((void**)&p->exScratch, sfft_exact_scratch_bytes(p->N));
+  dalloc((void**)&p->exBar, 2 * sizeof(unsigned));
   dalloc((void**)&p->Lw, sizeof(double) * (size_t)(p->N + 1) * p->ldL);
   dalloc((void**)&p->cholBar, 2 * sizeof(unsigned));
   dalloc((void**)&p->Etab, sizeof(cplx) * (size_t)p->TK * (2 * w + 1) * p->NC);
@@ -226,6 +227,7 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
       upload_twiddles(&p->twH, H) != cudaSuccess ||
       cudaMemcpy(p->d_pairs, p->h_pairs, sizeof(PairDesc) * p->nPair, cudaMemcpyHostToDevice) != cudaSuccess ||
       cudaMemcpy(p->d_groups, groups.data(), sizeof(CrossGroup) * groups.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemset(p->exBar, 0, 2 * sizeof(unsigned)) != cudaSuccess ||
       cudaMemset(p->cholBar, 0, 2 * sizeof(unsigned)) != cudaSuccess ||
       cudaMemset(p->T, 0, Tbytes) != cudaSuccess ||
       cudaMemset(p->F, 0, Fbytes) != cudaSuccess ||
@@ -303,6 +305,10 @@ sfft_status sfft_build_system_exact(sfft_plan* p, const double* R, const double*
   sfft_status s = sfft_build_system(p, R, S, nullptr, A, b, stream);
   if (s != SFFT_OK || !mask) return s;
   if (!aligned16(mask)) return SFFT_ERR_INVALID_ARG;
+  if (!p->exRows) {   // first use: the chunk buffer of generated rows (this allocation may synchronise, once)
+    if (cudaMalloc((void**)&p->exRows, sfft_exact_rows_bytes(p->N)) != cudaSuccess) { cudaGetLastError(); return SFFT_ERR_ALLOC; }
+    p->ws_bytes += sfft_exact_rows_bytes(p->N);
+  }
   int nl = p->launches[0];
   s = sfft_launch_exact_update(p, R, S, mask, A, b, (cudaStream_t)stream, &nl);
   if (s != SFFT_OK) return s;

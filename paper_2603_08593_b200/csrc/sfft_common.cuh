@@ -123,6 +123,8 @@ struct sfft_plan {
   double* kbStrip;  // [L*TK*TB] part of the fully masked target rows (from row moments)
   double* Lw;       // Cholesky workspace (N+1) x ldL
   double* exScratch; // sfft_build_system_exact: partial tiles of the masked pixels' rank-K update
+  double* exRows;    //   generated design-matrix rows of one chunk of masked pixels (allocated on first use)
+  unsigned* exBar;   //   grid-barrier counters of k_exact_syrk
   int cholMaxCtas;   // cap on the CTAs of k_chol_fused (0 = one per SM); see sfft_plan_set_solve_ctas
   unsigned* cholBar; // grid-barrier counters of k_chol_fused (arrivals, finished CTAs)
   cplx* Etab;       // subtract: E[TK][2w+1][NC]
@@ -183,6 +185,7 @@ sfft_status sfft_launch_col_fwd(sfft_plan* p, cudaStream_t st, int* nl);
 sfft_status sfft_launch_cross(sfft_plan* p, cudaStream_t st, int* nl);
 sfft_status sfft_launch_colx(sfft_plan* p, cudaStream_t st, int* nl);
 size_t sfft_exact_scratch_bytes(int N);
+size_t sfft_exact_rows_bytes(int N);
 sfft_status sfft_launch_exact_update(sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
                                      double* A, double* b, cudaStream_t st, int* nl);
 int sfft_colx_dinst(int w);
