@@ -271,14 +271,17 @@ k_chol_fused(const double* __restrict__ A, const double* __restrict__ b, double*
     const int rbelow = k0 + nb;                 // first row below the diagonal block
     // ---- panel phase: CTAs that own panel rows (and CTA 0) factor the diagonal block
     const bool has_rows = blockIdx.x * CH_WARPS < (N + 1 - rbelow);
-    if (has_rows || blockIdx.x == 0) {
+    // the factored block is written back by a CTA that owns no panel rows when there is one (the
+    // store then stays off the critical path of the rows), else by CTA 0
+    const unsigned storer = (nblocks - 1) * CH_WARPS >= (unsigned)(N + 1 - rbelow) ? nblocks - 1 : 0u;
+    if (has_rows || blockIdx.x == storer) {
       for (int e = tid; e < CH_PB * CH_PB; e += CH_THREADS) {
         const int i = e >> 6, j = e & 63;
         sd[i * CH_LDS + j] = (i < nb && j <= i) ? ld_cg(Lw + (size_t)(k0 + i) * ld + k0 + j) : (i == j ? 1.0 : 0.0);
       }
       const int bad = cta_potrf64(sd, ss, srd, colb, tid);
-      if (bad >= 0 && bad < nb && blockIdx.x == 0 && tid == 0 && info) atomicCAS(info, 0, k0 + bad + 1);
-      if (blockIdx.x == 0) {
+      if (bad >= 0 && bad < nb && blockIdx.x == storer && tid == 0 && info) atomicCAS(info, 0, k0 + bad + 1);
+      if (blockIdx.x == storer) {
         for (int e = tid; e < CH_PB * CH_PB; e += CH_THREADS) {
           const int i = e >> 6, j = e & 63;
           if (i < nb && j <= i) Lw[(size_t)(k0 + i) * ld + k0 + j] = sd[i * CH_LDS + j];
