@@ -275,6 +275,14 @@ k_chol_fused(const double* __restrict__ A, const double* __restrict__ b, double*
     // store then stays off the critical path of the rows), else by CTA 0
     const unsigned storer = (nblocks - 1) * CH_WARPS >= (unsigned)(N + 1 - rbelow) ? nblocks - 1 : 0u;
     if (has_rows || blockIdx.x == storer) {
+      // the warp's first panel row is final already: request it now, its L2 latency hides under the factor
+      const int row0 = rbelow + gw;
+      double pre0 = 0.0, pre1 = 0.0;
+      if (row0 <= N) {
+        const double* src = Lw + (size_t)row0 * ld + k0;
+        if (lane < nb) pre0 = ld_cg(src + lane);
+        if (lane + CH_NB < nb) pre1 = ld_cg(src + lane + CH_NB);
+      }
       for (int e = tid; e < CH_PB * CH_PB; e += CH_THREADS) {
         const int i = e >> 6, j = e & 63;
         sd[i * CH_LDS + j] = (i < nb && j <= i) ? ld_cg(Lw + (size_t)(k0 + i) * ld + k0 + j) : (i == j ? 1.0 : 0.0);
@@ -293,8 +301,11 @@ k_chol_fused(const double* __restrict__ A, const double* __restrict__ b, double*
       // dependent chain; the divisions are off it
       for (int row = rbelow + gw; row <= N; row += ngw) {
         double* src = Lw + (size_t)row * ld + k0;
-        double x0 = (lane < nb) ? ld_cg(src + lane) : 0.0;
-        double x1 = (lane + CH_NB < nb) ? ld_cg(src + lane + CH_NB) : 0.0;
+        double x0 = pre0, x1 = pre1;
+        if (row != row0) {
+          x0 = (lane < nb) ? ld_cg(src + lane) : 0.0;
+          x1 = (lane + CH_NB < nb) ? ld_cg(src + lane + CH_NB) : 0.0;
+        }
         const double* s0 = ss + lane * CH_LDS, *s1 = ss + (lane + CH_NB) * CH_LDS;
 #pragma unroll
         for (int j = 0; j < CH_NB; ++j) {
