@@ -467,8 +467,8 @@ def run_cuda(args, rank, world, local_rank):
         syrk_flop = 2.0 * nmask * (ntb * (ntb + 1) // 2) * 128 * 128
         post["build_system_exact"] = {"ms": round(t_ex, 3), "masked_pixels": nmask,
                                       "rank_k_update_tflops": round(syrk_flop / ((t_ex - 0.72) * 1e-3) / 1e12, 2),
-                                      "note": "ordinary build (0.72 ms) + masked-pixel list + cooperative 128x128-tiled fp64 SYRK "
-                                              "over rows generated once per 16384-pixel chunk (8 warps/SM, 250 registers)"}
+                                      "note": "ordinary build (0.72 ms) + masked-pixel list + cooperative 128x128-tiled fp64 SYRK on the "
+                                              "fp64 tensor path (mma.sync m8n8k4) over rows generated once per 16384-pixel chunk"}
         del Dt, outm
         torch.cuda.empty_cache()
 

@@ -11,8 +11,9 @@
 //  k_exact_syrk          : cooperative kernel, one CTA = one 128 x 128 tile of the lower triangle x
 //                          one slice of the pixel list.  Per chunk of 16384 masked pixels all CTAs
 //                          first generate the chunk's rows of Gm once (coalesced), then each adds its
-//                          slice to its tile: 8 x 8 register tiles, double-buffered 16 x 128 panels,
-//                          the next panels' loads in flight under the current panel's 1024 DFMAs.
+//                          slice to its tile with the fp64 tensor path (mma.sync m8n8k4, warp tiles of
+//                          64 x 32: a dense contraction is where tensor cores belong), double-buffered
+//                          16 x 128 panels, the next panels' loads in flight under the current one's MMAs.
 //  k_exact_apply         : adds the slices in order and subtracts the tile from A (both triangles), b.
 // Every sum has a fixed order, so the result is reproducible run to run.
 #include "sfft_common.cuh"
@@ -20,6 +21,7 @@
 #define EX_T 128      // tile edge
 #define EX_KS 16      // pixels per panel
 #define EX_TH 256
+#define EX_PITCH (EX_T + 4)   // panel row pitch in doubles: the (row, k) lanes of an mma fragment hit distinct banks
 #define EX_KC 16384  // masked pixels per chunk of the generated rows
 #ifndef EX_UNR
 #define EX_UNR 4
@@ -155,9 +157,9 @@ __device__ __forceinline__ double ex_element(const ExactParams& P, int pixel, in
 // Cooperative kernel, grid = (tiles of the lower triangle) x (slices).  The pixel list is walked in
 // chunks of EX_KC pixels: all CTAs first write the chunk's rows Gm[k][Npad] (every element generated
 // once, coalesced along the columns), meet at a grid barrier, then every CTA adds its slice of the
-// chunk to its 128 x 128 tile (8 x 8 register tiles; the next 16-row panels travel global -> registers
-// under the current panel's 1024 DFMAs, then into the other shared buffer), and a second barrier
-// frees the chunk buffer.
+// chunk to its 128 x 128 tile (mma.sync m8n8k4 on 64 x 32 warp tiles; the next 16-row panels travel
+// global -> registers under the current panel's MMAs, then into the other shared buffer), and a
+// second barrier frees the chunk buffer.
 __global__ void __launch_bounds__(EX_TH, 1) k_exact_syrk(ExactParams P) {
   extern __shared__ __align__(16) double ex_pan[];   // [2 buffers][2 blocks][EX_KS][EX_T]
   const int tid = threadIdx.x;
@@ -171,12 +173,18 @@ __global__ void __launch_bounds__(EX_TH, 1) k_exact_syrk(ExactParams P) {
   const int tj = blockIdx.x - ti * (ti + 1) / 2;
   const int nm = P.off[P.H];
   const int Npad = P.ntb * EX_T;
-  const int tx = tid & 15, ty = tid >> 4;   // rows {32 i + 2 ty, +1}, columns {32 i + 2 tx, +1}, i < 4
-  double acc[8][8];
+  // product role: 8 warps as 2 (rows) x 4 (columns), warp tile 64 x 32 = 8 x 4 mma tiles of
+  // m8n8k4 (fp64 tensor path, mma.sync): lane holds A[row = lane/4][k = lane%4], B[k = lane%4][col = lane/4]
+  // and C[row = lane/4][2 (lane%4), +1] of every tile -- one shared load feeds 8 multiply-adds per
+  // thread instead of 4 in the scalar form, which was bound by the shared-memory pipe
+  const int lane = tid & 31, wrp = tid >> 5;
+  const int wr = (wrp >> 2) * 64, wc = (wrp & 3) * 32;
+  const int fr = lane >> 2, fk = lane & 3;
+  double acc[8][4][2];
 #pragma unroll
-  for (int r = 0; r < 8; ++r)
+  for (int mt = 0; mt < 8; ++mt)
 #pragma unroll
-    for (int c = 0; c < 8; ++c) acc[r][c] = 0.0;
+    for (int nt = 0; nt < 4; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
 
   for (int c0 = 0; c0 < nm; c0 += EX_KC) {
     const int kc = min(EX_KC, nm - c0);
@@ -210,7 +218,7 @@ __global__ void __launch_bounds__(EX_TH, 1) k_exact_syrk(ExactParams P) {
       for (int q = 0; q < 8; ++q) {
         const int e = tid + q * EX_TH;
         const int blk = e >> 10, r = (e >> 6) & 15, c2 = e & 63;
-        reinterpret_cast<double2*>(ex_pan + ((size_t)(buf * 2 + blk) * EX_KS + r) * EX_T)[c2] = stg[q];
+        reinterpret_cast<double2*>(ex_pan + ((size_t)(buf * 2 + blk) * EX_KS + r) * EX_PITCH)[c2] = stg[q];
       }
     };
     if (kbeg < kend) {
@@ -222,22 +230,22 @@ __global__ void __launch_bounds__(EX_TH, 1) k_exact_syrk(ExactParams P) {
     for (int k0 = kbeg; k0 < kend; k0 += EX_KS, buf ^= 1) {
       const bool more = k0 + EX_KS < kend;
       if (more) fetch(k0 + EX_KS);
-      const double* pa = ex_pan + ((size_t)(buf * 2 + 0) * EX_KS) * EX_T + 2 * ty;
-      const double* pb = ex_pan + ((size_t)(buf * 2 + 1) * EX_KS) * EX_T + 2 * tx;
-#pragma unroll EXU
-      for (int kk = 0; kk < EX_KS; ++kk) {
-        double a[8], b[8];
+      const double* pa = ex_pan + ((size_t)(buf * 2 + 0) * EX_KS + fk) * EX_PITCH + wr + fr;
+      const double* pb = ex_pan + ((size_t)(buf * 2 + 1) * EX_KS + fk) * EX_PITCH + wc + fr;
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          const double2 ta = *reinterpret_cast<const double2*>(pa + kk * EX_T + 32 * i);
-          const double2 tb = *reinterpret_cast<const double2*>(pb + kk * EX_T + 32 * i);
-          a[2 * i] = ta.x; a[2 * i + 1] = ta.y;
-          b[2 * i] = tb.x; b[2 * i + 1] = tb.y;
-        }
+      for (int k4 = 0; k4 < EX_KS; k4 += 4) {
+        double a[8], b[4];
 #pragma unroll
-        for (int r = 0; r < 8; ++r)
+        for (int mt = 0; mt < 8; ++mt) a[mt] = pa[k4 * EX_PITCH + 8 * mt];
 #pragma unroll
-          for (int c = 0; c < 8; ++c) acc[r][c] = fma(a[r], b[c], acc[r][c]);
+        for (int nt = 0; nt < 4; ++nt) b[nt] = pb[k4 * EX_PITCH + 8 * nt];
+#pragma unroll
+        for (int mt = 0; mt < 8; ++mt)
+#pragma unroll
+          for (int nt = 0; nt < 4; ++nt)
+            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                         : "+d"(acc[mt][nt][0]), "+d"(acc[mt][nt][1])
+                         : "d"(a[mt]), "d"(b[nt]));
       }
       if (more) stash(buf ^ 1);
       __syncthreads();
@@ -246,12 +254,11 @@ __global__ void __launch_bounds__(EX_TH, 1) k_exact_syrk(ExactParams P) {
   }
   double* out = P.Cpart + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * EX_T * EX_T;
 #pragma unroll
-  for (int r = 0; r < 8; ++r) {
-    const int row = 32 * (r >> 1) + 2 * ty + (r & 1);
+  for (int mt = 0; mt < 8; ++mt)
 #pragma unroll
-    for (int i = 0; i < 4; ++i)
-      *reinterpret_cast<double2*>(out + (size_t)row * EX_T + 32 * i + 2 * tx) = make_double2(acc[r][2 * i], acc[r][2 * i + 1]);
-  }
+    for (int nt = 0; nt < 4; ++nt)
+      *reinterpret_cast<double2*>(out + (size_t)(wr + 8 * mt + fr) * EX_T + wc + 8 * nt + 2 * fk) =
+          make_double2(acc[mt][nt][0], acc[mt][nt][1]);
   // last CTA out resets the barrier counter for the next launch
   __syncthreads();
   if (tid == 0) {
@@ -330,7 +337,7 @@ sfft_status sfft_launch_exact_update(sfft_plan* p, const double* R, const double
   P.Gm = p->exRows; P.bar = p->exBar;
   for (int t = 0; t < p->TK; ++t) { P.monoK[t][0] = p->monoK[t][0]; P.monoK[t][1] = p->monoK[t][1]; }
   for (int t = 0; t < p->TB; ++t) { P.monoB[t][0] = p->monoB[t][0]; P.monoB[t][1] = p->monoB[t][1]; }
-  const size_t smem = (size_t)2 * 2 * EX_KS * EX_T * sizeof(double);
+  const size_t smem = (size_t)2 * 2 * EX_KS * EX_PITCH * sizeof(double);
   SFFT_CUDA_TRY(cudaFuncSetAttribute(k_exact_syrk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   void* args[] = {(void*)&P};
   SFFT_CUDA_TRY(cudaLaunchCooperativeKernel((const void*)k_exact_syrk, dim3(ntiles, ks), dim3(EX_TH), args, smem, st));
