@@ -306,13 +306,17 @@ def aperture_stats(D, mask, xs, ys, radius, stream=None):
     return flux, stats
 
 
-def resample_affine(img, M, Hout, Wout, a=3, stream=None):
+def resample_affine(img, M, Hout, Wout, a=3, out=None, outside=None, stream=None):
     """sfft_resample_affine: (out, outside) of a CUDA float64 image through the affine map M (6 floats)."""
     import torch
     lib = load_library()
     assert img.is_cuda and img.dtype == torch.float64 and img.is_contiguous() and img.dim() == 2
-    out = torch.empty((Hout, Wout), dtype=torch.float64, device=img.device)
-    outside = torch.empty((Hout, Wout), dtype=torch.uint8, device=img.device)
+    if out is None:
+        out = torch.empty((Hout, Wout), dtype=torch.float64, device=img.device)
+    if outside is None:
+        outside = torch.empty((Hout, Wout), dtype=torch.uint8, device=img.device)
+    assert out.shape == (Hout, Wout) and out.dtype == torch.float64 and out.is_contiguous()
+    assert outside.shape == (Hout, Wout) and outside.dtype == torch.uint8 and outside.is_contiguous()
     Mc = (ctypes.c_double * 6)(*[float(v) for v in M])
     st = torch.cuda.current_stream() if stream is None else stream
     _check(lib, lib.sfft_resample_affine(img.data_ptr(), img.shape[0], img.shape[1], Mc, int(a), out.data_ptr(),
