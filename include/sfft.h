@@ -22,8 +22,10 @@
  * aligned, contiguous; images are H rows x W columns, row-major, element (y,x) at y*W+x, fp64.
  * The library never allocates, frees or modifies caller buffers other than the stated outputs.
  * The four hot calls only enqueue work on `stream` (a cudaStream_t passed as void*; NULL = the
- * legacy default stream): they never synchronise the stream or the device.  A plan owns scratch
- * memory and is NOT re-entrant: use one plan per stream in flight.  No call throws; every call
+ * legacy default stream): they never synchronise the stream or the device.  Internally a plan also
+ * owns one side stream that is forked from and joined back into `stream` with events inside a call
+ * (or between sfft_subtract_prepare and the sfft_subtract that consumes it); the caller never sees it.
+ * A plan owns scratch memory and is NOT re-entrant: use one plan per stream in flight.  No call throws; every call
  * returns an sfft_status.  There is no CPU fallback: without a CUDA device plan creation fails.
  */
 #ifndef SFFT_H
