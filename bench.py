@@ -138,6 +138,16 @@ def oracle_cores():
     return len(os.sched_getaffinity(0))
 
 
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.lower().startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 # ------------------------------------------------------------------------------------------------
 # reference arm: the CPU oracle on a bounded sample
 
@@ -169,7 +179,9 @@ def run_reference(args, rank, world):
         step()
     dt = time.perf_counter() - t0
     value = args.steps * frac / dt
-    sample = f"{ch}x{cw} centre crop (1/{int(round(1 / frac))} of the CCD's pixels) of the configs[3] pair, same w/DK/DB; CCD/s = crop fraction / time"
+    sample = (f"{ch}x{cw} centre crop (1/{int(round(1 / frac))} of the CCD's pixels) of the configs[3] pair, same w/DK/DB; "
+              "CCD/s = crop fraction / time, i.e. extrapolated LINEARLY in pixels -- the full-CCD oracle leg of the "
+              "CUDA arm (cpu_baseline) runs ~1.9x slower per pixel (cache effects, N log N), so this line flatters the CPU")
     out = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
@@ -271,11 +283,50 @@ def run_exposure(torch, synth, cfg, plans, streams, nccd):
     wall = time.perf_counter() - t0
     ok = bool((infos == 0).all().item())
     inputs_gb = nccd * (2 * cfg.H * cfg.W * 8 + cfg.H * cfg.W) / 1e9
-    return {"ccds": nccd, "wall_s": wall, "ccd_per_s": nccd / wall, "plans_in_flight": NS, "solve_ctas": SOLVE_CTAS_PIPELINED, "all_spd": ok,
-            "inputs_resident_gb": round(inputs_gb, 2), "generation_s": round(gen_s, 1),
-            "how": "configs[4]: per-CCD seed 2000+k, sky0~U[800,3000], S FWHM~U[3.5,6]; inputs and outputs resident "
-                   "in HBM; host wall-clock of the second pass from first launch to final synchronize; the paper's "
-                   "~50 s per exposure (PAPER.md:305, whole Stage 2 on 64 cores + 2x A100) is context only"}
+
+    # the same exposure with the 60 pairs in PINNED HOST memory: every CCD's R, S, mask cross PCIe inside
+    # the timed region; D and the coefficients stay in HBM as above
+    wall_h2d = None
+    try:
+        hostp = [tuple(t.cpu().pin_memory() for t in trip) for trip in dev]
+        stg = [tuple(torch.empty_like(t) for t in dev[0]) for _ in range(NS)]
+
+        def run_all_h2d():
+            for k in range(nccd):
+                s = k % NS
+                st, pl = streams[s], plans[s]
+                R, S, M = stg[s]
+                with torch.cuda.stream(st):
+                    for d, h in zip((R, S, M), hostp[k]):
+                        d.copy_(h, non_blocking=True)
+                pl.build_system(R, S, M, As[s], bs[s], stream=st)
+                pl.solve(As[s], bs[s], cs[k], infos[k:k + 1], stream=st)
+                pl.subtract(R, S, cs[k], Ds[k], stream=st)
+
+        torch.cuda.synchronize()
+        run_all_h2d()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        run_all_h2d()
+        torch.cuda.synchronize()
+        wall_h2d = time.perf_counter() - t0
+        ok = ok and bool((infos == 0).all().item())
+        del hostp
+    except RuntimeError as e:       # not enough pinnable host memory on this box
+        wall_h2d = None
+        h2d_err = str(e).splitlines()[0][:120]
+    out = {"ccds": nccd, "wall_s": wall, "ccd_per_s": nccd / wall, "plans_in_flight": NS, "solve_ctas": SOLVE_CTAS_PIPELINED, "all_spd": ok,
+           "inputs_resident_gb": round(inputs_gb, 2), "generation_s": round(gen_s, 1),
+           "wall_s_incl_h2d": wall_h2d, "ccd_per_s_incl_h2d": (nccd / wall_h2d) if wall_h2d else None,
+           "h2d_gb": round(inputs_gb, 2),
+           "how": "configs[4]: per-CCD seed 2000+k, sky0~U[800,3000], S FWHM~U[3.5,6]; wall_s: inputs and outputs resident "
+                  "in HBM; wall_s_incl_h2d: the 60 pairs start in pinned host memory and R, S, mask of every CCD are copied "
+                  "to the device inside the timed region (PCIe-bound); host wall-clock of the second pass from first launch "
+                  "to final synchronize; the paper's ~50 s per exposure (PAPER.md:305, whole Stage 2 on 64 cores + 2x A100) "
+                  "is context only"}
+    if wall_h2d is None:
+        out["h2d_error"] = h2d_err
+    return out
 
 
 def run_cuda(args, rank, world, local_rank):
@@ -355,35 +406,12 @@ def run_cuda(args, rank, world, local_rank):
     plans = [plan] + [SfftPlan(cfg.H, cfg.W, cfg.w, cfg.DK, cfg.DB) for _ in range(NS - 1)]
     for pl in plans:   # several plans in flight: a small Cholesky grid leaves whole SMs to the others
         pl.set_solve_ctas(SOLVE_CTAS_PIPELINED)
-    bufs = []
-    for s in range(NS):
-        bufs.append(dict(
-            R=torch.empty((cfg.H, cfg.W), dtype=torch.float64, device="cuda"),
-            S=torch.empty((cfg.H, cfg.W), dtype=torch.float64, device="cuda"),
-            M=torch.empty((cfg.H, cfg.W), dtype=torch.uint8, device="cuda"),
-            A=torch.empty((N, N), dtype=torch.float64, device="cuda"),
-            b=torch.empty(N, dtype=torch.float64, device="cuda"),
-            c=torch.empty(N, dtype=torch.float64, device="cuda"),
-            info=torch.zeros(1, dtype=torch.int32, device="cuda"),
-            D=torch.empty((cfg.H, cfg.W), dtype=torch.float64, device="cuda"),
-            Dh=torch.empty((cfg.H, cfg.W), dtype=torch.float64).pin_memory(),
-            ch=torch.empty(N, dtype=torch.float64).pin_memory()))
-    h2d = 2 * cfg.H * cfg.W * 8 + cfg.H * cfg.W
-    d2h = cfg.H * cfg.W * 8 + N * 8
+    h2d, d2h = SfftPlan.host_bytes_per_call(cfg.H, cfg.W, N)
 
     def e2e_step(k):
-        s = k % NS
-        B, st, pl = bufs[s], streams[s], plans[s]
+        # the repo's public end-to-end call: pinned host R, S, mask in; D, coefficients, info out
         hR, hS, hM = host[k % NPAIR]
-        with torch.cuda.stream(st):
-            B["R"].copy_(hR, non_blocking=True)
-            B["S"].copy_(hS, non_blocking=True)
-            B["M"].copy_(hM, non_blocking=True)
-            pl.build_system(B["R"], B["S"], B["M"], B["A"], B["b"], stream=st)
-            pl.solve(B["A"], B["b"], B["c"], B["info"], stream=st)
-            pl.subtract(B["R"], B["S"], B["c"], B["D"], stream=st)
-            B["Dh"].copy_(B["D"], non_blocking=True)
-            B["ch"].copy_(B["c"], non_blocking=True)
+        return plans[k % NS].difference_host_async(hR, hS, hM, stream=streams[k % NS])
 
     for k in range(warm):
         e2e_step(k)
@@ -404,7 +432,7 @@ def run_cuda(args, rank, world, local_rank):
     ms_e2e = f0.elapsed_time(f1)
     ms_e2e = shard.max_over_ranks(ms_e2e, device="cuda")
     e2e_value = shard.aggregate_rate(args.steps, world, ms_e2e)
-    assert all(int(B["info"].item()) == 0 for B in bufs)
+    assert all(int(pl._stage["ih"].item()) == 0 for pl in plans)
 
     # ---- the two steps after the differencing, timed alone on the device
     post = None
@@ -479,7 +507,8 @@ def run_cuda(args, rank, world, local_rank):
 
     exposure = None
     if world == 1 and args.exposure_ccds > 0:
-        del bufs
+        for pl in plans:
+            pl._stage = None
         torch.cuda.empty_cache()
         exposure = run_exposure(torch, synth, cfg, plans, streams, args.exposure_ccds)
 
@@ -532,7 +561,8 @@ def run_cuda(args, rank, world, local_rank):
         dfma_tf = None
     roof["alu_peak_probed_tflops"] = dfma_tf
 
-    # ---- CPU baseline: the oracle as it stands, one CCD of the same workload
+    # ---- CPU baseline: the oracle as it stands, one CCD of the same workload, with all host cores and
+    # once more with scipy.fft workers=1 (SURVEY 8(d) "Timing the oracle beside it")
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         from oracle import sfft_oracle as orc
@@ -541,9 +571,15 @@ def run_cuda(args, rank, world, local_rank):
         tc = time.perf_counter()
         orc.sfft_difference(p0.R, p0.S, p0.mask, cfg.w, cfg.DK, cfg.DB, workers=cores)
         dtc = time.perf_counter() - tc
+        tc = time.perf_counter()
+        orc.sfft_difference(p0.R, p0.S, p0.mask, cfg.w, cfg.DK, cfg.DB, workers=1)
+        dt1 = time.perf_counter() - tc
         cpu = {"value": 1.0 / dtc, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": "1 full CCD pair (pair 0 of this run): FFT-route build + Cholesky + FFT-route subtract, "
-                         f"scipy.fft workers={cores}; {dtc:.1f} s"}
+                         f"scipy.fft workers={cores}; {dtc:.1f} s",
+               "workers1": {"value": 1.0 / dt1, "unit": UNIT, "cores": 1, "seconds": round(dt1, 1),
+                            "sample": "the same pair and code with scipy.fft workers=1 (numpy's own BLAS/threads untouched)"},
+               "cpu_model": cpu_model()}
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warm,

@@ -117,7 +117,8 @@ sfft_status sfft_subtract_prepare(sfft_plan* p, const double* R, void* stream);
 /* Multi-template combination (§2.3.2: the N_TEMP difference images of one science
  * exposure are "normalized to a common photometric zero point ... and median-combined"; N_TEMP
  * defaults to 5):  out[i] = median over k of scale[k] * D[k][i],  i < npix.
- * For even n the median is the mean of the two middle values (reading M1).
+ * For even n the median is the mean of the two middle values (reading M1); a NaN in any of
+ * the n values makes out[i] NaN (reading M2).
  *   D     in : HOST array of n DEVICE pointers, each npix fp64, 16-byte aligned, none aliasing out.
  *   scale in : HOST array of n flux factors (10^(0.4 (zp_ref - zp_k))).
  *   out  out : npix fp64 (device, 16-byte aligned).      1 <= n <= SFFT_MAX_TEMPLATES.
@@ -131,7 +132,8 @@ sfft_status sfft_median_combine(const double* const* D, const double* scale, int
  *   D in: H*W fp64 (device);  mask in: H*W uint8 (device), nonzero = not background, NULL = none.
  *   xs, ys in: n real-valued pixel positions (device; pixel (y,x) is centred at integer coordinates).
  *   flux out: n fp64 (device): sum of D over the pixels whose centres lie within `radius` of the
- *     position; NaN when that disc leaves the frame or touches a masked pixel (readings L1, L2).
+ *     position; NaN when that disc leaves the frame or touches a masked pixel, or when the position
+ *     itself is not finite (readings L1, L2).
  *   stats out: 3 fp64 (device): number of kept positions, their mean flux, their population
  *     standard deviation sigma.  The limiting magnitude is zp - 2.5 log10(5 sigma) (host arithmetic).
  * 0 < radius <= 64.  Enqueues two kernels on `stream`; never synchronises.  Needs no plan. */

@@ -12,6 +12,8 @@ It shares no code with the CUDA path and does not import the package.  Plain num
     brings image k to the common zero point (scale_k = 10^(0.4 (zp_ref - zp_k))).
     Reading M1 (paper silent): for an even number of images the median is the mean of the two
     middle values (the usual convention; the default N_TEMP = 5 is odd).
+    Reading M2 (paper silent): a NaN in any of the images makes the combined pixel NaN (what
+    numpy.median does; a resampled template flags its missing pixels this way).
 
 (2) Monte-Carlo limiting flux -- PAPER.md:164 (§2.3.3): "We measure aperture fluxes at 1024 randomly
     selected background positions using the same aperture definition, and deriving the 5 sigma
@@ -41,9 +43,9 @@ def median_combine(Ds, scales):
     stack = np.stack([np.asarray(D, dtype=np.float64) * float(s) for D, s in zip(Ds, scales)], axis=0)
     n = stack.shape[0]
     srt = np.sort(stack, axis=0)
-    if n % 2 == 1:
-        return srt[n // 2].copy()
-    return 0.5 * (srt[n // 2 - 1] + srt[n // 2])
+    out = srt[n // 2].copy() if n % 2 == 1 else 0.5 * (srt[n // 2 - 1] + srt[n // 2])
+    out[np.isnan(stack).any(axis=0)] = np.nan      # reading M2: a NaN in any image makes the pixel NaN
+    return out
 
 
 def aperture_flux(D, mask, x0, y0, radius):
@@ -51,6 +53,8 @@ def aperture_flux(D, mask, x0, y0, radius):
     leaves the frame or touches a masked pixel (readings L1, L2).  Explicit loops."""
     H, W = D.shape
     r2 = radius * radius
+    if not (math.isfinite(x0) and math.isfinite(y0)):
+        return float("nan")                        # reading L2: not a position inside the frame
     ylo, yhi = int(math.ceil(y0 - radius)), int(math.floor(y0 + radius))
     xlo, xhi = int(math.ceil(x0 - radius)), int(math.floor(x0 + radius))
     if ylo < 0 or xlo < 0 or yhi > H - 1 or xhi > W - 1:

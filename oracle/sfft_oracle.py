@@ -120,14 +120,6 @@ def normal_entry(R, S, mask, w, DK, DB, i, j=None):
 # --------------------------------------------------------------------------- O2: Fourier route
 
 
-def cross_correlation(f, g, workers=1):
-    """C_{f,g}[dy,dx] = sum_x f(x) g(x+d), circular, all lags:
-    irfft2(conj(rfft2 f) * rfft2 g), unnormalised forward, 1/P on the inverse (A8)."""
-    F = scipy.fft.rfft2(f, workers=workers)
-    Gg = scipy.fft.rfft2(g, workers=workers)
-    return scipy.fft.irfft2(np.conj(F) * Gg, s=f.shape, workers=workers)
-
-
 def build_system_fft(R, S, mask, w, DK, DB, workers=1, dtype=np.float64):
     """O2: A, b from cross-correlation maps read at the shift differences (north_star (3),(4)).
 

@@ -211,7 +211,9 @@ class SfftPlan:
 
     def subtract_prepare(self, R, stream=None):
         """sfft_subtract_prepare: start the coefficient-independent stage of the next subtract(R, ...)
-        on the plan's side stream (overlaps the solve).  R must stay unmodified until that subtract."""
+        on the plan's side stream (overlaps the solve).  R must stay ALIVE and unmodified until that
+        subtract has been enqueued: the side stream is not known to torch's caching allocator, so a
+        dropped R could be handed out again while the side stream still reads it."""
         import torch
         _check(self._lib, self._lib.sfft_subtract_prepare(
             self._p, _dev_ptr(R, torch.float64, self.H * self.W, "R"), _stream_handle(stream)), "sfft_subtract_prepare")
@@ -224,15 +226,61 @@ class SfftPlan:
         D = self.subtract(R, S, c, stream=stream)
         return A, b, c, info, D
 
-    def difference_host(self, R_host, S_host, mask_host, stream=None):
-        """End-to-end call with HOST (pinned) buffers: H2D copies, hot path, D2H of D and coeffs."""
+    def difference_host_async(self, R_host, S_host, mask_host, stream=None, D_host=None, c_host=None):
+        """End-to-end call with HOST buffers: H2D copies of R, S, mask, the hot path (build -> solve ->
+        subtract) and D2H copies of D, the coefficients and `info`, ALL enqueued on one stream (default:
+        the current one); nothing synchronises.  Returns (D_host, c_host, info_host, done) with `done` a
+        CUDA event recorded after the last copy: the host tensors are valid once it has completed.
+        Pinned host tensors make the copies asynchronous; the plan keeps its device staging buffers and,
+        unless D_host / c_host are given, its pinned result buffers between calls (so a second call on
+        the same plan overwrites the first call's results).  Copies and marshalling only."""
         import torch
+        st = torch.cuda.current_stream() if stream is None else stream
         dev = torch.device("cuda", torch.cuda.current_device())
-        R = R_host.to(dev, non_blocking=True)
-        S = S_host.to(dev, non_blocking=True)
-        mask = None if mask_host is None else mask_host.to(dev, non_blocking=True)
-        A, b, c, info, D = self.difference(R, S, mask, stream=stream)
-        return D.to("cpu", non_blocking=False), c.to("cpu"), info.to("cpu")
+        sg = getattr(self, "_stage", None)
+        if sg is None:
+            sg = dict(
+                R=torch.empty((self.H, self.W), dtype=torch.float64, device=dev),
+                S=torch.empty((self.H, self.W), dtype=torch.float64, device=dev),
+                M=torch.empty((self.H, self.W), dtype=torch.uint8, device=dev),
+                A=torch.empty((self.N, self.N), dtype=torch.float64, device=dev),
+                b=torch.empty(self.N, dtype=torch.float64, device=dev),
+                c=torch.empty(self.N, dtype=torch.float64, device=dev),
+                info=torch.zeros(1, dtype=torch.int32, device=dev),
+                D=torch.empty((self.H, self.W), dtype=torch.float64, device=dev),
+                Dh=torch.empty((self.H, self.W), dtype=torch.float64).pin_memory(),
+                ch=torch.empty(self.N, dtype=torch.float64).pin_memory(),
+                ih=torch.zeros(1, dtype=torch.int32).pin_memory())
+            self._stage = sg
+        Dh = sg["Dh"] if D_host is None else D_host
+        ch = sg["ch"] if c_host is None else c_host
+        with torch.cuda.stream(st):
+            sg["R"].copy_(R_host.reshape(self.H, self.W), non_blocking=True)
+            sg["S"].copy_(S_host.reshape(self.H, self.W), non_blocking=True)
+            M = None
+            if mask_host is not None:
+                sg["M"].copy_(mask_host.reshape(self.H, self.W), non_blocking=True)
+                M = sg["M"]
+            self.build_system(sg["R"], sg["S"], M, sg["A"], sg["b"], stream=st)
+            self.solve(sg["A"], sg["b"], sg["c"], sg["info"], stream=st)
+            self.subtract(sg["R"], sg["S"], sg["c"], sg["D"], stream=st)
+            Dh.copy_(sg["D"], non_blocking=True)
+            ch.copy_(sg["c"], non_blocking=True)
+            sg["ih"].copy_(sg["info"], non_blocking=True)
+            done = torch.cuda.Event()
+            done.record(st)
+        return Dh, ch, sg["ih"], done
+
+    def difference_host(self, R_host, S_host, mask_host, stream=None):
+        """difference_host_async, then wait for its event: (D, coeffs, info) as host tensors."""
+        Dh, ch, ih, done = self.difference_host_async(R_host, S_host, mask_host, stream=stream)
+        done.synchronize()
+        return Dh, ch, ih
+
+    @staticmethod
+    def host_bytes_per_call(H, W, N, with_mask=True):
+        """(h2d, d2h) bytes difference_host moves per call, counted from the tensors it copies."""
+        return 2 * H * W * 8 + (H * W if with_mask else 0), H * W * 8 + N * 8 + 4
 
     # -- diagnostics
     def last_launch_count(self, which: int) -> int:

@@ -443,7 +443,7 @@ sfft_status sfft_launch_lag_gather(sfft_plan* p, double* A, double* b, cudaStrea
   for (int t = 0; t < p->TK; ++t) { GP.monoK[t][0] = p->monoK[t][0]; GP.monoK[t][1] = p->monoK[t][1]; }
   const size_t total = (size_t)p->N * p->N + p->N;
   int blocks = (int)((total + 255) / 256);
-  if (blocks > 148 * 16) blocks = 148 * 16;
+  if (blocks > p->num_sms * 16) blocks = p->num_sms * 16;
   k_gather<<<blocks, 256, 0, st>>>(GP);
   SFFT_LAUNCH_CHECK();
   ++*nl;

@@ -341,7 +341,7 @@ sfft_status sfft_launch_exact_update(sfft_plan* p, const double* R, const double
   SFFT_CUDA_TRY(cudaFuncSetAttribute(k_exact_syrk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   void* args[] = {(void*)&P};
   SFFT_CUDA_TRY(cudaLaunchCooperativeKernel((const void*)k_exact_syrk, dim3(ntiles, ks), dim3(EX_TH), args, smem, st));
-  k_exact_apply<<<148 * 4, 256, 0, st>>>(p->exScratch, A, b, p->N, ntiles, ks);
+  k_exact_apply<<<p->num_sms * 4, 256, 0, st>>>(p->exScratch, A, b, p->N, ntiles, ks);
   SFFT_LAUNCH_CHECK();
   *nl += 5;
   return SFFT_OK;

@@ -27,6 +27,12 @@ struct MedianParams {
 
 template <int N>
 __device__ __forceinline__ double median_of(double* v) {
+  // a NaN in any template makes the combined pixel NaN (reading M2; fmin/fmax below would
+  // silently drop it)
+  bool anynan = false;
+#pragma unroll
+  for (int i = 0; i < N; ++i) anynan |= (v[i] != v[i]);
+  if (anynan) return nan("");
   // insertion sort with compile-time indices (stays in registers)
 #pragma unroll
   for (int i = 1; i < N; ++i) {
@@ -65,7 +71,8 @@ __global__ void __launch_bounds__(256) k_median(MedianParams P) {
 template <int N>
 static sfft_status launch_median_t(const MedianParams& P, cudaStream_t st) {
   size_t blocks = ((P.npix >> 1) + 255) / 256;
-  if (blocks > 148 * 16) blocks = 148 * 16;
+  const size_t cap = (size_t)sfft_device_sms() * 16;
+  if (blocks > cap) blocks = cap;
   if (blocks < 1) blocks = 1;
   k_median<N><<<(unsigned)blocks, 256, 0, st>>>(P);
   SFFT_LAUNCH_CHECK();
@@ -81,7 +88,8 @@ __global__ void __launch_bounds__(256) k_aperture_flux(const double* __restrict_
   const double x0 = xs[a], y0 = ys[a], r2 = radius * radius;
   const int ylo = (int)ceil(y0 - radius), yhi = (int)floor(y0 + radius);
   const int xlo = (int)ceil(x0 - radius), xhi = (int)floor(x0 + radius);
-  const bool inside = ylo >= 0 && xlo >= 0 && yhi <= H - 1 && xhi <= W - 1;   // warp-uniform
+  // a non-finite position is dropped like one outside the frame (its int conversions are meaningless)
+  const bool inside = isfinite(x0) && isfinite(y0) && ylo >= 0 && xlo >= 0 && yhi <= H - 1 && xhi <= W - 1;   // warp-uniform
   double acc = 0.0;
   int bad = 0;
   if (inside) {

@@ -203,30 +203,31 @@ sfft_status sfft_launch_subtract(sfft_plan* p, const double* R, const double* S,
     if (s != SFFT_OK) return s;
   }
   p->prepValid = 0;
-  ProfScope* pmix = new ProfScope(p, 7, st);
-  // 2. x-phase table of the kernel coefficients
-  ETabParams EP;
-  EP.coeffs = c; EP.E = p->Etab; EP.w = p->w; EP.L = p->L; EP.NC = p->NC; EP.W = p->W; EP.twW = p->twW;
-  dim3 ge((p->NC + 127) / 128, p->TK * (2 * p->w + 1));
-  k_etable<<<ge, 128, 0, st>>>(EP);
-  SFFT_LAUNCH_CHECK();
-  ++*nl;
-  // 3. y-mixing
-  MixParams MP;
-  MP.G = p->T; MP.E = p->Etab; MP.Mhat = p->Mhat; MP.H = p->H; MP.NC = p->NC;
-  MP.DK = p->DK; MP.TK = p->TK;
-  MP.KT = p->NC < 32 ? p->NC : 32;
-  for (int t = 0; t < p->TK; ++t) { MP.monoK[t][0] = p->monoK[t][0]; MP.monoK[t][1] = p->monoK[t][1]; }
-  switch (p->w) {
-    case 0: s = launch_mix_t<0>(MP, st); break;
-    case 1: s = launch_mix_t<1>(MP, st); break;
-    case 2: s = launch_mix_t<2>(MP, st); break;
-    case 3: s = launch_mix_t<3>(MP, st); break;
-    case 4: s = launch_mix_t<4>(MP, st); break;
-    case 5: s = launch_mix_t<5>(MP, st); break;
-    default: s = SFFT_ERR_UNSUPPORTED; break;
+  {
+    ProfScope pmix(p, 7, st);
+    // 2. x-phase table of the kernel coefficients
+    ETabParams EP;
+    EP.coeffs = c; EP.E = p->Etab; EP.w = p->w; EP.L = p->L; EP.NC = p->NC; EP.W = p->W; EP.twW = p->twW;
+    dim3 ge((p->NC + 127) / 128, p->TK * (2 * p->w + 1));
+    k_etable<<<ge, 128, 0, st>>>(EP);
+    SFFT_LAUNCH_CHECK();
+    ++*nl;
+    // 3. y-mixing
+    MixParams MP;
+    MP.G = p->T; MP.E = p->Etab; MP.Mhat = p->Mhat; MP.H = p->H; MP.NC = p->NC;
+    MP.DK = p->DK; MP.TK = p->TK;
+    MP.KT = p->NC < 32 ? p->NC : 32;
+    for (int t = 0; t < p->TK; ++t) { MP.monoK[t][0] = p->monoK[t][0]; MP.monoK[t][1] = p->monoK[t][1]; }
+    switch (p->w) {
+      case 0: s = launch_mix_t<0>(MP, st); break;
+      case 1: s = launch_mix_t<1>(MP, st); break;
+      case 2: s = launch_mix_t<2>(MP, st); break;
+      case 3: s = launch_mix_t<3>(MP, st); break;
+      case 4: s = launch_mix_t<4>(MP, st); break;
+      case 5: s = launch_mix_t<5>(MP, st); break;
+      default: s = SFFT_ERR_UNSUPPORTED; break;
+    }
   }
-  delete pmix;
   if (s != SFFT_OK) return s;
   ++*nl;
   // 4. inverse rows + subtraction

@@ -78,6 +78,8 @@ static void plan_free(sfft_plan* p) {
   delete p;
 }
 
+static bool aligned16(const void* q) { return (((uintptr_t)q) & 15) == 0; }
+
 extern "C" {
 
 const char* sfft_version(void) { return "sfft-b200 0.1 (sm_100a)"; }
@@ -210,6 +212,7 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
     dalloc((void**)&p->kbStrip, sizeof(double) * (size_t)p->TK * p->L * p->TB);
   }
   dalloc((void**)&p->exScratch, sfft_exact_scratch_bytes(p->N));
+  dalloc((void**)&p->exRows, sfft_exact_rows_bytes(p->N));   // here, so that no hot call ever allocates
   dalloc((void**)&p->exBar, 2 * sizeof(unsigned));
   dalloc((void**)&p->Lw, sizeof(double) * (size_t)(p->N + 1) * p->ldL);
   dalloc((void**)&p->cholBar, 2 * sizeof(unsigned));
@@ -253,14 +256,21 @@ sfft_status sfft_plan_destroy(sfft_plan* p) {
 int sfft_num_coeffs(const sfft_plan* p) { return p ? p->N : -1; }
 size_t sfft_workspace_bytes(const sfft_plan* p) { return p ? p->ws_bytes : 0; }
 
-static bool aligned16(const void* q) { return (((uintptr_t)q) & 15) == 0; }
+// A CUDA error left pending by earlier, unrelated work would be reported as a launch failure of this
+// library (the launch checks peek at the last error): the hot calls refuse to start on top of one.
+static bool cuda_error_pending() { return cudaPeekAtLastError() != cudaSuccess; }
 
-sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
-                              double* A, double* b, void* stream) {
-  if (!p || !R || !S || !A || !b) return SFFT_ERR_INVALID_ARG;
-  if (!aligned16(R) || !aligned16(S) || !aligned16(A) || !aligned16(b) || (mask && !aligned16(mask)))
-    return SFFT_ERR_INVALID_ARG;
-  cudaStream_t st = (cudaStream_t)stream;
+// After the fork every failure path must join the side stream back into the caller stream: the side
+// stream may still be reading the caller's R and mask, which the caller is free to reuse once the
+// call has returned and its stream has drained.
+static sfft_status fail_joined(sfft_plan* p, cudaStream_t st, sfft_status s) {
+  if (cudaEventRecord(p->evJoin, p->side) == cudaSuccess) cudaStreamWaitEvent(st, p->evJoin, 0);
+  cudaGetLastError();
+  return s;
+}
+
+static sfft_status build_system_impl(sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
+                                     double* A, double* b, cudaStream_t st) {
   int nl = 0;
   // the row-pass scratch is about to be overwritten: an unconsumed prepare finishes first, then is dropped
   if (p->prepValid) SFFT_CUDA_TRY(cudaStreamWaitEvent(st, p->evPrep, 0));
@@ -273,25 +283,24 @@ sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S, co
   SFFT_CUDA_TRY(cudaEventRecord(p->evFork, st));
   SFFT_CUDA_TRY(cudaStreamWaitEvent(p->side, p->evFork, 0));
   { ProfScope ps(p, 9, p->side); s = sfft_launch_kb(p, R, mask, p->side, &nl); }
-  if (s != SFFT_OK) return s;
+  if (s != SFFT_OK) return fail_joined(p, st, s);
   { ProfScope ps(p, 0, st); s = sfft_launch_row_fwd(p, R, S, mask, true, p->T, p->pitchT, !p->fused, p->fused != 0, st, &nl); }
-  if (s != SFFT_OK) return s;
+  if (s != SFFT_OK) return fail_joined(p, st, s);
   // the final moment reduction needs only the row pass: it follows the sparse chain on the side stream
-  SFFT_CUDA_TRY(cudaEventRecord(p->evRow, st));
-  SFFT_CUDA_TRY(cudaStreamWaitEvent(p->side, p->evRow, 0));
+  if (cudaEventRecord(p->evRow, st) != cudaSuccess || cudaStreamWaitEvent(p->side, p->evRow, 0) != cudaSuccess)
+    return fail_joined(p, st, SFFT_ERR_CUDA);
   s = sfft_launch_moments(p, p->side, &nl);
-  if (s != SFFT_OK) return s;
-  SFFT_CUDA_TRY(cudaEventRecord(p->evJoin, p->side));
+  if (s != SFFT_OK) return fail_joined(p, st, s);
+  if (cudaEventRecord(p->evJoin, p->side) != cudaSuccess) return fail_joined(p, st, SFFT_ERR_CUDA);
   if (p->fused) {
     // a2 (column pass, applies eta^q) + a3 (cross products + lag-pruned inverse along ky), fused
     ProfScope ps(p, 1, st);
     s = sfft_launch_colx(p, st, &nl);
   } else {
     { ProfScope ps(p, 1, st); s = sfft_launch_col_fwd(p, st, &nl); }
-    if (s != SFFT_OK) return s;
-    s = sfft_launch_cross(p, st, &nl);
+    if (s == SFFT_OK) s = sfft_launch_cross(p, st, &nl);
   }
-  if (s != SFFT_OK) return s;
+  if (s != SFFT_OK) return fail_joined(p, st, s);
   SFFT_CUDA_TRY(cudaStreamWaitEvent(st, p->evJoin, 0));
   { ProfScope ps(p, 4, st); s = sfft_launch_lag_gather(p, A, b, st, &nl); }  // a3 (kx inverse on lag rows) + a4
   if (s != SFFT_OK) return s;
@@ -299,16 +308,27 @@ sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S, co
   return SFFT_OK;
 }
 
+static bool build_args_ok(const sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
+                          const double* A, const double* b) {
+  return p && R && S && A && b && aligned16(R) && aligned16(S) && aligned16(A) && aligned16(b) &&
+         (!mask || aligned16(mask));
+}
+
+sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
+                              double* A, double* b, void* stream) {
+  if (!build_args_ok(p, R, S, mask, A, b)) return SFFT_ERR_INVALID_ARG;
+  if (cuda_error_pending()) return SFFT_ERR_CUDA;
+  return build_system_impl(p, R, S, mask, A, b, (cudaStream_t)stream);
+}
+
 sfft_status sfft_build_system_exact(sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
                                     double* A, double* b, void* stream) {
+  // every argument is validated before anything is enqueued
+  if (!build_args_ok(p, R, S, mask, A, b)) return SFFT_ERR_INVALID_ARG;
+  if (cuda_error_pending()) return SFFT_ERR_CUDA;
   // the ordinary build on the unmasked images, then the masked pixels' rank-one terms are taken out
-  sfft_status s = sfft_build_system(p, R, S, nullptr, A, b, stream);
+  sfft_status s = build_system_impl(p, R, S, nullptr, A, b, (cudaStream_t)stream);
   if (s != SFFT_OK || !mask) return s;
-  if (!aligned16(mask)) return SFFT_ERR_INVALID_ARG;
-  if (!p->exRows) {   // first use: the chunk buffer of generated rows (this allocation may synchronise, once)
-    if (cudaMalloc((void**)&p->exRows, sfft_exact_rows_bytes(p->N)) != cudaSuccess) { cudaGetLastError(); return SFFT_ERR_ALLOC; }
-    p->ws_bytes += sfft_exact_rows_bytes(p->N);
-  }
   int nl = p->launches[0];
   s = sfft_launch_exact_update(p, R, S, mask, A, b, (cudaStream_t)stream, &nl);
   if (s != SFFT_OK) return s;
@@ -318,6 +338,7 @@ sfft_status sfft_build_system_exact(sfft_plan* p, const double* R, const double*
 
 sfft_status sfft_solve(sfft_plan* p, const double* A, const double* b, double* coeffs, int* info, void* stream) {
   if (!p || !A || !b || !coeffs) return SFFT_ERR_INVALID_ARG;
+  if (cuda_error_pending()) return SFFT_ERR_CUDA;
   int nl = 0;
   sfft_status s;
   { ProfScope ps(p, 5, (cudaStream_t)stream); s = sfft_launch_solve(p, A, b, coeffs, info, (cudaStream_t)stream, &nl); }
@@ -330,6 +351,7 @@ sfft_status sfft_subtract(sfft_plan* p, const double* R, const double* S, const 
                           void* stream) {
   if (!p || !R || !S || !coeffs || !D) return SFFT_ERR_INVALID_ARG;
   if (!aligned16(R) || !aligned16(S) || !aligned16(D) || D == R || D == S) return SFFT_ERR_INVALID_ARG;
+  if (cuda_error_pending()) return SFFT_ERR_CUDA;
   int nl = (p->prepValid && p->prepR == R) ? p->launches[2] : 0;
   sfft_status s = sfft_launch_subtract(p, R, S, coeffs, D, (cudaStream_t)stream, &nl);
   if (s != SFFT_OK) return s;
@@ -339,6 +361,7 @@ sfft_status sfft_subtract(sfft_plan* p, const double* R, const double* S, const 
 
 sfft_status sfft_subtract_prepare(sfft_plan* p, const double* R, void* stream) {
   if (!p || !R || !aligned16(R)) return SFFT_ERR_INVALID_ARG;
+  if (cuda_error_pending()) return SFFT_ERR_CUDA;
   cudaStream_t st = (cudaStream_t)stream;
   int nl = 0;
   // ordered after everything already enqueued on `stream` (the build that used the scratch before),
@@ -346,8 +369,8 @@ sfft_status sfft_subtract_prepare(sfft_plan* p, const double* R, void* stream) {
   SFFT_CUDA_TRY(cudaEventRecord(p->evFork, st));
   SFFT_CUDA_TRY(cudaStreamWaitEvent(p->side, p->evFork, 0));
   sfft_status s = sfft_launch_subtract_rows(p, R, p->side, &nl);
-  if (s != SFFT_OK) return s;
-  SFFT_CUDA_TRY(cudaEventRecord(p->evPrep, p->side));
+  if (s != SFFT_OK) return fail_joined(p, st, s);
+  if (cudaEventRecord(p->evPrep, p->side) != cudaSuccess) return fail_joined(p, st, SFFT_ERR_CUDA);
   p->prepR = R;
   p->prepValid = 1;
   p->launches[2] = nl;   // counted with the subtract call it belongs to

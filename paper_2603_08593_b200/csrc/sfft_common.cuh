@@ -176,6 +176,18 @@ struct ProfScope {  // RAII: record an event pair around one stage when profilin
     }                                                \
   } while (0)
 
+// SM count of the current device (cached; 148 on B200), for the plan-less calls' grid sizes
+inline int sfft_device_sms() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0, v = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) n = v;
+    else { cudaGetLastError(); return 148; }
+  }
+  return n;
+}
+
 // ---- stage entry points implemented in the k_*.cu files (host functions) ----------------------
 // build = true: images m xi^p R (p <= DK) and m S with the fused row moments; false: xi^p R only
 sfft_status sfft_launch_row_fwd(sfft_plan* p, const double* R, const double* S,

@@ -334,3 +334,79 @@ def test_exact_objective_full_config_sampled():
         assert abs(A[i, j] - orc.exact_entry(pr.R, pr.S, pr.mask, cfg.w, cfg.DK, cfg.DB, int(i), int(j))) <= TOL_AB * scale
     for i in (0, 61, 725, 731):
         assert abs(b[i] - orc.exact_entry(pr.R, pr.S, pr.mask, cfg.w, cfg.DK, cfg.DB, i)) <= TOL_AB * np.max(np.abs(b))
+
+
+def test_exposure_configuration_three_plans_in_flight():
+    """The launch configuration bench.py's exposure and end-to-end legs time (BASELINE.json configs[4];
+    PAPER.md:324, a GPU works through a queue of CCDs): 3 plans on 3 streams in flight at once,
+    sfft_plan_set_solve_ctas(48), no sfft_subtract_prepare, exposure-recipe pairs (seed 2000+k) at the
+    extremes of the recipe (sky 800 / FWHM 6 and sky 3000 / FWHM 3.5) plus one mid draw.  A, b, c, D of
+    the two extreme pairs against the oracle at the A5 tolerances, and every pair bitwise equal to the
+    same pair run alone on one plan with the default solve grid (sfft.h: "Results are bitwise
+    independent of the setting")."""
+    prs = [synth.make_pair("full", seed=2000, sky0=800.0, fwhm_s=6.0),
+           synth.make_pair("full", seed=2001, sky0=3000.0, fwhm_s=3.5),
+           synth.make_exposure_pair(2)]
+    cfg = prs[0].cfg
+    N = cfg.N
+    devp = [(dev(p.R), dev(p.S), dev(p.mask)) for p in prs]
+    streams = [torch.cuda.Stream() for _ in prs]
+    plans = [SfftPlan(cfg.H, cfg.W, cfg.w, cfg.DK, cfg.DB) for _ in prs]
+    outs = []
+    try:
+        for pl in plans:
+            pl.set_solve_ctas(48)
+        torch.cuda.synchronize()
+        res = [None] * len(prs)
+        for rep in range(2):                      # second round: every plan's scratch has been used once
+            for k, (pl, st) in enumerate(zip(plans, streams)):
+                R, S, M = devp[k]
+                with torch.cuda.stream(st):
+                    A, b = pl.build_system(R, S, M, stream=st)
+                    c, info = pl.solve(A, b, stream=st)
+                    D = pl.subtract(R, S, c, stream=st)
+                res[k] = (A, b, c, info, D)
+        torch.cuda.synchronize()
+        # the same pairs alone, one plan, default grid, with the prepare hint (the single-stream path)
+        with SfftPlan(cfg.H, cfg.W, cfg.w, cfg.DK, cfg.DB) as solo:
+            for k in range(len(prs)):
+                R, S, M = devp[k]
+                A0, b0, c0, info0, D0 = solo.difference(R, S, M)
+                torch.cuda.synchronize()
+                A, b, c, info, D = res[k]
+                assert int(info.item()) == 0 and int(info0.item()) == 0
+                assert torch.equal(A, A0) and torch.equal(b, b0), k
+                assert torch.equal(c, c0), k
+                assert torch.equal(D, D0), k
+        outs = [tuple(t.cpu().numpy() for t in (r[0], r[1], r[2], r[4])) for r in res[:2]]
+    finally:
+        for pl in plans:
+            pl.close()
+    L, TK = cfg.L, (cfg.DK + 1) * (cfg.DK + 2) // 2
+    for k, (A, b, c, D) in enumerate(outs):
+        pr = prs[k]
+        Ao, bo = orc.build_system_fft(pr.R, pr.S, pr.mask, cfg.w, cfg.DK, cfg.DB, workers=8)
+        co = orc.solve(Ao, bo)
+        check_system(A, b, Ao, bo, L, TK)
+        assert np.max(np.abs(c - co)) <= TOL_C * np.max(np.abs(co))
+        Df = orc.subtract_fft(pr.R, pr.S, co, cfg.w, cfg.DK, cfg.DB, workers=8)
+        assert np.max(np.abs(D - Df)) <= TOL_D * pr.sky_rms
+        rng = np.random.default_rng(50 + k)
+        ys, xs = rng.integers(0, cfg.H, 20), rng.integers(0, cfg.W, 20)
+        Dp = orc.subtract_at_pixels(pr.R, pr.S, co, cfg.w, cfg.DK, cfg.DB, ys, xs)
+        assert np.max(np.abs(D[ys, xs] - Dp)) <= TOL_D * pr.sky_rms
+
+
+def test_difference_host_end_to_end_call():
+    """SfftPlan.difference_host (pinned host buffers in, D and coefficients out -- the call bench.py's
+    e2e leg times) on a non-default stream equals the device-resident path bitwise."""
+    pr = synth.make_pair("small", force_saturated=3)
+    cfg = pr.cfg
+    hR, hS, hM = (torch.from_numpy(x).pin_memory() for x in (pr.R, pr.S, pr.mask))
+    st = torch.cuda.Stream()
+    with SfftPlan(cfg.H, cfg.W, cfg.w, cfg.DK, cfg.DB) as plan:
+        Dh, ch, ih = plan.difference_host(hR, hS, hM, stream=st)
+        assert int(ih.item()) == 0 and not Dh.is_cuda and not ch.is_cuda
+        A, b, c, info, D = plan.difference(dev(pr.R), dev(pr.S), dev(pr.mask))
+        torch.cuda.synchronize()
+        assert torch.equal(Dh, D.cpu()) and torch.equal(ch, c.cpu())

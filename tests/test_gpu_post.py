@@ -24,6 +24,31 @@ def test_median_combine_bit_exact(n, shape):
     assert np.array_equal(out, po.median_combine(Ds, sc))
 
 
+@pytest.mark.parametrize("n", [1, 2, 4, 5, 9])
+def test_median_combine_nan_propagates(n):
+    """Reading M2: a NaN in any template gives a NaN pixel, everything else is untouched (bit-exact)."""
+    rng = np.random.default_rng(n)
+    Ds = [40.0 * rng.standard_normal((33, 47)) for _ in range(n)]
+    Ds[0][5, 6] = np.nan
+    Ds[n - 1][32, 46] = np.nan          # odd tail element (33*47 is odd)
+    Ds[n // 2][0, 0] = np.nan
+    sc = rng.uniform(0.7, 1.4, n)
+    out = median_combine([torch.from_numpy(D).cuda() for D in Ds], sc).cpu().numpy()
+    ref = po.median_combine(Ds, sc)
+    assert np.isnan(ref).sum() == 3
+    assert np.array_equal(out, ref, equal_nan=True)
+
+
+def test_aperture_non_finite_positions_are_dropped():
+    D = torch.ones((40, 40), dtype=torch.float64, device="cuda")
+    xs = torch.tensor([float("nan"), 20.0, float("inf"), 20.0, 1e300], dtype=torch.float64, device="cuda")
+    ys = torch.tensor([20.0, float("-inf"), 20.0, 20.0, 20.0], dtype=torch.float64, device="cuda")
+    flux, st = aperture_stats(D, None, xs, ys, 3.0)
+    fo, (cnt, mean, sigma) = po.aperture_stats(np.ones((40, 40)), None, xs.cpu().numpy(), ys.cpu().numpy(), 3.0)
+    assert np.array_equal(np.isnan(flux.cpu().numpy()), np.isnan(fo)) and cnt == 1
+    assert flux[3].item() == 29 and st[0].item() == 1
+
+
 def test_median_combine_full_ccd_sampled():
     """5 templates at the full CCD size (the launch bench.py times): sampled pixels against the
     definition, and the order-statistic property min <= median <= max everywhere."""

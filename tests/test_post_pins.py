@@ -35,6 +35,20 @@ def test_median_known_values_and_invariances():
     assert out2.tolist() == [[1.0, 0.4]]
 
 
+def test_median_nan_reading_M2_matches_numpy_median():
+    """A NaN in any image makes the pixel NaN -- numpy.median's behaviour (library routine)."""
+    rng = np.random.default_rng(4)
+    for n in (3, 4, 5):
+        Ds = [rng.standard_normal((6, 7)) for _ in range(n)]
+        Ds[1][2, 3] = np.nan
+        Ds[n - 1][0, 0] = np.nan
+        Ds[0][0, 0] = np.nan
+        out = po.median_combine(Ds, [1.0] * n)
+        ref = np.median(np.stack(Ds), axis=0)
+        assert np.isnan(out[2, 3]) and np.isnan(out[0, 0]) and np.isnan(out).sum() == 2
+        assert np.array_equal(out, ref, equal_nan=True)
+
+
 @pytest.mark.parametrize("r,count", [(1.0, 5), (2.0, 13), (3.0, 29), (4.0, 49), (5.0, 81), (1.5, 9), (2.5, 21)])
 def test_disc_pixel_count_is_the_gauss_circle_number(r, count):
     """N(r) = #{(i,j) in Z^2 : i^2 + j^2 <= r^2}: 5, 13, 29, 49, 81 for r = 1..5 (OEIS A000328)."""
@@ -64,6 +78,9 @@ def test_frame_edge_and_mask_drop_the_position():
     mask[15, 17] = 1
     assert math.isnan(po.aperture_flux(D, mask, 15.0, 15.0, 3.0))      # (17,15) is inside the disc
     assert po.aperture_flux(D, mask, 15.0, 15.0, 1.5) == 9              # and outside the smaller one
+    for bad in (float("nan"), float("inf"), -float("inf")):              # not a position at all: dropped
+        assert math.isnan(po.aperture_flux(D, None, bad, 15.0, 3.0))
+        assert math.isnan(po.aperture_flux(D, None, 15.0, bad, 3.0))
 
 
 def test_stats_constant_and_white_noise():
@@ -83,8 +100,11 @@ def test_stats_constant_and_white_noise():
     _, (n2, m2, s2) = po.aperture_stats(noise, None, xs_i, ys_i, 4.2)
     assert n2 == 1024
     assert s2 == pytest.approx(5.0 * math.sqrt(57), rel=0.12)
-    assert po.limiting_magnitude(s2, 30.0) == pytest.approx(30.0 - 2.5 * math.log10(5 * s2))
-    assert po.limiting_magnitude(1.0, 25.0) == pytest.approx(25.0 - 2.5 * math.log10(5.0))
+    # hand values (reading L5): 2.5 log10(5) = 1.7474250108..., and a 100x larger sigma is
+    # exactly 5 magnitudes brighter
+    assert po.limiting_magnitude(1.0, 25.0) == pytest.approx(23.2525749891600, abs=1e-12)
+    assert po.limiting_magnitude(0.2, 25.0) == pytest.approx(25.0, abs=1e-12)
+    assert po.limiting_magnitude(100.0, 25.0) == pytest.approx(18.2525749891600, abs=1e-12)
 
 
 # --------------------------------------------------------------------------- resampling pins
