@@ -24,7 +24,7 @@ struct RowFwdParams {
   cplx* T;       // [nimg][H][pitchT]
   int pitchT;    // row pitch of T in complex elements
   int packed;    // 1: T[y][0] = X[0] + i X[W/2];  0: T[y][0] = X[0], T[y][NC] = X[W/2]
-  int pairT;     // 1 (unpacked only): column-pair-major layout T[img][kx/2][y][kx%2] read by k_colx
+  int colT;      // 1 (unpacked only): column-major layout T[img][kx][y], kx in [0, NC], read by k_colb
   const cplx* twP;   // per-pass twiddle tables for length NC
   const cplx* twW;
   int moments, DB, nMomA, nMomS, nMomR;
@@ -207,10 +207,10 @@ __global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
     fft_regs_to_smem<NC, -1, false>(v, s, tid, nth, RB, P.twP, C::SEQ_STRIDE);
     fetch(im + 1);
     // split: X[k] = Xe + w^k Xo, X[NC-k] = conj(Xe - w^k Xo), w = e^{-2 pi i / W}
-    // element k of this row: row-major out[k], or pair-major ((im*NP + k/2)*H + y)*2 + k%2
-    cplx* out = P.pairT ? P.T + ((size_t)im * (NC / 2 + 1) * H + y) * 2 : P.T + ((size_t)im * H + y) * P.pitchT;
-    const size_t kmul = P.pairT ? (size_t)H * 2 : 2;   // offset of column pair k/2
-    auto at = [&](int k) -> cplx* { return out + (size_t)(k >> 1) * kmul + (k & 1); };
+    // element k of this row: row-major out[k], or column-major (im*(NC+1) + k)*H + y
+    cplx* out = P.colT ? P.T + (size_t)im * (NC + 1) * H + y : P.T + ((size_t)im * H + y) * P.pitchT;
+    const size_t kmul = P.colT ? (size_t)H : 1;   // offset of column k
+    auto at = [&](int k) -> cplx* { return out + (size_t)k * kmul; };
     // all twiddles and sequence elements of the thread's NIT bins are requested up front (the loop
     // is latency bound otherwise: one shared and one global load chain per bin)
     constexpr int NIT = (NC / 2) / TPR;
@@ -426,11 +426,11 @@ static sfft_status launch_row_inv_t(const RowInvParams& P, cudaStream_t st) {
 
 sfft_status sfft_launch_row_fwd(sfft_plan* p, const double* R, const double* S,
                                 const unsigned char* mask, bool build, cplx* Tout, int pitchT, bool packed,
-                                bool pairT, cudaStream_t st, int* nl) {
+                                bool colT, cudaStream_t st, int* nl) {
   RowFwdParams P;
   P.R = R; P.S = S; P.mask = mask; P.H = p->H; P.W = p->W;
   P.nR = p->DK + 1; P.withS = build ? 1 : 0;
-  P.T = Tout; P.pitchT = pitchT; P.packed = packed ? 1 : 0; P.pairT = pairT ? 1 : 0; P.twP = p->twPNC; P.twW = p->twW;
+  P.T = Tout; P.pitchT = pitchT; P.packed = packed ? 1 : 0; P.colT = colT ? 1 : 0; P.twP = p->twPNC; P.twW = p->twW;
   P.moments = build ? 1 : 0; P.DB = p->DB; P.nMomA = p->nMomA; P.nMomS = p->nMomS; P.nMomR = p->nMomR;
   P.rowMom = p->rowMom;
   for (int a = 0; a < ROW_NMA; ++a) P.fullA[a] = p->fullA[a];

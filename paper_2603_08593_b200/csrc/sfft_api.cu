@@ -64,7 +64,7 @@ static cudaError_t upload_pass_tables(cplx** dst, int n) {
 
 static void plan_free(sfft_plan* p) {
   if (!p) return;
-  cudaFree(p->twP512);
+  cudaFree(p->tw128);
   cudaFree(p->twPNC); cudaFree(p->twPH); cudaFree(p->twW); cudaFree(p->twH); cudaFree(p->d_pairs); cudaFree(p->d_groups);
   cudaFree(p->T); cudaFree(p->F); cudaFree(p->Y); cudaFree(p->Cmap); cudaFree(p->rowMom);
   cudaFree(p->mom); cudaFree(p->spCount); cudaFree(p->spOff); cudaFree(p->spList); cudaFree(p->fmFlag); cudaFree(p->fmList); cudaFree(p->kbPart); cudaFree(p->kbCorr); cudaFree(p->kbStrip); cudaFree(p->Lw); cudaFree(p->exScratch); cudaFree(p->exRows); cudaFree(p->exBar); cudaFree(p->cholBar); cudaFree(p->Etab); cudaFree(p->Mhat);
@@ -126,8 +126,8 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   p->nMomR = DK + DB + 1;
   p->ldL = (p->N + 1 + 3) & ~3;
   p->fused = sfft_colx_supported(H, p->nPair) ? 1 : 0;
-  p->nPart = p->fused ? H / 512 : 1;
-  p->pitchT = p->fused ? p->NC + 8 : p->NC;
+  p->nPart = 1;
+  p->pitchT = p->NC;
   for (int a = 0; a <= 2 * SFFT_MAX_DEG; ++a) {   // whole-row sums of xi^a (odd powers cancel exactly)
     long double acc = 0.0L;
     if ((a & 1) == 0)
@@ -189,9 +189,9 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
     ws += bytes;
   };
   const size_t HN = (size_t)H * p->NC, HP = (size_t)H * p->pitch;
-  // fused path: pair-major T[img][NC/2+1][H][2]; subtract always uses row-major packed [DK+1][H][NC]
+  // fused path: column-major T[img][NC+1][H]; subtract always uses row-major packed [DK+1][H][NC]
   size_t Tbytes = sizeof(cplx) * (size_t)H * p->pitchT * p->nRowImg;
-  if (p->fused) Tbytes = sizeof(cplx) * (size_t)H * 2 * (p->NC / 2 + 1) * p->nRowImg;
+  if (p->fused) Tbytes = sizeof(cplx) * (size_t)H * (p->NC + 1) * p->nRowImg;
   const size_t Fbytes = p->fused ? 256 : sizeof(cplx) * HP * p->nSpec;   // no spectra in HBM on the fused path
   const size_t Ybytes = sizeof(cplx) * (size_t)p->nPart * p->nPair * p->nLag * p->pitch;
   dalloc((void**)&p->T, Tbytes);
@@ -221,7 +221,7 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   dalloc((void**)&p->d_pairs, sizeof(PairDesc) * p->nPair);
   dalloc((void**)&p->d_groups, sizeof(CrossGroup) * groups.size());
   if (!ok) { plan_free(p); return SFFT_ERR_ALLOC; }
-  if (p->fused && (upload_pass_tables(&p->twP512, 512) != cudaSuccess || sfft_colx_init() != SFFT_OK)) {
+  if (p->fused && upload_twiddles(&p->tw128, 128) != cudaSuccess) {
     cudaGetLastError();
     plan_free(p);
     return SFFT_ERR_CUDA;

@@ -93,10 +93,10 @@ struct sfft_plan {
   // device tables
   cplx* twPNC;   // per-pass FFT twiddle tables for length NC (fft_smem.cuh)
   cplx* twPH;    // per-pass FFT twiddle tables for length H
-  cplx* twP512;  // per-pass FFT twiddle tables for length 512 (fused column/cross kernel)
-  int fused;     // 1: k_colx replaces k_col_fwd + k_cross (H in {1024,2048,4096}, <= 32 pairs)
-  int nPart;     // partial lag-row sets in Y (H/512 on the fused path, else 1)
-  int pitchT;    // row pitch of T on the build path (NC + 8 unpacked when fused, else NC packed)
+  cplx* tw128;   // e^{-2 pi i m/128}: block transforms of the blocked column/cross kernel (k_colb.cu)
+  int fused;     // 1: k_colb replaces k_col_fwd + k_cross (H in {1024,2048,4096}, <= 32 pairs)
+  int nPart;     // partial lag-row sets in Y (1 on both paths)
+  int pitchT;    // row pitch of T on the generic build path (NC packed); the fused path is column-major
   cplx* twW;     // e^{-2 pi i m / W},  m in [0, W)
   cplx* twH;     // e^{-2 pi i m / H},  m in [0, H)
   PairDesc* d_pairs;
@@ -192,7 +192,7 @@ inline int sfft_device_sms() {
 // build = true: images m xi^p R (p <= DK) and m S with the fused row moments; false: xi^p R only
 sfft_status sfft_launch_row_fwd(sfft_plan* p, const double* R, const double* S,
                                 const unsigned char* mask, bool build, cplx* Tout, int pitchT, bool packed,
-                                bool pairT, cudaStream_t st, int* nl);
+                                bool colT, cudaStream_t st, int* nl);
 sfft_status sfft_launch_col_fwd(sfft_plan* p, cudaStream_t st, int* nl);
 sfft_status sfft_launch_cross(sfft_plan* p, cudaStream_t st, int* nl);
 sfft_status sfft_launch_colx(sfft_plan* p, cudaStream_t st, int* nl);
@@ -200,8 +200,6 @@ size_t sfft_exact_scratch_bytes(int N);
 size_t sfft_exact_rows_bytes(int N);
 sfft_status sfft_launch_exact_update(sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
                                      double* A, double* b, cudaStream_t st, int* nl);
-int sfft_colx_dinst(int w);
-sfft_status sfft_colx_init();
 bool sfft_colx_supported(int H, int nPair);
 sfft_status sfft_launch_kb(sfft_plan* p, const double* R, const unsigned char* mask, cudaStream_t st, int* nl);
 sfft_status sfft_launch_moments(sfft_plan* p, cudaStream_t st, int* nl);
