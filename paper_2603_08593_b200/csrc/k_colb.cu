@@ -35,7 +35,8 @@
 //   phase 4  (once per column) accumulators -> shared memory, 16-point inverse over b (k = a + 8 b),
 //            then the 2D+1 lags of every pair (8 twiddled terms each), Y[pair][dy][kx].
 // Shared-memory positions are XOR-swizzled (slot k1*16 + (j ^ k1)): every pass is conflict free with no
-// padding.  T is column-major (T[img][kx][y]), so every load is a contiguous 256-byte run per half warp.
+// padding.  T has the row-group layout T[img][y/G][kx][y%G], G = SFFT_T_G = 8 (k_row2_fwd): a half warp's 16
+// rows of a column are two whole 128-byte lines.
 #include <math.h>
 #include "fft_smem.cuh"
 
@@ -45,7 +46,7 @@
 #define CB_LAGS 21        // 2 * 10 + 1
 
 struct ColbParams {
-  const cplx* T;          // [nimg][NC+1][H] column-major row spectra
+  const cplx* T;          // [nimg][H/G][NC+1][G] row spectra, row-group layout (G = SFFT_T_G)
   cplx* Y;                // [nPair][nLag][pitch]
   const PairDesc* pairs;
   const cplx* tw128;      // e^{-2 pi i m/128}, m < 128
@@ -103,6 +104,10 @@ __host__ __device__ constexpr int cb_part_pairs(int T0, int T1, int U0, int U1) 
   return n;
 }
 
+// offset of row y inside one image of T (column 0): T[img][y/G][kx][y%G], G = SFFT_T_G
+__device__ __forceinline__ size_t cb_toff(int y, size_t grpStride) {
+  return (size_t)(y / SFFT_T_G) * grpStride + (size_t)(y % SFFT_T_G);
+}
 __device__ __forceinline__ int cb_slot(int k1, int j) { return k1 * 16 + (j ^ k1); }   // k1 < 8, j < 16
 
 // Phase 3 for one block: acc[] += conj(C_t) E_t2 over the part's pairs, every operand read once.
@@ -219,7 +224,8 @@ __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
   const int tid = threadIdx.x;
   const int H = P.H, D = P.D, B = P.B, nblk = P.nblk, nst = P.nst;
   const double invH = 1.0 / (double)H;
-  const size_t imgStride = (size_t)(P.NC + 1) * H;
+  const size_t imgStride = (size_t)(P.NC + 1) * H;      // T[img][y/G][kx][y%G] (k_row2_fwd)
+  const size_t grpStride = (size_t)(P.NC + 1) * SFFT_T_G;
   for (int i = tid; i < CB_N; i += CB_TH) s_tw[i] = ldg2(P.tw128 + i);
   for (int i = tid; i < NPAIR; i += CB_TH) s_Dp[i] = P.pairs[i].D;
   for (int i = tid; i < 7 * 16; i += CB_TH) s_w[i] = ldg2(P.tw128 + ((i >> 4) + 1) * (i & 15));
@@ -242,7 +248,7 @@ __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
     const cplx* src = Tcol + (size_t)img * imgStride;
     const int y0 = c0 - D + p1_j + H;
 #pragma unroll
-    for (int r = 0; r < 8; ++r) x[r] = (p1_j + 16 * r < lim) ? src[(y0 + 16 * r) & (H - 1)] : cmake(0.0, 0.0);
+    for (int r = 0; r < 8; ++r) x[r] = (p1_j + 16 * r < lim) ? src[cb_toff((y0 + 16 * r) & (H - 1), grpStride)] : cmake(0.0, 0.0);
   };
   // the thread's inputs of stage st of column nkx: the group's first row image into registers (xa), its
   // second one (if any) by cp.async into the half warp's staging slot
@@ -252,7 +258,7 @@ __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
     if (nkx > P.NC) return;
     const int bs = (st * nblk) / nst, be = ((st + 1) * nblk) / nst;
     if (bs + p1_u >= be) return;
-    const cplx* Tn = P.T + (size_t)nkx * H;
+    const cplx* Tn = P.T + SFFT_T_G * (size_t)nkx;
     if (p1_img0 >= 0) fetch(xa, Tn, bs + p1_u, p1_img0);
     if (p1_img1 >= 0) {
       const int c0 = (bs + p1_u) * B;
@@ -260,7 +266,8 @@ __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
       const cplx* src = Tn + (size_t)p1_img1 * imgStride;
       const int y0 = c0 - D + p1_j + H;
 #pragma unroll
-      for (int r = 0; r < 8; ++r) cb_cp_async16(xs + 16 * r, src + ((y0 + 16 * r) & (H - 1)), p1_j + 16 * r < lim);
+      for (int r = 0; r < 8; ++r)
+        cb_cp_async16(xs + 16 * r, src + cb_toff((y0 + 16 * r) & (H - 1), grpStride), p1_j + 16 * r < lim);
     }
     asm volatile("cp.async.commit_group;\n" ::: "memory");
   };

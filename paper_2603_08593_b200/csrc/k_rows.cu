@@ -24,7 +24,7 @@ struct RowFwdParams {
   cplx* T;       // [nimg][H][pitchT]
   int pitchT;    // row pitch of T in complex elements
   int packed;    // 1: T[y][0] = X[0] + i X[W/2];  0: T[y][0] = X[0], T[y][NC] = X[W/2]
-  int colT;      // 1 (unpacked only): column-major layout T[img][kx][y], kx in [0, NC], read by k_colb
+  int colT;      // 1 (unpacked only): row-pair layout T[img][y/2][kx][y%2], kx in [0, NC], written by k_row2_fwd, read by k_colb
   const cplx* twP;   // per-pass twiddle tables for length NC
   const cplx* twW;
   int moments, DB, nMomA, nMomS, nMomR;
@@ -207,10 +207,8 @@ __global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
     fft_regs_to_smem<NC, -1, false>(v, s, tid, nth, RB, P.twP, C::SEQ_STRIDE);
     fetch(im + 1);
     // split: X[k] = Xe + w^k Xo, X[NC-k] = conj(Xe - w^k Xo), w = e^{-2 pi i / W}
-    // element k of this row: row-major out[k], or column-major (im*(NC+1) + k)*H + y
-    cplx* out = P.colT ? P.T + (size_t)im * (NC + 1) * H + y : P.T + ((size_t)im * H + y) * P.pitchT;
-    const size_t kmul = P.colT ? (size_t)H : 1;   // offset of column k
-    auto at = [&](int k) -> cplx* { return out + (size_t)k * kmul; };
+    cplx* out = P.T + ((size_t)im * H + y) * P.pitchT;
+    auto at = [&](int k) -> cplx* { return out + k; };
     // all twiddles and sequence elements of the thread's NIT bins are requested up front (the loop
     // is latency bound otherwise: one shared and one global load chain per bin)
     constexpr int NIT = (NC / 2) / TPR;
@@ -275,6 +273,233 @@ __global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
       ROW_ST(at(NC / 2), cadd(xe, cmul(ldg2(P.twW + NC / 2), xo)));
     }
     __syncthreads();
+  }
+}
+
+
+// ------------------------------------------------------------------------------------------------
+// Row pass of the fused build path: one CTA = one image (blockIdx.x % nimg) of RB row PAIRS (2b, 2b+1).
+// The two rows of a pair are transformed one after the other into two shared-memory buffers and leave
+// the CTA together: the split step writes, per column kx, the 32-byte pair {X_2b[kx], X_2b+1[kx]}, so
+// T has the row-pair layout T[img][y/2][kx][y%2] (kx in [0, NC]) -- a warp's stores are one contiguous
+// 1 KB run (full lines), and k_colb reads whole 32-byte sectors along y.  Row 2b's inputs go from
+// global memory through the weighting into the first butterfly (registers only); row 2b+1's inputs are
+// requested at the same time by cp.async into the second buffer (free until that row's first pass),
+// so no global-memory latency is exposed between the two transforms.  Fused reductions as in k_row_fwd.
+__device__ __forceinline__ void row_cp_async16(void* smem_dst, const void* gsrc) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void row_st_pair(cplx* dst, cplx a, cplx b) {   // 32-byte streaming store
+  asm volatile("st.global.cs.v4.f64 [%0], {%1, %2, %3, %4};\n" ::"l"(dst), "d"(a.x), "d"(a.y), "d"(b.x), "d"(b.y) : "memory");
+}
+
+template <int NC, int MINB>
+__global__ void __launch_bounds__(128, MINB) k_row2_fwd(RowFwdParams P) {
+  using C = FftCfg<NC>;
+  constexpr int EPT = C::EPT;
+  constexpr int TPR = NC / EPT;  // threads per row
+  constexpr int LW = TPR < 32 ? TPR : 32;           // lanes of one row inside a warp
+  constexpr int WPR = TPR / 32 > 0 ? TPR / 32 : 1;  // warps per row
+  constexpr int NSLOT = 128 / LW;                   // (pair, warp-of-row) slots of a CTA
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ double redM[2][ROW_NMA][NSLOT];
+  __shared__ double redX[2][SFFT_MAX_DEG][NSLOT];
+  cplx* s = reinterpret_cast<cplx*>(smem_raw);
+  const int tid = threadIdx.x, nth = blockDim.x;
+  const int RB = nth / TPR;
+  const int r = tid / TPR, tr = tid - r * TPR;
+  const int nimg = P.nR + P.withS;
+  const int im = blockIdx.x % nimg;                 // images of one pair run side by side (R rows stay in L2)
+  const int pairIdx = (blockIdx.x / nimg) * RB + r;
+  const int y0 = 2 * pairIdx;
+  const int W = P.W, H = P.H;
+  const double invW = 1.0 / (double)W;
+  const double xb = (double)(4 * tr + 1 - W) * invW, step = (double)(4 * TPR) * invW, dx1 = 2.0 * invW;
+  const int slot = tid / LW;
+  const int pw = im < P.nR ? im : 0;
+  const double* src = (im < P.nR ? P.R : P.S) + (size_t)y0 * W;
+  cplx* buf[2] = {s, s + RB * C::SEQ_STRIDE};
+  cplx* raw1s = buf[1] + r * C::SEQ_STRIDE;         // row 2b+1's inputs, unpadded, until its first pass
+
+#pragma unroll
+  for (int e = 0; e < EPT; ++e) row_cp_async16(raw1s + tr + e * TPR, src + W + 2 * (tr + e * TPR));
+  asm volatile("cp.async.commit_group;\n" ::: "memory");
+  double2 raw[EPT];
+#pragma unroll
+  for (int e = 0; e < EPT; ++e) raw[e] = ROW_LD(reinterpret_cast<const double2*>(src + 2 * (tr + e * TPR)));
+
+  // mask bits of both rows: bit 2e = element 2j masked, bit 2e+1 = element 2j+1 masked, j = tr + e*TPR
+  unsigned mbits[2] = {0u, 0u};
+  if (P.mask) {
+    uchar2 mk[2][EPT];
+#pragma unroll
+    for (int rr = 0; rr < 2; ++rr)
+#pragma unroll
+      for (int e = 0; e < EPT; ++e)
+        mk[rr][e] = *reinterpret_cast<const uchar2*>(P.mask + (size_t)(y0 + rr) * W + 2 * (tr + e * TPR));
+#pragma unroll
+    for (int rr = 0; rr < 2; ++rr)
+#pragma unroll
+      for (int e = 0; e < EPT; ++e)
+        mbits[rr] |= (mk[rr][e].x ? 1u : 0u) << (2 * e) | (mk[rr][e].y ? 1u : 0u) << (2 * e + 1);
+  }
+  const bool momA = P.moments && im == 0;
+  if (momA) {
+    // masked part of sum_x m xi^a: only warps that hold a masked pixel do any work
+#pragma unroll
+    for (int rr = 0; rr < 2; ++rr) {
+      double ms[ROW_NMA];
+#pragma unroll
+      for (int a = 0; a < ROW_NMA; ++a) ms[a] = 0.0;
+      if (__any_sync(0xffffffffu, mbits[rr] != 0u)) {
+        unsigned mm = mbits[rr];
+        while (mm) {
+          const int bit = __ffs(mm) - 1;
+          mm &= mm - 1;
+          const int j = tr + (bit >> 1) * TPR;
+          const double x = (double)(4 * j + 1 + 2 * (bit & 1) - W) * invW;
+          double pwr = 1.0;
+#pragma unroll
+          for (int a = 0; a < ROW_NMA; ++a) { ms[a] += pwr; pwr *= x; }
+        }
+#pragma unroll
+        for (int a = 0; a < ROW_NMA; ++a) {
+#pragma unroll
+          for (int off = LW / 2; off > 0; off >>= 1) ms[a] += __shfl_xor_sync(0xffffffffu, ms[a], off);
+        }
+      }
+      if ((tid & (LW - 1)) == 0) {
+#pragma unroll
+        for (int a = 0; a < ROW_NMA; ++a) redM[rr][a][slot] = ms[a];
+      }
+    }
+  }
+  const bool extra = P.moments && P.DB > 0 && im >= P.nR - 1;
+
+#pragma unroll
+  for (int rr = 0; rr < 2; ++rr) {
+    if (rr == 1) {
+      asm volatile("cp.async.wait_all;\n" ::: "memory");   // the thread's own copies have landed
+#pragma unroll
+      for (int e = 0; e < EPT; ++e) raw[e] = raw1s[tr + e * TPR];
+      __syncthreads();                                      // every thread holds its inputs: the buffer may be rewritten
+    }
+    if (mbits[rr]) {
+#pragma unroll
+      for (int e = 0; e < EPT; ++e) {
+        if ((mbits[rr] >> (2 * e)) & 1u) raw[e].x = 0.0;
+        if ((mbits[rr] >> (2 * e + 1)) & 1u) raw[e].y = 0.0;
+      }
+    }
+    cplx v[EPT];
+    switch (pw) {
+      case 0:
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) v[e] = raw[e];
+        break;
+      case 1: row_weight<EPT, 1>(raw, v, xb, step, dx1); break;
+      case 2: row_weight<EPT, 2>(raw, v, xb, step, dx1); break;
+      default: row_weight<EPT, 3>(raw, v, xb, step, dx1); break;
+    }
+    if (extra) {
+      double hi[SFFT_MAX_DEG];
+      switch (P.DB) {
+        case 1: row_extra_moments<EPT, 1>(v, xb, step, dx1, hi); break;
+        case 2: row_extra_moments<EPT, 2>(v, xb, step, dx1, hi); break;
+        default: row_extra_moments<EPT, 3>(v, xb, step, dx1, hi); break;
+      }
+#pragma unroll
+      for (int i = 0; i < SFFT_MAX_DEG; ++i) {
+#pragma unroll
+        for (int off = LW / 2; off > 0; off >>= 1) hi[i] += __shfl_xor_sync(0xffffffffu, hi[i], off);
+      }
+      if ((tid & (LW - 1)) == 0) {
+#pragma unroll
+        for (int i = 0; i < SFFT_MAX_DEG; ++i) redX[rr][i][slot] = hi[i];
+      }
+    }
+    fft_regs_to_smem<NC, -1, false>(v, buf[rr], tid, nth, RB, P.twP, C::SEQ_STRIDE);
+  }
+
+  // split of both rows: X[k] = Xe + w^k Xo, X[NC-k] = conj(Xe - w^k Xo), w = e^{-2 pi i / W}
+  const cplx* sA = buf[0] + r * C::SEQ_STRIDE;
+  const cplx* sB = buf[1] + r * C::SEQ_STRIDE;
+  // T[img][y/G][kx][y%G]: column k of the pair's rows at out + G k
+  constexpr int G = SFFT_T_G;
+  cplx* out = P.T + ((size_t)im * (H / G) + y0 / G) * (size_t)(NC + 1) * G + (y0 % G);
+  constexpr int NIT = (NC / 2) / TPR;
+  constexpr int NBT = NIT >= SFFT_ROW_NBT ? SFFT_ROW_NBT : NIT;
+#pragma unroll 1
+  for (int i0 = 0; i0 < NIT; i0 += NBT) {
+    cplx tws[NBT], zk[2][NBT], zm[2][NBT];
+#pragma unroll
+    for (int i = 0; i < NBT; ++i) tws[i] = ldg2(P.twW + tr + (i0 + i) * TPR);
+#pragma unroll
+    for (int i = 0; i < NBT; ++i) {
+      const int k = tr + (i0 + i) * TPR;
+      const int pk = C::phys(k), pm = C::phys((NC - k) & (NC - 1));
+      zk[0][i] = sA[pk]; zm[0][i] = cconj(sA[pm]);
+      zk[1][i] = sB[pk]; zm[1][i] = cconj(sB[pm]);
+    }
+#pragma unroll
+    for (int i = 0; i < NBT; ++i) {
+      const int k = tr + (i0 + i) * TPR;
+      cplx xe[2], xo[2];
+#pragma unroll
+      for (int rr = 0; rr < 2; ++rr) {
+        xe[rr] = cscale(cadd(zk[rr][i], zm[rr][i]), 0.5);
+        xo[rr] = cmul_mi(cscale(csub(zk[rr][i], zm[rr][i]), 0.5));
+      }
+      if (i0 + i == 0 && tr == 0) {
+        double dc[2], ny[2];
+#pragma unroll
+        for (int rr = 0; rr < 2; ++rr) { dc[rr] = xe[rr].x + xo[rr].x; ny[rr] = xe[rr].x - xo[rr].x; }
+        row_st_pair(out, cmake(dc[0], 0.0), cmake(dc[1], 0.0));
+        row_st_pair(out + G * NC, cmake(ny[0], 0.0), cmake(ny[1], 0.0));
+        if (P.moments) {   // tr == 0 here: the pair's moment writer
+          const int s0 = r * WPR;
+          for (int rr = 0; rr < 2; ++rr) {
+            const int y = y0 + rr;
+            double* momS = P.rowMom + (size_t)P.nMomA * H + y;
+            double* momR = momS + (size_t)P.nMomS * H;
+            if (im < P.nR) momR[(size_t)im * H] = dc[rr]; else momS[0] = dc[rr];
+            if (extra) {
+              double* dst = im < P.nR ? momR + (size_t)P.nR * H : momS + H;
+              for (int ii = 0; ii < P.DB; ++ii) {
+                double t = 0.0;
+                for (int k2 = 0; k2 < WPR; ++k2) t += redX[rr][ii][s0 + k2];
+                dst[(size_t)ii * H] = t;
+              }
+            }
+            if (momA) {
+              for (int a = 0; a < P.nMomA; ++a) {
+                double t = 0.0;
+                for (int k2 = 0; k2 < WPR; ++k2) t += redM[rr][a][s0 + k2];
+                P.rowMom[(size_t)a * H + y] = P.fullA[a] - t;
+              }
+            }
+          }
+        }
+      } else {
+        const cplx t0 = cmul(tws[i], xo[0]), t1 = cmul(tws[i], xo[1]);
+        row_st_pair(out + G * k, cadd(xe[0], t0), cadd(xe[1], t1));
+        row_st_pair(out + G * (NC - k), cconj(csub(xe[0], t0)), cconj(csub(xe[1], t1)));
+      }
+    }
+  }
+  if (tr == 0) {   // the middle bin k = NC/2 pairs with itself
+    const cplx tw = ldg2(P.twW + NC / 2);
+    cplx o[2];
+#pragma unroll
+    for (int rr = 0; rr < 2; ++rr) {
+      const cplx z = (rr ? sB : sA)[C::phys(NC / 2)];
+      const cplx zc = cconj(z);
+      const cplx xe = cscale(cadd(z, zc), 0.5);
+      const cplx xo = cmul_mi(cscale(csub(z, zc), 0.5));
+      o[rr] = cadd(xe, cmul(tw, xo));
+    }
+    row_st_pair(out + G * (NC / 2), o[0], o[1]);
   }
 }
 
@@ -399,6 +624,19 @@ static sfft_status launch_row_fwd_t(const RowFwdParams& P, cudaStream_t st) {
 }
 
 template <int NC>
+static sfft_status launch_row2_fwd_t(const RowFwdParams& P, cudaStream_t st) {
+  using C = FftCfg<NC>;
+  int nth = row_threads(NC, P.H / 2, C::EPT);
+  const int RB = nth / (NC / C::EPT);
+  const size_t smem = (size_t)2 * RB * C::SEQ_STRIDE * sizeof(cplx);
+  constexpr int MINB = SFFT_ROW_MINB;
+  SFFT_CUDA_TRY(cudaFuncSetAttribute(k_row2_fwd<NC, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  k_row2_fwd<NC, MINB><<<(P.H / 2 / RB) * (P.nR + P.withS), nth, smem, st>>>(P);
+  SFFT_LAUNCH_CHECK();
+  return SFFT_OK;
+}
+
+template <int NC>
 static sfft_status launch_row_inv_t(const RowInvParams& P, cudaStream_t st) {
   using C = FftCfg<NC>;
   const int nth = row_threads(NC, P.H, C::EPT);
@@ -435,6 +673,9 @@ sfft_status sfft_launch_row_fwd(sfft_plan* p, const double* R, const double* S,
   P.rowMom = p->rowMom;
   for (int a = 0; a < ROW_NMA; ++a) P.fullA[a] = p->fullA[a];
   ++*nl;
+  if (colT) {
+    SFFT_DISPATCH_NC(p->NC, launch_row2_fwd_t)
+  }
   SFFT_DISPATCH_NC(p->NC, launch_row_fwd_t)
 }
 

@@ -13,6 +13,9 @@
 #define SFFT_CR_GP 21        // k_cross: pairs per CTA (threads = SFFT_CR_GP * SFFT_CR_CT)
 #define SFFT_CR_MAXSPEC 24   // k_cross: spectra a group may stage
 #define SFFT_KB_NBLK 296     // x-CTAs of the kernel-background correction kernel (2 per SM)
+#ifndef SFFT_T_G
+#define SFFT_T_G 8          // fused path: rows per group of the row-spectra layout T[img][y/G][kx][y%G]
+#endif
 #define SFFT_NSTAGE 10     // see sfft_profile_read in include/sfft.h
 #define SFFT_PROF_MAX 512
 
