@@ -26,6 +26,21 @@ It shares no code with the CUDA path and does not import the package.  Plain num
     (divide by the number of kept apertures); L4 the positions are inputs (the random draw is the
     caller's), so both sides see the same ones; L5 m_lim = zp - 2.5 log10(5 sigma).
 
+(3) Multi-template MODE, the whole chain of (1) -- PAPER.md:158 (§2.3.2) with N_TEMP of PAPER.md:94:
+    multi_template_difference = N_TEMP runs of the differencing oracle (oracle/sfft_oracle.py, one per
+    template exposure, all against the same science image), then (1).  Reading MT1 (paper silent on
+    which pixels enter each fit): one common mask -- the union of the science and template data-quality
+    masks (PAPER.md:162 treats a pixel as bad when it is flagged "in either the science or template
+    images") -- is used in all N_TEMP fits; a list of per-template masks is accepted too.
+
+(4) Three-channel stamps for the real-bogus classifier -- PAPER.md:168 (§2.3.4): "the classifier takes
+    as input a set of three-channel image stamps -- consisting of the science image, template image,
+    and their difference -- centered on the candidate position".  The paper gives neither the stamp
+    size nor an edge rule; readings: ST1 channel order (science, template, difference), as listed;
+    ST2 the stamp is size x size pixels, its centre pixel (index size//2 along each axis) is the pixel
+    nearest the position, (floor(x + 1/2), floor(y + 1/2)), pixel centres at integer coordinates;
+    ST3 pixels outside the frame are 0; ST4 a non-finite position gives an all-NaN stamp.
+
 Pins (tests/test_post_pins.py): statistics.median on small stacks, permutation and scale
 invariance, known order statistics; Gauss circle lattice counts N(r) for the disc, a constant image
 (flux = c N(r), sigma = 0), a linear ramp (flux = N(r) * value at the centre for integer centres),
@@ -84,6 +99,42 @@ def aperture_stats(D, mask, xs, ys, radius):
 def limiting_magnitude(sigma, zero_point):
     """m_lim = zp - 2.5 log10(5 sigma)  (reading L5)."""
     return zero_point - 2.5 * math.log10(5.0 * sigma)
+
+
+def multi_template_difference(Rs, S, masks, w, DK, DB, scales, workers=1):
+    """(D_final, [D_k], [c_k]): one differencing per template R_k against the same S,
+    D_final = median_k(scales[k] * D_k).  `masks`: one common mask (reading MT1), None, or a list."""
+    from oracle import sfft_oracle as orc
+    if masks is None or isinstance(masks, np.ndarray):
+        masks = [masks] * len(Rs)
+    Ds, cs = [], []
+    for R, m in zip(Rs, masks):
+        _, _, c, D = orc.sfft_difference(R, S, m, w, DK, DB, workers=workers, fourier_subtract=True)
+        Ds.append(D)
+        cs.append(c)
+    return median_combine(Ds, scales), Ds, cs
+
+
+def cut_stamps(S, R, D, xs, ys, size):
+    """[n, 3, size, size] stamps (science, template, difference) centred on the positions
+    (readings ST1-ST4).  Explicit loops."""
+    H, W = S.shape
+    n = len(xs)
+    out = np.zeros((n, 3, size, size))
+    half = size // 2
+    for k in range(n):
+        x, y = float(xs[k]), float(ys[k])
+        if not (math.isfinite(x) and math.isfinite(y)):
+            out[k] = np.nan
+            continue
+        cx, cy = math.floor(x + 0.5), math.floor(y + 0.5)
+        for ch, img in enumerate((S, R, D)):
+            for j in range(size):
+                for i in range(size):
+                    yy, xx = cy - half + j, cx - half + i
+                    if 0 <= yy < H and 0 <= xx < W:
+                        out[k, ch, j, i] = img[yy, xx]
+    return out
 
 
 # --------------------------------------------------------------------------- resampling (NEXT-4)

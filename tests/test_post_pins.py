@@ -158,3 +158,83 @@ def test_resample_mask_threshold():
     # L(1.5) = -0.135 < 0.3
     out = po.resample_mask_affine(mask, [0.5, 1.0, 0.0, 0.0, 0.0, 1.0], 20, 20)
     assert out[10, 9] == 2 and out[10, 10] == 2 and out[10, 8] == 1 and out[10, 11] == 1
+
+
+# --------------------------------------------------------------------------- stamps
+def test_stamps_hand_written_values():
+    """5x6 images with value 10 y + x (science), 100 + that (template), -that (difference): stamps
+    written out by hand for an interior, a corner and an off-frame position (readings ST1-ST3)."""
+    H, W = 5, 6
+    base = np.array([[10.0 * y + x for x in range(W)] for y in range(H)])
+    S, R, D = base, 100.0 + base, -base
+    st = po.cut_stamps(S, R, D, [2.0, 0.0, 5.4, -3.0], [2.0, 0.0, 4.2, 1.0], 3)
+    assert st.shape == (4, 3, 3, 3)
+    assert st[0, 0].tolist() == [[11, 12, 13], [21, 22, 23], [31, 32, 33]]
+    assert st[0, 1].tolist() == [[111, 112, 113], [121, 122, 123], [131, 132, 133]]
+    assert st[0, 2].tolist() == [[-11, -12, -13], [-21, -22, -23], [-31, -32, -33]]
+    assert st[1, 0].tolist() == [[0, 0, 0], [0, 0, 1], [0, 10, 11]]          # top-left corner: zero fill
+    assert st[2, 0].tolist() == [[34, 35, 0], [44, 45, 0], [0, 0, 0]]        # (5.4, 4.2) -> pixel (5, 4)
+    assert st[3].tolist() == np.zeros((3, 3, 3)).tolist()                    # wholly outside the frame
+
+
+def test_stamps_rounding_even_size_and_nonfinite():
+    H, W = 8, 8
+    S = np.arange(64.0).reshape(H, W)
+    # nearest pixel: floor(x + 1/2) -- 2.5 -> 3, 2.49 -> 2, -0.5 -> 0, -0.51 -> -1
+    st = po.cut_stamps(S, S, S, [2.5, 2.49, -0.5, -0.51], [3.0, 3.0, 3.0, 3.0], 1)
+    assert st[:, 0, 0, 0].tolist() == [27.0, 26.0, 24.0, 0.0]
+    # even size: the centre pixel has index size//2, so the stamp starts size//2 before it
+    st = po.cut_stamps(S, S, S, [4.0], [4.0], 4)
+    assert st[0, 0, 2, 2] == S[4, 4] and st[0, 0, 0, 0] == S[2, 2] and st[0, 0, 3, 3] == S[5, 5]
+    st = po.cut_stamps(S, S, S, [float("nan"), float("inf")], [1.0, 1.0], 3)
+    assert np.isnan(st).all()
+
+
+# ------------------------------------------------------------- multi-template mode (PAPER.md:158)
+def _mt_pair(seed, H=32, W=32):
+    rng = np.random.default_rng(seed)
+    R = 50.0 * rng.standard_normal((H, W)) + 400.0 * (rng.random((H, W)) > 0.97)
+    S = 0.8 * np.roll(R, (1, -1), (0, 1)) + 5.0 * rng.standard_normal((H, W)) + 120.0
+    mask = (rng.random((H, W)) < 0.04).astype(np.uint8)
+    return R, S, mask
+
+
+def test_multi_template_identical_templates_equal_the_single_difference():
+    from oracle import sfft_oracle as orc
+    R, S, mask = _mt_pair(1)
+    _, _, _, D1 = orc.sfft_difference(R, S, mask, 1, 1, 1)
+    Dm, Ds, cs = po.multi_template_difference([R] * 5, S, mask, 1, 1, 1, [1.0] * 5)
+    assert len(Ds) == 5 and np.array_equal(Dm, D1)
+
+
+def test_multi_template_permutation_invariance_and_outlier_rejection():
+    rng = np.random.default_rng(2)
+    R, S, mask = _mt_pair(2)
+    # five different templates (independent noise realisations of the same field)
+    Rs = [R + 3.0 * rng.standard_normal(R.shape) for _ in range(5)]
+    sc = [1.0, 1.1, 0.9, 1.05, 0.95]
+    Dm, Ds, _ = po.multi_template_difference(Rs, S, mask, 1, 0, 0, sc)
+    perm = [3, 0, 4, 1, 2]
+    Dp, _, _ = po.multi_template_difference([Rs[i] for i in perm], S, mask, 1, 0, 0, [sc[i] for i in perm])
+    assert np.array_equal(Dm, Dp)
+    # the result is, pixel by pixel, one of the scaled individual differences (odd count)
+    stack = np.stack([s * D for s, D in zip(sc, Ds)])
+    assert np.all(np.any(stack == Dm[None], axis=0))
+    # four identical templates and one carrying an artefact: at least three of the five values of
+    # every pixel agree exactly, so the artefact never reaches the median
+    Rbad = R.copy()
+    Rbad[10:14, 10:14] += 5000.0
+    Dclean, _, _ = po.multi_template_difference([R] * 5, S, mask, 1, 0, 0, [1.0] * 5)
+    for pos in range(5):
+        Rs2 = [R] * 5
+        Rs2[pos] = Rbad
+        Dout, Ds2, _ = po.multi_template_difference(Rs2, S, mask, 1, 0, 0, [1.0] * 5)
+        assert np.array_equal(Dout, Dclean)
+        assert np.max(np.abs(Ds2[pos] - Dclean)) > 100.0      # the artefact is in that one difference
+
+
+def test_multi_template_per_template_masks_and_common_mask_agree_when_equal():
+    R, S, mask = _mt_pair(3)
+    a, _, _ = po.multi_template_difference([R, 1.01 * R, 0.99 * R], S, mask, 1, 0, 0, [1.0, 1.0, 1.0])
+    b, _, _ = po.multi_template_difference([R, 1.01 * R, 0.99 * R], S, [mask, mask, mask], 1, 0, 0, [1.0, 1.0, 1.0])
+    assert np.array_equal(a, b)
