@@ -502,7 +502,52 @@ def run_cuda(args, rank, world, local_rank):
                                       "rank_k_update_tflops": round(syrk_flop / ((t_ex - 0.72) * 1e-3) / 1e12, 2),
                                       "note": "ordinary build (0.72 ms) + masked-pixel list + cooperative 128x128-tiled fp64 SYRK on the "
                                               "fp64 tensor path (mma.sync m8n8k4) over rows generated once per 16384-pixel chunk"}
-        del Dt, outm
+        # multi-template MODE (NEXT-2): S against N_TEMP = 5 templates in one call (the science
+        # image's row transform computed once), against 5 x the single-template chain + the median
+        from paper_2603_08593_b200 import cut_stamps
+        gt = torch.Generator(device="cuda").manual_seed(11)
+        Rt = [Rx + 3.0 * torch.randn(Rx.shape, dtype=torch.float64, device="cuda", generator=gt) for _ in range(nT)]
+        for _ in range(2):
+            mt = plan.multi_template_difference(Rt, Sx, Mx, sc)
+        g6, g7, g8 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        g6.record()
+        for _ in range(3):
+            mt = plan.multi_template_difference(Rt, Sx, Mx, sc)
+        g7.record()
+        for _ in range(3):
+            sep = []
+            for k in range(nT):
+                plan.build_system(Rt[k], Sx, Mx, A, b)
+                plan.subtract_prepare(Rt[k])
+                plan.solve(A, b, c, info)
+                sep.append(plan.subtract(Rt[k], Sx, c, mt[1][k]))
+            median_combine(sep, sc, out=outm)
+        g8.record()
+        torch.cuda.synchronize()
+        assert mt[3].cpu().tolist() == [0] * nT and torch.equal(outm, mt[0])
+        t_mt, t_sep = g6.elapsed_time(g7) / 3, g7.elapsed_time(g8) / 3
+        post["multi_template"] = {"templates": nT, "ms": round(t_mt, 3), "ms_separate_calls": round(t_sep, 3),
+                                  "ccd_per_s": round(1e3 / t_mt, 1),
+                                  "note": "one sfft_multi_template_difference call (row transform and moments of m S "
+                                          "reused by templates 2..5) vs 5 x (build, prepare, solve, subtract) + "
+                                          "sfft_median_combine; bitwise equal results (asserted)"}
+        del mt, sep, Rt
+        # three-channel stamps (NEXT-3): 1024 candidates, 63 x 63 pixels (size is the caller's)
+        for _ in range(2):
+            stp = cut_stamps(Sx, Rx, D, xs, ys, 63)
+        g9, g10 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g9.record()
+        for _ in range(reps):
+            stp = cut_stamps(Sx, Rx, D, xs, ys, 63)
+        g10.record()
+        torch.cuda.synchronize()
+        t_st = g9.elapsed_time(g10) / reps
+        st_bytes = 2 * stp.numel() * 8
+        post["cut_stamps"] = {"candidates": 1024, "size": 63, "ms": round(t_st, 4), "bytes": st_bytes,
+                              "gbs": round(st_bytes / t_st / 1e6, 1),
+                              "note": "gather of 1024 x 3 x 63 x 63 fp64 (read + write bytes counted; the output "
+                                      "tensor is allocated inside the timed call)"}
+        del Dt, outm, stp
         torch.cuda.empty_cache()
 
     exposure = None

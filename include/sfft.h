@@ -126,6 +126,25 @@ sfft_status sfft_subtract_prepare(sfft_plan* p, const double* R, void* stream);
 sfft_status sfft_median_combine(const double* const* D, const double* scale, int n, size_t npix,
                                 double* out, void* stream);
 
+/* Multi-template MODE (§2.3.2: "the science image is differenced against each individual
+ * template exposure, producing N_TEMP difference images per science exposure.  All difference images
+ * are subsequently normalized to a common photometric zero point ... and median-combined"; N_TEMP
+ * default 5).  One call = n x (sfft_build_system, sfft_solve, sfft_subtract) against the
+ * same science image S, then sfft_median_combine.  The science image's share of the build -- the row
+ * transform of m S and its row moments -- is computed for the first template only and reused by the
+ * other n - 1 builds, which is why ONE mask serves all n fits (reading MT1: the union of the
+ * science and template data-quality masks; NULL = none).  Every D_k, c_k is bitwise what the three
+ * separate calls give for (R[k], S, mask).
+ *   R      in : HOST array of n DEVICE pointers, each H*W fp64, 16-byte aligned.
+ *   scale  in : HOST array of n flux factors to the common zero point.
+ *   Dk    out : n*H*W fp64 (device): the individual difference images D_k (unscaled).
+ *   coeffs out: n*N fp64 (device);  info out (nullable): n ints (device), as sfft_solve.
+ *   out   out : H*W fp64 (device): median_k(scale[k] * D_k).    1 <= n <= SFFT_MAX_TEMPLATES.
+ * All work is enqueued on `stream` (and the plan's side stream, joined back); never synchronises. */
+sfft_status sfft_multi_template_difference(sfft_plan* p, const double* const* R, const double* S,
+                                           const unsigned char* mask, const double* scale, int n,
+                                           double* Dk, double* coeffs, int* info, double* out, void* stream);
+
 /* Monte-Carlo limiting flux of a difference image (§2.3.3: "aperture fluxes at 1024
  * randomly selected background positions ... deriving the 5 sigma threshold from their standard
  * deviation").  The positions are INPUTS (the random draw is the caller's).
@@ -140,6 +159,19 @@ sfft_status sfft_median_combine(const double* const* D, const double* scale, int
 sfft_status sfft_aperture_stats(const double* D, const unsigned char* mask, int H, int W,
                                 const double* xs, const double* ys, int n, double radius,
                                 double* flux, double* stats, void* stream);
+
+/* Three-channel stamps for the real-bogus classifier (§2.3.4: "three-channel image
+ * stamps -- consisting of the science image, template image, and their difference -- centered on the
+ * candidate position").  The paper fixes neither the size nor an edge rule; readings ST1-ST4:
+ * channel order (science, template, difference); the stamp is size x size pixels and its centre pixel
+ * (index size/2 along each axis) is the pixel nearest the position, (floor(x + 1/2), floor(y + 1/2)),
+ * pixel (y,x) centred at integer coordinates; pixels outside the frame are 0; a non-finite position
+ * gives an all-NaN stamp.
+ *   S, R, D in: H*W fp64 (device);  xs, ys in: n real-valued positions (device);
+ *   out: n*3*size*size fp64 (device), out[k][channel][j][i].   1 <= size <= 1024.
+ * A gather (bit-exact copies).  Enqueues one kernel on `stream`; needs no plan. */
+sfft_status sfft_cut_stamps(const double* S, const double* R, const double* D, int H, int W,
+                            const double* xs, const double* ys, int n, int size, double* out, void* stream);
 
 /* Resampling onto another pixel grid, the step before the differencing (§2.3.2: the
  * science image is reprojected "onto the WCS of the corresponding template image(s) using SWARP";

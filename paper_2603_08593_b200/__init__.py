@@ -15,7 +15,8 @@ from .binding import (  # noqa: F401
     aperture_stats,
     resample_affine,
     resample_mask_affine,
+    cut_stamps,
 )
 
 __all__ = ["synth", "SfftPlan", "SfftError", "lib_path", "load_library", "EXPORTED_SYMBOLS",
-           "median_combine", "aperture_stats", "resample_affine", "resample_mask_affine"]
+           "median_combine", "aperture_stats", "resample_affine", "resample_mask_affine", "cut_stamps"]

@@ -19,6 +19,7 @@ EXPORTED_SYMBOLS = [
     "sfft_status_string", "sfft_build_system", "sfft_build_system_exact", "sfft_solve", "sfft_subtract", "sfft_subtract_prepare",
     "sfft_probe_fp64", "sfft_last_launch_count", "sfft_plan_fused", "sfft_plan_set_solve_ctas", "sfft_version",
     "sfft_profile_enable", "sfft_profile_read", "sfft_median_combine", "sfft_aperture_stats", "sfft_resample_affine", "sfft_resample_mask_affine",
+    "sfft_cut_stamps", "sfft_multi_template_difference",
 ]
 
 STAGE_NAMES = ["build.row_fwd", "build.col_fwd", "build.cross_KK", "build.cross_KS",
@@ -81,6 +82,10 @@ def load_library():
     lib.sfft_plan_set_solve_ctas.restype = i32
     lib.sfft_median_combine.argtypes = [vp, vp, i32, ctypes.c_size_t, vp, vp]
     lib.sfft_median_combine.restype = i32
+    lib.sfft_cut_stamps.argtypes = [vp, vp, vp, i32, i32, vp, vp, i32, i32, vp, vp]
+    lib.sfft_cut_stamps.restype = i32
+    lib.sfft_multi_template_difference.argtypes = [vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp]
+    lib.sfft_multi_template_difference.restype = i32
     lib.sfft_aperture_stats.argtypes = [vp, vp, i32, i32, vp, vp, i32, ctypes.c_double, vp, vp, vp]
     lib.sfft_aperture_stats.restype = i32
     lib.sfft_resample_affine.argtypes = [vp, i32, i32, vp, i32, vp, i32, i32, vp, vp]
@@ -218,6 +223,26 @@ class SfftPlan:
         _check(self._lib, self._lib.sfft_subtract_prepare(
             self._p, _dev_ptr(R, torch.float64, self.H * self.W, "R"), _stream_handle(stream)), "sfft_subtract_prepare")
 
+    def multi_template_difference(self, Rs, S, mask, scales, stream=None):
+        """sfft_multi_template_difference: S against every template of Rs with one
+        common mask, then the median of the scaled differences.  Returns (out, Dk, coeffs, info) with
+        Dk [n, H, W], coeffs [n, N], info [n]."""
+        import torch
+        n, P = len(Rs), self.H * self.W
+        dev = S.device
+        ptrs = (ctypes.c_void_p * n)(*[_dev_ptr(R, torch.float64, P, f"Rs[{k}]").value for k, R in enumerate(Rs)])
+        sc = (ctypes.c_double * n)(*[float(x) for x in scales])
+        Dk = torch.empty((n, self.H, self.W), dtype=torch.float64, device=dev)
+        coeffs = torch.empty((n, self.N), dtype=torch.float64, device=dev)
+        info = torch.zeros(n, dtype=torch.int32, device=dev)
+        out = torch.empty((self.H, self.W), dtype=torch.float64, device=dev)
+        _check(self._lib, self._lib.sfft_multi_template_difference(
+            self._p, ptrs, _dev_ptr(S, torch.float64, P, "S"), _dev_ptr(mask, torch.uint8, P, "mask"), sc, n,
+            _dev_ptr(Dk, torch.float64, n * P, "Dk"), _dev_ptr(coeffs, torch.float64, n * self.N, "coeffs"),
+            _dev_ptr(info, torch.int32, n, "info"), _dev_ptr(out, torch.float64, P, "out"),
+            _stream_handle(stream)), "sfft_multi_template_difference")
+        return out, Dk, coeffs, info
+
     def difference(self, R, S, mask, stream=None):
         """One pass of the whole hot path: build -> (subtract_prepare) -> solve -> subtract."""
         A, b = self.build_system(R, S, mask, stream=stream)
@@ -352,6 +377,22 @@ def aperture_stats(D, mask, xs, ys, radius, stream=None):
                                         ys.data_ptr(), n, float(radius), flux.data_ptr(), stats.data_ptr(),
                                         st.cuda_stream), "sfft_aperture_stats")
     return flux, stats
+
+
+def cut_stamps(S, R, D, xs, ys, size, stream=None):
+    """sfft_cut_stamps: [n, 3, size, size] (science, template, difference) stamps centred on the
+    positions.  S, R, D: CUDA float64 [H, W]; xs, ys: CUDA float64 [n]."""
+    import torch
+    lib = load_library()
+    H, W = S.shape
+    n = xs.numel()
+    out = torch.empty((n, 3, size, size), dtype=torch.float64, device=S.device)
+    _check(lib, lib.sfft_cut_stamps(_dev_ptr(S, torch.float64, H * W, "S"), _dev_ptr(R, torch.float64, H * W, "R"),
+                                    _dev_ptr(D, torch.float64, H * W, "D"), H, W, _dev_ptr(xs, torch.float64, n, "xs"),
+                                    _dev_ptr(ys, torch.float64, n, "ys"), n, int(size),
+                                    _dev_ptr(out, torch.float64, out.numel(), "out"), _stream_handle(stream)),
+           "sfft_cut_stamps")
+    return out
 
 
 def resample_affine(img, M, Hout, Wout, a=3, out=None, outside=None, stream=None):

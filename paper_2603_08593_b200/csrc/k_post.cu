@@ -11,6 +11,10 @@
 //                     whose centres lie within `radius`; NaN if the disc leaves the frame or touches
 //                     a masked pixel (readings L1, L2).  The positions are inputs.
 //  k_aperture_stats : count, mean and population sigma of the kept fluxes, fixed-order tree sums.
+//  k_cut_stamps     : three-channel (science, template, difference) stamps centred on candidate positions,
+//                     the input of the real-bogus classifier (§2.3.4; NEXT-3).  A gather:
+//                     one CTA per (candidate, channel), lanes along the stamp row; zero fill outside
+//                     the frame, all-NaN stamp for a non-finite position (readings ST1-ST4).
 //  k_resample<A>    : the step BEFORE the differencing (NEXT-4): Lanczos-A resampling of an image or a
 //                     data-quality mask through an affine pixel map.
 #include <math.h>
@@ -263,7 +267,43 @@ static sfft_status launch_resample(const ResampleParams& P, int a, cudaStream_t 
   return SFFT_OK;
 }
 
+
+__global__ void __launch_bounds__(256) k_cut_stamps(const double* __restrict__ S, const double* __restrict__ R,
+                                                    const double* __restrict__ D, int H, int W,
+                                                    const double* __restrict__ xs, const double* __restrict__ ys,
+                                                    int size, double* out) {
+  const int k = blockIdx.x, ch = blockIdx.y;
+  const double* img = ch == 0 ? S : (ch == 1 ? R : D);
+  double* dst = out + ((size_t)k * 3 + ch) * size * size;
+  const double x = xs[k], y = ys[k];
+  const int npx = size * size;
+  if (!(isfinite(x) && isfinite(y))) {
+    for (int e = threadIdx.x; e < npx; e += blockDim.x) dst[e] = nan("");
+    return;
+  }
+  // nearest pixel floor(x + 1/2); positions far outside the frame are clamped before the int
+  // conversion (the stamp is all zero either way)
+  const double lim = 1.0e9;
+  const long long cx = (long long)floor(fmin(fmax(x, -lim), lim) + 0.5);
+  const long long cy = (long long)floor(fmin(fmax(y, -lim), lim) + 0.5);
+  const int half = size / 2;
+  for (int e = threadIdx.x; e < npx; e += blockDim.x) {
+    const int j = e / size, i = e - j * size;
+    const long long yy = cy - half + j, xx = cx - half + i;
+    dst[e] = (yy >= 0 && yy < H && xx >= 0 && xx < W) ? img[(size_t)yy * W + (size_t)xx] : 0.0;
+  }
+}
+
 extern "C" {
+
+sfft_status sfft_cut_stamps(const double* S, const double* R, const double* D, int H, int W, const double* xs,
+                            const double* ys, int n, int size, double* out, void* stream) {
+  if (!S || !R || !D || !xs || !ys || !out || H < 1 || W < 1 || n < 1 || size < 1 || size > 1024)
+    return SFFT_ERR_INVALID_ARG;
+  k_cut_stamps<<<dim3((unsigned)n, 3), 256, 0, (cudaStream_t)stream>>>(S, R, D, H, W, xs, ys, size, out);
+  SFFT_LAUNCH_CHECK();
+  return SFFT_OK;
+}
 
 sfft_status sfft_median_combine(const double* const* D, const double* scale, int n, size_t npix, double* out,
                                 void* stream) {

@@ -667,7 +667,7 @@ sfft_status sfft_launch_row_fwd(sfft_plan* p, const double* R, const double* S,
                                 bool colT, cudaStream_t st, int* nl) {
   RowFwdParams P;
   P.R = R; P.S = S; P.mask = mask; P.H = p->H; P.W = p->W;
-  P.nR = p->DK + 1; P.withS = build ? 1 : 0;
+  P.nR = p->DK + 1; P.withS = (build && S) ? 1 : 0;   // S == NULL in a build: its row spectra are reused
   P.T = Tout; P.pitchT = pitchT; P.packed = packed ? 1 : 0; P.colT = colT ? 1 : 0; P.twP = p->twPNC; P.twW = p->twW;
   P.moments = build ? 1 : 0; P.DB = p->DB; P.nMomA = p->nMomA; P.nMomS = p->nMomS; P.nMomR = p->nMomR;
   P.rowMom = p->rowMom;

@@ -67,7 +67,7 @@ static void plan_free(sfft_plan* p) {
   cudaFree(p->tw128);
   cudaFree(p->twPNC); cudaFree(p->twPH); cudaFree(p->twW); cudaFree(p->twH); cudaFree(p->d_pairs); cudaFree(p->d_groups);
   cudaFree(p->T); cudaFree(p->F); cudaFree(p->Y); cudaFree(p->Cmap); cudaFree(p->rowMom);
-  cudaFree(p->mom); cudaFree(p->spCount); cudaFree(p->spOff); cudaFree(p->spList); cudaFree(p->fmFlag); cudaFree(p->fmList); cudaFree(p->kbPart); cudaFree(p->kbCorr); cudaFree(p->kbStrip); cudaFree(p->Lw); cudaFree(p->exScratch); cudaFree(p->exRows); cudaFree(p->exBar); cudaFree(p->cholBar); cudaFree(p->Etab); cudaFree(p->Mhat);
+  cudaFree(p->mom); cudaFree(p->spCount); cudaFree(p->spOff); cudaFree(p->spList); cudaFree(p->fmFlag); cudaFree(p->fmList); cudaFree(p->kbPart); cudaFree(p->kbCorr); cudaFree(p->kbStrip); cudaFree(p->Lw); cudaFree(p->exScratch); cudaFree(p->exRows); cudaFree(p->exBar); cudaFree(p->cholBar); cudaFree(p->mtA); cudaFree(p->mtB); cudaFree(p->Etab); cudaFree(p->Mhat);
   free(p->h_pairs);
   if (p->side) cudaStreamDestroy(p->side);
   if (p->evFork) cudaEventDestroy(p->evFork);
@@ -216,6 +216,8 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   dalloc((void**)&p->exBar, 2 * sizeof(unsigned));
   dalloc((void**)&p->Lw, sizeof(double) * (size_t)(p->N + 1) * p->ldL);
   dalloc((void**)&p->cholBar, 2 * sizeof(unsigned));
+  dalloc((void**)&p->mtA, sizeof(double) * (size_t)p->N * p->N);   // normal equations of the multi-template mode
+  dalloc((void**)&p->mtB, sizeof(double) * (size_t)p->N);
   dalloc((void**)&p->Etab, sizeof(cplx) * (size_t)p->TK * (2 * w + 1) * p->NC);
   dalloc((void**)&p->Mhat, sizeof(cplx) * HN);
   dalloc((void**)&p->d_pairs, sizeof(PairDesc) * p->nPair);
@@ -269,8 +271,10 @@ static sfft_status fail_joined(sfft_plan* p, cudaStream_t st, sfft_status s) {
   return s;
 }
 
+// reuseS: the row spectra and row moments of m S are already in the scratch (same S and mask as the
+// previous build of this plan: the multi-template mode), only the R images are transformed
 static sfft_status build_system_impl(sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
-                                     double* A, double* b, cudaStream_t st) {
+                                     double* A, double* b, cudaStream_t st, bool reuseS = false) {
   int nl = 0;
   // the row-pass scratch is about to be overwritten: an unconsumed prepare finishes first, then is dropped
   if (p->prepValid) SFFT_CUDA_TRY(cudaStreamWaitEvent(st, p->evPrep, 0));
@@ -284,7 +288,7 @@ static sfft_status build_system_impl(sfft_plan* p, const double* R, const double
   SFFT_CUDA_TRY(cudaStreamWaitEvent(p->side, p->evFork, 0));
   { ProfScope ps(p, 9, p->side); s = sfft_launch_kb(p, R, mask, p->side, &nl); }
   if (s != SFFT_OK) return fail_joined(p, st, s);
-  { ProfScope ps(p, 0, st); s = sfft_launch_row_fwd(p, R, S, mask, true, p->T, p->pitchT, !p->fused, p->fused != 0, st, &nl); }
+  { ProfScope ps(p, 0, st); s = sfft_launch_row_fwd(p, R, reuseS ? nullptr : S, mask, true, p->T, p->pitchT, !p->fused, p->fused != 0, st, &nl); }
   if (s != SFFT_OK) return fail_joined(p, st, s);
   // the final moment reduction needs only the row pass: it follows the sparse chain on the side stream
   if (cudaEventRecord(p->evRow, st) != cudaSuccess || cudaStreamWaitEvent(p->side, p->evRow, 0) != cudaSuccess)
@@ -359,10 +363,8 @@ sfft_status sfft_subtract(sfft_plan* p, const double* R, const double* S, const 
   return SFFT_OK;
 }
 
-sfft_status sfft_subtract_prepare(sfft_plan* p, const double* R, void* stream) {
-  if (!p || !R || !aligned16(R)) return SFFT_ERR_INVALID_ARG;
-  if (cuda_error_pending()) return SFFT_ERR_CUDA;
-  cudaStream_t st = (cudaStream_t)stream;
+// sfft_subtract_prepare without the argument checks (shared with the multi-template mode)
+static sfft_status subtract_prepare_impl(sfft_plan* p, const double* R, cudaStream_t st) {
   int nl = 0;
   // ordered after everything already enqueued on `stream` (the build that used the scratch before),
   // then concurrent with whatever the caller enqueues next (typically sfft_solve)
@@ -374,6 +376,51 @@ sfft_status sfft_subtract_prepare(sfft_plan* p, const double* R, void* stream) {
   p->prepR = R;
   p->prepValid = 1;
   p->launches[2] = nl;   // counted with the subtract call it belongs to
+  return SFFT_OK;
+}
+
+sfft_status sfft_subtract_prepare(sfft_plan* p, const double* R, void* stream) {
+  if (!p || !R || !aligned16(R)) return SFFT_ERR_INVALID_ARG;
+  if (cuda_error_pending()) return SFFT_ERR_CUDA;
+  return subtract_prepare_impl(p, R, (cudaStream_t)stream);
+}
+
+sfft_status sfft_multi_template_difference(sfft_plan* p, const double* const* R, const double* S,
+                                           const unsigned char* mask, const double* scale, int n,
+                                           double* Dk, double* coeffs, int* info, double* out, void* stream) {
+  if (!p || !R || !S || !scale || !Dk || !coeffs || !out || n < 1 || n > SFFT_MAX_TEMPLATES) return SFFT_ERR_INVALID_ARG;
+  if (!aligned16(S) || !aligned16(Dk) || !aligned16(out) || (mask && !aligned16(mask))) return SFFT_ERR_INVALID_ARG;
+  const size_t npix = (size_t)p->H * p->W;
+  for (int k = 0; k < n; ++k)
+    if (!R[k] || !aligned16(R[k]) || R[k] == out || R[k] == S) return SFFT_ERR_INVALID_ARG;
+  if (out == S || (out >= Dk && out < Dk + (size_t)n * npix)) return SFFT_ERR_INVALID_ARG;
+  if (cuda_error_pending()) return SFFT_ERR_CUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  const double* dptr[SFFT_MAX_TEMPLATES];
+  int nlTot = 0;
+  for (int k = 0; k < n; ++k) {
+    double* Dcur = Dk + (size_t)k * npix;
+    sfft_status s = build_system_impl(p, R[k], S, mask, p->mtA, p->mtB, st, k > 0);
+    if (s != SFFT_OK) return s;
+    nlTot += p->launches[0];
+    // the coefficient-independent row transforms of the subtraction run beside the latency-bound solve
+    s = subtract_prepare_impl(p, R[k], st);
+    if (s != SFFT_OK) return s;
+    int nl = 0;
+    { ProfScope ps(p, 5, st); s = sfft_launch_solve(p, p->mtA, p->mtB, coeffs + (size_t)k * p->N, info ? info + k : nullptr, st, &nl); }
+    if (s != SFFT_OK) return fail_joined(p, st, s);
+    nlTot += nl;
+    nl = p->launches[2];
+    s = sfft_launch_subtract(p, R[k], S, coeffs + (size_t)k * p->N, Dcur, st, &nl);
+    if (s != SFFT_OK) return s;
+    nlTot += nl;
+    dptr[k] = Dcur;
+  }
+  sfft_status s = sfft_median_combine(dptr, scale, n, npix, out, stream);
+  if (s != SFFT_OK) return s;
+  p->launches[0] = nlTot + 1;   // the whole chain is reported as one "build" count
+  p->launches[1] = 0;
+  p->launches[2] = 0;
   return SFFT_OK;
 }
 

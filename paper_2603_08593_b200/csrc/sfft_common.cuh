@@ -129,6 +129,8 @@ struct sfft_plan {
   double* exRows;    //   generated design-matrix rows of one chunk of masked pixels (allocated on first use)
   unsigned* exBar;   //   grid-barrier counters of k_exact_syrk
   int cholMaxCtas;   // cap on the CTAs of k_chol_fused (0 = one per SM); see sfft_plan_set_solve_ctas
+  double* mtA;       // sfft_multi_template_difference: normal matrix and right-hand side of the current template
+  double* mtB;
   unsigned* cholBar; // grid-barrier counters of k_chol_fused (arrivals, finished CTAs)
   cplx* Etab;       // subtract: E[TK][2w+1][NC]
   cplx* Mhat;       // subtract: mixed row spectra [H][NC]

@@ -1,4 +1,5 @@
-"""Parity of the two post-differencing kernels (sfft_median_combine, sfft_aperture_stats) against
+"""Parity of the post-differencing calls (sfft_median_combine, sfft_aperture_stats, sfft_cut_stamps,
+sfft_multi_template_difference, sfft_resample_*) against
 oracle/post_oracle.py, through the C ABI.  Median: bit-exact (it selects values, or averages two).
 Aperture fluxes: 1e-12 of sum|D| over the disc (the summation order differs); dropped positions
 must agree exactly; sigma to 1e-10 relative."""
@@ -130,3 +131,81 @@ def test_resample_identity_is_bit_exact_on_gpu():
     assert bool(inner[2:125, 2:253].all()) and torch.equal(out[inner], img[inner])
     out, outside = resample_affine(img, [5, 1, 0, -2, 0, 1], 128, 256, 3)   # integer shift
     assert torch.equal(out[10:100, 10:200], img[8:98, 15:205])
+
+
+# ------------------------------------------------------------------- stamps (NEXT-3)
+@pytest.mark.parametrize("H,W,size,n", [(40, 56, 7, 40), (64, 64, 63, 9), (33, 47, 4, 25), (16, 16, 1, 10)])
+def test_cut_stamps_bit_exact(H, W, size, n):
+    """A gather: bit-exact against the oracle, including stamps that hang over every edge, positions
+    wholly outside the frame, half-pixel positions and non-finite positions (all-NaN stamps)."""
+    from paper_2603_08593_b200 import cut_stamps
+    rng = np.random.default_rng(H * 3 + size)
+    S, R, D = (rng.standard_normal((H, W)) for _ in range(3))
+    xs = rng.uniform(-size, W + size, n)
+    ys = rng.uniform(-size, H + size, n)
+    xs[:6] = [0.0, W - 1.0, 2.5, -0.5, W + 5.0 * size, 1e300]
+    ys[:6] = [0.0, H - 1.0, 3.5, H - 0.5, 1.0, 2.0]
+    xs[6], ys[7] = np.nan, np.inf
+    ref = po.cut_stamps(S, R, D, xs, ys, size)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    out = cut_stamps(t(S), t(R), t(D), t(xs), t(ys), size).cpu().numpy()
+    assert out.shape == (n, 3, size, size)
+    assert np.array_equal(out, ref, equal_nan=True)
+    assert np.isnan(ref[6]).all() and np.isnan(ref[7]).all() and not np.isnan(ref[:6]).any()
+
+
+# ------------------------------------------------------ multi-template mode (PAPER.md:158; NEXT-2)
+def _templates(seed, H, W, n):
+    rng = np.random.default_rng(seed)
+    base = 50.0 * rng.standard_normal((H, W)) + 500.0 * (rng.random((H, W)) > 0.98)
+    Rs = [base + 4.0 * rng.standard_normal((H, W)) for _ in range(n)]
+    S = 0.7 * np.roll(base, (1, -1), (0, 1)) + 30.0 * rng.standard_normal((H, W)) + 200.0
+    mask = (rng.random((H, W)) < 0.03).astype(np.uint8)
+    return Rs, S, mask
+
+
+@pytest.mark.parametrize("H,W,w,DK,DB,n,masked", [(64, 64, 2, 1, 1, 5, True), (1024, 64, 2, 2, 2, 5, True),
+                                                   (128, 256, 3, 2, 1, 3, False), (1024, 32, 1, 0, 0, 4, True)])
+def test_multi_template_mode_parity_and_reuse(H, W, w, DK, DB, n, masked):
+    """sfft_multi_template_difference (the science image's row transform computed once, reused by the
+    other templates) against the oracle chain: every D_k and the median at 1e-6 sigma_sky, every c_k
+    at 1e-7; and bitwise equal to n separate build/solve/subtract calls plus sfft_median_combine.
+    Covers the fused (H = 1024) and the generic column paths."""
+    from paper_2603_08593_b200 import SfftPlan, median_combine
+    Rs, S, mask = _templates(H + W + n, H, W, n)
+    if not masked:
+        mask = None
+    scales = list(np.linspace(0.9, 1.1, n))
+    Dm_o, Ds_o, cs_o = po.multi_template_difference(Rs, S, mask, w, DK, DB, scales, workers=8)
+    t = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    Rd, Sd, Md = [t(R) for R in Rs], t(S), t(mask)
+    sky = 30.0
+    with SfftPlan(H, W, w, DK, DB) as plan:
+        out, Dk, coeffs, info = plan.multi_template_difference(Rd, Sd, Md, scales)
+        torch.cuda.synchronize()
+        assert info.cpu().tolist() == [0] * n
+        for k in range(n):
+            assert np.max(np.abs(coeffs[k].cpu().numpy() - cs_o[k])) <= 1e-7 * np.max(np.abs(cs_o[k]))
+            assert np.max(np.abs(Dk[k].cpu().numpy() - Ds_o[k])) <= 1e-6 * sky
+        assert np.max(np.abs(out.cpu().numpy() - Dm_o)) <= 1e-6 * sky * max(scales)
+        # the reuse changes nothing: separate calls give the same bits
+        sep = []
+        for k in range(n):
+            A, b, c, inf1, D = plan.difference(Rd[k], Sd, Md)
+            assert torch.equal(c, coeffs[k]) and torch.equal(D, Dk[k])
+            sep.append(D)
+        assert torch.equal(median_combine(sep, scales), out)
+
+
+def test_multi_template_mode_rejects_an_artefact_in_one_template():
+    from paper_2603_08593_b200 import SfftPlan
+    Rs, S, mask = _templates(77, 64, 64, 1)
+    R = Rs[0]
+    Rbad = R.copy()
+    Rbad[20:24, 30:34] += 5000.0
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    with SfftPlan(64, 64, 2, 0, 0) as plan:
+        clean, _, _, _ = plan.multi_template_difference([t(R)] * 5, t(S), t(mask), [1.0] * 5)
+        mixed, Dk, _, _ = plan.multi_template_difference([t(R), t(R), t(Rbad), t(R), t(R)], t(S), t(mask), [1.0] * 5)
+        assert torch.equal(clean, mixed)
+        assert float((Dk[2] - clean).abs().max()) > 100.0
