@@ -15,34 +15,47 @@
 //   Y[dy][kx] = H sum_y conj(f) g(y+dy) = (H/128) sum_k e^{+2 pi i k dy/128} sum_blocks conj(C_f[k]) E_g[k].
 //
 // Against the full-length formulation (one 2048-point FFT per spectrum, products, pruned inverse with
-// 2D+1 twiddled accumulations per 8 frequencies) this needs 1.6x fewer fp64 operations at the full
-// CCD, and a third of them become plain complex multiply-accumulates.  The sequences are the column kx
-// of the row spectra T (k_row_fwd), f = eta^q T_p for every kernel monomial t = (p,q) ("centre" AND
+// 2D+1 twiddled accumulations per 8 frequencies) this needs 1.5x fewer fp64 operations at the full
+// CCD, and a quarter of them are plain complex multiply-accumulates.  The sequences are the column kx
+// of the row spectra T (k_row2_fwd), f = eta^q T_p for every kernel monomial t = (p,q) ("centre" AND
 // "extended" version: 2 TK sequences) and g = the row spectrum of m S ("extended" only).
 //
-// One CTA per SM (persistent, columns round-robin), 384 threads (three warps per scheduler, so a thread
-// may hold 168 registers), a stage = up to CB_G = 7 blocks whose 2TK+1 sequences sit in shared memory
-// (182 KB at DK = 2).  With one column in flight per SM the column's 27 x 128 complex accumulators cost
-// 36 registers per thread (a third of the pairs each), which leaves room for the radix-16 butterflies:
-//   phase 1  warp = (group g < 3, pair of blocks), half warp = one block, lane j < 16.  A group owns a
-//            compile-time list of the block's sequences (5, 5 and 3 of the 13 at DK = 2) that reads at most
-//            two row images; their 8 x 16 block elements (n = j + 16 r) were requested during phase 3 of
-//            the stage before (the first image into registers, the second by cp.async into a staging slot).  Per sequence: eta^q weighting, zero padding, radix-8 butterfly over r,
-//            twiddle w128^(j k1), store.  Both halves of a warp run the same list: no divergence;
-//   phase 2  radix-16 butterflies over j for every (block, sequence, k1): X[k1 + 8 k2];
-//   phase 3  thread = (frequency k, third of the pairs): the stage's products accumulate in registers
-//            (6-7 operand loads per 9 pairs);
-//   phase 4  (once per column) accumulators -> shared memory, 16-point inverse over b (k = a + 8 b),
-//            then the 2D+1 lags of every pair (8 twiddled terms each), Y[pair][dy][kx].
+// One persistent CTA per SM (columns round-robin), 12 warps; after the prologue the warps meet only at
+// mbarriers while a column is in flight, and at three block barriers per column for its final inverse.
+// Every warp does both kinds of work:
+//   transform "tasks" of four sequences, warp-synchronously: each half warp (lane j < 16) takes the 8 x 16
+//            block elements n = j + 16 r of its row image from global memory (requested one task ahead,
+//            registers only), and per sequence weights them by eta^q, zero-pads (centre version), runs the
+//            radix-8 butterfly over r, multiplies by w128^(j k1) and stores to the block's slot of the
+//            shared-memory ring; after a __syncwarp the 32 lanes run the radix-16 butterflies over j of
+//            the four sequences (X[k1 + 8 k2]) in place, and lane 0 arrives on the slot's "full" barrier.
+//            The science sequence (one per block) is batched over four consecutive blocks into a task of
+//            its own.  Task g of the CTA's task list (all its columns, block by block) runs on warp g mod 12;
+//   products thread = (frequency k, third of the pairs): once a slot is full the thread accumulates its
+//            pairs' products conj(C_t) E_t2 of that block in registers (6-7 operand loads per 9 pairs) and
+//            the warp arrives on the slot's "empty" barrier (12 arrivals free it).
+// A warp runs transform tasks while the block its products wait for is not full yet, so the two kinds of
+// work interleave on every scheduler and the ring (CB_NSLOT blocks) lets the transforms run ahead, also
+// across the column boundary.  End of a column: accumulators -> shared memory, 16-point inverse over b
+// (k = a + 8 b), then the 2D+1 lags of every pair (8 twiddled terms each) -> Y[pair][dy][kx].
 // Shared-memory positions are XOR-swizzled (slot k1*16 + (j ^ k1)): every pass is conflict free with no
-// padding.  T has the row-group layout T[img][y/G][kx][y%G], G = SFFT_T_G = 8 (k_row2_fwd): a half warp's 16
-// rows of a column are two whole 128-byte lines.
+// padding.  T has the row-group layout T[img][y/G][kx][y%G], G = SFFT_T_G = 8 (k_row2_fwd): a half warp's
+// 16 rows of a column are two whole 128-byte lines.
 #include <math.h>
 #include "fft_smem.cuh"
 
 #define CB_N 128          // block transform length
-#define CB_TH 384         // 12 warps = 3 per scheduler: 168 registers per thread
-#define CB_G 7            // most blocks per stage (shared memory)
+#define CB_TH 512         // 16 warps = 4 warpgroups: 3 transform + 1 product (registers rebalanced by setmaxnreg)
+#define CB_NW (CB_TH / 32)
+#define CB_FW 12          // transform warps
+#ifndef CB_PREG
+#define CB_PREG 5           // block elements (of 8) a transform lane prefetches into registers (the rest: cp.async)
+#endif
+#define CB_REG_F 120       // registers per thread of the transform warpgroups
+#define CB_REG_P 152       // ... of the product warpgroup (3 x 120 + 152 = 4 x 128)
+#define CB_PT 128         // product threads (one per frequency)
+#define CB_NSLOT 6        // blocks in the shared-memory ring
+#define CB_NS2 16         // blocks in the ring of the S~ spectra (DK = 2: they are produced four blocks at a time, ahead of the rest)
 #define CB_LAGS 21        // 2 * 10 + 1
 
 struct ColbParams {
@@ -54,42 +67,60 @@ struct ColbParams {
   int D;                  // lag half-range (halo)
   int B;                  // centre rows per block = CB_N - 2 D
   int nblk;               // blocks per column = ceil(H / B)
-  int nst;                // stages per column = ceil(nblk / CB_G); stage i holds blocks [i nblk/nst, (i+1) nblk/nst)
 };
 
-// Phase-1 job lists.  Sequence index: centre version of monomial t at t, extended version at TK + t,
-// S~ (extended only) at 2 TK.  Monomial order (p,q): DK = 2: (0,0),(1,0),(0,1),(2,0),(1,1),(0,2); DK = 1:
-// (0,0),(1,0),(0,1); row image = p, q = power of eta.  A job = (buffer 0/1, q, centre?, sequence); group
-// g reads row image IMG[g][0] into buffer 0 and IMG[g][1] into buffer 1 (-1: none); the extended
-// sequences of an image come before its centre ones.
-template <int TK> struct CbP1;
-template <> struct CbP1<6> {
-  static constexpr int N[3] = {5, 5, 3};
-  static constexpr int IMG[3][2] = {{0, -1}, {1, 3}, {0, 2}};
-  //                                   E(0,0)      E(0,1)      E(0,2)       C(0,0)     C(0,1)
-  static constexpr int BUF[3][5] = {{0, 0, 0, 0, 0}, {0, 0, 0, 0, 1}, {0, 1, 1, 0, 0}};
-  static constexpr int Q[3][5] = {{0, 1, 2, 0, 1}, {0, 1, 0, 1, 0}, {2, 0, 0, 0, 0}};
-  static constexpr int CEN[3][5] = {{0, 0, 0, 1, 1}, {0, 0, 1, 1, 0}, {1, 0, 1, 0, 0}};
-  static constexpr int SEQ[3][5] = {{6, 8, 11, 0, 2}, {7, 10, 1, 4, 12}, {5, 9, 3, 0, 0}};
+// ---- task tables ---------------------------------------------------------------------------------------
+// Sequence index inside a slot: centre version of monomial t at t, extended version at TK + t, S~
+// (extended only) at 2 TK.  Monomial order (p,q): DK = 2: (0,0),(1,0),(0,1),(2,0),(1,1),(0,2); DK = 1:
+// (0,0),(1,0),(0,1); row image = p (S~ is image DK + 1), q = power of eta.
+// A per-block task = 2 half warps x 2 jobs; a half warp reads ONE row image.  Descriptor of a half warp:
+//   bits 0-1 image | job 0: bits 2-3 q, bit 4 centre, bits 5-8 sequence, bit 9 valid | job 1: the same at 10-17.
+// Where the images allow it the two half warps of a job share q (no divergence on the weighting branch).
+__host__ __device__ constexpr unsigned cb_job(int q, int cen, int seq) { return (unsigned)(q | (cen << 2) | (seq << 3) | (1 << 7)); }
+__host__ __device__ constexpr unsigned cb_half(int img, unsigned j0, unsigned j1) { return (unsigned)img | (j0 << 2) | (j1 << 10); }
+template <int TK> struct CbTasks;
+template <> struct CbTasks<6> {
+  static constexpr int NT = 3;            // tasks per block
+  static constexpr bool STASK = true;     // S~ sequences: a task of their own over 4 consecutive blocks
+  static constexpr int SIMG = 3, SSEQ = 12;
+  __device__ static constexpr unsigned desc(int task, int half) {
+    return task == 0 ? (half == 0 ? cb_half(0, cb_job(0, 0, 6), cb_job(1, 0, 8))      // E(0,0) E(0,1)
+                                  : cb_half(0, cb_job(0, 1, 0), cb_job(1, 1, 2)))     // C(0,0) C(0,1)
+         : task == 1 ? (half == 0 ? cb_half(1, cb_job(0, 0, 7), cb_job(1, 0, 10))     // E(1,0) E(1,1)
+                                  : cb_half(1, cb_job(0, 1, 1), cb_job(1, 1, 4)))     // C(1,0) C(1,1)
+                     : (half == 0 ? cb_half(2, cb_job(0, 0, 9), cb_job(0, 1, 3))      // E(2,0) C(2,0)
+                                  : cb_half(0, cb_job(2, 0, 11), cb_job(2, 1, 5)));   // E(0,2) C(0,2)
+  }
 };
-template <> struct CbP1<3> {
-  static constexpr int N[3] = {4, 3, 0};
-  static constexpr int IMG[3][2] = {{0, -1}, {1, 2}, {-1, -1}};
-  static constexpr int BUF[3][5] = {{0, 0, 0, 0, 0}, {0, 0, 1, 0, 0}, {0, 0, 0, 0, 0}};
-  static constexpr int Q[3][5] = {{0, 1, 0, 1, 0}, {0, 0, 0, 0, 0}, {0, 0, 0, 0, 0}};
-  static constexpr int CEN[3][5] = {{0, 0, 1, 1, 0}, {0, 1, 0, 0, 0}, {0, 0, 0, 0, 0}};
-  static constexpr int SEQ[3][5] = {{3, 5, 0, 2, 0}, {4, 1, 6, 0, 0}, {0, 0, 0, 0, 0}};
+template <> struct CbTasks<3> {
+  static constexpr int NT = 2;
+  static constexpr bool STASK = false;
+  static constexpr int SIMG = 2, SSEQ = 6;
+  __device__ static constexpr unsigned desc(int task, int half) {
+    return task == 0 ? (half == 0 ? cb_half(0, cb_job(0, 0, 3), cb_job(1, 0, 5))      // E(0,0) E(0,1)
+                                  : cb_half(0, cb_job(0, 1, 0), cb_job(1, 1, 2)))     // C(0,0) C(0,1)
+                     : (half == 0 ? cb_half(1, cb_job(0, 0, 4), cb_job(0, 1, 1))      // E(1,0) C(1,0)
+                                  : cb_half(2, cb_job(0, 0, 6), 0u));                 // S~
+  }
 };
-template <> struct CbP1<1> {
-  static constexpr int N[3] = {2, 1, 0};
-  static constexpr int IMG[3][2] = {{0, -1}, {1, -1}, {-1, -1}};
-  static constexpr int BUF[3][5] = {{0, 0, 0, 0, 0}, {0, 0, 0, 0, 0}, {0, 0, 0, 0, 0}};
-  static constexpr int Q[3][5] = {{0, 0, 0, 0, 0}, {0, 0, 0, 0, 0}, {0, 0, 0, 0, 0}};
-  static constexpr int CEN[3][5] = {{0, 1, 0, 0, 0}, {0, 0, 0, 0, 0}, {0, 0, 0, 0, 0}};
-  static constexpr int SEQ[3][5] = {{1, 0, 0, 0, 0}, {2, 0, 0, 0, 0}, {0, 0, 0, 0, 0}};
+template <> struct CbTasks<1> {
+  static constexpr int NT = 1;
+  static constexpr bool STASK = false;
+  static constexpr int SIMG = 1, SSEQ = 2;
+  __device__ static constexpr unsigned desc(int task, int half) {
+    return half == 0 ? cb_half(0, cb_job(0, 0, 1), cb_job(0, 1, 0))                   // E(0,0) C(0,0)
+                     : cb_half(1, cb_job(0, 0, 2), 0u);                               // S~
+  }
 };
 
-// Pair partition for phase 3.  Part (T0, T1, U0, U1) owns the pairs (t, t2), T0 <= t < T1,
+__device__ __forceinline__ int cb_slot(int k1, int j) { return k1 * 16 + (j ^ k1); }   // k1 < 8, j < 16
+
+// offset of row y inside one image of T (column 0): T[img][y/G][kx][y%G], G = SFFT_T_G
+__device__ __forceinline__ size_t cb_toff(int y, size_t grpStride) {
+  return (size_t)(y / SFFT_T_G) * grpStride + (size_t)(y % SFFT_T_G);
+}
+
+// Pair partition of the products.  Part (T0, T1, U0, U1) owns the pairs (t, t2), T0 <= t < T1,
 // max(t, U0) <= t2 <= U1 (t2 = TK stands for S~).  For TK = 6 the three parts hold 9 pairs each and
 // read 7, 6 and 7 operands: (C0-2 x E0-3), (C0-2 x E4,5,S), (C3-5 x E3,4,5,S).
 template <int TK> struct CbParts;
@@ -104,13 +135,7 @@ __host__ __device__ constexpr int cb_part_pairs(int T0, int T1, int U0, int U1) 
   return n;
 }
 
-// offset of row y inside one image of T (column 0): T[img][y/G][kx][y%G], G = SFFT_T_G
-__device__ __forceinline__ size_t cb_toff(int y, size_t grpStride) {
-  return (size_t)(y / SFFT_T_G) * grpStride + (size_t)(y % SFFT_T_G);
-}
-__device__ __forceinline__ int cb_slot(int k1, int j) { return k1 * 16 + (j ^ k1); }   // k1 < 8, j < 16
-
-// Phase 3 for one block: acc[] += conj(C_t) E_t2 over the part's pairs, every operand read once.
+// products of one block: acc[] += conj(C_t) E_t2 over the part's pairs, every operand read once
 template <int TK, int T0, int T1, int U0, int U1>
 __device__ __forceinline__ void cb_accumulate(cplx* acc, const cplx* __restrict__ ub, int pk) {
   cplx C[TK], E[TK + 1];
@@ -129,8 +154,8 @@ __device__ __forceinline__ void cb_accumulate(cplx* acc, const cplx* __restrict_
   }
 }
 
-// Phase 4a: the part's accumulators -> shared memory acs[pair][k] (pair index of the plan's list:
-// kernel-kernel pairs (t <= t2) row-major upper-triangular, then (t, S) at nKK + t)
+// the part's accumulators -> shared memory acs[pair][k] (pair index of the plan's list: kernel-kernel
+// pairs (t <= t2) row-major upper-triangular, then (t, S) at nKK + t)
 template <int TK, int T0, int T1, int U0, int U1>
 __device__ __forceinline__ void cb_flush(const cplx* acc, cplx* acs, int k) {
   constexpr int NKK = TK * (TK + 1) / 2;
@@ -146,36 +171,66 @@ __device__ __forceinline__ void cb_flush(const cplx* acc, cplx* acs, int k) {
   }
 }
 
-// eta of the rows n = j + 16 r of a block: eta_r = e0 + r (32/H) for the unwrapped row, and -/+ 2 where the
-// row index wrapped around the frame (only the halo of a column's first and last block does); every
-// value is a multiple of 1/H, so the arithmetic is exact.
-struct CbRows {
-  double e0, step;
-  unsigned cenbits;   // bit r: element r lies in the block's centre rows
-  unsigned lobits;    // bit r: row index below 0 before wrapping (eta + 2)
-  unsigned hibits;    // bit r: row index >= H before wrapping (eta - 2)
-};
-__device__ __forceinline__ double cb_eta(const CbRows& R, int r) {
-  double e = fma((double)r, R.step, R.e0);
-  if ((R.lobits >> r) & 1u) e += 2.0;
-  if ((R.hibits >> r) & 1u) e -= 2.0;
-  return e;
+// ---- mbarrier helpers (CTA scope) ---------------------------------------------------------------------
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  unsigned done;
+  do {
+    asm volatile(
+        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+        : "=r"(done) : "r"(a), "r"(parity) : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void cb_bar_products() {   // the 128 product threads only
+  asm volatile("bar.sync 1, %0;\n" ::"n"(CB_PT) : "memory");
+}
+// non-blocking: has the phase with this parity completed?  (acquire, CTA scope)
+__device__ __forceinline__ bool mbar_test(unsigned long long* bar, unsigned parity) {
+  unsigned done;
+  asm volatile(
+      "{\n .reg .pred p;\n mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+      : "=r"(done) : "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+  return done != 0u;
 }
 
-// One phase-1 job: sequence = DFT8 over r of (x[r] * eta_r^Q, zero outside the centre rows when CEN),
-// twiddled by w128^(j k1) (table row k1 - 1 of s_w, lane j) and stored at the lane's slots of `dst`.
-template <int Q, bool CEN>
-__device__ __forceinline__ void cb_job(const cplx* x, const CbRows& R, cplx* dst, int j, const cplx* __restrict__ swj) {
+// One phase-1 job of a half warp: sequence = DFT8 over r of (x[r] * eta_r^q, zero outside the centre rows
+// when cen), twiddled by w128^(j k1) (table row k1 - 1 of s_w, lane j) and stored at the lane's positions
+// of `dst`.  q and cen are uniform over a half warp.  e0 = eta of the lane's element r = 0 (unwrapped row),
+// estep = 32/H; edge: the block is the first or one of the last two of its column (rows may wrap, the centre may be
+// short), Yrow = unwrapped row of element 0, Bi = the block's centre rows.
+__device__ __forceinline__ void cb_job_run(const cplx* x, int q, bool cen, cplx* dst, int j, const cplx* __restrict__ swj,
+                                           double e0, double estep, bool edge, int Yrow, int Bi, int D, int H) {
   cplx v[8];
 #pragma unroll
-  for (int r = 0; r < 8; ++r) {
-    if (Q == 0) {
-      v[r] = x[r];
-    } else {
-      const double e = cb_eta(R, r);
-      v[r] = cscale(x[r], Q == 1 ? e : e * e);
+  for (int r = 0; r < 8; ++r) v[r] = x[r];
+  if (q > 0) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+      double e = fma((double)r, estep, e0);
+      if (edge) {                         // every value is a multiple of 1/H: exact
+        if (Yrow + 16 * r < 0) e += 2.0;
+        if (Yrow + 16 * r >= H) e -= 2.0;
+      }
+      if (q == 2) e *= e;
+      v[r] = cscale(v[r], e);
     }
-    if (CEN && !((R.cenbits >> r) & 1u)) v[r] = cmake(0.0, 0.0);
+  }
+  if (cen) {
+    // centre rows: n = j + 16 r in [D, D + Bi); with D <= 16 only r = 0 (and r = 7 for a whole block) can fall outside
+    if (j < D) v[0] = cmake(0.0, 0.0);
+    if (!edge) {
+      if (j + 112 >= D + Bi) v[7] = cmake(0.0, 0.0);
+    } else {
+#pragma unroll
+      for (int r = 1; r < 8; ++r)
+        if (j + 16 * r >= D + Bi) v[r] = cmake(0.0, 0.0);
+    }
   }
   Dft<8, -1>::run(v);
   dst[cb_slot(0, j)] = v[0];
@@ -183,188 +238,274 @@ __device__ __forceinline__ void cb_job(const cplx* x, const CbRows& R, cplx* dst
   for (int k1 = 1; k1 < 8; ++k1) dst[cb_slot(k1, j)] = cmul(v[k1], swj[(k1 - 1) * 16]);
 }
 
-// the whole job list of group G on one block (ub = the block's sequences in shared memory).  x holds the
-// group's first row image; its second one was staged in shared memory (xs, the lane's own 8 elements
-// 16 apart) and replaces x when the list reaches its first buffer-1 job.
-template <int TK, int G, int E>
-__device__ __forceinline__ void cb_group_jobs(cplx* x, const cplx* xs, const CbRows& R, cplx* ub, int j,
-                                              const cplx* __restrict__ swj) {
-  using T = CbP1<TK>;
-  if constexpr (E < T::N[G]) {
-    if constexpr (T::BUF[G][E] == 1 && (E == 0 || T::BUF[G][E > 0 ? E - 1 : 0] == 0)) {
-#pragma unroll
-      for (int r = 0; r < 8; ++r) x[r] = xs[16 * r];
-    }
-    cb_job<T::Q[G][E], T::CEN[G][E] != 0>(x, R, ub + T::SEQ[G][E] * CB_N, j, swj);
-    cb_group_jobs<TK, G, E + 1>(x, xs, R, ub, j, swj);
-  }
-}
-
-__device__ __forceinline__ void cb_cp_async16(cplx* smem_dst, const cplx* gsrc, bool valid) {   // zero fill when !valid
-  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
-  const int sz = valid ? 16 : 0;
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(sa), "l"(gsrc), "r"(sz) : "memory");
-}
-
 template <int TK>
 __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
   constexpr int NSEQ = 2 * TK + 1;
+  constexpr int NPAIR = TK * (TK + 1) / 2 + TK;
+  using TT = CbTasks<TK>;
   using PT = CbParts<TK>;
-  using P1 = CbP1<TK>;
   constexpr int NACC = cb_max(cb_max(cb_part_pairs(PT::T0[0], PT::T1[0], PT::U0[0], PT::U1[0]),
                                      cb_part_pairs(PT::T0[1], PT::T1[1], PT::U0[1], PT::U1[1])),
                               cb_max(cb_part_pairs(PT::T0[2], PT::T1[2], PT::U0[2], PT::U1[2]), 1));
-  constexpr int NPAIR = TK * (TK + 1) / 2 + TK;
+  constexpr unsigned FULL_COUNT = TT::NT;                         // lane-0 arrivals that complete a block
+  constexpr int NGRP_T = TT::STASK ? (1 + 4 * TT::NT) : TT::NT;   // tasks of a group of 4 blocks (or of one block)
+  constexpr int NSEQ_R = TT::STASK ? NSEQ - 1 : NSEQ;             // sequences per slot of the main ring
+  constexpr int SRING = CB_NSLOT * NSEQ_R * CB_N;                 // element offset of the S~ ring
+  constexpr int NPASS4 = NPAIR > 16 ? 2 : 1;                      // the end-of-column inverse runs in NPASS4 passes
+  constexpr int PP4 = (NPAIR + NPASS4 - 1) / NPASS4;              // over PP4 pairs each (scratch size)
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  cplx* sq = reinterpret_cast<cplx*>(smem_raw);   // [CB_G][NSEQ][CB_N]; phase 4: acs[NPAIR][CB_N]
-  cplx* xstage = sq + CB_G * NSEQ * CB_N;         // [2 groups][8 blocks][CB_N]: staged second row images
-  __shared__ cplx s_tw[CB_N];                     // e^{-2 pi i m/128}
-  __shared__ int s_Dp[NPAIR];                     // lag half-range of every pair
-  __shared__ cplx s_w[7 * 16];                    // w128^(j k1): row k1 - 1, lane j
-  const int tid = threadIdx.x;
-  const int H = P.H, D = P.D, B = P.B, nblk = P.nblk, nst = P.nst;
-  const double invH = 1.0 / (double)H;
-  const size_t imgStride = (size_t)(P.NC + 1) * H;      // T[img][y/G][kx][y%G] (k_row2_fwd)
-  const size_t grpStride = (size_t)(P.NC + 1) * SFFT_T_G;
+  cplx* ring = reinterpret_cast<cplx*>(smem_raw);        // [CB_NSLOT][NSEQ_R][CB_N], then [CB_NS2][CB_N] (S~ ring)
+  cplx* acs = ring + SRING + (TT::STASK ? CB_NS2 * CB_N : 0);   // [PP4][CB_N]: end-of-column scratch
+  __shared__ cplx s_tw[CB_N];                            // e^{-2 pi i m/128}
+  __shared__ cplx s_w[7 * 16];                           // w128^(j k1): row k1 - 1, lane j
+  __shared__ int s_Dp[NPAIR];                            // lag half-range of every pair
+  __shared__ cplx s_xs[(8 - CB_PREG) * CB_FW * 32];      // a transform lane's prefetched elements r >= CB_PREG (cp.async)
+  __shared__ __align__(8) unsigned long long s_full[CB_NSLOT], s_empty[CB_NSLOT], s_sfull[CB_NS2], s_sempty[CB_NS2];
+  const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
+  const int H = P.H, D = P.D, B = P.B, nblk = P.nblk;
+  const double invH = 1.0 / (double)H, estep = 32.0 * invH;
+  const size_t imgStride = (size_t)(P.NC + 1) * H;       // T[img][y/G][kx][y%G] (k_row2_fwd)
+  const unsigned grpStride = (unsigned)(P.NC + 1) * SFFT_T_G;
   for (int i = tid; i < CB_N; i += CB_TH) s_tw[i] = ldg2(P.tw128 + i);
-  for (int i = tid; i < NPAIR; i += CB_TH) s_Dp[i] = P.pairs[i].D;
   for (int i = tid; i < 7 * 16; i += CB_TH) s_w[i] = ldg2(P.tw128 + ((i >> 4) + 1) * (i & 15));
+  for (int i = tid; i < NPAIR; i += CB_TH) s_Dp[i] = P.pairs[i].D;
+  if (tid < CB_NSLOT) {
+    mbar_init(&s_full[tid], FULL_COUNT);
+    mbar_init(&s_empty[tid], CB_PT / 32);
+  }
+  if (tid < CB_NS2) {
+    mbar_init(&s_sfull[tid], 1);
+    mbar_init(&s_sempty[tid], CB_PT / 32);
+  }
+  __syncthreads();
+  const int ncolMine = (P.NC + 1 - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // columns of this CTA
 
-  // phase-1 identity: warp = (group, block pair), half warp = block u of the stage, lane j
-  const int p1_g = (tid >> 5) % 3, p1_u = ((tid >> 5) / 3) * 2 + ((tid >> 4) & 1), p1_j = tid & 15;
-  constexpr int i00 = P1::IMG[0][0], i10 = P1::IMG[1][0], i20 = P1::IMG[2][0];
-  constexpr int i01 = P1::IMG[0][1], i11 = P1::IMG[1][1], i21 = P1::IMG[2][1];
-  const int p1_img0 = p1_g == 0 ? i00 : (p1_g == 1 ? i10 : i20);
-  const int p1_img1 = p1_g == 0 ? i01 : (p1_g == 1 ? i11 : i21);
-  const cplx* swj = s_w + p1_j;
-  const int p2_k1 = tid & 7, p2_sub = tid >> 3;                        // phase 2
-  const int p3_k = tid & (CB_N - 1), p3_part = tid >> 7;               // phase 3
-  const int p3_pk = cb_slot(p3_k & 7, p3_k >> 3);
-
-  // requests the 8 x 16 elements (n = j + 16 r) of block blk of row image img (zero past the block's end)
-  auto fetch = [&](cplx* x, const cplx* Tcol, int blk, int img) {
-    const int c0 = blk * B;
-    const int lim = min(B, H - c0) + 2 * D;          // the last block may be short
-    const cplx* src = Tcol + (size_t)img * imgStride;
-    const int y0 = c0 - D + p1_j + H;
-#pragma unroll
-    for (int r = 0; r < 8; ++r) x[r] = (p1_j + 16 * r < lim) ? src[cb_toff((y0 + 16 * r) & (H - 1), grpStride)] : cmake(0.0, 0.0);
+  // ---- transform side: the warp's task cursor (ti = task index inside column iteration tci)
+  const int half = lane >> 4, j = lane & 15;
+  const cplx* swj = s_w + j;
+  const int tasksPerCol = TT::STASK ? (TT::NT * nblk + (nblk + 3) / 4) : TT::NT * nblk;
+  int tci = 0, ti = wrp;   // (transform warps only)
+  while (ti >= tasksPerCol && tci < ncolMine) { ti -= tasksPerCol; ++tci; }
+  // decode ti -> (type, first block); type < NT: per-block task, type == NT: S~ task over blocks blk .. blk + 3
+  auto decode = [&](int lid, int& type, int& blk) {
+    if (TT::STASK) {
+      const int m = lid / NGRP_T, rem = lid - m * NGRP_T;
+      if (rem == 0) { type = TT::NT; blk = 4 * m; }
+      else { type = (rem - 1) % TT::NT; blk = 4 * m + (rem - 1) / TT::NT; }
+    } else {
+      type = lid % TT::NT; blk = lid / TT::NT;
+    }
   };
-  // the thread's inputs of stage st of column nkx: the group's first row image into registers (xa), its
-  // second one (if any) by cp.async into the half warp's staging slot
-  cplx xa[8];
-  cplx* xs = xstage + ((p1_g > 0 ? p1_g - 1 : 0) * 8 + p1_u) * CB_N + p1_j;
-  auto prefetch = [&](int nkx, int st) {
-    if (nkx > P.NC) return;
-    const int bs = (st * nblk) / nst, be = ((st + 1) * nblk) / nst;
-    if (bs + p1_u >= be) return;
-    const cplx* Tn = P.T + SFFT_T_G * (size_t)nkx;
-    if (p1_img0 >= 0) fetch(xa, Tn, bs + p1_u, p1_img0);
-    if (p1_img1 >= 0) {
-      const int c0 = (bs + p1_u) * B;
-      const int lim = min(B, H - c0) + 2 * D;
-      const cplx* src = Tn + (size_t)p1_img1 * imgStride;
-      const int y0 = c0 - D + p1_j + H;
+  auto lane_img = [&](int type) -> int { return type == TT::NT ? TT::SIMG : (int)(TT::desc(type, half) & 3u); };
+  auto job_blk = [&](int type, int blk, int jb) -> int { return type == TT::NT ? blk + 2 * half + jb : blk; };
+  // requests the 8 x 16 elements (n = j + 16 r) of block b of row image img, column kx (zero past the block's end)
+  // (elements r in [R0, R1): the prefetch of a task is issued in two parts, see run_task)
+  auto fetch = [&](cplx* x, int kx, int b, int img, int R0 = 0, int R1 = 8) {
+    const int c0 = b * B;
+    const int lim = b < nblk ? min(B, H - c0) + 2 * D : 0;   // the last block may be short
+    const cplx* src = P.T + SFFT_T_G * (size_t)kx + (size_t)img * imgStride;
+    const int y0 = (c0 - D + j + H) & (H - 1);               // row of element r = 0; rows r differ by 16 = 2 groups
+    const unsigned gi0 = (unsigned)y0 / SFFT_T_G, sub = (unsigned)y0 % SFFT_T_G, gmask = (unsigned)(H / SFFT_T_G) - 1u;
 #pragma unroll
-      for (int r = 0; r < 8; ++r)
-        cb_cp_async16(xs + 16 * r, src + cb_toff((y0 + 16 * r) & (H - 1), grpStride), p1_j + 16 * r < lim);
+    for (int r = R0; r < R1; ++r) {
+      const unsigned gi = (gi0 + (unsigned)(16 / SFFT_T_G) * r) & gmask;
+      x[r] = (j + 16 * r < lim) ? src[gi * grpStride + sub] : cmake(0.0, 0.0);
+    }
+  };
+  // prefetch of a task's first job: elements r < CB_PREG into registers, the others by cp.async into the
+  // lane's staging words (the radix-16 pass that runs meanwhile needs the registers); prefetch_land()
+  // completes it
+  auto prefetch = [&](cplx* x, int kx, int b, int img) {
+    fetch(x, kx, b, img, 0, CB_PREG);
+    const int c0 = b * B;
+    const int lim = b < nblk ? min(B, H - c0) + 2 * D : 0;
+#pragma unroll
+    for (int r = CB_PREG; r < 8; ++r) {
+      const int yr = (c0 - D + j + 16 * r + H) & (H - 1);
+      const cplx* src = P.T + SFFT_T_G * (size_t)kx + (size_t)img * imgStride + (size_t)(yr / SFFT_T_G) * grpStride + (yr % SFFT_T_G);
+      const unsigned sa = (unsigned)__cvta_generic_to_shared(&s_xs[(r - CB_PREG) * CB_FW * 32 + tid]);
+      const int sz = (j + 16 * r < lim) ? 16 : 0;           // zero fill past the block's end
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(sa), "l"(sz ? src : P.T), "r"(sz) : "memory");
     }
     asm volatile("cp.async.commit_group;\n" ::: "memory");
   };
-  prefetch(blockIdx.x, 0);
-  __syncthreads();
-
-  for (int kx = blockIdx.x; kx <= P.NC; kx += gridDim.x) {
-    cplx acc[NACC];
+  auto prefetch_land = [&](cplx* x) {
+    asm volatile("cp.async.wait_all;\n" ::: "memory");
 #pragma unroll
-    for (int i = 0; i < NACC; ++i) acc[i] = cmake(0.0, 0.0);
-
-    for (int st = 0; st < nst; ++st) {
-      const int b0 = (st * nblk) / nst, na = ((st + 1) * nblk) / nst - b0;     // blocks of this stage
-      // ---- phase 1: weight, radix-8 over r (n = j + 16 r), twiddle, store ---------------------------
-      if (p1_u < na) {
-        const int c0 = (b0 + p1_u) * B;
-        const int Bi = min(B, H - c0);
-        const int Y = c0 - D + p1_j;             // unwrapped row of element r = 0
-        CbRows R;
-        R.e0 = (double)(2 * Y + 1 - H) * invH;
-        R.step = 32.0 * invH;
-        R.cenbits = R.lobits = R.hibits = 0u;
+    for (int r = CB_PREG; r < 8; ++r) x[r] = s_xs[(r - CB_PREG) * CB_FW * 32 + tid];
+  };
+  cplx xa[8];
+  int ttype = 0, tblk = 0;
+  if (tci < ncolMine && wrp < CB_FW) {
+    decode(ti, ttype, tblk);
+    prefetch(xa, (int)blockIdx.x + tci * (int)gridDim.x, job_blk(ttype, tblk, 0), lane_img(ttype));
+  }
+  // are the slots the pending task writes free?  (block sequence number n = column iteration * nblk + block)
+  auto task_ready = [&]() -> bool {
+    const int nb = tci * nblk + tblk;
+    bool ok = true;
+    if (TT::STASK && ttype == TT::NT) {
 #pragma unroll
-        for (int r = 0; r < 8; ++r) {
-          const int n = p1_j + 16 * r;
-          R.cenbits |= (n >= D && n < D + Bi) ? (1u << r) : 0u;
-          R.lobits |= (Y + 16 * r < 0) ? (1u << r) : 0u;
-          R.hibits |= (Y + 16 * r >= H) ? (1u << r) : 0u;
-        }
-        cplx* ub = sq + p1_u * NSEQ * CB_N;
-        asm volatile("cp.async.wait_all;\n" ::: "memory");      // the lane's own staged elements have landed
-        if (p1_g == 0) cb_group_jobs<TK, 0, 0>(xa, xs, R, ub, p1_j, swj);
-        else if (p1_g == 1) cb_group_jobs<TK, 1, 0>(xa, xs, R, ub, p1_j, swj);
-        else cb_group_jobs<TK, 2, 0>(xa, xs, R, ub, p1_j, swj);
+      for (int i = 0; i < 4; ++i) {
+        const int n = nb + i;
+        if (tblk + i < nblk) ok = ok && mbar_test(&s_empty[n % CB_NSLOT], (unsigned)(((n / CB_NSLOT) & 1) ^ 1));
       }
-      __syncthreads();
-      // ---- phase 2: radix-16 over j for every (block, sequence, k1) --------------------------------
-      for (int it = p2_sub; it < na * NSEQ; it += CB_TH / 8) {
-        cplx* sb = sq + it * CB_N + p2_k1 * 16;
+    } else {
+      ok = mbar_test(&s_empty[nb % CB_NSLOT], (unsigned)(((nb / CB_NSLOT) & 1) ^ 1));
+    }
+    return __all_sync(0xffffffffu, ok);
+  };
+  auto run_task = [&]() {
+    const int kx = (int)blockIdx.x + tci * (int)gridDim.x;
+    const int nbase = tci * nblk;
+    const bool stask = TT::STASK && ttype == TT::NT;
+    const unsigned desc = stask ? cb_half(TT::SIMG, cb_job(0, 0, TT::SSEQ), cb_job(0, 0, TT::SSEQ)) : TT::desc(ttype, half);
+    prefetch_land(xa);
+    // ---- phase 1: two jobs per half warp
+    int soff[2];        // element offset of the job's sequence in the ring, -1 = no job
+#pragma unroll
+    for (int jb = 0; jb < 2; ++jb) {
+      const unsigned jd = (desc >> (2 + 8 * jb)) & 0xffu;
+      const int b = job_blk(ttype, tblk, jb);
+      const bool valid = ((jd >> 7) & 1u) && b < nblk;
+      soff[jb] = !valid ? -1 : stask ? SRING + ((nbase + b) % CB_NS2) * CB_N
+                                     : (((nbase + b) % CB_NSLOT) * NSEQ_R + (int)((jd >> 3) & 15u)) * CB_N;
+      if (stask && jb == 1) fetch(xa, kx, b, TT::SIMG);   // the S~ task reads a new block per job
+      if (valid) {
+        const int c0 = b * B, Yrow = c0 - D + j;
+        cb_job_run(xa, (int)(jd & 3u), ((jd >> 2) & 1u) != 0u, ring + soff[jb], j, swj,
+                   (double)(2 * Yrow + 1 - H) * invH, estep, b == 0 || b >= nblk - 2, Yrow, min(B, H - c0), D, H);
+      }
+    }
+    // ---- advance the cursor; the next task's inputs are requested now (their latency hides under phase 2,
+    //      the products and the waits)
+    const int pblk = tblk;
+    ti += CB_FW;
+    while (ti >= tasksPerCol && tci < ncolMine) { ti -= tasksPerCol; ++tci; }
+    if (tci < ncolMine) {
+      decode(ti, ttype, tblk);
+      prefetch(xa, (int)blockIdx.x + tci * (int)gridDim.x, job_blk(ttype, tblk, 0), lane_img(ttype));
+    }
+    __syncwarp();
+    // ---- phase 2: radix-16 over j; lane = (sequence sq = (half, job), k1)
+    {
+      const int sq = lane >> 3, k1 = lane & 7;
+      const int o0 = __shfl_sync(0xffffffffu, soff[0], (sq >> 1) * 16), o1 = __shfl_sync(0xffffffffu, soff[1], (sq >> 1) * 16);
+      const int off = (sq & 1) ? o1 : o0;
+      if (off >= 0) {
+        cplx* base = ring + off + k1 * 16;
         cplx v[16];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) { v[j] = sb[j ^ p2_k1]; v[j + 8] = sb[(j ^ p2_k1) + 8]; }
+        for (int jj = 0; jj < 8; ++jj) { v[jj] = base[jj ^ k1]; v[jj + 8] = base[(jj ^ k1) + 8]; }
         Dft<16, -1>::run(v);
 #pragma unroll
-        for (int k2 = 0; k2 < 8; ++k2) { sb[k2 ^ p2_k1] = v[k2]; sb[(k2 ^ p2_k1) + 8] = v[k2 + 8]; }   // X[k1 + 8 k2]
+        for (int k2 = 0; k2 < 8; ++k2) { base[k2 ^ k1] = v[k2]; base[(k2 ^ k1) + 8] = v[k2 + 8]; }   // X[k1 + 8 k2]
       }
-      // the inputs of the thread's next stage (or of the next column's first stage) are requested now:
-      // their latency hides under phase 3
-      if (st + 1 < nst) prefetch(kx, st + 1);
-      else prefetch(kx + gridDim.x, 0);
-      __syncthreads();
-      // ---- phase 3: products of the stage's blocks, accumulated in registers -----------------------
-      for (int u = 0; u < na; ++u) {
-        const cplx* ub = sq + u * NSEQ * CB_N;
-        if (p3_part == 0) cb_accumulate<TK, PT::T0[0], PT::T1[0], PT::U0[0], PT::U1[0]>(acc, ub, p3_pk);
-        else if (p3_part == 1) cb_accumulate<TK, PT::T0[1], PT::T1[1], PT::U0[1], PT::U1[1]>(acc, ub, p3_pk);
-        else cb_accumulate<TK, PT::T0[2], PT::T1[2], PT::U0[2], PT::U1[2]>(acc, ub, p3_pk);
-      }
-      __syncthreads();
     }
+    __syncwarp();
+    if (lane == 0) {
+      if (stask) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+          if (pblk + i < nblk) mbar_arrive(&s_sfull[(nbase + pblk + i) % CB_NS2]);
+      } else {
+        mbar_arrive(&s_full[(nbase + pblk) % CB_NSLOT]);
+      }
+    }
+  };
 
-    // ---- phase 4: accumulators -> lags ---------------------------------------------------------------
-    cplx* acs = sq;
-    if (p3_part == 0) cb_flush<TK, PT::T0[0], PT::T1[0], PT::U0[0], PT::U1[0]>(acc, acs, p3_k);
-    else if (p3_part == 1) cb_flush<TK, PT::T0[1], PT::T1[1], PT::U0[1], PT::U1[1]>(acc, acs, p3_k);
-    else cb_flush<TK, PT::T0[2], PT::T1[2], PT::U0[2], PT::U1[2]>(acc, acs, p3_k);
-    __syncthreads();
-    // (pair, a): V_a[m] = sum_b acs[a + 8 b] e^{+2 pi i b m/16}, in place (slot a + 8 m)
-    {
-      const int p4_a = tid & 7, p4_pair = tid >> 3;
-      if (p4_pair < NPAIR) {     // NPAIR <= 27 < 48
-        cplx V[16];
-        cplx* base = acs + p4_pair * CB_N + p4_a;
+  if (wrp < CB_FW) {
+    // =============================== transform warps ===============================================
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(CB_REG_F));
+    while (tci < ncolMine) {
+      const int nb = tci * nblk + tblk;
+      if (TT::STASK && ttype == TT::NT) {
 #pragma unroll
-        for (int b = 0; b < 16; ++b) V[b] = base[8 * b];
-        Dft<16, +1>::run(V);
-#pragma unroll
-        for (int m = 0; m < 16; ++m) base[8 * m] = V[m];
+        for (int i = 0; i < 4; ++i) {
+          const int n = nb + i;
+          if (tblk + i < nblk) mbar_wait(&s_sempty[n % CB_NS2], (unsigned)(((n / CB_NS2) & 1) ^ 1));
+        }
+      } else {
+        mbar_wait(&s_empty[nb % CB_NSLOT], (unsigned)(((nb / CB_NSLOT) & 1) ^ 1));
       }
+      run_task();
     }
-    __syncthreads();
-    // Y[dy] = (H/128) sum_a e^{+2 pi i a dy/128} V_a[dy mod 16]; the lanes start at different a (banks)
+  } else {
+    // =============================== product warps ================================================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(CB_REG_P));
+    constexpr int NKK = TK * (TK + 1) / 2;
+    const int k = tid - CB_FW * 32;                      // frequency
+    const int pk = cb_slot(k & 7, k >> 3);
     const double scale = (double)H / (double)CB_N;
-    for (int o = tid; o < NPAIR * CB_LAGS; o += CB_TH) {
-      const int pair = o / CB_LAGS, dy = o - pair * CB_LAGS - 10;
-      const int Dp = s_Dp[pair];
-      if (dy < -Dp || dy > Dp) continue;
-      const cplx* base = acs + pair * CB_N + 8 * ((dy + 16) & 15);
-      cplx s = cmake(0.0, 0.0);
+    int n = 0;                                           // block sequence number
+    for (int ci = 0; ci < ncolMine; ++ci) {
+      const int kx = (int)blockIdx.x + ci * (int)gridDim.x;
+      cplx acc[NPAIR];
 #pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        const int a = (i + tid) & 7;
-        s = cadd(s, cmulc(s_tw[(a * (dy + 128)) & 127], base[a]));
+      for (int i = 0; i < NPAIR; ++i) acc[i] = cmake(0.0, 0.0);
+      for (int b = 0; b < nblk; ++b, ++n) {
+        const int slot = n % CB_NSLOT;
+        mbar_wait(&s_full[slot], (unsigned)((n / CB_NSLOT) & 1));
+        if (TT::STASK) mbar_wait(&s_sfull[n % CB_NS2], (unsigned)((n / CB_NS2) & 1));
+        const cplx* ub = ring + (size_t)slot * NSEQ_R * CB_N + pk;
+        const cplx* us = TT::STASK ? ring + SRING + (n % CB_NS2) * CB_N + pk : ub + 2 * TK * CB_N;
+        cplx C[TK];
+#pragma unroll
+        for (int t = 0; t < TK; ++t) C[t] = ub[t * CB_N];
+#pragma unroll
+        for (int t2 = 0; t2 <= TK; ++t2) {
+          const cplx E = t2 < TK ? ub[(TK + t2) * CB_N] : us[0];
+#pragma unroll
+          for (int t = 0; t < TK; ++t) {
+            if (t <= t2) {
+              const int pair = (t2 < TK) ? (t * TK - t * (t - 1) / 2 + (t2 - t)) : (NKK + t);
+              cfmac(acc[pair], C[t], E);
+            }
+          }
+        }
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive(&s_empty[slot]);
+          if (TT::STASK) mbar_arrive(&s_sempty[n % CB_NS2]);
+        }
       }
-      P.Y[((size_t)pair * P.nLag + (dy + Dp)) * P.pitch + kx] = cscale(s, scale);
+      // ---- end of the column: accumulators -> lags, PP4 pairs at a time
+#pragma unroll
+      for (int ps = 0; ps < NPASS4; ++ps) {
+        const int p0 = ps * PP4, np = (NPAIR - p0 < PP4) ? NPAIR - p0 : PP4;
+#pragma unroll
+        for (int i = 0; i < NPAIR; ++i)
+          if (i >= p0 && i < p0 + PP4) acs[(i - p0) * CB_N + k] = acc[i];
+        cb_bar_products();
+        // (pair, a): V_a[m] = sum_b acs[a + 8 b] e^{+2 pi i b m/16}, in place (position a + 8 m)
+        for (int it = k; it < np * 8; it += CB_PT) {
+          const int a = it & 7, pl = it >> 3;
+          cplx V[16];
+          cplx* base = acs + pl * CB_N + a;
+#pragma unroll
+          for (int bb = 0; bb < 16; ++bb) V[bb] = base[8 * bb];
+          Dft<16, +1>::run(V);
+#pragma unroll
+          for (int m = 0; m < 16; ++m) base[8 * m] = V[m];
+        }
+        cb_bar_products();
+        // Y[dy] = (H/128) sum_a e^{+2 pi i a dy/128} V_a[dy mod 16]; the lanes start at different a (banks)
+        for (int o = k; o < np * CB_LAGS; o += CB_PT) {
+          const int pl = o / CB_LAGS, dy = o - pl * CB_LAGS - 10, pair = p0 + pl;
+          const int Dp = s_Dp[pair];
+          if (dy < -Dp || dy > Dp) continue;
+          const cplx* base = acs + pl * CB_N + 8 * ((dy + 16) & 15);
+          cplx s = cmake(0.0, 0.0);
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const int a = (i + k) & 7;
+            s = cadd(s, cmulc(s_tw[(a * (dy + 128)) & 127], base[a]));
+          }
+          P.Y[((size_t)pair * P.nLag + (dy + Dp)) * P.pitch + kx] = cscale(s, scale);
+        }
+        cb_bar_products();   // the scratch is rewritten by the next pass / at the end of the next column
+      }
     }
-    __syncthreads();   // the stage buffer is reused by the next column
   }
 }
 
@@ -373,8 +514,10 @@ bool sfft_colx_supported(int H, int nPair) { return (H == 1024 || H == 2048 || H
 template <int TK>
 static sfft_status launch_colb_t(const ColbParams& P, int num_sms, cudaStream_t st) {
   constexpr int NSEQ = 2 * TK + 1, NPAIR = TK * (TK + 1) / 2 + TK;
-  const size_t smem = (size_t)(CB_G * NSEQ + 2 * 8) * CB_N * sizeof(cplx);   // stage buffer + staged second images
-  static_assert((size_t)NPAIR * CB_N <= (size_t)CB_G * NSEQ * CB_N, "phase 4 scratch must fit the stage buffer");
+  constexpr bool ST = CbTasks<TK>::STASK;
+  constexpr int NP4 = NPAIR > 16 ? 2 : 1, PP4 = (NPAIR + NP4 - 1) / NP4;
+  // ring (+ S~ ring) + end-of-column scratch
+  const size_t smem = (size_t)(CB_NSLOT * (ST ? NSEQ - 1 : NSEQ) + (ST ? CB_NS2 : 0) + PP4) * CB_N * sizeof(cplx);
   SFFT_CUDA_TRY(cudaFuncSetAttribute(k_colb<TK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int grid = num_sms;
   if (grid > P.NC + 1) grid = P.NC + 1;
@@ -388,7 +531,6 @@ sfft_status sfft_launch_colx(sfft_plan* p, cudaStream_t st, int* nl) {
   P.T = p->T; P.Y = p->Y; P.pairs = p->d_pairs; P.tw128 = p->tw128;
   P.H = p->H; P.NC = p->NC; P.pitch = p->pitch; P.nLag = p->nLag; P.nPair = p->nPair; P.nimg = p->nRowImg;
   P.D = p->Dmax; P.B = CB_N - 2 * p->Dmax; P.nblk = (p->H + P.B - 1) / P.B;
-  P.nst = (P.nblk + CB_G - 1) / CB_G;
   ++*nl;
   switch (p->TK) {
     case 1: return launch_colb_t<1>(P, p->num_sms, st);
