@@ -382,22 +382,25 @@ __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
     const int pblk = tblk;
     ti += CB_FW;
     while (ti >= tasksPerCol && tci < ncolMine) { ti -= tasksPerCol; ++tci; }
-    if (tci < ncolMine) {
-      decode(ti, ttype, tblk);
-      prefetch(xa, (int)blockIdx.x + tci * (int)gridDim.x, job_blk(ttype, tblk, 0), lane_img(ttype));
-    }
+    if (tci < ncolMine) decode(ti, ttype, tblk);
     __syncwarp();
     // ---- phase 2: radix-16 over j; lane = (sequence sq = (half, job), k1)
     {
       const int sq = lane >> 3, k1 = lane & 7;
       const int o0 = __shfl_sync(0xffffffffu, soff[0], (sq >> 1) * 16), o1 = __shfl_sync(0xffffffffu, soff[1], (sq >> 1) * 16);
       const int off = (sq & 1) ? o1 : o0;
-      if (off >= 0) {
-        cplx* base = ring + off + k1 * 16;
-        cplx v[16];
+      cplx* base = ring + (off >= 0 ? off : 0) + k1 * 16;
+      cplx v[16];   // (a lane without a sequence transforms slot 0 and stores nothing)
 #pragma unroll
-        for (int jj = 0; jj < 8; ++jj) { v[jj] = base[jj ^ k1]; v[jj + 8] = base[(jj ^ k1) + 8]; }
-        Dft<16, -1>::run(v);
+      for (int jj = 0; jj < 8; ++jj) { v[jj] = base[jj ^ k1]; v[jj + 8] = base[(jj ^ k1) + 8]; }
+      // the next task's inputs are requested HERE, after the shared-memory loads of this pass have been
+      // issued (issued earlier, the global loads' scoreboard would hold up those loads and the shuffles):
+      // their latency hides under the butterfly, the stores and the waits that follow
+      asm volatile("" ::: "memory");
+      if (tci < ncolMine) prefetch(xa, (int)blockIdx.x + tci * (int)gridDim.x, job_blk(ttype, tblk, 0), lane_img(ttype));
+      asm volatile("" ::: "memory");
+      Dft<16, -1>::run(v);
+      if (off >= 0) {
 #pragma unroll
         for (int k2 = 0; k2 < 8; ++k2) { base[k2 ^ k1] = v[k2]; base[(k2 ^ k1) + 8] = v[k2 + 8]; }   // X[k1 + 8 k2]
       }
