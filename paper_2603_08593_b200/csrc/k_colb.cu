@@ -39,8 +39,8 @@
 // across the column boundary.  End of a column: accumulators -> shared memory, 16-point inverse over b
 // (k = a + 8 b), then the 2D+1 lags of every pair (8 twiddled terms each) -> Y[pair][dy][kx].
 // Shared-memory positions are XOR-swizzled (slot k1*16 + (j ^ k1)): every pass is conflict free with no
-// padding.  T has the row-group layout T[img][y/G][kx][y%G], G = SFFT_T_G = 8 (k_row2_fwd): a half warp's
-// 16 rows of a column are two whole 128-byte lines.
+// padding.  T has the row-group layout T[img][y/G][kx][y%G], G = SFFT_T_G = 4 (k_row2_fwd): a half warp's
+// 16 rows of a column are four 64-byte runs.
 #include <math.h>
 #include "fft_smem.cuh"
 

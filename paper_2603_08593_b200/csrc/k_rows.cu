@@ -24,7 +24,7 @@ struct RowFwdParams {
   cplx* T;       // [nimg][H][pitchT]
   int pitchT;    // row pitch of T in complex elements
   int packed;    // 1: T[y][0] = X[0] + i X[W/2];  0: T[y][0] = X[0], T[y][NC] = X[W/2]
-  int colT;      // 1 (unpacked only): row-pair layout T[img][y/2][kx][y%2], kx in [0, NC], written by k_row2_fwd, read by k_colb
+  int colT;      // 1 (unpacked only): row-group layout T[img][y/G][kx][y%G], G = SFFT_T_G, kx in [0, NC]; written by k_row2_fwd, read by k_colb
   const cplx* twP;   // per-pass twiddle tables for length NC
   const cplx* twW;
   int moments, DB, nMomA, nMomS, nMomR;
@@ -280,12 +280,13 @@ __global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
 // ------------------------------------------------------------------------------------------------
 // Row pass of the fused build path: one CTA = one image (blockIdx.x % nimg) of RB row PAIRS (2b, 2b+1).
 // The two rows of a pair are transformed one after the other into two shared-memory buffers and leave
-// the CTA together: the split step writes, per column kx, the 32-byte pair {X_2b[kx], X_2b+1[kx]}, so
-// T has the row-pair layout T[img][y/2][kx][y%2] (kx in [0, NC]) -- a warp's stores are one contiguous
-// 1 KB run (full lines), and k_colb reads whole 32-byte sectors along y.  Row 2b's inputs go from
-// global memory through the weighting into the first butterfly (registers only); row 2b+1's inputs are
-// requested at the same time by cp.async into the second buffer (free until that row's first pass),
-// so no global-memory latency is exposed between the two transforms.  Fused reductions as in k_row_fwd.
+// the CTA together: the split step writes, per column kx, the 32-byte pair {X_2b[kx], X_2b+1[kx]} into
+// the row-group layout T[img][y/G][kx][y%G] (G = SFFT_T_G rows of one column are contiguous; kx in
+// [0, NC]) -- whole 32-byte sectors, G/2 row pairs filling a 16 G-byte run that k_colb reads along y.
+// Row 2b's inputs go from global memory through the weighting into the first butterfly (registers
+// only); row 2b+1's inputs are requested at the same time by cp.async into the second buffer (free
+// until that row's first pass), so no global-memory latency is exposed between the two transforms.
+// Fused reductions as in k_row_fwd.
 __device__ __forceinline__ void row_cp_async16(void* smem_dst, const void* gsrc) {
   const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gsrc) : "memory");

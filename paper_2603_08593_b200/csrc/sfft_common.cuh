@@ -14,7 +14,7 @@
 #define SFFT_CR_MAXSPEC 24   // k_cross: spectra a group may stage
 #define SFFT_KB_NBLK 296     // x-CTAs of the kernel-background correction kernel (2 per SM)
 #ifndef SFFT_T_G
-#define SFFT_T_G 8          // fused path: rows per group of the row-spectra layout T[img][y/G][kx][y%G]
+#define SFFT_T_G 4          // fused path: rows per group of the row-spectra layout T[img][y/G][kx][y%G] (2, 4 and 8 measured: 4 is best)
 #endif
 #define SFFT_NSTAGE 10     // see sfft_profile_read in include/sfft.h
 #define SFFT_PROF_MAX 512
