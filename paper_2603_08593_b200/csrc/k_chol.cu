@@ -404,7 +404,8 @@ k_chol_fused(const double* __restrict__ A, const double* __restrict__ b, double*
 }
 
 // Back substitution Lc^T c = z; z is row N of the workspace.  Per 32-block (last to first): the
-// block's triangular system is solved by warp 0 (lane m holds r_m), then every thread j < k0
+// block's triangular system is solved by warp 0 (lane m holds r_m; row-scaled factor, so one shuffle and
+// one fma per dependent step), then every thread j < k0
 // updates r_j -= sum_i L[k0+i][j] x_i with its 32 loads issued together (coalesced along j).
 __global__ void __launch_bounds__(1024, 1) k_chol_back(const double* __restrict__ Lw, double* c, int N, int ld) {
   extern __shared__ double sm[];
@@ -425,16 +426,20 @@ __global__ void __launch_bounds__(1024, 1) k_chol_back(const double* __restrict_
     const int k0 = kb * CH_NB;
     const int nb = min(CH_NB, N - k0);
     if (tid < 32) {
-      rd[lane] = 1.0 / ls[lane * (CH_NB + 1) + lane];
+      // x_j = r_j / L_jj, r_m -= L[j][m] x_j = r_j (L[j][m] / L[j][j]): with the row-scaled factor the
+      // dependent chain is one shuffle and one fma per step; the scalings and the final division are off it
+      const double dl = ls[lane * (CH_NB + 1) + lane];
+      const double rl = 1.0 / dl;
+      rd[lane] = rl;
       __syncwarp();
       double rm = (lane < nb) ? r[k0 + lane] : 0.0;
 #pragma unroll
       for (int j = CH_NB - 1; j >= 0; --j) {
+        const double sj = ls[j * (CH_NB + 1) + lane] * rd[j];
         const double rj = __shfl_sync(0xffffffffu, rm, j);
-        const double xj = div_by(rj, ls[j * (CH_NB + 1) + j], rd[j]);
-        if (lane == j) rm = xj;
-        else if (lane < j) rm = fma(-ls[j * (CH_NB + 1) + lane], xj, rm);
+        if (lane < j) rm = fma(-sj, rj, rm);
       }
+      rm = div_by(rm, dl, rl);
       if (lane < nb) {
         cb[lane] = rm;
         c[k0 + lane] = rm;
