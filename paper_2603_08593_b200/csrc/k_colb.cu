@@ -54,8 +54,12 @@
 #define CB_REG_F 120       // registers per thread of the transform warpgroups
 #define CB_REG_P 152       // ... of the product warpgroup (3 x 120 + 152 = 4 x 128)
 #define CB_PT 128         // product threads (one per frequency)
+#ifndef CB_NSLOT
 #define CB_NSLOT 6        // blocks in the shared-memory ring
+#endif
+#ifndef CB_NS2
 #define CB_NS2 16         // blocks in the ring of the S~ spectra (DK = 2: they are produced four blocks at a time, ahead of the rest)
+#endif
 #define CB_LAGS 21        // 2 * 10 + 1
 
 struct ColbParams {
