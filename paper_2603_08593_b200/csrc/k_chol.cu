@@ -271,8 +271,8 @@ k_chol_fused(const double* __restrict__ A, const double* __restrict__ b, double*
     const int rbelow = k0 + nb;                 // first row below the diagonal block
     // ---- panel phase: CTAs that own panel rows (and CTA 0) factor the diagonal block
     const bool has_rows = blockIdx.x * CH_WARPS < (N + 1 - rbelow);
-    // the factored block is written back by a CTA that owns no panel rows when there is one (the
-    // store then stays off the critical path of the rows), else by CTA 0
+    // the factored block is written back (after the grid barrier) by a CTA that owns no panel rows when
+    // there is one, else by CTA 0
     const unsigned storer = (nblocks - 1) * CH_WARPS >= (unsigned)(N + 1 - rbelow) ? nblocks - 1 : 0u;
     if (has_rows || blockIdx.x == storer) {
       // the warp's first panel row is final already: request it now, its L2 latency hides under the factor
@@ -289,12 +289,6 @@ k_chol_fused(const double* __restrict__ A, const double* __restrict__ b, double*
       }
       const int bad = cta_potrf64(sd, ss, srd, colb, tid);
       if (bad >= 0 && bad < nb && blockIdx.x == storer && tid == 0 && info) atomicCAS(info, 0, k0 + bad + 1);
-      if (blockIdx.x == storer) {
-        for (int e = tid; e < CH_PB * CH_PB; e += CH_THREADS) {
-          const int i = e >> 6, j = e & 63;
-          if (i < nb && j <= i) Lw[(size_t)(k0 + i) * ld + k0 + j] = sd[i * CH_LDS + j];
-        }
-      }
       CH_STAMP(stamp + 0)
       // rows below (including the rhs row N): one row per warp, lane holds entries lane and lane+32.
       // x_j = a_j / L_jj, a_m -= x_j L_mj = a_j ss[m][j]: per step one shuffle and one fma on the
@@ -326,6 +320,17 @@ k_chol_fused(const double* __restrict__ A, const double* __restrict__ b, double*
     CH_STAMP(stamp + 1)
     grid_barrier(bar, target, nblocks);
     CH_STAMP(stamp + 2)
+    // The factored diagonal block is written back only now: before the barrier the other CTAs were still
+    // reading the UNFACTORED block from the same addresses.  The storer's copy in shared memory is intact
+    // until the update phase below reuses the buffers; nothing in this kernel reads the block again
+    // (k_chol_back does), so the store is off every critical path.
+    if (blockIdx.x == storer) {
+      for (int e = tid; e < CH_PB * CH_PB; e += CH_THREADS) {
+        const int i = e >> 6, j = e & 63;
+        if (i < nb && j <= i) Lw[(size_t)(k0 + i) * ld + k0 + j] = sd[i * CH_LDS + j];
+      }
+      __syncthreads();
+    }
     // ---- update phase: 32x32 tiles (ti, tj), tj <= ti, of the trailing matrix starting at r0,
     //      A22 -= L21 L21^T with the panel's 64 columns
     const int r0 = k0 + CH_PB;
