@@ -32,6 +32,9 @@ __device__ unsigned long long sfft_chol_dbg[256];
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));                       \
     sfft_chol_dbg[i] = t_;                                                       \
   }
+extern "C" int sfft_chol_dbg_read(unsigned long long* out, int n) {   // development builds only
+  return (int)cudaMemcpyFromSymbol(out, sfft_chol_dbg, sizeof(unsigned long long) * (size_t)(n < 256 ? n : 256));
+}
 #else
 #define CH_STAMP(i)
 #endif
