@@ -175,15 +175,15 @@ __device__ __forceinline__ void cb_flush(const cplx* acc, cplx* acs, int k) {
   }
 }
 
-// ---- mbarrier helpers (CTA scope) ---------------------------------------------------------------------
-__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+// ---- mbarrier helpers (CTA scope; `a` = 32-bit shared-memory address of the barrier) -------------------
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned a, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(a), "r"(count) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+__device__ __forceinline__ void mbar_arrive(unsigned a) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(a) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
-  const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+__device__ __forceinline__ void mbar_wait(unsigned a, unsigned parity) {
   unsigned done;
   do {
     asm volatile(
@@ -193,14 +193,6 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
 }
 __device__ __forceinline__ void cb_bar_products() {   // the 128 product threads only
   asm volatile("bar.sync 1, %0;\n" ::"n"(CB_PT) : "memory");
-}
-// non-blocking: has the phase with this parity completed?  (acquire, CTA scope)
-__device__ __forceinline__ bool mbar_test(unsigned long long* bar, unsigned parity) {
-  unsigned done;
-  asm volatile(
-      "{\n .reg .pred p;\n mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
-      : "=r"(done) : "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
-  return done != 0u;
 }
 
 // One phase-1 job of a half warp: sequence = DFT8 over r of (x[r] * eta_r^q, zero outside the centre rows
@@ -273,13 +265,15 @@ __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
   for (int i = tid; i < CB_N; i += CB_TH) s_tw[i] = ldg2(P.tw128 + i);
   for (int i = tid; i < 7 * 16; i += CB_TH) s_w[i] = ldg2(P.tw128 + ((i >> 4) + 1) * (i & 15));
   for (int i = tid; i < NPAIR; i += CB_TH) s_Dp[i] = P.pairs[i].D;
+  // 32-bit shared addresses of the barrier arrays (barrier i at base + 8 i)
+  const unsigned aFull = smem_addr(s_full), aEmpty = smem_addr(s_empty), aSFull = smem_addr(s_sfull), aSEmpty = smem_addr(s_sempty);
   if (tid < CB_NSLOT) {
-    mbar_init(&s_full[tid], FULL_COUNT);
-    mbar_init(&s_empty[tid], CB_PT / 32);
+    mbar_init(aFull + 8u * tid, FULL_COUNT);
+    mbar_init(aEmpty + 8u * tid, CB_PT / 32);
   }
   if (tid < CB_NS2) {
-    mbar_init(&s_sfull[tid], 1);
-    mbar_init(&s_sempty[tid], CB_PT / 32);
+    mbar_init(aSFull + 8u * tid, 1);
+    mbar_init(aSEmpty + 8u * tid, CB_PT / 32);
   }
   __syncthreads();
   const int ncolMine = (P.NC + 1 - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // columns of this CTA
@@ -319,17 +313,21 @@ __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
   // prefetch of a task's first job: elements r < CB_PREG into registers, the others by cp.async into the
   // lane's staging words (the radix-16 pass that runs meanwhile needs the registers); prefetch_land()
   // completes it
+  const unsigned aStage = smem_addr(&s_xs[tid < CB_FW * 32 ? tid : 0]);   // the lane's staging words, CB_FW*32*16 bytes apart
   auto prefetch = [&](cplx* x, int kx, int b, int img) {
     fetch(x, kx, b, img, 0, CB_PREG);
     const int c0 = b * B;
     const int lim = b < nblk ? min(B, H - c0) + 2 * D : 0;
+    const cplx* src = P.T + SFFT_T_G * (size_t)kx + (size_t)img * imgStride;
+    const int y0 = (c0 - D + j + H) & (H - 1);
+    const unsigned gi0 = (unsigned)y0 / SFFT_T_G, sub = (unsigned)y0 % SFFT_T_G, gmask = (unsigned)(H / SFFT_T_G) - 1u;
 #pragma unroll
     for (int r = CB_PREG; r < 8; ++r) {
-      const int yr = (c0 - D + j + 16 * r + H) & (H - 1);
-      const cplx* src = P.T + SFFT_T_G * (size_t)kx + (size_t)img * imgStride + (size_t)(yr / SFFT_T_G) * grpStride + (yr % SFFT_T_G);
-      const unsigned sa = (unsigned)__cvta_generic_to_shared(&s_xs[(r - CB_PREG) * CB_FW * 32 + tid]);
-      const int sz = (j + 16 * r < lim) ? 16 : 0;           // zero fill past the block's end
-      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(sa), "l"(sz ? src : P.T), "r"(sz) : "memory");
+      const unsigned gi = (gi0 + (unsigned)(16 / SFFT_T_G) * r) & gmask;
+      const bool in = j + 16 * r < lim;
+      const int sz = in ? 16 : 0;                           // zero fill past the block's end
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n"
+                   ::"r"(aStage + (unsigned)((r - CB_PREG) * CB_FW * 32 * sizeof(cplx))), "l"(src + (in ? gi * grpStride + sub : 0u)), "r"(sz) : "memory");
     }
     asm volatile("cp.async.commit_group;\n" ::: "memory");
   };
@@ -344,21 +342,6 @@ __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
     decode(ti, ttype, tblk);
     prefetch(xa, (int)blockIdx.x + tci * (int)gridDim.x, job_blk(ttype, tblk, 0), lane_img(ttype));
   }
-  // are the slots the pending task writes free?  (block sequence number n = column iteration * nblk + block)
-  auto task_ready = [&]() -> bool {
-    const int nb = tci * nblk + tblk;
-    bool ok = true;
-    if (TT::STASK && ttype == TT::NT) {
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const int n = nb + i;
-        if (tblk + i < nblk) ok = ok && mbar_test(&s_empty[n % CB_NSLOT], (unsigned)(((n / CB_NSLOT) & 1) ^ 1));
-      }
-    } else {
-      ok = mbar_test(&s_empty[nb % CB_NSLOT], (unsigned)(((nb / CB_NSLOT) & 1) ^ 1));
-    }
-    return __all_sync(0xffffffffu, ok);
-  };
   auto run_task = [&]() {
     const int kx = (int)blockIdx.x + tci * (int)gridDim.x;
     const int nbase = tci * nblk;
@@ -414,9 +397,9 @@ __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
       if (stask) {
 #pragma unroll
         for (int i = 0; i < 4; ++i)
-          if (pblk + i < nblk) mbar_arrive(&s_sfull[(nbase + pblk + i) % CB_NS2]);
+          if (pblk + i < nblk) mbar_arrive(aSFull + 8u * (unsigned)((nbase + pblk + i) % CB_NS2));
       } else {
-        mbar_arrive(&s_full[(nbase + pblk) % CB_NSLOT]);
+        mbar_arrive(aFull + 8u * (unsigned)((nbase + pblk) % CB_NSLOT));
       }
     }
   };
@@ -430,10 +413,10 @@ __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
           const int n = nb + i;
-          if (tblk + i < nblk) mbar_wait(&s_sempty[n % CB_NS2], (unsigned)(((n / CB_NS2) & 1) ^ 1));
+          if (tblk + i < nblk) mbar_wait(aSEmpty + 8u * (unsigned)(n % CB_NS2), (unsigned)(((n / CB_NS2) & 1) ^ 1));
         }
       } else {
-        mbar_wait(&s_empty[nb % CB_NSLOT], (unsigned)(((nb / CB_NSLOT) & 1) ^ 1));
+        mbar_wait(aEmpty + 8u * (unsigned)(nb % CB_NSLOT), (unsigned)(((nb / CB_NSLOT) & 1) ^ 1));
       }
       run_task();
     }
@@ -452,8 +435,8 @@ __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
       for (int i = 0; i < NPAIR; ++i) acc[i] = cmake(0.0, 0.0);
       for (int b = 0; b < nblk; ++b, ++n) {
         const int slot = n % CB_NSLOT;
-        mbar_wait(&s_full[slot], (unsigned)((n / CB_NSLOT) & 1));
-        if (TT::STASK) mbar_wait(&s_sfull[n % CB_NS2], (unsigned)((n / CB_NS2) & 1));
+        mbar_wait(aFull + 8u * (unsigned)slot, (unsigned)((n / CB_NSLOT) & 1));
+        if (TT::STASK) mbar_wait(aSFull + 8u * (unsigned)(n % CB_NS2), (unsigned)((n / CB_NS2) & 1));
         const cplx* ub = ring + (size_t)slot * NSEQ_R * CB_N + pk;
         const cplx* us = TT::STASK ? ring + SRING + (n % CB_NS2) * CB_N + pk : ub + 2 * TK * CB_N;
         cplx C[TK];
@@ -472,8 +455,8 @@ __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
         }
         __syncwarp();
         if (lane == 0) {
-          mbar_arrive(&s_empty[slot]);
-          if (TT::STASK) mbar_arrive(&s_sempty[n % CB_NS2]);
+          mbar_arrive(aEmpty + 8u * (unsigned)slot);
+          if (TT::STASK) mbar_arrive(aSEmpty + 8u * (unsigned)(n % CB_NS2));
         }
       }
       // ---- end of the column: accumulators -> lags, PP4 pairs at a time
