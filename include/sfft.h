@@ -209,8 +209,8 @@ sfft_status sfft_probe_fp64(int kind, int iters, double* tflops, double* elapsed
  * event pair on the caller stream around each stage (no synchronisation; at most 512 pending
  * pairs between reads).  sfft_profile_read synchronises on the pending events, folds them into
  * per-stage totals and returns the accumulated milliseconds and pair count of `stage`:
- *   0 build: row pass (k_row_fwd)          1 build: column pass (k_col_fwd), or the fused
- *                                            column-pass + cross kernel (k_colx)
+ *   0 build: row pass (k_row2_fwd/k_row_fwd) 1 build: column pass (k_col_fwd), or the fused
+ *                                            column/cross kernel (k_colb)
  *   2 build: cross+pruned inverse, K-K     3 build: cross+pruned inverse, K-S
  *   4 build: lag-row inverse + moments + gather      5 solve (all kernels)
  *   6 subtract: row pass   7 subtract: phase table + y-mixing   8 subtract: inverse rows + D
@@ -223,7 +223,7 @@ sfft_status sfft_profile_read(sfft_plan* p, int stage, double* total_ms, int* co
  * for bench.py's "gpu_launches"): which = 0 build, 1 solve, 2 subtract.  -1 on bad arguments. */
 int sfft_last_launch_count(const sfft_plan* p, int which);
 
-/* 1 if the plan runs the fused column-FFT + cross-spectra kernel (H in {1024, 2048, 4096} and at
+/* 1 if the plan runs the fused (blocked) column/cross-spectra kernel (H in {1024, 2048, 4096} and at
  * most 32 map pairs, i.e. DK <= 2), 0 if it runs the separate column-pass and cross kernels, -1 if
  * p is NULL.  Both are CUDA paths with identical results up to rounding order; profile stage 1 then
  * holds the fused kernel and stages 2, 3 stay empty. */

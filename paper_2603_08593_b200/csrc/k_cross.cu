@@ -177,7 +177,7 @@ struct LagParams {
   double* Cmap;  // [nPair][nLag][nLag]; pair with half-range D uses rows/cols [0, 2D]
   const PairDesc* pairs;
   int NC, W, pitch, nLag;
-  int nPart;            // partial lag-row sets (residue classes of k_colx), added in order
+  int nPart;            // partial lag-row sets, added in order (1 on both build paths)
   size_t partStride;    // elements between two sets
   double invP;
   const cplx* twW;
