@@ -25,6 +25,9 @@
 #pragma once
 #include "sfft_common.cuh"
 
+#ifndef SFFT_TW_TABLE
+#define SFFT_TW_RECUR 1   // twiddles w^r, r >= 3, as products of w^1, w^2 (see fft_twiddle_load); -DSFFT_TW_TABLE: all from the table
+#endif
 #define SFFT_SQRT1_2 0.70710678118654752440
 #define SFFT_COS_PI_8 0.92387953251128675613
 #define SFFT_SIN_PI_8 0.38268343236508977173
@@ -187,17 +190,50 @@ __device__ __forceinline__ void fft_map(int i, int nseq, int& seq, int& j) {
 }
 
 // twiddle + butterfly + Stockham store of one radix-R butterfly held in v[]
+// a^2 and a*b for unit-modulus twiddles
+__device__ __forceinline__ cplx csqr(cplx a) { return cmake(fma(a.x, a.x, -(a.y * a.y)), 2.0 * a.x * a.y); }
+// The R-1 twiddles w^r, w = exp(-2 pi i k/(NS R)), of one butterfly.  SFFT_TW_RECUR: only w^1 (and w^2 for
+// radix 16) come from the table; the others are products of at most three table values' powers
+// (w^4 = (w^2)^2, w^8 = (w^4)^2, w^(a+b) = w^a w^b: depth <= 3 multiplications, error a few ulp), which
+// trades ~13 table loads per radix-16 butterfly for ~50 fp64 operations: the row kernels are bound by
+// the L1/shared-memory pipe with the fp64 pipe a third busy.
 template <int N, int R, int NS>
 __device__ __forceinline__ void fft_twiddle_load(cplx* t, int j, const cplx* __restrict__ tw) {
   if constexpr (NS > 1) {
     const int k = j & (NS - 1);
+#ifdef SFFT_TW_RECUR
+    t[1] = ldg2(tw + k);
+    if constexpr (R >= 4) t[2] = ldg2(tw + NS + k);
+#else
 #pragma unroll
     for (int r = 1; r < R; ++r) t[r] = ldg2(tw + (r - 1) * NS + k);
+#endif
   }
+}
+// completes t[] after the loads above have landed (no-op without SFFT_TW_RECUR)
+template <int R, int NS>
+__device__ __forceinline__ void fft_twiddle_complete(cplx* t) {
+#ifdef SFFT_TW_RECUR
+  if constexpr (NS > 1 && R >= 4) {
+    t[3] = cmul(t[1], t[2]);
+    if constexpr (R >= 8) {
+      t[4] = csqr(t[2]);
+      t[5] = cmul(t[1], t[4]);
+      t[6] = cmul(t[2], t[4]);
+      t[7] = cmul(t[3], t[4]);
+    }
+    if constexpr (R >= 16) {
+      t[8] = csqr(t[4]);
+#pragma unroll
+      for (int r = 1; r < 8; ++r) t[8 + r] = cmul(t[r], t[8]);
+    }
+  }
+#endif
 }
 template <int N, int R, int NS, int DIR>
 __device__ __forceinline__ void fft_twiddle_apply(cplx* v, cplx* t) {
   if constexpr (NS > 1) {
+    fft_twiddle_complete<R, NS>(t);
 #pragma unroll
     for (int r = 1; r < R; ++r) {
       if (DIR > 0) t[r].y = -t[r].y;
