@@ -61,6 +61,25 @@ __device__ __forceinline__ cplx mul_w16(cplx a) {
   else return a;
 }
 
+// exp(-2 pi i m / 32), m in [0, 16): compile-time constants once m is (the rows' split/merge twiddles of
+// one thread are w^(tr + e TPR) = w^tr * exp(-2 pi i e / (2 EPT)) -- one table load, EPT-1 constant products)
+__host__ __device__ constexpr double sfft_cos32(int m) {
+  constexpr double c[17] = {1.0, 0.98078528040323044913, 0.92387953251128675613, 0.83146961230254523708,
+                            0.70710678118654752440, 0.55557023301960222474, 0.38268343236508977173,
+                            0.19509032201612826785, 0.0, -0.19509032201612826785, -0.38268343236508977173,
+                            -0.55557023301960222474, -0.70710678118654752440, -0.83146961230254523708,
+                            -0.92387953251128675613, -0.98078528040323044913, -1.0};
+  return c[m];
+}
+// a * exp(-2 pi i e / (2 EPT)),  e < EPT, EPT in {8, 16}
+template <int EPT>
+__device__ __forceinline__ cplx mul_split_root(cplx a, int e) {
+  const int m = e * (16 / EPT);                     // exp(-2 pi i m/32) = cos(pi m/16) - i sin(pi m/16)
+  const double cr = sfft_cos32(m), ci = -sfft_cos32(m < 8 ? 8 - m : m - 8) * (m < 8 ? 1.0 : 1.0);
+  // sin(pi m/16) = cos(pi (8 - m)/16) for m <= 8 and = cos(pi (m - 8)/16) for m >= 8
+  return cmake(fma(a.x, cr, -(a.y * ci)), fma(a.x, ci, a.y * cr));
+}
+
 template <int DIR>
 __device__ __forceinline__ void dft4(cplx& x0, cplx& x1, cplx& x2, cplx& x3) {
   cplx a = cadd(x0, x2), b = csub(x0, x2), c = cadd(x1, x3), d = mul_qi<DIR>(csub(x1, x3));

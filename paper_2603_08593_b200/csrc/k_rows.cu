@@ -213,11 +213,13 @@ __global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
     // is latency bound otherwise: one shared and one global load chain per bin)
     constexpr int NIT = (NC / 2) / TPR;
     constexpr int NBT = NIT >= SFFT_ROW_NBT ? SFFT_ROW_NBT : NIT;   // bins per batch (register budget: raw[] is live here)
+    // w^(tr + i TPR) = w^tr e^{-2 pi i i/(2 EPT)}: one table load per image, then constant products
+    cplx twrun = ldg2(P.twW + tr);
 #pragma unroll 1
     for (int i0 = 0; i0 < NIT; i0 += NBT) {
     cplx tws[NBT], zks[NBT], zms[NBT];
 #pragma unroll
-    for (int i = 0; i < NBT; ++i) tws[i] = ldg2(P.twW + tr + (i0 + i) * TPR);
+    for (int i = 0; i < NBT; ++i) { tws[i] = twrun; twrun = mul_split_root<EPT>(twrun, 1); }
 #pragma unroll
     for (int i = 0; i < NBT; ++i) {
       const int k = tr + (i0 + i) * TPR;
@@ -431,11 +433,13 @@ __global__ void __launch_bounds__(128, MINB) k_row2_fwd(RowFwdParams P) {
   cplx* out = P.T + ((size_t)im * (H / G) + y0 / G) * (size_t)(NC + 1) * G + (y0 % G);
   constexpr int NIT = (NC / 2) / TPR;
   constexpr int NBT = NIT >= SFFT_ROW_NBT ? SFFT_ROW_NBT : NIT;
+  // w^(tr + i TPR) = w^tr e^{-2 pi i i/(2 EPT)}: one table load, then constant products
+  cplx twrun = ldg2(P.twW + tr);
 #pragma unroll 1
   for (int i0 = 0; i0 < NIT; i0 += NBT) {
     cplx tws[NBT], zk[2][NBT], zm[2][NBT];
 #pragma unroll
-    for (int i = 0; i < NBT; ++i) tws[i] = ldg2(P.twW + tr + (i0 + i) * TPR);
+    for (int i = 0; i < NBT; ++i) { tws[i] = twrun; twrun = mul_split_root<EPT>(twrun, 1); }
 #pragma unroll
     for (int i = 0; i < NBT; ++i) {
       const int k = tr + (i0 + i) * TPR;
@@ -539,13 +543,15 @@ __global__ void __launch_bounds__(128, MINB) k_row_inv_sub(RowInvParams P) {
   cplx v[EPT];
   {
     cplx xk[EPT], xm[EPT], tw[EPT];
+    const cplx tw0 = ldg2(P.twW + tr);   // w^(tr + e TPR) = w^tr e^{-2 pi i e/(2 EPT)}: one table load, constant products
 #pragma unroll
     for (int e = 0; e < EPT; ++e) {
       const int k = tr + e * TPR;
       xk[e] = in[k];
       xm[e] = in[(NC - k) & (NC - 1)];
-      tw[e] = ldg2(P.twW + k);
     }
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) tw[e] = e == 0 ? tw0 : mul_split_root<EPT>(tw0, e);
 #pragma unroll
     for (int e = 0; e < EPT; ++e) {
       const int k = tr + e * TPR;
