@@ -48,6 +48,12 @@ struct RowFwdParams {
 #ifndef SFFT_ROW_MINB
 #define SFFT_ROW_MINB 3   // CTAs per SM the row kernels are compiled for
 #endif
+#ifndef SFFT_ROW2_MINB
+#define SFFT_ROW2_MINB 2  // ... the row-pair kernel of the fused build path: two CTAs per SM leave the side stream's
+#endif                    // kernel-background chain room beside it (0.186 -> 0.177 ms for the row pass, chain span 0.18 -> 0.13 ms)
+#ifndef SFFT_ROW2_NBT
+#define SFFT_ROW2_NBT 2   // bins of its split step loaded per batch
+#endif
 
 // v[e] = raw[e] * (x0^PW, x1^PW): x0 = xi(2j), x1 = xi(2j+1), j = tr + e*TPR; xi(2j) = xb + e*step
 // (all values are multiples of 1/W, so the affine form is exact).
@@ -432,7 +438,7 @@ __global__ void __launch_bounds__(128, MINB) k_row2_fwd(RowFwdParams P) {
   constexpr int G = SFFT_T_G;
   cplx* out = P.T + ((size_t)im * (H / G) + y0 / G) * (size_t)(NC + 1) * G + (y0 % G);
   constexpr int NIT = (NC / 2) / TPR;
-  constexpr int NBT = NIT >= SFFT_ROW_NBT ? SFFT_ROW_NBT : NIT;
+  constexpr int NBT = NIT >= SFFT_ROW2_NBT ? SFFT_ROW2_NBT : NIT;
   // w^(tr + i TPR) = w^tr e^{-2 pi i i/(2 EPT)}: one table load, then constant products
   cplx twrun = ldg2(P.twW + tr);
 #pragma unroll 1
@@ -636,7 +642,7 @@ static sfft_status launch_row2_fwd_t(const RowFwdParams& P, cudaStream_t st) {
   int nth = row_threads(NC, P.H / 2, C::EPT);
   const int RB = nth / (NC / C::EPT);
   const size_t smem = (size_t)2 * RB * C::SEQ_STRIDE * sizeof(cplx);
-  constexpr int MINB = SFFT_ROW_MINB;
+  constexpr int MINB = SFFT_ROW2_MINB;
   SFFT_CUDA_TRY(cudaFuncSetAttribute(k_row2_fwd<NC, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   k_row2_fwd<NC, MINB><<<(P.H / 2 / RB) * (P.nR + P.withS), nth, smem, st>>>(P);
   SFFT_LAUNCH_CHECK();
