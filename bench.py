@@ -686,8 +686,8 @@ def run_cuda(args, rank, world, local_rank):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture of the final
 # kernels of this round, summarised in NCU_SOURCE (null where that capture holds no such kernel).
 NCU_SOURCE = "profiles/r02_ncu_full.md"
-NCU_TRAFFIC = {"build.colx": 283.0e6, "build.row_fwd": 361.8e6, "subtract.row_fwd": 209.9e6, "subtract.mix": 267.3e6,
-               "subtract.row_inv": 172.3e6, "solve": 4.6e6}
+NCU_TRAFFIC = {"build.colx": 283.6e6, "build.row_fwd": 358.3e6, "subtract.row_fwd": 209.8e6, "subtract.mix": 254.3e6,
+               "subtract.row_inv": 171.9e6, "solve": 4.5e6}
 
 
 def main():
