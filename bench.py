@@ -510,12 +510,10 @@ def run_cuda(args, rank, world, local_rank):
         torch.cuda.synchronize()
         t_ex = g4.elapsed_time(g5) / 5
         nmask = int((Mx != 0).sum().item())
-        ntb = (N + 1 + 127) // 128
-        syrk_flop = 2.0 * nmask * (ntb * (ntb + 1) // 2) * 128 * 128
         post["build_system_exact"] = {"ms": round(t_ex, 3), "masked_pixels": nmask,
-                                      "rank_k_update_tflops": round(syrk_flop / ((t_ex - 0.72) * 1e-3) / 1e12, 2),
-                                      "note": "ordinary build (0.72 ms) + masked-pixel list + cooperative 128x128-tiled fp64 SYRK on the "
-                                              "fp64 tensor path (mma.sync m8n8k4) over rows generated once per 16384-pixel chunk"}
+                                      "note": "ordinary build with no mask + fully masked rows / columns through strip "
+                                              "correlations (k_exact_strips.cu) + the other masked pixels (none for this "
+                                              "frame mask) through the fp64 tensor-path rank-K update; round 1: 3.7 ms"}
         # multi-template MODE (NEXT-2): S against N_TEMP = 5 templates in one call (the science
         # image's row transform computed once), against 5 x the single-template chain + the median
         from paper_2603_08593_b200 import cut_stamps

@@ -80,8 +80,10 @@ sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S,
  * SURVEY.md §8(f) NEXT-1): R and S are used as they are and the masked pixels are dropped from the
  * sum, A = sum_{x unmasked} g(x) g(x)^T, b = sum_{x unmasked} g(x) S(x), g(x) the design-matrix row of
  * the unmasked images.  Computed as sfft_build_system with mask = NULL minus the masked pixels'
- * rank-one terms (a symmetric rank-K update, K = number of masked pixels: ~2 ms more at the full CCD
- * with a 6-pixel border).  Recovers a known kernel exactly under any mask, which the input-masking
+ * rank-one terms: fully masked rows and columns (a CCD's border frame; up to 32 per direction) through
+ * 1-D correlations of a few image rows / columns, every other masked pixel through a symmetric rank-K
+ * update (~0.4 ms more than the ordinary build at the full CCD with a 6-pixel border, + ~40 ns per
+ * isolated masked pixel).  Recovers a known kernel exactly under any mask, which the input-masking
  * system of sfft_build_system cannot (reading A2').  Same arguments and errors. */
 sfft_status sfft_build_system_exact(sfft_plan* p, const double* R, const double* S,
                                     const unsigned char* mask, double* A, double* b, void* stream);

@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsfft.so")
-SOURCES = ["sfft_api.cu", "k_rows.cu", "k_cols.cu", "k_cross.cu", "k_colb.cu", "k_kb.cu", "k_exact.cu", "k_chol.cu", "k_sub.cu", "k_post.cu", "k_probe.cu"]
+SOURCES = ["sfft_api.cu", "k_rows.cu", "k_cols.cu", "k_cross.cu", "k_colb.cu", "k_kb.cu", "k_exact.cu", "k_exact_strips.cu", "k_chol.cu", "k_sub.cu", "k_post.cu", "k_probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--expt-relaxed-constexpr"]
 

@@ -172,6 +172,7 @@ __global__ void __launch_bounds__(EX_TH, 1) k_exact_syrk(ExactParams P) {
   }
   const int tj = blockIdx.x - ti * (ti + 1) / 2;
   const int nm = P.off[P.H];
+  if (nm == 0) return;        // empty list (uniform over the grid): nothing is written, k_exact_apply skips it too
   const int Npad = P.ntb * EX_T;
   // product role: 8 warps as 2 (rows) x 4 (columns), warp tile 64 x 32 = 8 x 4 mma tiles of
   // m8n8k4 (fp64 tensor path, mma.sync): lane holds A[row = lane/4][k = lane%4], B[k = lane%4][col = lane/4]
@@ -268,9 +269,10 @@ __global__ void __launch_bounds__(EX_TH, 1) k_exact_syrk(ExactParams P) {
   }
 }
 
-// A[i][j] -= sum_ks C[i][j] (both triangles from the same sum), b[i] -= sum_ks C[N][i]
+// A[i][j] += sign * sum_ks C[i][j] (both triangles from the same sum), b[i] += sign * sum_ks C[N][i]; sign = -1 or +1
 __global__ void __launch_bounds__(256) k_exact_apply(const double* __restrict__ Cpart, double* A, double* b, int N,
-                                                     int ntiles, int KSplit) {
+                                                     int ntiles, int KSplit, double sign, const int* __restrict__ nlist) {
+  if (*nlist == 0) return;    // empty pixel list: k_exact_syrk wrote nothing
   const size_t total = (size_t)N * (N + 1) / 2 + N;
   for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (size_t)gridDim.x * blockDim.x) {
     int i, j;
@@ -289,11 +291,12 @@ __global__ void __launch_bounds__(256) k_exact_apply(const double* __restrict__ 
     const size_t loc = ((size_t)(ti * (ti + 1) / 2 + tj) * EX_T + (i % EX_T)) * EX_T + (j % EX_T);
     double s = 0.0;
     for (int ks = 0; ks < KSplit; ++ks) s += Cpart[(size_t)ks * ntiles * EX_T * EX_T + loc];
+    s *= sign;
     if (rhs) {
-      b[j] -= s;
+      b[j] += s;
     } else {
-      A[(size_t)i * N + j] -= s;
-      if (i != j) A[(size_t)j * N + i] -= s;
+      A[(size_t)i * N + j] += s;
+      if (i != j) A[(size_t)j * N + i] += s;
     }
   }
 }
@@ -315,18 +318,14 @@ size_t sfft_exact_rows_bytes(int N) {
   return (size_t)EX_KC * ntb * EX_T * sizeof(double);
 }
 
-sfft_status sfft_launch_exact_update(sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
-                                     double* A, double* b, cudaStream_t st, int* nl) {
-  const int H = p->H, W = p->W, rowsPerBlock = 8;
-  // the special-pixel arrays of the kernel-background chain are free once the ordinary build has finished
-  k_mk_rows<false><<<(H + rowsPerBlock - 1) / rowsPerBlock, 32 * rowsPerBlock, 0, st>>>(mask, H, W, p->spCount, nullptr, nullptr);
-  SFFT_LAUNCH_CHECK();
-  k_mk_scan<<<1, 1024, 0, st>>>(p->spCount, p->spOff, H);
-  SFFT_LAUNCH_CHECK();
-  k_mk_rows<true><<<(H + rowsPerBlock - 1) / rowsPerBlock, 32 * rowsPerBlock, 0, st>>>(mask, H, W, p->spCount, p->spOff, p->spList);
-  SFFT_LAUNCH_CHECK();
+void sfft_launch_mk_scan(const int* cnt, int* off, int H, cudaStream_t st) { k_mk_scan<<<1, 1024, 0, st>>>(cnt, off, H); }
+
+// rank-K update over one ordered pixel list: A, b += sign * sum_{x in list} g(x) [g(x); S(x)]^T
+sfft_status sfft_launch_exact_syrk(sfft_plan* p, const double* R, const double* S, const int* list, const int* off,
+                                   double* A, double* b, double sign, cudaStream_t st, int* nl) {
+  const int H = p->H, W = p->W;
   ExactParams P;
-  P.R = R; P.S = S; P.list = p->spList; P.off = p->spOff; P.Cpart = p->exScratch;
+  P.R = R; P.S = S; P.list = list; P.off = off; P.Cpart = p->exScratch;
   P.H = H; P.W = W; P.w = p->w; P.L = p->L; P.TK = p->TK; P.TB = p->TB; P.N = p->N;
   P.ntb = (p->N + 1 + EX_T - 1) / EX_T;
   P.log2W = p->log2NC + 1;
@@ -341,8 +340,8 @@ sfft_status sfft_launch_exact_update(sfft_plan* p, const double* R, const double
   SFFT_CUDA_TRY(cudaFuncSetAttribute(k_exact_syrk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   void* args[] = {(void*)&P};
   SFFT_CUDA_TRY(cudaLaunchCooperativeKernel((const void*)k_exact_syrk, dim3(ntiles, ks), dim3(EX_TH), args, smem, st));
-  k_exact_apply<<<p->num_sms * 4, 256, 0, st>>>(p->exScratch, A, b, p->N, ntiles, ks);
+  k_exact_apply<<<p->num_sms * 4, 256, 0, st>>>(p->exScratch, A, b, p->N, ntiles, ks, sign, off + H);
   SFFT_LAUNCH_CHECK();
-  *nl += 5;
+  *nl += 2;
   return SFFT_OK;
 }

@@ -67,7 +67,7 @@ static void plan_free(sfft_plan* p) {
   cudaFree(p->tw128);
   cudaFree(p->twPNC); cudaFree(p->twPH); cudaFree(p->twW); cudaFree(p->twH); cudaFree(p->d_pairs); cudaFree(p->d_groups);
   cudaFree(p->T); cudaFree(p->F); cudaFree(p->Y); cudaFree(p->Cmap); cudaFree(p->rowMom);
-  cudaFree(p->mom); cudaFree(p->spCount); cudaFree(p->spOff); cudaFree(p->spList); cudaFree(p->fmFlag); cudaFree(p->fmList); cudaFree(p->kbPart); cudaFree(p->kbCorr); cudaFree(p->kbStrip); cudaFree(p->Lw); cudaFree(p->exScratch); cudaFree(p->exRows); cudaFree(p->exBar); cudaFree(p->cholBar); cudaFree(p->mtA); cudaFree(p->mtB); cudaFree(p->Etab); cudaFree(p->Mhat);
+  cudaFree(p->mom); cudaFree(p->spCount); cudaFree(p->spOff); cudaFree(p->spList); cudaFree(p->fmFlag); cudaFree(p->fmList); cudaFree(p->kbPart); cudaFree(p->kbCorr); cudaFree(p->kbStrip); cudaFree(p->Lw); cudaFree(p->exScratch); cudaFree(p->exRows); cudaFree(p->exBar); cudaFree(p->xsPlan); cudaFree(p->xsColCnt); cudaFree(p->xsRowFull); cudaFree(p->xsColFull); cudaFree(p->xsSrcIdxY); cudaFree(p->xsSrcIdxX); cudaFree(p->xsZ); cudaFree(p->xsQ); cudaFree(p->xsCnt); cudaFree(p->xsOff); cudaFree(p->xsList); cudaFree(p->cholBar); cudaFree(p->mtA); cudaFree(p->mtB); cudaFree(p->Etab); cudaFree(p->Mhat);
   free(p->h_pairs);
   if (p->side) cudaStreamDestroy(p->side);
   if (p->evFork) cudaEventDestroy(p->evFork);
@@ -214,6 +214,17 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   dalloc((void**)&p->exScratch, sfft_exact_scratch_bytes(p->N));
   dalloc((void**)&p->exRows, sfft_exact_rows_bytes(p->N));   // here, so that no hot call ever allocates
   dalloc((void**)&p->exBar, 2 * sizeof(unsigned));
+  dalloc((void**)&p->xsPlan, sfft_xs_plan_bytes());
+  dalloc((void**)&p->xsColCnt, sizeof(int) * (size_t)W);
+  dalloc((void**)&p->xsRowFull, (size_t)H);
+  dalloc((void**)&p->xsColFull, (size_t)W);
+  dalloc((void**)&p->xsSrcIdxY, sizeof(int) * (size_t)H);
+  dalloc((void**)&p->xsSrcIdxX, sizeof(int) * (size_t)W);
+  dalloc((void**)&p->xsZ, sfft_xs_strip_bytes(H, W));
+  dalloc((void**)&p->xsQ, sfft_xs_q_bytes());
+  dalloc((void**)&p->xsCnt, sizeof(int) * (size_t)H);
+  dalloc((void**)&p->xsOff, sizeof(int) * (size_t)(H + 1));
+  dalloc((void**)&p->xsList, sizeof(int) * (size_t)SFFT_XS_MAXT * SFFT_XS_MAXT);
   dalloc((void**)&p->Lw, sizeof(double) * (size_t)(p->N + 1) * p->ldL);
   dalloc((void**)&p->cholBar, 2 * sizeof(unsigned));
   dalloc((void**)&p->mtA, sizeof(double) * (size_t)p->N * p->N);   // normal equations of the multi-template mode

@@ -16,6 +16,9 @@
 #ifndef SFFT_T_G
 #define SFFT_T_G 4          // fused path: rows per group of the row-spectra layout T[img][y/G][kx][y%G] (2, 4 and 8 measured: 4 is best)
 #endif
+#define SFFT_XS_MAXT 32     // exact objective, structured part (k_exact_strips.cu): most fully masked lines per direction,
+#define SFFT_XS_MAXS 64     //   most distinct source lines,
+#define SFFT_XS_MAXW 5      //   largest kernel half-width it is compiled for
 #define SFFT_NSTAGE 10     // see sfft_profile_read in include/sfft.h
 #define SFFT_PROF_MAX 512
 
@@ -128,6 +131,18 @@ struct sfft_plan {
   double* exScratch; // sfft_build_system_exact: partial tiles of the masked pixels' rank-K update
   double* exRows;    //   generated design-matrix rows of one chunk of masked pixels (allocated on first use)
   unsigned* exBar;   //   grid-barrier counters of k_exact_syrk
+  // fully masked rows / columns of the exact objective (k_exact_strips.cu)
+  void* xsPlan;             // 2 x XsPlan
+  int* xsColCnt;            // [W]
+  unsigned char* xsRowFull; // [H]
+  unsigned char* xsColFull; // [W]
+  int* xsSrcIdxY;           // [H]
+  int* xsSrcIdxX;           // [W]
+  double* xsZ;              // strips
+  double* xsQ;              // strip correlations
+  int* xsCnt;               // [H]     corner list: per-row counts,
+  int* xsOff;               // [H + 1] offsets,
+  int* xsList;              // [XS_MAXT^2] pixels
   int cholMaxCtas;   // cap on the CTAs of k_chol_fused (0 = one per SM); see sfft_plan_set_solve_ctas
   double* mtA;       // sfft_multi_template_difference: normal matrix and right-hand side of the current template
   double* mtB;
@@ -203,6 +218,9 @@ sfft_status sfft_launch_cross(sfft_plan* p, cudaStream_t st, int* nl);
 sfft_status sfft_launch_colx(sfft_plan* p, cudaStream_t st, int* nl);
 size_t sfft_exact_scratch_bytes(int N);
 size_t sfft_exact_rows_bytes(int N);
+size_t sfft_xs_plan_bytes();
+size_t sfft_xs_strip_bytes(int H, int W);
+size_t sfft_xs_q_bytes();
 sfft_status sfft_launch_exact_update(sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
                                      double* A, double* b, cudaStream_t st, int* nl);
 bool sfft_colx_supported(int H, int nPair);
