@@ -286,6 +286,39 @@ def test_exact_objective_parity(H, W, w, DK, DB, border):
         assert torch.equal(A0, A1) and torch.equal(b0, b1)
 
 
+@pytest.mark.parametrize("H,W,w,DK,DB,kind", [
+    (128, 128, 2, 1, 1, "frame+lines"), (64, 256, 3, 2, 2, "frame+lines"), (256, 64, 1, 2, 0, "many_rows"),
+    (128, 64, 5, 1, 1, "scattered_rows"), (64, 64, 0, 2, 2, "frame+lines"), (128, 128, 2, 0, 3, "cols_only")])
+def test_exact_objective_structured_masks(H, W, w, DK, DB, kind):
+    """The structured part of sfft_build_system_exact (fully masked rows / columns through strip
+    correlations, corners added back, the rest through the pixel list) against the oracle: frames with
+    extra full lines in the interior and isolated pixels; more full rows than the strip path accepts
+    (the surplus stays in the pixel list); full rows so far apart that the source-line cap is hit;
+    w = 0; columns only."""
+    rng = np.random.default_rng(7 * H + W + w)
+    R = 50.0 * rng.standard_normal((H, W)) + 500.0 * (rng.random((H, W)) > 0.98)
+    S = 0.7 * np.roll(R, (1 if w else 0, -1 if w else 0), (0, 1)) + 30.0 * rng.standard_normal((H, W)) + 200.0
+    mask = (rng.random((H, W)) < 0.02).astype(np.uint8)
+    if kind == "frame+lines":
+        mask[:3] = 1; mask[-2:] = 1; mask[:, :2] = 1; mask[:, -3:] = 1
+        mask[H // 2] = 1; mask[:, W // 3] = 1; mask[:, W // 3 + 1] = 1
+    elif kind == "many_rows":
+        mask[10:50] = 1                      # 40 full rows: 32 take the strip path
+        mask[:, 5] = 1
+    elif kind == "scattered_rows":
+        mask[::16] = 1                       # 8 isolated full rows, 11 source rows each: the 64-line cap is hit
+    elif kind == "cols_only":
+        mask[:, 7:11] = 1; mask[:, -1] = 1
+    Ao, bo = orc.build_system_exact_fft(R, S, mask, w, DK, DB, workers=8)
+    with SfftPlan(H, W, w, DK, DB) as plan:
+        A, b = plan.build_system_exact(dev(R), dev(S), dev(mask))
+        A2, b2 = plan.build_system_exact(dev(R), dev(S), dev(mask))
+        assert torch.equal(A, A2) and torch.equal(b, b2)          # reproducible
+        L = (2 * w + 1) ** 2
+        TK = (DK + 1) * (DK + 2) // 2
+        check_system(A.cpu().numpy(), b.cpu().numpy(), Ao, bo, L, TK)
+
+
 def test_exact_objective_recovers_kernel_under_mask_on_gpu():
     """S = M(R; c0) with a border + random mask: the exact objective returns c0 to 1e-9 and D = 0 on
     the GPU path alone; the input-masking system does not (reading A2')."""
