@@ -20,24 +20,26 @@
 // of the row spectra T (k_row2_fwd), f = eta^q T_p for every kernel monomial t = (p,q) ("centre" AND
 // "extended" version: 2 TK sequences) and g = the row spectrum of m S ("extended" only).
 //
-// One persistent CTA per SM (columns round-robin), 12 warps; after the prologue the warps meet only at
-// mbarriers while a column is in flight, and at three block barriers per column for its final inverse.
-// Every warp does both kinds of work:
-//   transform "tasks" of four sequences, warp-synchronously: each half warp (lane j < 16) takes the 8 x 16
-//            block elements n = j + 16 r of its row image from global memory (requested one task ahead,
-//            registers only), and per sequence weights them by eta^q, zero-pads (centre version), runs the
-//            radix-8 butterfly over r, multiplies by w128^(j k1) and stores to the block's slot of the
-//            shared-memory ring; after a __syncwarp the 32 lanes run the radix-16 butterflies over j of
-//            the four sequences (X[k1 + 8 k2]) in place, and lane 0 arrives on the slot's "full" barrier.
-//            The science sequence (one per block) is batched over four consecutive blocks into a task of
-//            its own.  Task g of the CTA's task list (all its columns, block by block) runs on warp g mod 12;
-//   products thread = (frequency k, third of the pairs): once a slot is full the thread accumulates its
-//            pairs' products conj(C_t) E_t2 of that block in registers (6-7 operand loads per 9 pairs) and
-//            the warp arrives on the slot's "empty" barrier (12 arrivals free it).
-// A warp runs transform tasks while the block its products wait for is not full yet, so the two kinds of
-// work interleave on every scheduler and the ring (CB_NSLOT blocks) lets the transforms run ahead, also
-// across the column boundary.  End of a column: accumulators -> shared memory, 16-point inverse over b
-// (k = a + 8 b), then the 2D+1 lags of every pair (8 twiddled terms each) -> Y[pair][dy][kx].
+// One persistent CTA per SM (columns round-robin), 16 warps in two ROLES that meet only at mbarriers (no
+// block-wide barrier after the prologue); registers are rebalanced between the warpgroups with setmaxnreg:
+//   transform warps (12, 120 registers)  run "tasks" of four sequences, warp-synchronously: each half warp
+//            (lane j < 16) takes the 8 x 16 block elements n = j + 16 r of its row image from global memory
+//            (requested one task ahead: CB_PREG in registers, the rest by cp.async, issued after the
+//            radix-16 pass has issued its shared-memory loads), and per sequence weights them by eta^q,
+//            zero-pads (centre version), runs the radix-8 butterfly over r, multiplies by w128^(j k1) and
+//            stores to the block's slot of the shared-memory ring; after a __syncwarp the 32 lanes run the
+//            radix-16 butterflies over j of the four sequences (X[k1 + 8 k2]) in place, and lane 0 arrives
+//            on the slot's "full" barrier.  Task g of the CTA's task list (all its columns, block by block)
+//            runs on warp g mod 12.  The science sequence (one per block) is batched over four consecutive
+//            blocks into a task of its own and goes to a ring of its own (CB_NS2 blocks), so that it never
+//            waits for the main ring;
+//   product warps (4, 152 registers)  thread = frequency k; they wait for a slot to be full, read each of its
+//            2TK+1 spectra ONCE and accumulate all TK(TK+1)/2 + TK pair products conj(C_t) E_t2 in registers
+//            over the blocks of a column, then free the slot ("empty" barrier).  End of a column:
+//            accumulators -> shared memory (two passes over half of the pairs), 16-point inverse over b
+//            (k = a + 8 b), the 2D+1 lags of every pair (8 twiddled terms each) -> Y[pair][dy][kx].
+// The ring holds CB_NSLOT blocks, so the transforms run up to CB_NSLOT blocks ahead of the products, also
+// across the column boundary; both roles issue to the same fp64 pipes at the same time.
 // Shared-memory positions are XOR-swizzled (slot k1*16 + (j ^ k1)): every pass is conflict free with no
 // padding.  T has the row-group layout T[img][y/G][kx][y%G], G = SFFT_T_G = 4 (k_row2_fwd): a half warp's
 // 16 rows of a column are four 64-byte runs.
@@ -46,7 +48,6 @@
 
 #define CB_N 128          // block transform length
 #define CB_TH 512         // 16 warps = 4 warpgroups: 3 transform + 1 product (registers rebalanced by setmaxnreg)
-#define CB_NW (CB_TH / 32)
 #define CB_FW 12          // transform warps
 #ifndef CB_PREG
 #define CB_PREG 5           // block elements (of 8) a transform lane prefetches into registers (the rest: cp.async)
@@ -124,57 +125,6 @@ __device__ __forceinline__ size_t cb_toff(int y, size_t grpStride) {
   return (size_t)(y / SFFT_T_G) * grpStride + (size_t)(y % SFFT_T_G);
 }
 
-// Pair partition of the products.  Part (T0, T1, U0, U1) owns the pairs (t, t2), T0 <= t < T1,
-// max(t, U0) <= t2 <= U1 (t2 = TK stands for S~).  For TK = 6 the three parts hold 9 pairs each and
-// read 7, 6 and 7 operands: (C0-2 x E0-3), (C0-2 x E4,5,S), (C3-5 x E3,4,5,S).
-template <int TK> struct CbParts;
-template <> struct CbParts<6> { static constexpr int T0[3] = {0, 0, 3}, T1[3] = {3, 3, 6}, U0[3] = {0, 4, 3}, U1[3] = {3, 6, 6}; };
-template <> struct CbParts<3> { static constexpr int T0[3] = {0, 1, 2}, T1[3] = {1, 2, 3}, U0[3] = {0, 1, 2}, U1[3] = {3, 3, 3}; };
-template <> struct CbParts<1> { static constexpr int T0[3] = {0, 0, 0}, T1[3] = {1, 0, 0}, U0[3] = {0, 0, 0}, U1[3] = {1, 0, 0}; };
-__host__ __device__ constexpr int cb_max(int a, int b) { return a > b ? a : b; }
-__host__ __device__ constexpr int cb_part_pairs(int T0, int T1, int U0, int U1) {
-  int n = 0;
-  for (int t = T0; t < T1; ++t)
-    for (int t2 = cb_max(t, U0); t2 <= U1; ++t2) ++n;
-  return n;
-}
-
-// products of one block: acc[] += conj(C_t) E_t2 over the part's pairs, every operand read once
-template <int TK, int T0, int T1, int U0, int U1>
-__device__ __forceinline__ void cb_accumulate(cplx* acc, const cplx* __restrict__ ub, int pk) {
-  cplx C[TK], E[TK + 1];
-#pragma unroll
-  for (int t = T0; t < T1; ++t) C[t] = ub[t * CB_N + pk];
-#pragma unroll
-  for (int t2 = cb_max(T0, U0); t2 <= U1; ++t2) E[t2] = ub[(TK + t2) * CB_N + pk];
-  int idx = 0;
-#pragma unroll
-  for (int t = T0; t < T1; ++t) {
-#pragma unroll
-    for (int t2 = cb_max(t, U0); t2 <= U1; ++t2) {
-      cfmac(acc[idx], C[t], E[t2]);
-      ++idx;
-    }
-  }
-}
-
-// the part's accumulators -> shared memory acs[pair][k] (pair index of the plan's list: kernel-kernel
-// pairs (t <= t2) row-major upper-triangular, then (t, S) at nKK + t)
-template <int TK, int T0, int T1, int U0, int U1>
-__device__ __forceinline__ void cb_flush(const cplx* acc, cplx* acs, int k) {
-  constexpr int NKK = TK * (TK + 1) / 2;
-  int idx = 0;
-#pragma unroll
-  for (int t = T0; t < T1; ++t) {
-#pragma unroll
-    for (int t2 = cb_max(t, U0); t2 <= U1; ++t2) {
-      const int pair = (t2 < TK) ? (t * TK - t * (t - 1) / 2 + (t2 - t)) : (NKK + t);
-      acs[pair * CB_N + k] = acc[idx];
-      ++idx;
-    }
-  }
-}
-
 // ---- mbarrier helpers (CTA scope; `a` = 32-bit shared-memory address of the barrier) -------------------
 __device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned a, unsigned count) {
@@ -239,10 +189,6 @@ __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
   constexpr int NSEQ = 2 * TK + 1;
   constexpr int NPAIR = TK * (TK + 1) / 2 + TK;
   using TT = CbTasks<TK>;
-  using PT = CbParts<TK>;
-  constexpr int NACC = cb_max(cb_max(cb_part_pairs(PT::T0[0], PT::T1[0], PT::U0[0], PT::U1[0]),
-                                     cb_part_pairs(PT::T0[1], PT::T1[1], PT::U0[1], PT::U1[1])),
-                              cb_max(cb_part_pairs(PT::T0[2], PT::T1[2], PT::U0[2], PT::U1[2]), 1));
   constexpr unsigned FULL_COUNT = TT::NT;                         // lane-0 arrivals that complete a block
   constexpr int NGRP_T = TT::STASK ? (1 + 4 * TT::NT) : TT::NT;   // tasks of a group of 4 blocks (or of one block)
   constexpr int NSEQ_R = TT::STASK ? NSEQ - 1 : NSEQ;             // sequences per slot of the main ring
