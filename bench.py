@@ -30,7 +30,7 @@ if ROOT not in sys.path:
 METRIC = "SFFT subtractions/sec per 2048x4096 fp64 CCD"
 UNIT = "CCD/s"
 WORKLOAD = "full DECam CCD (BASELINE.json configs[3]): 2048x4096 fp64, w=5, DK=2, DB=2, N=732"
-SOLVE_CTAS_PIPELINED = 48   # sfft_plan_set_solve_ctas for the multi-plan legs (e2e, exposure)
+SOLVE_CTAS_PIPELINED = 16   # sfft_plan_set_solve_ctas for the multi-plan legs (e2e, exposure); 8..74 swept: 16 is best
 NPAIR = 3  # distinct resident pairs cycled through (3 x 143 MB of inputs > 126 MB L2)
 
 # fp64-pipe peak derived from unit counts and clocks: 148 SMs x 4 SMSPs x 16
@@ -284,6 +284,7 @@ def run_exposure(torch, synth, cfg, plans, streams, nccd):
             R, S, M = dev[k]
             st, pl = streams[s], plans[s]
             pl.build_system(R, S, M, As[s], bs[s], stream=st)
+            pl.subtract_prepare(R, stream=st)
             pl.solve(As[s], bs[s], cs[k], infos[k:k + 1], stream=st)
             pl.subtract(R, S, cs[k], Ds[k], stream=st)
 
@@ -313,6 +314,7 @@ def run_exposure(torch, synth, cfg, plans, streams, nccd):
                     for d, h in zip((R, S, M), hostp[k]):
                         d.copy_(h, non_blocking=True)
                 pl.build_system(R, S, M, As[s], bs[s], stream=st)
+                pl.subtract_prepare(R, stream=st)
                 pl.solve(As[s], bs[s], cs[k], infos[k:k + 1], stream=st)
                 pl.subtract(R, S, cs[k], Ds[k], stream=st)
 

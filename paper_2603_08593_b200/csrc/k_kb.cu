@@ -21,7 +21,9 @@
 #include "sfft_common.cuh"
 
 #define KB_TH 128
+#ifndef KB_CH
 #define KB_CH 128   // special pixels staged per chunk
+#endif
 
 // Monomial t of the order "for d: for q <= d: p = d - q" as compile-time functions, so that the
 // unrolled loops below multiply by register-held powers without any table lookups.

@@ -372,7 +372,7 @@ def test_exact_objective_full_config_sampled():
 def test_exposure_configuration_three_plans_in_flight():
     """The launch configuration bench.py's exposure and end-to-end legs time (BASELINE.json configs[4];
     PAPER.md:324, a GPU works through a queue of CCDs): 3 plans on 3 streams in flight at once,
-    sfft_plan_set_solve_ctas(48), no sfft_subtract_prepare, exposure-recipe pairs (seed 2000+k) at the
+    sfft_plan_set_solve_ctas(16), sfft_subtract_prepare before the solve, exposure-recipe pairs (seed 2000+k) at the
     extremes of the recipe (sky 800 / FWHM 6 and sky 3000 / FWHM 3.5) plus one mid draw.  A, b, c, D of
     the two extreme pairs against the oracle at the A5 tolerances, and every pair bitwise equal to the
     same pair run alone on one plan with the default solve grid (sfft.h: "Results are bitwise
@@ -388,7 +388,7 @@ def test_exposure_configuration_three_plans_in_flight():
     outs = []
     try:
         for pl in plans:
-            pl.set_solve_ctas(48)
+            pl.set_solve_ctas(16)
         torch.cuda.synchronize()
         res = [None] * len(prs)
         for rep in range(2):                      # second round: every plan's scratch has been used once
@@ -396,6 +396,7 @@ def test_exposure_configuration_three_plans_in_flight():
                 R, S, M = devp[k]
                 with torch.cuda.stream(st):
                     A, b = pl.build_system(R, S, M, stream=st)
+                    pl.subtract_prepare(R, stream=st)
                     c, info = pl.solve(A, b, stream=st)
                     D = pl.subtract(R, S, c, stream=st)
                 res[k] = (A, b, c, info, D)
