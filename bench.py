@@ -461,6 +461,7 @@ def run_cuda(args, rank, world, local_rank):
 
     # ---- the two steps after the differencing, timed alone on the device
     post = None
+    plan.set_solve_ctas(0)   # the single-plan legs below run with the default solve grid again
     if world == 1:
         from paper_2603_08593_b200 import aperture_stats, median_combine
         nT = 5   # N_TEMP default
@@ -577,6 +578,7 @@ def run_cuda(args, rank, world, local_rank):
     if world == 1 and args.exposure_ccds > 0:
         for pl in plans:
             pl._stage = None
+            pl.set_solve_ctas(SOLVE_CTAS_PIPELINED)
         torch.cuda.empty_cache()
         exposure = run_exposure(torch, synth, cfg, plans, streams, args.exposure_ccds)
 
@@ -696,7 +698,7 @@ def run_cuda(args, rank, world, local_rank):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture of the final
 # kernels of this round, summarised in NCU_SOURCE (null where that capture holds no such kernel).
 NCU_SOURCE = "profiles/r02_ncu_full.md"
-NCU_TRAFFIC = {"build.colx": 283.6e6, "build.row_fwd": 358.3e6, "subtract.row_fwd": 209.8e6, "subtract.mix": 254.3e6,
+NCU_TRAFFIC = {"build.colx": 283.8e6, "build.row_fwd": 359.6e6, "subtract.row_fwd": 209.9e6, "subtract.mix": 254.5e6,
                "subtract.row_inv": 171.9e6, "solve": 4.5e6}
 
 
