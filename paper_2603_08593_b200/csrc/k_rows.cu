@@ -48,13 +48,6 @@ struct RowFwdParams {
 #ifndef SFFT_ROW_MINB
 #define SFFT_ROW_MINB 3   // CTAs per SM the row kernels are compiled for
 #endif
-#ifndef SFFT_ROW2_MINB
-#define SFFT_ROW2_MINB 2  // ... the row-pair kernel of the fused build path: two CTAs per SM leave the side stream's
-#endif                    // kernel-background chain room beside it (0.186 -> 0.177 ms for the row pass, chain span 0.18 -> 0.13 ms)
-#ifndef SFFT_ROW2_NBT
-#define SFFT_ROW2_NBT 2   // bins of its split step loaded per batch
-#endif
-
 // v[e] = raw[e] * (x0^PW, x1^PW): x0 = xi(2j), x1 = xi(2j+1), j = tr + e*TPR; xi(2j) = xb + e*step
 // (all values are multiples of 1/W, so the affine form is exact).
 template <int EPT, int PW>
@@ -286,229 +279,197 @@ __global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
 
 
 // ------------------------------------------------------------------------------------------------
-// Row pass of the fused build path: one CTA = one image (blockIdx.x % nimg) of RB row PAIRS (2b, 2b+1).
-// The two rows of a pair are transformed one after the other into two shared-memory buffers and leave
-// the CTA together: the split step writes, per column kx, the 32-byte pair {X_2b[kx], X_2b+1[kx]} into
-// the row-group layout T[img][y/G][kx][y%G] (G = SFFT_T_G rows of one column are contiguous; kx in
-// [0, NC]) -- whole 32-byte sectors, G/2 row pairs filling a 16 G-byte run that k_colb reads along y.
-// Row 2b's inputs go from global memory through the weighting into the first butterfly (registers
-// only); row 2b+1's inputs are requested at the same time by cp.async into the second buffer (free
-// until that row's first pass), so no global-memory latency is exposed between the two transforms.
-// Fused reductions as in k_row_fwd.
-__device__ __forceinline__ void row_cp_async16(void* smem_dst, const void* gsrc) {
-  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gsrc) : "memory");
-}
+// Row pass of the fused build path: one CTA = one image (blockIdx.x % nimg, so the images of a pair run
+// side by side and R stays in L2) of RB row PAIRS (2b, 2b+1), 2 RB TPR threads (256 at W = 4096), thread =
+// (pair, row of the pair, tr).  The two rows of a pair are transformed side by side -- both go from global
+// memory through the weighting into their first butterflies (registers only), the passes run on 2 RB
+// sequences at once -- and leave the CTA together: the split step is shared, a thread takes half of its
+// tr's bins for BOTH rows and writes, per column kx, the 32-byte pair {X_2b[kx], X_2b+1[kx]} into the
+// row-group layout T[img][y/G][kx][y%G] (G = SFFT_T_G rows of one column are contiguous; kx in [0, NC]):
+// whole 32-byte sectors, G/2 row pairs filling a 16 G-byte run that k_colb reads along y.  128 registers,
+// two CTAs = 16 warps per SM (the kernel is latency-bound; a variant that transformed the two rows one
+// after the other in 128-thread CTAs, the second row staged by cp.async, had 8-12 warps per SM and took
+// 0.175 instead of 0.165 ms).  Fused reductions as in k_row_fwd.
 __device__ __forceinline__ void row_st_pair(cplx* dst, cplx a, cplx b) {   // 32-byte streaming store
   asm volatile("st.global.cs.v4.f64 [%0], {%1, %2, %3, %4};\n" ::"l"(dst), "d"(a.x), "d"(a.y), "d"(b.x), "d"(b.y) : "memory");
 }
 
 template <int NC, int MINB>
-__global__ void __launch_bounds__(128, MINB) k_row2_fwd(RowFwdParams P) {
+__global__ void __launch_bounds__(256, MINB) k_row2_fwd(RowFwdParams P) {
   using C = FftCfg<NC>;
   constexpr int EPT = C::EPT;
   constexpr int TPR = NC / EPT;  // threads per row
   constexpr int LW = TPR < 32 ? TPR : 32;           // lanes of one row inside a warp
   constexpr int WPR = TPR / 32 > 0 ? TPR / 32 : 1;  // warps per row
-  constexpr int NSLOT = 128 / LW;                   // (pair, warp-of-row) slots of a CTA
+  constexpr int NSLOT = 256 / LW;                   // (row, warp-of-row) slots of a CTA
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  __shared__ double redM[2][ROW_NMA][NSLOT];
-  __shared__ double redX[2][SFFT_MAX_DEG][NSLOT];
+  __shared__ double redM[ROW_NMA][NSLOT];
+  __shared__ double redX[SFFT_MAX_DEG][NSLOT];
   cplx* s = reinterpret_cast<cplx*>(smem_raw);
   const int tid = threadIdx.x, nth = blockDim.x;
-  const int RB = nth / TPR;
-  const int r = tid / TPR, tr = tid - r * TPR;
+  const int nseq = nth / TPR;                       // rows of the CTA = 2 RB
+  const int seq = tid / TPR, tr = tid - seq * TPR;
+  const int pr = seq >> 1, rr = seq & 1;
   const int nimg = P.nR + P.withS;
   const int im = blockIdx.x % nimg;                 // images of one pair run side by side (R rows stay in L2)
-  const int pairIdx = (blockIdx.x / nimg) * RB + r;
-  const int y0 = 2 * pairIdx;
+  const int pairIdx = (blockIdx.x / nimg) * (nseq >> 1) + pr;
+  const int y0 = 2 * pairIdx, y = y0 + rr;
   const int W = P.W, H = P.H;
   const double invW = 1.0 / (double)W;
   const double xb = (double)(4 * tr + 1 - W) * invW, step = (double)(4 * TPR) * invW, dx1 = 2.0 * invW;
   const int slot = tid / LW;
   const int pw = im < P.nR ? im : 0;
-  const double* src = (im < P.nR ? P.R : P.S) + (size_t)y0 * W;
-  cplx* buf[2] = {s, s + RB * C::SEQ_STRIDE};
-  cplx* raw1s = buf[1] + r * C::SEQ_STRIDE;         // row 2b+1's inputs, unpadded, until its first pass
+  const double* src = (im < P.nR ? P.R : P.S) + (size_t)y * W;
 
-#pragma unroll
-  for (int e = 0; e < EPT; ++e) row_cp_async16(raw1s + tr + e * TPR, src + W + 2 * (tr + e * TPR));
-  asm volatile("cp.async.commit_group;\n" ::: "memory");
   double2 raw[EPT];
 #pragma unroll
   for (int e = 0; e < EPT; ++e) raw[e] = ROW_LD(reinterpret_cast<const double2*>(src + 2 * (tr + e * TPR)));
-
-  // mask bits of both rows: bit 2e = element 2j masked, bit 2e+1 = element 2j+1 masked, j = tr + e*TPR
-  unsigned mbits[2] = {0u, 0u};
+  // mask bits: bit 2e = element 2j masked, bit 2e+1 = element 2j+1 masked, j = tr + e*TPR
+  unsigned mbits = 0u;
   if (P.mask) {
-    uchar2 mk[2][EPT];
+    uchar2 mk[EPT];
 #pragma unroll
-    for (int rr = 0; rr < 2; ++rr)
+    for (int e = 0; e < EPT; ++e) mk[e] = *reinterpret_cast<const uchar2*>(P.mask + (size_t)y * W + 2 * (tr + e * TPR));
 #pragma unroll
-      for (int e = 0; e < EPT; ++e)
-        mk[rr][e] = *reinterpret_cast<const uchar2*>(P.mask + (size_t)(y0 + rr) * W + 2 * (tr + e * TPR));
-#pragma unroll
-    for (int rr = 0; rr < 2; ++rr)
-#pragma unroll
-      for (int e = 0; e < EPT; ++e)
-        mbits[rr] |= (mk[rr][e].x ? 1u : 0u) << (2 * e) | (mk[rr][e].y ? 1u : 0u) << (2 * e + 1);
+    for (int e = 0; e < EPT; ++e) mbits |= (mk[e].x ? 1u : 0u) << (2 * e) | (mk[e].y ? 1u : 0u) << (2 * e + 1);
   }
   const bool momA = P.moments && im == 0;
   if (momA) {
     // masked part of sum_x m xi^a: only warps that hold a masked pixel do any work
+    double ms[ROW_NMA];
 #pragma unroll
-    for (int rr = 0; rr < 2; ++rr) {
-      double ms[ROW_NMA];
+    for (int a = 0; a < ROW_NMA; ++a) ms[a] = 0.0;
+    if (__any_sync(0xffffffffu, mbits != 0u)) {
+      unsigned mm = mbits;
+      while (mm) {
+        const int bit = __ffs(mm) - 1;
+        mm &= mm - 1;
+        const int j = tr + (bit >> 1) * TPR;
+        const double x = (double)(4 * j + 1 + 2 * (bit & 1) - W) * invW;
+        double pwr = 1.0;
 #pragma unroll
-      for (int a = 0; a < ROW_NMA; ++a) ms[a] = 0.0;
-      if (__any_sync(0xffffffffu, mbits[rr] != 0u)) {
-        unsigned mm = mbits[rr];
-        while (mm) {
-          const int bit = __ffs(mm) - 1;
-          mm &= mm - 1;
-          const int j = tr + (bit >> 1) * TPR;
-          const double x = (double)(4 * j + 1 + 2 * (bit & 1) - W) * invW;
-          double pwr = 1.0;
-#pragma unroll
-          for (int a = 0; a < ROW_NMA; ++a) { ms[a] += pwr; pwr *= x; }
-        }
-#pragma unroll
-        for (int a = 0; a < ROW_NMA; ++a) {
-#pragma unroll
-          for (int off = LW / 2; off > 0; off >>= 1) ms[a] += __shfl_xor_sync(0xffffffffu, ms[a], off);
-        }
+        for (int a = 0; a < ROW_NMA; ++a) { ms[a] += pwr; pwr *= x; }
       }
-      if ((tid & (LW - 1)) == 0) {
 #pragma unroll
-        for (int a = 0; a < ROW_NMA; ++a) redM[rr][a][slot] = ms[a];
+      for (int a = 0; a < ROW_NMA; ++a) {
+#pragma unroll
+        for (int off = LW / 2; off > 0; off >>= 1) ms[a] += __shfl_xor_sync(0xffffffffu, ms[a], off);
       }
     }
+    if ((tid & (LW - 1)) == 0) {
+#pragma unroll
+      for (int a = 0; a < ROW_NMA; ++a) redM[a][slot] = ms[a];
+    }
+  }
+  if (mbits) {
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+      if ((mbits >> (2 * e)) & 1u) raw[e].x = 0.0;
+      if ((mbits >> (2 * e + 1)) & 1u) raw[e].y = 0.0;
+    }
+  }
+  cplx v[EPT];
+  switch (pw) {
+    case 0:
+#pragma unroll
+      for (int e = 0; e < EPT; ++e) v[e] = raw[e];
+      break;
+    case 1: row_weight<EPT, 1>(raw, v, xb, step, dx1); break;
+    case 2: row_weight<EPT, 2>(raw, v, xb, step, dx1); break;
+    default: row_weight<EPT, 3>(raw, v, xb, step, dx1); break;
   }
   const bool extra = P.moments && P.DB > 0 && im >= P.nR - 1;
-
-#pragma unroll
-  for (int rr = 0; rr < 2; ++rr) {
-    if (rr == 1) {
-      asm volatile("cp.async.wait_all;\n" ::: "memory");   // the thread's own copies have landed
-#pragma unroll
-      for (int e = 0; e < EPT; ++e) raw[e] = raw1s[tr + e * TPR];
-      __syncthreads();                                      // every thread holds its inputs: the buffer may be rewritten
+  if (extra) {
+    double hi[SFFT_MAX_DEG];
+    switch (P.DB) {
+      case 1: row_extra_moments<EPT, 1>(v, xb, step, dx1, hi); break;
+      case 2: row_extra_moments<EPT, 2>(v, xb, step, dx1, hi); break;
+      default: row_extra_moments<EPT, 3>(v, xb, step, dx1, hi); break;
     }
-    if (mbits[rr]) {
 #pragma unroll
-      for (int e = 0; e < EPT; ++e) {
-        if ((mbits[rr] >> (2 * e)) & 1u) raw[e].x = 0.0;
-        if ((mbits[rr] >> (2 * e + 1)) & 1u) raw[e].y = 0.0;
-      }
+    for (int i = 0; i < SFFT_MAX_DEG; ++i) {
+#pragma unroll
+      for (int off = LW / 2; off > 0; off >>= 1) hi[i] += __shfl_xor_sync(0xffffffffu, hi[i], off);
     }
-    cplx v[EPT];
-    switch (pw) {
-      case 0:
+    if ((tid & (LW - 1)) == 0) {
 #pragma unroll
-        for (int e = 0; e < EPT; ++e) v[e] = raw[e];
-        break;
-      case 1: row_weight<EPT, 1>(raw, v, xb, step, dx1); break;
-      case 2: row_weight<EPT, 2>(raw, v, xb, step, dx1); break;
-      default: row_weight<EPT, 3>(raw, v, xb, step, dx1); break;
+      for (int i = 0; i < SFFT_MAX_DEG; ++i) redX[i][slot] = hi[i];
     }
-    if (extra) {
-      double hi[SFFT_MAX_DEG];
-      switch (P.DB) {
-        case 1: row_extra_moments<EPT, 1>(v, xb, step, dx1, hi); break;
-        case 2: row_extra_moments<EPT, 2>(v, xb, step, dx1, hi); break;
-        default: row_extra_moments<EPT, 3>(v, xb, step, dx1, hi); break;
-      }
-#pragma unroll
-      for (int i = 0; i < SFFT_MAX_DEG; ++i) {
-#pragma unroll
-        for (int off = LW / 2; off > 0; off >>= 1) hi[i] += __shfl_xor_sync(0xffffffffu, hi[i], off);
-      }
-      if ((tid & (LW - 1)) == 0) {
-#pragma unroll
-        for (int i = 0; i < SFFT_MAX_DEG; ++i) redX[rr][i][slot] = hi[i];
-      }
-    }
-    fft_regs_to_smem<NC, -1, false>(v, buf[rr], tid, nth, RB, P.twP, C::SEQ_STRIDE);
   }
+  fft_regs_to_smem<NC, -1, false>(v, s, tid, nth, nseq, P.twP, C::SEQ_STRIDE);
 
-  // split of both rows: X[k] = Xe + w^k Xo, X[NC-k] = conj(Xe - w^k Xo), w = e^{-2 pi i / W}
-  const cplx* sA = buf[0] + r * C::SEQ_STRIDE;
-  const cplx* sB = buf[1] + r * C::SEQ_STRIDE;
-  // T[img][y/G][kx][y%G]: column k of the pair's rows at out + G k
+  // split of both rows of the pair; this thread: half rr of tr's bins
+  const cplx* sA = s + (2 * pr) * C::SEQ_STRIDE;
+  const cplx* sB = sA + C::SEQ_STRIDE;
   constexpr int G = SFFT_T_G;
-  cplx* out = P.T + ((size_t)im * (H / G) + y0 / G) * (size_t)(NC + 1) * G + (y0 % G);
-  constexpr int NIT = (NC / 2) / TPR;
-  constexpr int NBT = NIT >= SFFT_ROW2_NBT ? SFFT_ROW2_NBT : NIT;
-  // w^(tr + i TPR) = w^tr e^{-2 pi i i/(2 EPT)}: one table load, then constant products
-  cplx twrun = ldg2(P.twW + tr);
-#pragma unroll 1
-  for (int i0 = 0; i0 < NIT; i0 += NBT) {
-    cplx tws[NBT], zk[2][NBT], zm[2][NBT];
+  cplx* out = P.T + ((size_t)im * (H / G) + y0 / G) * (size_t)(NC + 1) * G + (y0 % G);   // column k at out + G k
+  constexpr int NIT = (NC / 2) / TPR, NH = NIT / 2;
+  static_assert(NIT >= 2 && NIT % 2 == 0, "the split step is shared by the two rows' threads");
+  const cplx tw0 = ldg2(P.twW + tr);
+  cplx twrun = rr ? mul_split_root<EPT>(tw0, NH) : tw0;    // w^(tr + i TPR) = w^tr e^{-2 pi i i/(2 EPT)}
+  cplx zk[2][NH], zm[2][NH];
 #pragma unroll
-    for (int i = 0; i < NBT; ++i) { tws[i] = twrun; twrun = mul_split_root<EPT>(twrun, 1); }
+  for (int i = 0; i < NH; ++i) {
+    const int k = tr + (rr * NH + i) * TPR;
+    const int pk = C::phys(k), pm = C::phys((NC - k) & (NC - 1));
+    zk[0][i] = sA[pk]; zm[0][i] = cconj(sA[pm]);
+    zk[1][i] = sB[pk]; zm[1][i] = cconj(sB[pm]);
+  }
 #pragma unroll
-    for (int i = 0; i < NBT; ++i) {
-      const int k = tr + (i0 + i) * TPR;
-      const int pk = C::phys(k), pm = C::phys((NC - k) & (NC - 1));
-      zk[0][i] = sA[pk]; zm[0][i] = cconj(sA[pm]);
-      zk[1][i] = sB[pk]; zm[1][i] = cconj(sB[pm]);
+  for (int i = 0; i < NH; ++i) {
+    const int k = tr + (rr * NH + i) * TPR;
+    cplx xe[2], xo[2];
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      xe[q] = cscale(cadd(zk[q][i], zm[q][i]), 0.5);
+      xo[q] = cmul_mi(cscale(csub(zk[q][i], zm[q][i]), 0.5));
     }
+    if (k == 0) {     // rr == 0, tr == 0, i == 0: DC and Nyquist bins, and the pair's moment writer
+      double dc[2], ny[2];
 #pragma unroll
-    for (int i = 0; i < NBT; ++i) {
-      const int k = tr + (i0 + i) * TPR;
-      cplx xe[2], xo[2];
-#pragma unroll
-      for (int rr = 0; rr < 2; ++rr) {
-        xe[rr] = cscale(cadd(zk[rr][i], zm[rr][i]), 0.5);
-        xo[rr] = cmul_mi(cscale(csub(zk[rr][i], zm[rr][i]), 0.5));
-      }
-      if (i0 + i == 0 && tr == 0) {
-        double dc[2], ny[2];
-#pragma unroll
-        for (int rr = 0; rr < 2; ++rr) { dc[rr] = xe[rr].x + xo[rr].x; ny[rr] = xe[rr].x - xo[rr].x; }
-        row_st_pair(out, cmake(dc[0], 0.0), cmake(dc[1], 0.0));
-        row_st_pair(out + G * NC, cmake(ny[0], 0.0), cmake(ny[1], 0.0));
-        if (P.moments) {   // tr == 0 here: the pair's moment writer
-          const int s0 = r * WPR;
-          for (int rr = 0; rr < 2; ++rr) {
-            const int y = y0 + rr;
-            double* momS = P.rowMom + (size_t)P.nMomA * H + y;
-            double* momR = momS + (size_t)P.nMomS * H;
-            if (im < P.nR) momR[(size_t)im * H] = dc[rr]; else momS[0] = dc[rr];
-            if (extra) {
-              double* dst = im < P.nR ? momR + (size_t)P.nR * H : momS + H;
-              for (int ii = 0; ii < P.DB; ++ii) {
-                double t = 0.0;
-                for (int k2 = 0; k2 < WPR; ++k2) t += redX[rr][ii][s0 + k2];
-                dst[(size_t)ii * H] = t;
-              }
+      for (int q = 0; q < 2; ++q) { dc[q] = xe[q].x + xo[q].x; ny[q] = xe[q].x - xo[q].x; }
+      row_st_pair(out, cmake(dc[0], 0.0), cmake(dc[1], 0.0));
+      row_st_pair(out + G * NC, cmake(ny[0], 0.0), cmake(ny[1], 0.0));
+      if (P.moments) {
+        for (int q = 0; q < 2; ++q) {
+          const int yq = y0 + q, s0 = (2 * pr + q) * WPR;
+          double* momS = P.rowMom + (size_t)P.nMomA * H + yq;
+          double* momR = momS + (size_t)P.nMomS * H;
+          if (im < P.nR) momR[(size_t)im * H] = dc[q]; else momS[0] = dc[q];
+          if (extra) {
+            double* dst = im < P.nR ? momR + (size_t)P.nR * H : momS + H;
+            for (int ii = 0; ii < P.DB; ++ii) {
+              double t = 0.0;
+              for (int k2 = 0; k2 < WPR; ++k2) t += redX[ii][s0 + k2];
+              dst[(size_t)ii * H] = t;
             }
-            if (momA) {
-              for (int a = 0; a < P.nMomA; ++a) {
-                double t = 0.0;
-                for (int k2 = 0; k2 < WPR; ++k2) t += redM[rr][a][s0 + k2];
-                P.rowMom[(size_t)a * H + y] = P.fullA[a] - t;
-              }
+          }
+          if (momA) {
+            for (int a = 0; a < P.nMomA; ++a) {
+              double t = 0.0;
+              for (int k2 = 0; k2 < WPR; ++k2) t += redM[a][s0 + k2];
+              P.rowMom[(size_t)a * H + yq] = P.fullA[a] - t;
             }
           }
         }
-      } else {
-        const cplx t0 = cmul(tws[i], xo[0]), t1 = cmul(tws[i], xo[1]);
-        row_st_pair(out + G * k, cadd(xe[0], t0), cadd(xe[1], t1));
-        row_st_pair(out + G * (NC - k), cconj(csub(xe[0], t0)), cconj(csub(xe[1], t1)));
       }
+    } else {
+      const cplx t0 = cmul(twrun, xo[0]), t1 = cmul(twrun, xo[1]);
+      row_st_pair(out + G * k, cadd(xe[0], t0), cadd(xe[1], t1));
+      row_st_pair(out + G * (NC - k), cconj(csub(xe[0], t0)), cconj(csub(xe[1], t1)));
     }
+    twrun = mul_split_root<EPT>(twrun, 1);
   }
-  if (tr == 0) {   // the middle bin k = NC/2 pairs with itself
+  if (rr == 1 && tr == 0) {   // the middle bin k = NC/2 pairs with itself
     const cplx tw = ldg2(P.twW + NC / 2);
     cplx o[2];
 #pragma unroll
-    for (int rr = 0; rr < 2; ++rr) {
-      const cplx z = (rr ? sB : sA)[C::phys(NC / 2)];
+    for (int q = 0; q < 2; ++q) {
+      const cplx z = (q ? sB : sA)[C::phys(NC / 2)];
       const cplx zc = cconj(z);
       const cplx xe = cscale(cadd(z, zc), 0.5);
       const cplx xo = cmul_mi(cscale(csub(z, zc), 0.5));
-      o[rr] = cadd(xe, cmul(tw, xo));
+      o[q] = cadd(xe, cmul(tw, xo));
     }
     row_st_pair(out + G * (NC / 2), o[0], o[1]);
   }
@@ -639,10 +600,13 @@ static sfft_status launch_row_fwd_t(const RowFwdParams& P, cudaStream_t st) {
 template <int NC>
 static sfft_status launch_row2_fwd_t(const RowFwdParams& P, cudaStream_t st) {
   using C = FftCfg<NC>;
-  int nth = row_threads(NC, P.H / 2, C::EPT);
-  const int RB = nth / (NC / C::EPT);
+  constexpr int TPR = NC / C::EPT;
+  int RB = 128 / TPR;                               // row pairs per CTA
+  if (RB < 1) RB = 1;
+  if (RB > P.H / 2) RB = P.H / 2;
+  const int nth = 2 * RB * TPR;
   const size_t smem = (size_t)2 * RB * C::SEQ_STRIDE * sizeof(cplx);
-  constexpr int MINB = SFFT_ROW2_MINB;
+  constexpr int MINB = 2;
   SFFT_CUDA_TRY(cudaFuncSetAttribute(k_row2_fwd<NC, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   k_row2_fwd<NC, MINB><<<(P.H / 2 / RB) * (P.nR + P.withS), nth, smem, st>>>(P);
   SFFT_LAUNCH_CHECK();
