@@ -211,7 +211,7 @@ sfft_status sfft_probe_fp64(int kind, int iters, double* tflops, double* elapsed
  * event pair on the caller stream around each stage (no synchronisation; at most 512 pending
  * pairs between reads).  sfft_profile_read synchronises on the pending events, folds them into
  * per-stage totals and returns the accumulated milliseconds and pair count of `stage`:
- *   0 build: row pass (k_row2_fwd/k_row_fwd) 1 build: column pass (k_col_fwd), or the fused
+ *   0 build: row pass (k_row2_fwd)          1 build: column pass (k_col_fwd), or the fused
  *                                            column/cross kernel (k_colb)
  *   2 build: cross+pruned inverse, K-K     3 build: cross+pruned inverse, K-S
  *   4 build: lag-row inverse + moments + gather      5 solve (all kernels)

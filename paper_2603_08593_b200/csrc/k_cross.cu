@@ -13,7 +13,7 @@
 //                 double buffered); the 2D+1 accumulators live in registers.
 //  k_lag_idft   : C[dy][dx] = (1/P) [ Re Y[dy][0] + (-1)^dx Re Y[dy][NC]
 //                                     + 2 sum_{kx=1}^{NC-1} Re( Y[dy][kx] e^{2 pi i kx dx/W} ) ].
-//  k_mom_final  : reduces the per-row moments of k_row_fwd to sum m xi^a eta^b and sum m xi^p eta^q S.
+//  k_mom_final  : reduces the per-row moments of k_row2_fwd to sum m xi^a eta^b and sum m xi^p eta^q S.
 //  k_gather     : A[tL+s, t'L+s'] = C_{t,t'}[(u-u', v-v')], b[tL+s] = C_{t,S}[(u,v)],
 //                 A[tL+s, B t'] = C_{t,Psi t'}[(u,v)], A[B,B] and b_B from the moments.
 #include "fft_smem.cuh"

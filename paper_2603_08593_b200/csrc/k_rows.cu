@@ -1,6 +1,6 @@
 // Row-direction kernels.
 //
-//  k_row_fwd   : (a1)+(a2 first pass) -- generation of the polynomial-weighted, masked images
+//  k_row2_fwd  : (a1)+(a2 first pass) -- generation of the polynomial-weighted, masked images
 //                m xi^p R, m S fused into the first (row, R2C) pass of the 2-D FFT, plus the fused
 //                fp64 row reductions sum_x m xi^a, sum_x m xi^a S and sum_x m xi^a R
 //                (north_star subsystems (1),(2)).  The eta^q factor of a
@@ -10,8 +10,9 @@
 //                D = S - M - B (north_star subsystem (6)).
 //
 // Real rows of length W are transformed as W/2-point complex FFTs of z[j] = x[2j] + i x[2j+1]
-// with the standard split/merge post-(pre-)processing.  Output column 0 packs the two real
-// bins: T[y][0] = X[0] + i X[W/2].
+// with the standard split/merge post-(pre-)processing.  Two output layouts: the row-group layout of
+// the fused build path (see k_row2_fwd) and the row-major packed one, T[y][kx], kx < W/2, whose
+// column 0 packs the two real bins, T[y][0] = X[0] + i X[W/2] (generic build path, sfft_subtract).
 #include "fft_smem.cuh"
 
 struct RowFwdParams {
@@ -21,7 +22,7 @@ struct RowFwdParams {
   int H, W;
   int nR;        // images 0..nR-1 are xi^p R, p = image index
   int withS;     // image nR is S (weight 1)
-  cplx* T;       // [nimg][H][pitchT]
+  cplx* T;       // colT = 0: [nimg][H][pitchT];  colT = 1: [nimg][H/G][NC+1][G]
   int pitchT;    // row pitch of T in complex elements
   int packed;    // 1: T[y][0] = X[0] + i X[W/2];  0: T[y][0] = X[0], T[y][NC] = X[W/2]
   int colT;      // 1 (unpacked only): row-group layout T[img][y/G][kx][y%G], G = SFFT_T_G, kx in [0, NC]; written by k_row2_fwd, read by k_colb
@@ -41,9 +42,6 @@ struct RowFwdParams {
 #else
 #define ROW_LD(p) (*(p))
 #define ROW_ST(p, v) (*(p) = (v))
-#endif
-#ifndef SFFT_ROW_NBT
-#define SFFT_ROW_NBT 2    // bins of the split step loaded per batch
 #endif
 #ifndef SFFT_ROW_MINB
 #define SFFT_ROW_MINB 3   // CTAs per SM the row kernels are compiled for
@@ -80,204 +78,6 @@ __device__ __forceinline__ void row_extra_moments(const cplx* v, double xb, doub
   }
 }
 
-// One CTA = RB rows, NC/EPT threads per row.  A thread's EPT input elements j = tr + e*TPR are
-// exactly the inputs of its first-pass butterfly, so they go from global memory through the
-// weighting (mask, xi^p) into the butterfly without being staged in shared memory; the inputs of
-// the next image are requested before the split/store phase of the current one.  The mask is
-// read once and kept as two bits per element.
-//
-// Fused reductions (moments != 0), all in a fixed order:
-//   sum_x m xi^p R, p <= DK and sum_x m S : the DC bin of the image's own row transform;
-//   sum_x m xi^a R, DK < a <= DK+DB and sum_x m xi^a S, 0 < a <= DB: DB extra sums on the
-//     weighted values of the last R image and of the S image (shuffle tree, then warps in order);
-//   sum_x m xi^a, a <= 2 DB: the closed-form whole-row sum minus the (rare) masked pixels.
-template <int NC, int MINB>
-__global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
-  using C = FftCfg<NC>;
-  constexpr int EPT = C::EPT;
-  constexpr int TPR = NC / EPT;  // threads per row
-  constexpr int LW = TPR < 32 ? TPR : 32;           // lanes of one row inside a warp
-  constexpr int WPR = TPR / 32 > 0 ? TPR / 32 : 1;  // warps per row
-  constexpr int NSLOT = 128 / LW;                   // (row, warp-of-row) slots of a CTA
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  __shared__ double redM[ROW_NMA][NSLOT];
-  __shared__ double redX[SFFT_MAX_DEG][NSLOT];
-  cplx* s = reinterpret_cast<cplx*>(smem_raw);
-  const int tid = threadIdx.x, nth = blockDim.x;
-  const int RB = nth / TPR;
-  const int r = tid / TPR, tr = tid - r * TPR;
-  const int y = blockIdx.x * RB + r;
-  const int W = P.W, H = P.H;
-  const double invW = 1.0 / (double)W;
-  const double xb = (double)(4 * tr + 1 - W) * invW, step = (double)(4 * TPR) * invW, dx1 = 2.0 * invW;
-  const size_t rowoff = (size_t)y * W;
-  const int slot = tid / LW;
-  const int nimg = P.nR + P.withS;
-
-  // mask bits: bit 2e = element 2j masked, bit 2e+1 = element 2j+1 masked, j = tr + e*TPR
-  unsigned mbits = 0u;
-  if (P.mask) {
-    uchar2 mk[EPT];
-#pragma unroll
-    for (int e = 0; e < EPT; ++e) mk[e] = *reinterpret_cast<const uchar2*>(P.mask + rowoff + 2 * (tr + e * TPR));
-#pragma unroll
-    for (int e = 0; e < EPT; ++e) mbits |= (mk[e].x ? 1u : 0u) << (2 * e) | (mk[e].y ? 1u : 0u) << (2 * e + 1);
-  }
-
-  cplx* srow = s + r * C::SEQ_STRIDE;
-  double2 raw[EPT];
-  auto fetch = [&](int im) {
-    if (im < nimg) {
-      const double* src = (im < P.nR ? P.R : P.S) + rowoff;
-#pragma unroll
-      for (int e = 0; e < EPT; ++e) raw[e] = ROW_LD(reinterpret_cast<const double2*>(src + 2 * (tr + e * TPR)));
-    } else {
-#pragma unroll
-      for (int e = 0; e < EPT; ++e) raw[e] = make_double2(0.0, 0.0);
-    }
-  };
-  fetch(0);
-
-  if (P.moments) {
-    // masked part of sum_x m xi^a: only warps that hold a masked pixel do any work
-    double ms[ROW_NMA];
-#pragma unroll
-    for (int a = 0; a < ROW_NMA; ++a) ms[a] = 0.0;
-    if (__any_sync(0xffffffffu, mbits != 0u)) {
-      unsigned mm = mbits;
-      while (mm) {
-        const int bit = __ffs(mm) - 1;
-        mm &= mm - 1;
-        const int j = tr + (bit >> 1) * TPR;
-        const double x = (double)(4 * j + 1 + 2 * (bit & 1) - W) * invW;
-        double pw = 1.0;
-#pragma unroll
-        for (int a = 0; a < ROW_NMA; ++a) { ms[a] += pw; pw *= x; }
-      }
-#pragma unroll
-      for (int a = 0; a < ROW_NMA; ++a) {
-#pragma unroll
-        for (int off = LW / 2; off > 0; off >>= 1) ms[a] += __shfl_xor_sync(0xffffffffu, ms[a], off);
-      }
-    }
-    if ((tid & (LW - 1)) == 0) {
-#pragma unroll
-      for (int a = 0; a < ROW_NMA; ++a) redM[a][slot] = ms[a];
-    }
-  }
-
-  for (int im = 0; im < nimg; ++im) {
-    const int pw = im < P.nR ? im : 0;
-    if (mbits) {
-#pragma unroll
-      for (int e = 0; e < EPT; ++e) {
-        if ((mbits >> (2 * e)) & 1u) raw[e].x = 0.0;
-        if ((mbits >> (2 * e + 1)) & 1u) raw[e].y = 0.0;
-      }
-    }
-    cplx v[EPT];
-    switch (pw) {
-      case 0:
-#pragma unroll
-        for (int e = 0; e < EPT; ++e) v[e] = raw[e];
-        break;
-      case 1: row_weight<EPT, 1>(raw, v, xb, step, dx1); break;
-      case 2: row_weight<EPT, 2>(raw, v, xb, step, dx1); break;
-      default: row_weight<EPT, 3>(raw, v, xb, step, dx1); break;
-    }
-    const bool extra = P.moments && P.DB > 0 && im >= P.nR - 1;
-    if (extra) {
-      double hi[SFFT_MAX_DEG];
-      switch (P.DB) {
-        case 1: row_extra_moments<EPT, 1>(v, xb, step, dx1, hi); break;
-        case 2: row_extra_moments<EPT, 2>(v, xb, step, dx1, hi); break;
-        default: row_extra_moments<EPT, 3>(v, xb, step, dx1, hi); break;
-      }
-#pragma unroll
-      for (int i = 0; i < SFFT_MAX_DEG; ++i) {
-#pragma unroll
-        for (int off = LW / 2; off > 0; off >>= 1) hi[i] += __shfl_xor_sync(0xffffffffu, hi[i], off);
-      }
-      if ((tid & (LW - 1)) == 0) {
-#pragma unroll
-        for (int i = 0; i < SFFT_MAX_DEG; ++i) redX[i][slot] = hi[i];
-      }
-    }
-    fft_regs_to_smem<NC, -1, false>(v, s, tid, nth, RB, P.twP, C::SEQ_STRIDE);
-    fetch(im + 1);
-    // split: X[k] = Xe + w^k Xo, X[NC-k] = conj(Xe - w^k Xo), w = e^{-2 pi i / W}
-    cplx* out = P.T + ((size_t)im * H + y) * P.pitchT;
-    auto at = [&](int k) -> cplx* { return out + k; };
-    // all twiddles and sequence elements of the thread's NIT bins are requested up front (the loop
-    // is latency bound otherwise: one shared and one global load chain per bin)
-    constexpr int NIT = (NC / 2) / TPR;
-    constexpr int NBT = NIT >= SFFT_ROW_NBT ? SFFT_ROW_NBT : NIT;   // bins per batch (register budget: raw[] is live here)
-    // w^(tr + i TPR) = w^tr e^{-2 pi i i/(2 EPT)}: one table load per image, then constant products
-    cplx twrun = ldg2(P.twW + tr);
-#pragma unroll 1
-    for (int i0 = 0; i0 < NIT; i0 += NBT) {
-    cplx tws[NBT], zks[NBT], zms[NBT];
-#pragma unroll
-    for (int i = 0; i < NBT; ++i) { tws[i] = twrun; twrun = mul_split_root<EPT>(twrun, 1); }
-#pragma unroll
-    for (int i = 0; i < NBT; ++i) {
-      const int k = tr + (i0 + i) * TPR;
-      zks[i] = srow[C::phys(k)];
-      zms[i] = cconj(srow[C::phys((NC - k) & (NC - 1))]);
-    }
-#pragma unroll
-    for (int i = 0; i < NBT; ++i) {
-      const int k = tr + (i0 + i) * TPR;
-      const cplx xe = cscale(cadd(zks[i], zms[i]), 0.5);
-      const cplx xo = cmul_mi(cscale(csub(zks[i], zms[i]), 0.5));
-      if (i0 + i == 0 && tr == 0) {
-        const double dc = xe.x + xo.x, ny = xe.x - xo.x;
-        if (P.packed) {
-          out[0] = cmake(dc, ny);
-        } else {
-          ROW_ST(at(0), cmake(dc, 0.0));
-          ROW_ST(at(NC), cmake(ny, 0.0));
-        }
-        if (P.moments) {   // tr == 0 here: the row's moment writer
-          double* momS = P.rowMom + (size_t)P.nMomA * H + y;
-          double* momR = momS + (size_t)P.nMomS * H;
-          const int s0 = r * WPR;
-          if (im < P.nR) momR[(size_t)im * H] = dc; else momS[0] = dc;
-          if (extra) {
-            double* dst = im < P.nR ? momR + (size_t)P.nR * H : momS + H;
-            for (int ii = 0; ii < P.DB; ++ii) {
-              double t = 0.0;
-              for (int k2 = 0; k2 < WPR; ++k2) t += redX[ii][s0 + k2];
-              dst[(size_t)ii * H] = t;
-            }
-          }
-          if (im == 0) {
-            for (int a = 0; a < P.nMomA; ++a) {
-              double t = 0.0;
-              for (int k2 = 0; k2 < WPR; ++k2) t += redM[a][s0 + k2];
-              P.rowMom[(size_t)a * H + y] = P.fullA[a] - t;
-            }
-          }
-        }
-      } else {
-        const cplx t = cmul(tws[i], xo);
-        ROW_ST(at(k), cadd(xe, t));
-        ROW_ST(at(NC - k), cconj(csub(xe, t)));
-      }
-    }
-    }
-    if (tr == 0) {   // the middle bin k = NC/2 pairs with itself
-      const cplx z = srow[C::phys(NC / 2)];
-      const cplx zc = cconj(z);
-      const cplx xe = cscale(cadd(z, zc), 0.5);
-      const cplx xo = cmul_mi(cscale(csub(z, zc), 0.5));
-      ROW_ST(at(NC / 2), cadd(xe, cmul(ldg2(P.twW + NC / 2), xo)));
-    }
-    __syncthreads();
-  }
-}
-
-
 // ------------------------------------------------------------------------------------------------
 // Row pass of the fused build path: one CTA = one image (blockIdx.x % nimg, so the images of a pair run
 // side by side and R stays in L2) of RB row PAIRS (2b, 2b+1), 2 RB TPR threads (256 at W = 4096), thread =
@@ -289,7 +89,14 @@ __global__ void __launch_bounds__(128, MINB) k_row_fwd(RowFwdParams P) {
 // whole 32-byte sectors, G/2 row pairs filling a 16 G-byte run that k_colb reads along y.  128 registers,
 // two CTAs = 16 warps per SM (the kernel is latency-bound; a variant that transformed the two rows one
 // after the other in 128-thread CTAs, the second row staged by cp.async, had 8-12 warps per SM and took
-// 0.175 instead of 0.165 ms).  Fused reductions as in k_row_fwd.
+// 0.175 instead of 0.165 ms).  With colT = 0 the same kernel writes the row-major packed layout instead.
+// A thread's EPT input elements j = tr + e*TPR are exactly the inputs of its first-pass butterfly; the
+// mask is read once and kept as two bits per element.
+// Fused reductions (moments != 0), all in a fixed order:
+//   sum_x m xi^p R, p <= DK and sum_x m S : the DC bin of the image's own row transform;
+//   sum_x m xi^a R, DK < a <= DK+DB and sum_x m xi^a S, 0 < a <= DB: DB extra sums on the
+//     weighted values of the last R image and of the S image (shuffle tree, then warps in order);
+//   sum_x m xi^a, a <= 2 DB: the closed-form whole-row sum minus the (rare) masked pixels.
 __device__ __forceinline__ void row_st_pair(cplx* dst, cplx a, cplx b) {   // 32-byte streaming store
   asm volatile("st.global.cs.v4.f64 [%0], {%1, %2, %3, %4};\n" ::"l"(dst), "d"(a.x), "d"(a.y), "d"(b.x), "d"(b.y) : "memory");
 }
@@ -403,6 +210,14 @@ __global__ void __launch_bounds__(256, MINB) k_row2_fwd(RowFwdParams P) {
   const cplx* sB = sA + C::SEQ_STRIDE;
   constexpr int G = SFFT_T_G;
   cplx* out = P.T + ((size_t)im * (H / G) + y0 / G) * (size_t)(NC + 1) * G + (y0 % G);   // column k at out + G k
+  // row-major packed layout (generic build path, sfft_subtract): T[img][y][kx], kx < NC, column 0 = X[0] + i X[NC]
+  cplx* outA = P.T + ((size_t)im * H + y0) * P.pitchT;
+  cplx* outB = outA + P.pitchT;
+  const bool grp = P.colT != 0;
+  auto emit = [&](int k, cplx a, cplx b) {
+    if (grp) row_st_pair(out + (size_t)G * k, a, b);
+    else { ROW_ST(outA + k, a); ROW_ST(outB + k, b); }
+  };
   constexpr int NIT = (NC / 2) / TPR, NH = NIT / 2;
   static_assert(NIT >= 2 && NIT % 2 == 0, "the split step is shared by the two rows' threads");
   const cplx tw0 = ldg2(P.twW + tr);
@@ -428,8 +243,12 @@ __global__ void __launch_bounds__(256, MINB) k_row2_fwd(RowFwdParams P) {
       double dc[2], ny[2];
 #pragma unroll
       for (int q = 0; q < 2; ++q) { dc[q] = xe[q].x + xo[q].x; ny[q] = xe[q].x - xo[q].x; }
-      row_st_pair(out, cmake(dc[0], 0.0), cmake(dc[1], 0.0));
-      row_st_pair(out + G * NC, cmake(ny[0], 0.0), cmake(ny[1], 0.0));
+      if (grp) {
+        emit(0, cmake(dc[0], 0.0), cmake(dc[1], 0.0));
+        emit(NC, cmake(ny[0], 0.0), cmake(ny[1], 0.0));
+      } else {
+        emit(0, cmake(dc[0], ny[0]), cmake(dc[1], ny[1]));
+      }
       if (P.moments) {
         for (int q = 0; q < 2; ++q) {
           const int yq = y0 + q, s0 = (2 * pr + q) * WPR;
@@ -455,8 +274,8 @@ __global__ void __launch_bounds__(256, MINB) k_row2_fwd(RowFwdParams P) {
       }
     } else {
       const cplx t0 = cmul(twrun, xo[0]), t1 = cmul(twrun, xo[1]);
-      row_st_pair(out + G * k, cadd(xe[0], t0), cadd(xe[1], t1));
-      row_st_pair(out + G * (NC - k), cconj(csub(xe[0], t0)), cconj(csub(xe[1], t1)));
+      emit(k, cadd(xe[0], t0), cadd(xe[1], t1));
+      emit(NC - k, cconj(csub(xe[0], t0)), cconj(csub(xe[1], t1)));
     }
     twrun = mul_split_root<EPT>(twrun, 1);
   }
@@ -471,7 +290,7 @@ __global__ void __launch_bounds__(256, MINB) k_row2_fwd(RowFwdParams P) {
       const cplx xo = cmul_mi(cscale(csub(z, zc), 0.5));
       o[q] = cadd(xe, cmul(tw, xo));
     }
-    row_st_pair(out + G * (NC / 2), o[0], o[1]);
+    emit(NC / 2, o[0], o[1]);
   }
 }
 
@@ -585,19 +404,6 @@ static int row_threads(int NC, int H, int EPT) {
 }
 
 template <int NC>
-static sfft_status launch_row_fwd_t(const RowFwdParams& P, cudaStream_t st) {
-  using C = FftCfg<NC>;
-  const int nth = row_threads(NC, P.H, C::EPT);
-  const int RB = nth / (NC / C::EPT);
-  size_t smem = (size_t)RB * C::SEQ_STRIDE * sizeof(cplx);
-  constexpr int MINB = SFFT_ROW_MINB;
-  SFFT_CUDA_TRY(cudaFuncSetAttribute(k_row_fwd<NC, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  k_row_fwd<NC, MINB><<<P.H / RB, nth, smem, st>>>(P);
-  SFFT_LAUNCH_CHECK();
-  return SFFT_OK;
-}
-
-template <int NC>
 static sfft_status launch_row2_fwd_t(const RowFwdParams& P, cudaStream_t st) {
   using C = FftCfg<NC>;
   constexpr int TPR = NC / C::EPT;
@@ -650,10 +456,7 @@ sfft_status sfft_launch_row_fwd(sfft_plan* p, const double* R, const double* S,
   P.rowMom = p->rowMom;
   for (int a = 0; a < ROW_NMA; ++a) P.fullA[a] = p->fullA[a];
   ++*nl;
-  if (colT) {
-    SFFT_DISPATCH_NC(p->NC, launch_row2_fwd_t)
-  }
-  SFFT_DISPATCH_NC(p->NC, launch_row_fwd_t)
+  SFFT_DISPATCH_NC(p->NC, launch_row2_fwd_t)
 }
 
 sfft_status sfft_launch_row_inv_sub(sfft_plan* p, const double* S, const double* c, double* D,
