@@ -618,7 +618,7 @@ def run_cuda(args, rank, world, local_rank):
             r["overlapped"] = "side stream, concurrent with build.row_fwd / build.colx (span, not busy time)"
         if r["stage"] == "subtract.row_fwd":
             r["overlapped"] = ("side stream (sfft_subtract_prepare), concurrent with solve on about a third of the "
-                               "SMs (span, not busy time; 0.098 ms when run alone on the whole GPU)")
+                               "SMs (span, not busy time; ~0.065 ms when run alone on the whole GPU)")
     serial = [r for r in table if "overlapped" not in r]
     tot = sum(r["ms"] for r in serial)
     for r in serial:
@@ -698,8 +698,8 @@ def run_cuda(args, rank, world, local_rank):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture of the final
 # kernels of this round, summarised in NCU_SOURCE (null where that capture holds no such kernel).
 NCU_SOURCE = "profiles/r02_ncu_full.md"
-NCU_TRAFFIC = {"build.colx": 283.8e6, "build.row_fwd": 359.6e6, "subtract.row_fwd": 209.9e6, "subtract.mix": 254.5e6,
-               "subtract.row_inv": 171.9e6, "solve": 4.5e6}
+NCU_TRAFFIC = {"build.colx": 284.4e6, "build.row_fwd": 365.0e6, "subtract.row_fwd": 208.9e6, "subtract.mix": 254.7e6,
+               "subtract.row_inv": 173.0e6, "solve": 4.5e6}
 
 
 def main():
