@@ -23,7 +23,8 @@
 #define CH_WARPS (CH_THREADS / 32)
 
 // Optional phase timestamps (development builds only: -DSFFT_CHOL_TIMING): CTA 0 records
-// %globaltimer at every phase boundary into sfft_chol_dbg.
+// %globaltimer at every phase boundary into sfft_chol_dbg (k_chol_fused: entries 0.., its diagonal-block
+// factorisation 200..204; k_chol_back: 100 + 3 per block).
 #ifdef SFFT_CHOL_TIMING
 __device__ unsigned long long sfft_chol_dbg[256];
 #define CH_STAMP(i)                                                              \
@@ -435,6 +436,7 @@ __global__ void __launch_bounds__(CHB_TH, 1) k_chol_back(const double* __restric
     }
   }
   __syncthreads();
+  CH_STAMP(100)
   for (int kb = nblk - 1; kb >= 0; --kb) {
     const int k0 = kb * CHB_NB;
     const int nb = min(CHB_NB, N - k0);
@@ -467,6 +469,7 @@ __global__ void __launch_bounds__(CHB_TH, 1) k_chol_back(const double* __restric
       if (lane < nb) c[k0 + lane] = rm0;
       if (lane + 32 < nb) c[k0 + lane + 32] = rm1;
     }
+    CH_STAMP(101 + 3 * kb)
     // the next diagonal block is requested while warp 0 solves
     constexpr int NQ = CHB_NB * CHB_NB / CHB_TH;
     double nxt[NQ];
@@ -487,6 +490,7 @@ __global__ void __launch_bounds__(CHB_TH, 1) k_chol_back(const double* __restric
         ls[(e >> 6) * (CHB_NB + 1) + (e & 63)] = nxt[q];
       }
     }
+    CH_STAMP(102 + 3 * kb)
     for (int j = tid; j < k0; j += CHB_TH) {
       double a0 = r[j], a1 = 0.0;
 #pragma unroll
@@ -503,6 +507,7 @@ __global__ void __launch_bounds__(CHB_TH, 1) k_chol_back(const double* __restric
       r[j] = a0 + a1;
     }
     __syncthreads();
+    CH_STAMP(103 + 3 * kb)
   }
 }
 
