@@ -48,7 +48,7 @@ typedef enum {
 } sfft_status;
 
 /* Create a plan for H x W images, kernel half-width w, polynomial degrees DK (kernel) and DB
- * (background).  Supported: H, W powers of two, 32 <= H, W <= 4096; 0 <= w <= 5 (this build),
+ * (background).  Supported: H, W powers of two, 16 <= H, W <= 4096; 0 <= w <= 5 (this build),
  * 4w+1 <= min(H,W); 0 <= DK, DB <= 3.  Otherwise SFFT_ERR_UNSUPPORTED.  Allocates scratch on the current
  * device and uploads tables; may synchronise.  *out is set to NULL on failure.
  * (north_star: sfft_plan_create(H,W,w,DK,DB).) */

@@ -173,8 +173,9 @@ __device__ __forceinline__ void cb_job_run(const cplx* x, int q, bool cen, cplx*
     if (!edge) {
       if (j + 112 >= D + Bi) v[7] = cmake(0.0, 0.0);
     } else {
+      // (r = 0 included: the last block of a column can hold fewer than 16 - D centre rows, e.g. H = 2048, w = 2)
 #pragma unroll
-      for (int r = 1; r < 8; ++r)
+      for (int r = 0; r < 8; ++r)
         if (j + 16 * r >= D + Bi) v[r] = cmake(0.0, 0.0);
     }
   }
@@ -239,7 +240,11 @@ __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
   const int half = lane >> 4, j = lane & 15;
   const cplx* swj = s_w + j;
   const int tasksPerCol = TT::STASK ? (TT::NT * nblk + (nblk + 3) / 4) : TT::NT * nblk;
-  int tci = 0, ti = wrp;   // (transform warps only)
+  // A warp's consecutive tasks must lie at most one ring generation (CB_NSLOT blocks) apart: the parity wait on
+  // an empty-barrier only tells the previous generation from the current one.  With one task per block (TK = 1)
+  // twelve warps would span two generations, so only FWA of them take tasks there (the others idle).
+  constexpr int FWA = TT::STASK ? CB_FW : (CB_FW < TT::NT * CB_NSLOT ? CB_FW : TT::NT * CB_NSLOT);
+  int tci = wrp < FWA ? 0 : ncolMine, ti = wrp;   // (transform warps only)
   while (ti >= tasksPerCol && tci < ncolMine) { ti -= tasksPerCol; ++tci; }
   // decode ti -> (type, first block); type < NT: per-block task, type == NT: S~ task over blocks blk .. blk + 3
   auto decode = [&](int lid, int& type, int& blk) {
@@ -324,7 +329,7 @@ __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
     // ---- advance the cursor; the next task's inputs are requested now (their latency hides under phase 2,
     //      the products and the waits)
     const int pblk = tblk;
-    ti += CB_FW;
+    ti += FWA;
     while (ti >= tasksPerCol && tci < ncolMine) { ti -= tasksPerCol; ++tci; }
     if (tci < ncolMine) decode(ti, ttype, tblk);
     __syncwarp();

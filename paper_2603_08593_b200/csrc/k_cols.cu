@@ -141,6 +141,7 @@ sfft_status sfft_launch_col_fwd(sfft_plan* p, cudaStream_t st, int* nl) {
   P.ngrp = n;
   ++*nl;
   switch (p->H) {
+    case 16: return launch_col_fwd_t<16>(P, st);
     case 32: return launch_col_fwd_t<32>(P, st);
     case 64: return launch_col_fwd_t<64>(P, st);
     case 128: return launch_col_fwd_t<128>(P, st);

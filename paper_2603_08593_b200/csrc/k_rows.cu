@@ -434,6 +434,7 @@ static sfft_status launch_row_inv_t(const RowInvParams& P, cudaStream_t st) {
 
 #define SFFT_DISPATCH_NC(NCV, CALL)                       \
   switch (NCV) {                                          \
+    case 8: return CALL<8>(P, st);                        \
     case 16: return CALL<16>(P, st);                      \
     case 32: return CALL<32>(P, st);                      \
     case 64: return CALL<64>(P, st);                      \

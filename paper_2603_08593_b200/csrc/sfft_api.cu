@@ -98,7 +98,7 @@ const char* sfft_status_string(sfft_status s) {
 sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int DB) {
   if (!out) return SFFT_ERR_INVALID_ARG;
   *out = nullptr;
-  if (!is_pow2(H) || !is_pow2(W) || H < 32 || W < 32 || H > 4096 || W > 4096) return SFFT_ERR_UNSUPPORTED;
+  if (!is_pow2(H) || !is_pow2(W) || H < 16 || W < 16 || H > 4096 || W > 4096) return SFFT_ERR_UNSUPPORTED;
   if (w < 0 || w > SFFT_MAX_W || 4 * w + 1 > (H < W ? H : W)) return SFFT_ERR_UNSUPPORTED;
   if (w > 5) return SFFT_ERR_UNSUPPORTED;  // lag half-ranges above 10 need the split-range path (not built yet)
   if (DK < 0 || DK > SFFT_MAX_DEG || DB < 0 || DB > SFFT_MAX_DEG) return SFFT_ERR_UNSUPPORTED;

@@ -103,9 +103,25 @@ def test_ragged_shapes_and_degrees(H, W, w, DK, DB, masked):
 
 
 @pytest.mark.parametrize("H,W,w,DK,DB,masked", [
+    (16, 16, 3, 1, 1, True), (16, 16, 0, 0, 0, False), (16, 64, 2, 2, 0, True), (128, 16, 1, 0, 2, False),
+    (16, 32, 3, 1, 2, True), (2048, 16, 2, 1, 1, True)])
+def test_smallest_frame_sizes(H, W, w, DK, DB, masked):
+    """H or W = 16, the smallest size include/sfft.h admits (4w+1 <= min(H, W) caps w at 3 there): one
+    single-pass transform per row (8 complex points) or column; the last case takes the blocked
+    column/cross kernel with 8-point packed rows and a last block of 8 centre rows (fewer than 16 - 2w)."""
+    rng = np.random.default_rng(H * 11 + W)
+    R = 50.0 * rng.standard_normal((H, W)) + 500.0 * (rng.random((H, W)) > 0.97)
+    S = 0.8 * np.roll(R, (1 if w else 0, -1 if w else 0), (0, 1)) + 30.0 * rng.standard_normal((H, W)) + 150.0
+    mask = (rng.random((H, W)) < 0.04).astype(np.uint8) if masked else None
+    run_case(R, S, mask, w, DK, DB, 30.0)
+
+
+@pytest.mark.parametrize("H,W,w,DK,DB,masked", [
     (1024, 32, 0, 0, 0, True), (1024, 64, 1, 1, 3, True), (1024, 32, 2, 2, 1, False),
     (2048, 32, 3, 2, 2, True), (1024, 128, 5, 1, 0, True), (4096, 32, 2, 2, 2, True),
-    (1024, 64, 4, 3, 1, True)])
+    (1024, 64, 4, 3, 1, True),
+    # DK = 0 with more blocks per column than ring slots (one task per block), and a short last block
+    (2048, 32, 2, 0, 0, True), (4096, 32, 1, 0, 1, False), (2048, 64, 1, 0, 0, True), (2048, 32, 2, 1, 2, True)])
 def test_fused_column_cross_path(H, W, w, DK, DB, masked):
     """H in {1024, 2048, 4096}: the fused column-FFT + cross-spectra kernel (every residue-class
     count DR = 2, 4, 8, every instantiated lag range) against the oracle; DK = 3 (> 32 map pairs)
