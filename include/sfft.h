@@ -237,6 +237,26 @@ int sfft_plan_fused(const sfft_plan* p);
  * plan's latency-bound solve runs.  Results are bitwise independent of the setting. */
 sfft_status sfft_plan_set_solve_ctas(sfft_plan* p, int max_ctas);
 
+/* sfft_solve for callers that cannot allocate device memory (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): the same Cholesky kernels as sfft_solve (north_star
+ * (5), a5), but no plan -- the factorisation workspace is a static array inside the library instead of a
+ * plan's cudaMalloc'ed scratch.  The call performs NO cudaMalloc / cudaFree and calls no allocating
+ * library routine; it only enqueues work on `stream`.
+ *   A    in : N*N fp64 row-major (device, not modified; only the lower triangle is read).
+ *   b    in : N fp64 (device, not modified).      coeffs out: N fp64 (device).
+ *   info out: device int, may be NULL; meaning as in sfft_solve.
+ *   N       : 1 <= N <= SFFT_SOLVE_STATIC_MAX_N (the Full configuration has N = 732).
+ * Limit and cost: the static workspace holds (MAX_N + 1) * MAX_N fp64 = 4.7 MB and is resident on every
+ * GPU that loads the library, until the process exits.  N > SFFT_SOLVE_STATIC_MAX_N returns
+ * SFFT_ERR_UNSUPPORTED (nothing is enqueued); N < 1 or a NULL A/b/coeffs returns SFFT_ERR_INVALID_ARG.
+ * Sharing: ALL calls on a device use the one workspace, which keeps the previous call's contents (the
+ * call rewrites every word it later reads, and clears its grid-barrier words itself).  Two calls that
+ * overlap on the GPU (different streams, or different host threads' streams) RACE and give wrong results:
+ * order them on one stream or with events.  Results are bitwise those of sfft_solve. */
+#define SFFT_SOLVE_STATIC_MAX_N 768
+sfft_status sfft_solve_static(const double* A, const double* b, int N, double* coeffs, int* info,
+                              void* stream);
+
 /* Library version string, e.g. "sfft-b200 0.1 (sm_100a)". */
 const char* sfft_version(void);
 

@@ -16,7 +16,10 @@ from .binding import (  # noqa: F401
     resample_affine,
     resample_mask_affine,
     cut_stamps,
+    solve_static,
+    SOLVE_STATIC_MAX_N,
 )
 
 __all__ = ["synth", "SfftPlan", "SfftError", "lib_path", "load_library", "EXPORTED_SYMBOLS",
-           "median_combine", "aperture_stats", "resample_affine", "resample_mask_affine", "cut_stamps"]
+           "median_combine", "aperture_stats", "resample_affine", "resample_mask_affine", "cut_stamps",
+           "solve_static", "SOLVE_STATIC_MAX_N"]

@@ -19,8 +19,10 @@ EXPORTED_SYMBOLS = [
     "sfft_status_string", "sfft_build_system", "sfft_build_system_exact", "sfft_solve", "sfft_subtract", "sfft_subtract_prepare",
     "sfft_probe_fp64", "sfft_last_launch_count", "sfft_plan_fused", "sfft_plan_set_solve_ctas", "sfft_version",
     "sfft_profile_enable", "sfft_profile_read", "sfft_median_combine", "sfft_aperture_stats", "sfft_resample_affine", "sfft_resample_mask_affine",
-    "sfft_cut_stamps", "sfft_multi_template_difference",
+    "sfft_cut_stamps", "sfft_multi_template_difference", "sfft_solve_static",
 ]
+
+SOLVE_STATIC_MAX_N = 768   # SFFT_SOLVE_STATIC_MAX_N (include/sfft.h)
 
 STAGE_NAMES = ["build.row_fwd", "build.col_fwd", "build.cross_KK", "build.cross_KS",
                "build.lag_gather", "solve", "subtract.row_fwd", "subtract.mix", "subtract.row_inv",
@@ -66,6 +68,8 @@ def load_library():
     lib.sfft_build_system.restype = i32
     lib.sfft_solve.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.sfft_solve.restype = i32
+    lib.sfft_solve_static.argtypes = [vp, vp, i32, vp, vp, vp]
+    lib.sfft_solve_static.restype = i32
     lib.sfft_subtract.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.sfft_subtract.restype = i32
     lib.sfft_probe_fp64.argtypes = [i32, i32, dbl_p, dbl_p, vp]
@@ -332,6 +336,25 @@ class SfftPlan:
                                                           1 if reset else 0), "sfft_profile_read")
             out[name] = (ms.value, cnt.value)
         return out
+
+
+def solve_static(A, b, coeffs=None, info=None, stream=None):
+    """sfft_solve_static: A c = b without a plan and without any device allocation inside the library (the
+    workspace is a static array shared by every call on the device: calls that overlap on the GPU race).
+    N = len(b) <= SOLVE_STATIC_MAX_N.  The output tensors created here when coeffs / info are None are the
+    caller-side allocations; pass preallocated ones from code that must not allocate at all."""
+    import torch
+    lib = load_library()
+    N = int(b.numel())
+    if coeffs is None:
+        coeffs = torch.empty(N, dtype=torch.float64, device=A.device)
+    if info is None:
+        info = torch.zeros(1, dtype=torch.int32, device=A.device)
+    _check(lib, lib.sfft_solve_static(
+        _dev_ptr(A, torch.float64, N * N, "A"), _dev_ptr(b, torch.float64, N, "b"), N,
+        _dev_ptr(coeffs, torch.float64, N, "coeffs"), _dev_ptr(info, torch.int32, 1, "info"),
+        _stream_handle(stream)), "sfft_solve_static")
+    return coeffs, info
 
 
 def probe_fp64(kind: int = 0, iters: int = 4096, stream=None):

@@ -539,3 +539,68 @@ sfft_status sfft_launch_solve(sfft_plan* p, const double* A, const double* b, do
   ++*nl;
   return SFFT_OK;
 }
+
+// ------------------------------------------------------------------------------------------------
+// sfft_solve_static (include/sfft.h): the same two kernels with the factorisation workspace in a static
+// device array, for callers that must not allocate.  Layout of the array: (N + 1) rows of pitch ld =
+// round-up(N + 1, 4) doubles (the layout sfft_launch_solve uses in a plan's Lw), then, at a fixed offset
+// past the largest workspace, the two grid-barrier words of k_chol_fused.
+#define NA_MAXN SFFT_SOLVE_STATIC_MAX_N
+#define NA_LD ((NA_MAXN + 1 + 3) & ~3)
+#define NA_WORK ((size_t)(NA_MAXN + 1) * NA_LD)      // doubles
+#define NA_TOTAL (NA_WORK + 32)                      // + 256 bytes for the barrier words
+static __device__ __align__(256) double sfft_static_scratch[NA_TOTAL];
+
+#define NA_MAXDEV 64
+namespace {
+struct NaDevice {
+  double* scratch;   // device address of sfft_static_scratch on this device
+  int sms;
+  bool ready;
+};
+NaDevice na_dev[NA_MAXDEV];   // zero-initialised
+}  // namespace
+
+extern "C" sfft_status sfft_solve_static(const double* A, const double* b, int N, double* coeffs, int* info,
+                                         void* stream) {
+  if (!A || !b || !coeffs || N < 1) return SFFT_ERR_INVALID_ARG;
+  if (N > NA_MAXN) return SFFT_ERR_UNSUPPORTED;
+  if (cudaPeekAtLastError() != cudaSuccess) return SFFT_ERR_CUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  int dev = -1;
+  SFFT_CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= NA_MAXDEV) return SFFT_ERR_UNSUPPORTED;
+  NaDevice& nd = na_dev[dev];
+  if (!nd.ready) {
+    // once per device, with that device current: in host code the array's name is only a handle, the
+    // device address comes from the runtime.  (Concurrent first calls store the same values.)
+    double* ptr = nullptr;
+    int sms = 0;
+    SFFT_CUDA_TRY(cudaGetSymbolAddress((void**)&ptr, sfft_static_scratch));
+    SFFT_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (!ptr || sms < 1) return SFFT_ERR_CUDA;
+    nd.scratch = ptr;
+    nd.sms = sms;
+    nd.ready = true;
+  }
+  double* Lw = nd.scratch;
+  unsigned* bar = reinterpret_cast<unsigned*>(nd.scratch + NA_WORK);
+  int ld = (N + 1 + 3) & ~3;
+  // the barrier words must start at zero whatever an earlier (possibly aborted) call left there
+  SFFT_CUDA_TRY(cudaMemsetAsync(bar, 0, 2 * sizeof(unsigned), st));
+  void* args[] = {(void*)&A, (void*)&b, (void*)&Lw, (void*)&N, (void*)&ld, (void*)&info, (void*)&bar};
+  int grid = nd.sms;   // cooperative launch: one CTA per SM at most
+  const int rows = N + 1, maxUseful = (rows + CH_WARPS - 1) / CH_WARPS;
+  const int T = (N + CH_NB - 1) / CH_NB, tiles = T * (T + 1) / 2;
+  int want = maxUseful > tiles ? maxUseful : tiles;
+  if (want < 1) want = 1;
+  if (grid > want) grid = want;
+  const size_t smemF = (size_t)2 * CH_PB * CH_LDS * sizeof(double);
+  SFFT_CUDA_TRY(cudaFuncSetAttribute(k_chol_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smemF));
+  SFFT_CUDA_TRY(cudaLaunchCooperativeKernel((const void*)k_chol_fused, dim3(grid), dim3(CH_THREADS), args, smemF, st));
+  const size_t smem = ((size_t)N + CHB_NB * (CHB_NB + 1) + 2 * CHB_NB) * sizeof(double);
+  SFFT_CUDA_TRY(cudaFuncSetAttribute(k_chol_back, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  k_chol_back<<<1, CHB_TH, smem, st>>>(Lw, coeffs, N, ld);
+  SFFT_LAUNCH_CHECK();
+  return SFFT_OK;
+}

@@ -55,6 +55,12 @@ def test_argument_validation_needs_no_gpu():
     assert lib.sfft_solve(None, None, None, None, None, None) == 1
     assert lib.sfft_subtract(None, None, None, None, None, None) == 1
     assert lib.sfft_last_launch_count(None, 0) == -1
+    # the allocation-free solve validates before any CUDA call: NULL -> INVALID_ARG, N beyond the static
+    # workspace -> UNSUPPORTED (the pointers are never dereferenced on the host)
+    fake = ctypes.c_void_p(256)
+    assert lib.sfft_solve_static(None, None, 5, None, None, None) == 1
+    assert lib.sfft_solve_static(fake, fake, 0, fake, None, None) == 1
+    assert lib.sfft_solve_static(fake, fake, 769, fake, None, None) == 2
 
 
 def test_no_cpu_fallback_without_device():
