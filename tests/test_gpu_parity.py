@@ -135,6 +135,27 @@ def test_fused_column_cross_path(H, W, w, DK, DB, masked):
     run_case(R, S, mask, w, DK, DB, 30.0, full_D=False)
 
 
+@pytest.mark.parametrize("H,W", [(1024, 32), (2048, 32), (4096, 32), (2048, 64), (1024, 16)])
+def test_blocked_column_kernel_every_lag_range_and_degree(H, W):
+    """sfft_build_system on the blocked column/cross kernel for EVERY kernel half-width 0..5 (the block length
+    128 - 4w, the number of blocks per column and the length of the last block all depend on w and H) and
+    TK = 1, 3, 6 (the three task tables), plus DK = 3 on the generic kernels, against the oracle."""
+    for w in range(0, 6):
+        if 4 * w + 1 > min(H, W):
+            continue
+        for DK, DB in [(0, 0), (1, 2), (2, 1), (0, 3), (3, 0)]:
+            rng = np.random.default_rng(H * 13 + W * 7 + w * 3 + DK)
+            R = 50.0 * rng.standard_normal((H, W)) + 500.0 * (rng.random((H, W)) > 0.97)
+            S = 0.8 * np.roll(R, (1 if w else 0, -1 if w else 0), (0, 1)) + 30.0 * rng.standard_normal((H, W)) + 150.0
+            mask = (rng.random((H, W)) < 0.03).astype(np.uint8)
+            Ao, bo = orc.build_system_fft(R, S, mask, w, DK, DB, workers=8)
+            with SfftPlan(H, W, w, DK, DB) as plan:
+                assert plan.fused == (DK <= 2)
+                A, b = plan.build_system(dev(R), dev(S), dev(mask))
+                torch.cuda.synchronize()
+                check_system(A.cpu().numpy(), b.cpu().numpy(), Ao, bo, (2 * w + 1) ** 2, (DK + 1) * (DK + 2) // 2)
+
+
 def test_mid_config():
     pr = synth.make_pair("mid")
     run_case(pr.R, pr.S, pr.mask, pr.cfg.w, pr.cfg.DK, pr.cfg.DB, pr.sky_rms, full_D=False)
