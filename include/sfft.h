@@ -48,9 +48,12 @@ typedef enum {
 } sfft_status;
 
 /* Create a plan for H x W images, kernel half-width w, polynomial degrees DK (kernel) and DB
- * (background).  Supported: H, W powers of two, 16 <= H, W <= 4096; 0 <= w <= 5 (this build),
- * 4w+1 <= min(H,W); 0 <= DK, DB <= 3.  Otherwise SFFT_ERR_UNSUPPORTED.  Allocates scratch on the current
- * device and uploads tables; may synchronise.  *out is set to NULL on failure.
+ * (background).  Supported: H, W powers of two, 16 <= H, W <= 4096; 0 <= w <= 15, 4w+1 <= min(H,W);
+ * 0 <= DK, DB <= 3.  Otherwise SFFT_ERR_UNSUPPORTED.  w <= 5 (every BASELINE configuration) runs the tuned
+ * kernels; w > 5 (lag half-ranges above 10) runs the generic column/cross kernels with the lag range split
+ * into windows and a plain mixing kernel -- same results, not tuned.  Allocates scratch on the current
+ * device (it grows with N^2: N = 9620 for w = 15, DK = 3) and uploads tables; may synchronise.  *out is set
+ * to NULL on failure.
  * (north_star: sfft_plan_create(H,W,w,DK,DB).) */
 sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int DB);
 
@@ -84,7 +87,10 @@ sfft_status sfft_build_system(sfft_plan* p, const double* R, const double* S,
  * 1-D correlations of a few image rows / columns, every other masked pixel through a symmetric rank-K
  * update (~0.4 ms more than the ordinary build at the full CCD with a 6-pixel border, + ~40 ns per
  * isolated masked pixel).  Recovers a known kernel exactly under any mask, which the input-masking
- * system of sfft_build_system cannot (reading A2').  Same arguments and errors. */
+ * system of sfft_build_system cannot (reading A2').  Same arguments and errors, plus
+ * SFFT_ERR_UNSUPPORTED (nothing enqueued) when mask != NULL and N > 2047, which only kernel half-widths
+ * w > 5 can reach (the rank-K update keeps the whole triangle of A in one cooperative launch); for w > 5
+ * every masked pixel takes the rank-K update (the line shortcut is compiled for w <= 5). */
 sfft_status sfft_build_system_exact(sfft_plan* p, const double* R, const double* S,
                                     const unsigned char* mask, double* A, double* b, void* stream);
 

@@ -461,7 +461,8 @@ __global__ void __launch_bounds__(CB_TH, 1) k_colb(ColbParams P) {
   }
 }
 
-bool sfft_colx_supported(int H, int nPair) { return (H == 1024 || H == 2048 || H == 4096) && nPair <= 32; }
+// (lag half-ranges above 10, i.e. w > 5, take the generic column and cross kernels)
+bool sfft_colx_supported(int H, int nPair, int Dmax) { return (H == 1024 || H == 2048 || H == 4096) && nPair <= 32 && Dmax <= 10; }
 
 template <int TK>
 static sfft_status launch_colb_t(const ColbParams& P, int num_sms, cudaStream_t st) {

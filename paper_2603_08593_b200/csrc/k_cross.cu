@@ -25,6 +25,7 @@ struct CrossParams {
   int g0;
   int H, NC, pitch, nLag;
   int NB, log2NB;            // b values staged per pipeline stage (power of two, divides H/8)
+  int c0;                    // windowed launches (half-ranges above 10): centre of the launch's 21 lags
   const cplx* twH;
 };
 
@@ -41,7 +42,9 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // shared by all of its pairs, so every spectrum element leaves L2 once per group instead of once
 // per pair.  Per staged b: x[a] = conj(F_f) F_g at ky = b + (H/8) a, 8-point inverse DFT over a,
 // then the 2D+1 twiddled accumulations in registers.
-template <int D>
+// WIN (lag half-ranges above 10, i.e. w > 5): the launch computes the 2D+1 lags c0 - D .. c0 + D of a longer
+// range, one twiddle load per lag (the symmetric pairing of +dy and -dy needs the window centred on 0).
+template <int D, bool WIN = false>
 __global__ void __launch_bounds__(SFFT_CR_GP * SFFT_CR_CT, 1) k_cross(CrossParams P) {
   constexpr int CT = SFFT_CR_CT;
   constexpr int NTH = SFFT_CR_GP * SFFT_CR_CT;
@@ -99,12 +102,21 @@ __global__ void __launch_bounds__(SFFT_CR_GP * SFFT_CR_CT, 1) k_cross(CrossParam
 #pragma unroll
         for (int a = 0; a < 8; ++a) x[a] = cmulc(pa[(bb * 8 + a) * CT], pb[(bb * 8 + a) * CT]);
         Dft<8, +1>::run(x);
+        if constexpr (WIN) {
+#pragma unroll
+          for (int i = 0; i < 2 * D + 1; ++i) {
+            const int dy = P.c0 + i - D;                         // (two's complement: & gives dy mod H)
+            const cplx t = ldg2(P.twH + ((b * dy) & (P.H - 1)));  // e^{-2 pi i b dy/H}
+            cfmac(acc[i], t, x[(i - D) & 7]);                    // += e^{+...} * Z[dy mod 8], c0 a multiple of 8
+          }
+        } else {
         acc[D] = cadd(acc[D], x[0]);
 #pragma unroll
         for (int i = 1; i <= D; ++i) {
           const cplx t = ldg2(P.twH + ((b * i) & (P.H - 1)));  // e^{-2 pi i b i/H}
           cfmac(acc[D + i], t, x[i & 7]);                      // += e^{+...} * Z[i mod 8]
           cfma(acc[D - i], t, x[(8 - (i & 7)) & 7]);           // += e^{-...} * Z[-i mod 8]
+        }
         }
       }
     }
@@ -116,7 +128,7 @@ __global__ void __launch_bounds__(SFFT_CR_GP * SFFT_CR_CT, 1) k_cross(CrossParam
     cplx* out = P.Y + ((size_t)G.pair[pl] * P.nLag) * P.pitch + kx;
 #pragma unroll
     for (int i = 0; i < 2 * D + 1; ++i) {
-      const int dy = i - D;
+      const int dy = (WIN ? P.c0 : 0) + i - D;
       if (dy >= -Dp && dy <= Dp) out[(size_t)(dy + Dp) * P.pitch] = acc[i];
     }
   }
@@ -132,7 +144,25 @@ static sfft_status launch_cross_t(const CrossParams& P, int ngroups, int maxns, 
   return SFFT_OK;
 }
 
-static sfft_status launch_cross_D(int D, const CrossParams& P, int ngroups, int maxns, cudaStream_t st) {
+// half-range Dfull > 10: 2 M + 1 launches of 25 lags each, centred on multiples of 24 (a multiple of 8, so the
+// residue dy mod 8 of a lag is a compile-time constant in the unrolled loop)
+#define SFFT_CR_WD 12
+static sfft_status launch_cross_windows(int Dfull, CrossParams P, int ngroups, int maxns, cudaStream_t st, int* nl) {
+  const size_t smem = (size_t)2 * maxns * P.NB * 8 * SFFT_CR_CT * sizeof(cplx);
+  SFFT_CUDA_TRY(cudaFuncSetAttribute(k_cross<SFFT_CR_WD, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  dim3 grid(P.NC / SFFT_CR_CT + 1, ngroups);
+  const int M = Dfull > SFFT_CR_WD ? (Dfull - SFFT_CR_WD + 2 * SFFT_CR_WD - 1) / (2 * SFFT_CR_WD) : 0;
+  for (int m = -M; m <= M; ++m) {
+    P.c0 = 2 * SFFT_CR_WD * m;
+    k_cross<SFFT_CR_WD, true><<<grid, SFFT_CR_GP * SFFT_CR_CT, smem, st>>>(P);
+    SFFT_LAUNCH_CHECK();
+    if (m != -M) ++*nl;   // (the caller counts the first launch)
+  }
+  return SFFT_OK;
+}
+
+static sfft_status launch_cross_D(int D, const CrossParams& P, int ngroups, int maxns, cudaStream_t st, int* nl) {
+  if (D > 10) return launch_cross_windows(D, P, ngroups, maxns, st, nl);
   switch (D) {
     case 0: case 1: return launch_cross_t<1>(P, ngroups, maxns, st);
     case 2: return launch_cross_t<2>(P, ngroups, maxns, st);
@@ -149,7 +179,7 @@ static sfft_status launch_cross_D(int D, const CrossParams& P, int ngroups, int 
 sfft_status sfft_launch_cross(sfft_plan* p, cudaStream_t st, int* nl) {
   CrossParams P;
   P.F = p->F; P.Y = p->Y; P.groups = p->d_groups; P.H = p->H; P.NC = p->NC; P.pitch = p->pitch;
-  P.nLag = p->nLag; P.twH = p->twH;
+  P.nLag = p->nLag; P.twH = p->twH; P.c0 = 0;
   const int N1 = p->H / 8;
   auto pickNB = [&](int maxns) {  // largest staged depth whose double buffer fits in shared memory
     int nb = 4;
@@ -161,12 +191,12 @@ sfft_status sfft_launch_cross(sfft_plan* p, cudaStream_t st, int* nl) {
   P.g0 = 0;
   P.NB = pickNB(p->maxnsKK); P.log2NB = P.NB == 4 ? 2 : (P.NB == 2 ? 1 : 0);
   ++*nl;
-  { ProfScope ps(p, 2, st); s = launch_cross_D(2 * p->w, P, p->nGroupKK, p->maxnsKK, st); }
+  { ProfScope ps(p, 2, st); s = launch_cross_D(2 * p->w, P, p->nGroupKK, p->maxnsKK, st, nl); }
   if (s != SFFT_OK) return s;
   P.g0 = p->nGroupKK;
   P.NB = pickNB(p->maxnsKO); P.log2NB = P.NB == 4 ? 2 : (P.NB == 2 ? 1 : 0);
   ++*nl;
-  { ProfScope ps(p, 3, st); s = launch_cross_D(p->w, P, p->nGroupKO, p->maxnsKO, st); }
+  { ProfScope ps(p, 3, st); s = launch_cross_D(p->w, P, p->nGroupKO, p->maxnsKO, st, nl); }
   return s;
 }
 
@@ -184,11 +214,12 @@ struct LagParams {
 };
 
 #define LAG_TH 256
-#define LAG_MAXD 10
+// LAG_MAXD = largest lag half-range of the instantiation: 10 (w <= 5) or 30 (w <= 15)
 
 // One CTA per (pair, lag row): lanes run along kx (coalesced reads of the lag row), every thread
 // keeps the 2D+1 partial sums of its kx values in registers, then a fixed-order reduction
 // (warp shuffle tree, then the warps in order) so the result is reproducible.
+template <int LAG_MAXD>
 __global__ void __launch_bounds__(LAG_TH) k_lag_idft(LagParams P) {
   const int pair = blockIdx.x, dyi = blockIdx.y;
   const int D = P.pairs[pair].D;
@@ -431,7 +462,8 @@ sfft_status sfft_launch_lag_gather(sfft_plan* p, double* A, double* b, cudaStrea
   LP.twW = p->twW;
   LP.nPart = p->nPart; LP.partStride = (size_t)p->nPair * p->nLag * p->pitch;
   dim3 g1(p->nPair, p->nLag);
-  k_lag_idft<<<g1, LAG_TH, 0, st>>>(LP);
+  if (p->Dmax <= 10) k_lag_idft<10><<<g1, LAG_TH, 0, st>>>(LP);
+  else k_lag_idft<30><<<g1, LAG_TH, 0, st>>>(LP);
   SFFT_LAUNCH_CHECK();
   ++*nl;
   GatherParams GP;

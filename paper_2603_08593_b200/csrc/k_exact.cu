@@ -308,12 +308,21 @@ static int exact_ksplit(int ntiles, int num_sms) {   // every CTA of the coopera
   return ks;
 }
 
-size_t sfft_exact_scratch_bytes(int N) {
+// the rank-K update keeps one 128 x 128 tile of the lower triangle per CTA of a cooperative launch: N + 1 <= 16 * 128
+// on a 148-SM device (w <= 5 always fits; w = 8 with DK = 2 is the largest kernel model that does)
+bool sfft_exact_supported(int N, int num_sms) {
+  const int ntb = (N + 1 + EX_T - 1) / EX_T;
+  return ntb * (ntb + 1) / 2 <= num_sms;
+}
+
+size_t sfft_exact_scratch_bytes(int N, int num_sms) {
+  if (!sfft_exact_supported(N, num_sms)) return 256;
   const int ntb = (N + 1 + EX_T - 1) / EX_T, ntiles = ntb * (ntb + 1) / 2;
   return (size_t)16 * ntiles * EX_T * EX_T * sizeof(double);
 }
 
-size_t sfft_exact_rows_bytes(int N) {
+size_t sfft_exact_rows_bytes(int N, int num_sms) {
+  if (!sfft_exact_supported(N, num_sms)) return 256;
   const int ntb = (N + 1 + EX_T - 1) / EX_T;
   return (size_t)EX_KC * ntb * EX_T * sizeof(double);
 }

@@ -58,7 +58,7 @@ __global__ void __launch_bounds__(256) k_xs_colcount(const unsigned char* __rest
 // other by one thread per direction on shared-memory copies of the index arrays.
 #define XS_MAXC 128   // full lines looked at per direction
 __global__ void __launch_bounds__(1024) k_xs_plan(const int* __restrict__ rowcnt, const int* __restrict__ colcnt, int H, int W,
-                                                  int w, XsPlan* plans, unsigned char* rowFull, unsigned char* colFull,
+                                                  int w, int maxT, XsPlan* plans, unsigned char* rowFull, unsigned char* colFull,
                                                   int* srcIdxY, int* srcIdxX) {
   extern __shared__ int xs_sm[];
   int* sY = xs_sm;              // [H]
@@ -101,7 +101,7 @@ __global__ void __launch_bounds__(1024) k_xs_plan(const int* __restrict__ rowcnt
     int* sidx = dir ? sX : sY;
     XsPlan& P = sp[dir];
     int nT = 0, nS = 0;
-    for (int ic = 0; ic < ncand[dir] && nT < XS_MAXT; ++ic) {
+    for (int ic = 0; ic < ncand[dir] && nT < maxT; ++ic) {
       const int l = cand[dir][ic];
       int need = 0;
       for (int s = -w; s <= w; ++s) need += sidx[(l - s + M) % M] < 0 ? 1 : 0;
@@ -367,7 +367,8 @@ sfft_status sfft_launch_exact_update(sfft_plan* p, const double* R, const double
   const int H = p->H, W = p->W, rowsPerBlock = 8;
   const int rowBlocks = (H + rowsPerBlock - 1) / rowsPerBlock;
   XsPlan* plans = reinterpret_cast<XsPlan*>(p->xsPlan);
-  // 1. masked pixels per row and per column, the accepted full lines
+  // 1. masked pixels per row and per column, the accepted full lines (none for w > SFFT_XS_MAXW, whose lag
+  //    range the strip correlations are not compiled for: every masked pixel then takes the rank-K update)
   SFFT_CUDA_TRY(cudaMemsetAsync(p->xsColCnt, 0, sizeof(int) * (size_t)W, st));
   k_xs_colcount<<<dim3((W + 255) / 256, (H + 63) / 64), 256, 0, st>>>(mask, H, W, p->xsColCnt);
   SFFT_LAUNCH_CHECK();
@@ -376,7 +377,7 @@ sfft_status sfft_launch_exact_update(sfft_plan* p, const double* R, const double
   SFFT_CUDA_TRY(cudaMemsetAsync(p->xsColFull, 0, (size_t)W, st));
   k_xs_list<false, 1><<<rowBlocks, 32 * rowsPerBlock, 0, st>>>(mask, p->xsRowFull, p->xsColFull, H, W, p->spCount, nullptr, nullptr);
   SFFT_LAUNCH_CHECK();
-  k_xs_plan<<<1, 1024, sizeof(int) * (size_t)(H + W), st>>>(p->spCount, p->xsColCnt, H, W, p->w, plans, p->xsRowFull, p->xsColFull, p->xsSrcIdxY, p->xsSrcIdxX);
+  k_xs_plan<<<1, 1024, sizeof(int) * (size_t)(H + W), st>>>(p->spCount, p->xsColCnt, H, W, p->w, p->w <= SFFT_XS_MAXW ? XS_MAXT : 0, plans, p->xsRowFull, p->xsColFull, p->xsSrcIdxY, p->xsSrcIdxX);
   SFFT_LAUNCH_CHECK();
   *nl += 3;
   // 2. the two directions' strips, correlations and terms

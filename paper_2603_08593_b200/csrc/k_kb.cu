@@ -185,8 +185,11 @@ __device__ __forceinline__ void kb_corr_body(const KbParams& P) {
   __shared__ unsigned char sm[KB_CH];
   const int tid = threadIdx.x;
   const int W = P.W, H = P.H, w = P.w, S1 = 2 * w + 1;
-  const int s = tid % P.L, sub = tid / P.L;
-  const bool active = sub < P.nsub;
+  // L <= KB_TH: thread = (shift s, pixel subset sub), grid.z = 1; L > KB_TH (w > 5): one shift per thread, the
+  // shifts spread over grid.z CTAs, a single subset
+  const bool wide = P.L > KB_TH;
+  const int s = wide ? (int)blockIdx.z * KB_TH + tid : tid % P.L, sub = wide ? 0 : tid / P.L;
+  const bool active = wide ? s < P.L : sub < P.nsub;
   const int u = s % S1 - w, v = s / S1 - w;
   const double invW = 1.0 / (double)W, invH = 1.0 / (double)H;
   const int nsp = P.spOff[H];
@@ -301,7 +304,7 @@ __global__ void __launch_bounds__(256) k_kb_reduce(const double* __restrict__ pa
 
 template <int NT, int TB>
 static sfft_status launch_kb_corr_t(const KbParams& P, cudaStream_t st) {
-  dim3 grid(SFFT_KB_NBLK, P.TK / NT);
+  dim3 grid(SFFT_KB_NBLK, P.TK / NT, (P.L + KB_TH - 1) / KB_TH);
   k_kb_corr<NT, TB><<<grid, KB_TH, 0, st>>>(P);
   SFFT_LAUNCH_CHECK();
   return SFFT_OK;
@@ -330,7 +333,7 @@ sfft_status sfft_launch_kb(sfft_plan* p, const double* R, const unsigned char* m
   P.R = R; P.mask = mask; P.spOff = p->spOff; P.spList = p->spList; P.part = p->kbPart;
   P.H = H; P.W = W; P.w = p->w; P.L = p->L; P.TK = p->TK; P.TB = p->TB;
   P.nsub = KB_TH / p->L;
-  if (P.nsub < 1) return SFFT_ERR_UNSUPPORTED;
+  if (P.nsub < 1) P.nsub = 1;   // L > KB_TH: see kb_corr_body
   for (int t = 0; t < p->TK; ++t) { P.monoK[t][0] = p->monoK[t][0]; P.monoK[t][1] = p->monoK[t][1]; }
   for (int t = 0; t < p->TB; ++t) { P.monoB[t][0] = p->monoB[t][0]; P.monoB[t][1] = p->monoB[t][1]; }
   sfft_status rs;

@@ -176,6 +176,43 @@ __global__ void __launch_bounds__(MIX_TH, MIX_MINB) k_mix(MixParams P) {
   }
 }
 
+// y-mixing for kernel half-widths above 5 (no register window: 2w+1 > 11 source rows per output row do not
+// fit beside the accumulators).  Thread = one (y, kx); every (monomial, v) term is read from global memory
+// (L1/L2-resident: neighbouring rows share their source rows).  Same sums as k_mix, monomial-major order.
+__global__ void __launch_bounds__(MIX_TH) k_mix_gen(MixParams P, int w) {
+  const int H = P.H, NC = P.NC, KT = P.KT, S1 = 2 * w + 1;
+  const int kx = blockIdx.x * KT + threadIdx.x % KT;
+  const int y = blockIdx.y * (MIX_TH / KT) + threadIdx.x / KT;
+  if (y >= H || kx >= NC) return;
+  const double invH = 1.0 / (double)H;
+  cplx acc = cmake(0.0, 0.0);
+  for (int t = 0; t < P.TK; ++t) {
+    int d = 0;                       // monomial t = (p, q) of the order "for d: for q <= d: p = d - q"
+    while ((d + 1) * (d + 2) / 2 <= t) ++d;
+    const int q = t - d * (d + 1) / 2, p = d - q;
+    for (int vi = 0; vi < S1; ++vi) {
+      const int yy = (y - vi + w + H) & (H - 1);
+      const double eq = ipow((double)(2 * yy + 1 - H) * invH, q);
+      const cplx e = P.E[((size_t)t * S1 + vi) * NC + kx];
+      const cplx g = P.G[((size_t)p * H + yy) * NC + kx];
+      if (kx == 0) {                 // packed column (X[0], X[W/2]): both real with real factors, component-wise
+        acc.x = fma(e.x * eq, g.x, acc.x);
+        acc.y = fma(e.y * eq, g.y, acc.y);
+      } else {
+        cfma(acc, cmake(e.x * eq, e.y * eq), g);
+      }
+    }
+  }
+  P.Mhat[(size_t)y * NC + kx] = acc;
+}
+
+static sfft_status launch_mix_gen(const MixParams& MP, int w, cudaStream_t st) {
+  dim3 grid((MP.NC + MP.KT - 1) / MP.KT, (MP.H + MIX_TH / MP.KT - 1) / (MIX_TH / MP.KT));
+  k_mix_gen<<<grid, MIX_TH, 0, st>>>(MP, w);
+  SFFT_LAUNCH_CHECK();
+  return SFFT_OK;
+}
+
 template <int WK>
 static sfft_status launch_mix_t(const MixParams& MP, cudaStream_t st) {
   const int rowsPerBlock = (MIX_TH / MP.KT) * MIX_RY;
@@ -227,7 +264,7 @@ sfft_status sfft_launch_subtract(sfft_plan* p, const double* R, const double* S,
       case 3: s = launch_mix_t<3>(MP, st); break;
       case 4: s = launch_mix_t<4>(MP, st); break;
       case 5: s = launch_mix_t<5>(MP, st); break;
-      default: s = SFFT_ERR_UNSUPPORTED; break;
+      default: s = launch_mix_gen(MP, p->w, st); break;   // w > 5
     }
   }
   if (s != SFFT_OK) return s;

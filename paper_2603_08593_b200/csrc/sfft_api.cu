@@ -100,7 +100,6 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   *out = nullptr;
   if (!is_pow2(H) || !is_pow2(W) || H < 16 || W < 16 || H > 4096 || W > 4096) return SFFT_ERR_UNSUPPORTED;
   if (w < 0 || w > SFFT_MAX_W || 4 * w + 1 > (H < W ? H : W)) return SFFT_ERR_UNSUPPORTED;
-  if (w > 5) return SFFT_ERR_UNSUPPORTED;  // lag half-ranges above 10 need the split-range path (not built yet)
   if (DK < 0 || DK > SFFT_MAX_DEG || DB < 0 || DB > SFFT_MAX_DEG) return SFFT_ERR_UNSUPPORTED;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return SFFT_ERR_CUDA; }
@@ -125,7 +124,7 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   p->nMomS = DB + 1;
   p->nMomR = DK + DB + 1;
   p->ldL = (p->N + 1 + 3) & ~3;
-  p->fused = sfft_colx_supported(H, p->nPair) ? 1 : 0;
+  p->fused = sfft_colx_supported(H, p->nPair, p->Dmax) ? 1 : 0;
   p->nPart = 1;
   p->pitchT = p->NC;
   for (int a = 0; a <= 2 * SFFT_MAX_DEG; ++a) {   // whole-row sums of xi^a (odd powers cancel exactly)
@@ -211,8 +210,8 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
     dalloc((void**)&p->kbCorr, sizeof(double) * (size_t)p->TK * p->L * p->TB);
     dalloc((void**)&p->kbStrip, sizeof(double) * (size_t)p->TK * p->L * p->TB);
   }
-  dalloc((void**)&p->exScratch, sfft_exact_scratch_bytes(p->N));
-  dalloc((void**)&p->exRows, sfft_exact_rows_bytes(p->N));   // here, so that no hot call ever allocates
+  dalloc((void**)&p->exScratch, sfft_exact_scratch_bytes(p->N, p->num_sms));
+  dalloc((void**)&p->exRows, sfft_exact_rows_bytes(p->N, p->num_sms));   // here, so that no hot call ever allocates
   dalloc((void**)&p->exBar, 2 * sizeof(unsigned));
   dalloc((void**)&p->xsPlan, sfft_xs_plan_bytes());
   dalloc((void**)&p->xsColCnt, sizeof(int) * (size_t)W);
@@ -340,6 +339,7 @@ sfft_status sfft_build_system_exact(sfft_plan* p, const double* R, const double*
                                     double* A, double* b, void* stream) {
   // every argument is validated before anything is enqueued
   if (!build_args_ok(p, R, S, mask, A, b)) return SFFT_ERR_INVALID_ARG;
+  if (mask && !sfft_exact_supported(p->N, p->num_sms)) return SFFT_ERR_UNSUPPORTED;   // N > 2047 (some w > 5 models)
   if (cuda_error_pending()) return SFFT_ERR_CUDA;
   // the ordinary build on the unmasked images, then the masked pixels' rank-one terms are taken out
   sfft_status s = build_system_impl(p, R, S, nullptr, A, b, (cudaStream_t)stream);

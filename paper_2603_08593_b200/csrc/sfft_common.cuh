@@ -216,14 +216,15 @@ sfft_status sfft_launch_row_fwd(sfft_plan* p, const double* R, const double* S,
 sfft_status sfft_launch_col_fwd(sfft_plan* p, cudaStream_t st, int* nl);
 sfft_status sfft_launch_cross(sfft_plan* p, cudaStream_t st, int* nl);
 sfft_status sfft_launch_colx(sfft_plan* p, cudaStream_t st, int* nl);
-size_t sfft_exact_scratch_bytes(int N);
-size_t sfft_exact_rows_bytes(int N);
+bool sfft_exact_supported(int N, int num_sms);
+size_t sfft_exact_scratch_bytes(int N, int num_sms);
+size_t sfft_exact_rows_bytes(int N, int num_sms);
 size_t sfft_xs_plan_bytes();
 size_t sfft_xs_strip_bytes(int H, int W);
 size_t sfft_xs_q_bytes();
 sfft_status sfft_launch_exact_update(sfft_plan* p, const double* R, const double* S, const unsigned char* mask,
                                      double* A, double* b, cudaStream_t st, int* nl);
-bool sfft_colx_supported(int H, int nPair);
+bool sfft_colx_supported(int H, int nPair, int Dmax);
 sfft_status sfft_launch_kb(sfft_plan* p, const double* R, const unsigned char* mask, cudaStream_t st, int* nl);
 sfft_status sfft_launch_moments(sfft_plan* p, cudaStream_t st, int* nl);
 sfft_status sfft_launch_lag_gather(sfft_plan* p, double* A, double* b, cudaStream_t st, int* nl);

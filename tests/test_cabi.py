@@ -47,6 +47,7 @@ def test_argument_validation_needs_no_gpu():
     assert lib.sfft_plan_create(ctypes.byref(p), 32, 32, 9, 0, 0) == 2
     assert lib.sfft_plan_create(ctypes.byref(p), 8, 64, 0, 0, 0) == 2      # below the smallest size (16)
     assert lib.sfft_plan_create(ctypes.byref(p), 16, 16, 4, 0, 0) == 2     # 4w + 1 > min(H, W)
+    assert lib.sfft_plan_create(ctypes.byref(p), 128, 128, 16, 0, 0) == 2  # w above the largest half-width (15)
     assert lib.sfft_plan_create(None, 64, 64, 2, 0, 0) == 1
     assert p.value in (None, 0)
     assert lib.sfft_num_coeffs(None) == -1

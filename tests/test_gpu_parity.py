@@ -10,7 +10,7 @@ import pytest
 import torch
 
 from oracle import sfft_oracle as orc
-from paper_2603_08593_b200 import SfftPlan, synth
+from paper_2603_08593_b200 import SfftError, SfftPlan, synth
 
 pytestmark = pytest.mark.gpu
 
@@ -133,6 +133,35 @@ def test_fused_column_cross_path(H, W, w, DK, DB, masked):
     with SfftPlan(H, W, w, DK, DB) as plan:
         assert plan.fused == (DK <= 2)
     run_case(R, S, mask, w, DK, DB, 30.0, full_D=False)
+
+
+@pytest.mark.parametrize("H,W,w,DK,DB", [
+    (32, 64, 6, 1, 1), (32, 32, 7, 0, 0), (64, 64, 6, 2, 2), (64, 128, 8, 1, 0), (128, 64, 10, 1, 2),
+    (64, 64, 15, 0, 1), (64, 64, 11, 1, 1), (64, 64, 12, 0, 2), (64, 64, 13, 1, 0), (1024, 64, 6, 2, 1),
+    (2048, 32, 7, 1, 1), (64, 256, 9, 3, 0)])
+def test_kernel_half_widths_above_five(H, W, w, DK, DB):
+    """w = 6 .. 15 (lag half-ranges 12 .. 30): the cross kernel covers the lag range in windows of 25 lags
+    (1 window up to half-range 12, 3 above), the lag transform runs its 30-lag instantiation, the sparse
+    kernel-background kernel spreads L > 128 shifts over several CTAs and the mixing runs the plain kernel;
+    H >= 1024 falls back from the blocked column kernel to the generic column and cross kernels.  The
+    exact-objective system is compared too wherever N <= 2047 lets it run."""
+    rng = np.random.default_rng(H * 13 + W * 7 + w * 3 + DK)
+    R = 50.0 * rng.standard_normal((H, W)) + 500.0 * (rng.random((H, W)) > 0.97)
+    S = 0.8 * np.roll(R, (1, -1), (0, 1)) + 30.0 * rng.standard_normal((H, W)) + 150.0
+    mask = (rng.random((H, W)) < 0.03).astype(np.uint8)
+    run_case(R, S, mask, w, DK, DB, 30.0, full_D=False)
+    N = orc.num_coeffs(w, DK, DB)
+    with SfftPlan(H, W, w, DK, DB) as plan:
+        assert not plan.fused
+        if N <= 2047:
+            Ax, bx = orc.build_system_exact_fft(R, S, mask, w, DK, DB, workers=8)
+            Ae, be = plan.build_system_exact(dev(R), dev(S), dev(mask))
+            torch.cuda.synchronize()
+            check_system(Ae.cpu().numpy(), be.cpu().numpy(), Ax, bx, (2 * w + 1) ** 2, (DK + 1) * (DK + 2) // 2)
+        else:
+            with pytest.raises(SfftError) as e:
+                plan.build_system_exact(dev(R), dev(S), dev(mask))
+            assert e.value.code == 2
 
 
 @pytest.mark.parametrize("H,W", [(1024, 32), (2048, 32), (4096, 32), (2048, 64), (1024, 16)])
