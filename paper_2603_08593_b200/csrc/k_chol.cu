@@ -16,6 +16,7 @@
 // (<= 1 ulp), which keeps the 32 dependent steps of a diagonal block short.
 // info: 0, or the 1-based order of the first non-positive leading minor (no pivoting, no
 // regularisation: DESIGN.md reading A9).
+#include <mutex>
 #include "sfft_common.cuh"
 
 #define CH_NB 32
@@ -559,6 +560,7 @@ struct NaDevice {
   bool ready;
 };
 NaDevice na_dev[NA_MAXDEV];   // zero-initialised
+std::mutex na_mutex;
 }  // namespace
 
 extern "C" sfft_status sfft_solve_static(const double* A, const double* b, int N, double* coeffs, int* info,
@@ -571,9 +573,10 @@ extern "C" sfft_status sfft_solve_static(const double* A, const double* b, int N
   SFFT_CUDA_TRY(cudaGetDevice(&dev));
   if (dev < 0 || dev >= NA_MAXDEV) return SFFT_ERR_UNSUPPORTED;
   NaDevice& nd = na_dev[dev];
+  std::lock_guard<std::mutex> lock(na_mutex);   // set-up once per device; the launches below stay ordered per caller
   if (!nd.ready) {
     // once per device, with that device current: in host code the array's name is only a handle, the
-    // device address comes from the runtime.  (Concurrent first calls store the same values.)
+    // device address comes from the runtime
     double* ptr = nullptr;
     int sms = 0;
     SFFT_CUDA_TRY(cudaGetSymbolAddress((void**)&ptr, sfft_static_scratch));
