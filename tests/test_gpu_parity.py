@@ -281,6 +281,31 @@ def test_degenerate_all_masked_and_plan_reuse():
         assert plan.last_launch_count(0) > 0
 
 
+@pytest.mark.parametrize("cfg", [(2048, 4096, 5, 2, 2), (256, 256, 3, 1, 1), (32, 32, 0, 0, 0)])
+def test_solve_is_bitwise_independent_of_the_cta_cap(cfg):
+    """include/sfft.h, sfft_plan_set_solve_ctas: "Results are bitwise independent of the setting" -- grids of
+    1, 3, 16, 50 CTAs and the default (one per SM) on N = 732, 150 and 2, against the oracle's solve too."""
+    with SfftPlan(*cfg) as plan:
+        N = plan.N
+        rng = np.random.default_rng(N)
+        G = rng.standard_normal((2 * N + 20, N))
+        A = G.T @ G + 1e-3 * np.eye(N)
+        b = rng.standard_normal(N)
+        co = orc.solve(A, b)
+        Ad, bd = dev(A), dev(b)
+        ref = None
+        for cap in (0, 1, 3, 16, 50):
+            plan.set_solve_ctas(cap)
+            c, info = plan.solve(Ad, bd)
+            torch.cuda.synchronize()
+            assert int(info.item()) == 0
+            if ref is None:
+                ref = c.clone()
+                assert np.max(np.abs(ref.cpu().numpy() - co)) <= TOL_C * np.max(np.abs(co))
+            else:
+                assert torch.equal(c, ref), cap
+
+
 def test_non_default_stream():
     pr = synth.make_pair("tiny")
     cfg = pr.cfg
