@@ -550,12 +550,33 @@ def run_cuda(args, rank, world, local_rank):
         torch.cuda.synchronize()
         assert mt[3].cpu().tolist() == [0] * nT and torch.equal(outm, mt[0])
         t_mt, t_sep = g6.elapsed_time(g7) / 3, g7.elapsed_time(g8) / 3
+        # the same mode with the templates spread over three plans (sfft_multi_template_difference_plans: the
+        # solve of one template overlaps the transforms of the others; 16-CTA solve grids as in the exposure leg)
+        helpers = [SfftPlan(cfg.H, cfg.W, cfg.w, cfg.DK, cfg.DB) for _ in range(2)]
+        for q in [plan, *helpers]:
+            q.set_solve_ctas(SOLVE_CTAS_PIPELINED)
+        for _ in range(2):
+            mt3 = plan.multi_template_difference(Rt, Sx, Mx, sc, helpers=helpers)
+        g9, g10 = (torch.cuda.Event(enable_timing=True) for _ in range(2))
+        g9.record()
+        for _ in range(3):
+            mt3 = plan.multi_template_difference(Rt, Sx, Mx, sc, helpers=helpers)
+        g10.record()
+        torch.cuda.synchronize()
+        assert all(torch.equal(a, b) for a, b in zip(mt3, mt))
+        t_mt3 = g9.elapsed_time(g10) / 3
+        plan.set_solve_ctas(0)
+        for q in helpers:
+            q.close()
         post["multi_template"] = {"templates": nT, "ms": round(t_mt, 3), "ms_separate_calls": round(t_sep, 3),
-                                  "ccd_per_s": round(1e3 / t_mt, 1),
+                                  "ms_three_plans": round(t_mt3, 3),
+                                  "ccd_per_s": round(1e3 / t_mt, 1), "ccd_per_s_three_plans": round(1e3 / t_mt3, 1),
                                   "note": "one sfft_multi_template_difference call (row transform and moments of m S "
                                           "reused by templates 2..5) vs 5 x (build, prepare, solve, subtract) + "
-                                          "sfft_median_combine; bitwise equal results (asserted)"}
-        del mt, sep, Rt
+                                          "sfft_median_combine; ms_three_plans: sfft_multi_template_difference_plans "
+                                          "with the 5 templates spread over 3 plans (solves overlap the other "
+                                          "templates' transforms); bitwise equal results (asserted)"}
+        del mt, mt3, sep, Rt
         # three-channel stamps (NEXT-3): 1024 candidates, 63 x 63 pixels (size is the caller's)
         for _ in range(2):
             stp = cut_stamps(Sx, Rx, D, xs, ys, 63)

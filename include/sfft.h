@@ -153,6 +153,23 @@ sfft_status sfft_multi_template_difference(sfft_plan* p, const double* const* R,
                                            const unsigned char* mask, const double* scale, int n,
                                            double* Dk, double* coeffs, int* info, double* out, void* stream);
 
+/* The same mode with the n chains spread over several plans (the GPU works
+ * through a queue of independent differencings): template k runs on plans[k % nplans], so the
+ * latency-bound sfft_solve of one template overlaps the transforms of the others.  plans[0]'s chains are
+ * enqueued on `stream`; every other plan's go to a stream that plan owns, forked from `stream` at entry
+ * and joined back into it before the median (also on every error return) -- no host synchronisation,
+ * and work enqueued on `stream` after the call sees all outputs.  Each plan transforms m S once (for
+ * its first template).  Results are bitwise those of sfft_multi_template_difference.
+ *   plans in : HOST array of nplans distinct plans created with the same (H, W, w, DK, DB), none in
+ *              use by other in-flight work;  1 <= nplans <= SFFT_MAX_TEMPLATES (plans beyond n are
+ *              left untouched).  sfft_plan_set_solve_ctas applies per plan (a cap of about 16 CTAs
+ *              lets the solves run beside the other plans' transforms).
+ * Other arguments and errors as sfft_multi_template_difference (N, H, W are plans[0]'s). */
+sfft_status sfft_multi_template_difference_plans(sfft_plan* const* plans, int nplans, const double* const* R,
+                                                 const double* S, const unsigned char* mask, const double* scale,
+                                                 int n, double* Dk, double* coeffs, int* info, double* out,
+                                                 void* stream);
+
 /* Monte-Carlo limiting flux of a difference image (§2.3.3: "aperture fluxes at 1024
  * randomly selected background positions ... deriving the 5 sigma threshold from their standard
  * deviation").  The positions are INPUTS (the random draw is the caller's).

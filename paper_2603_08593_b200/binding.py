@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = [
     "sfft_status_string", "sfft_build_system", "sfft_build_system_exact", "sfft_solve", "sfft_subtract", "sfft_subtract_prepare",
     "sfft_probe_fp64", "sfft_last_launch_count", "sfft_plan_fused", "sfft_plan_set_solve_ctas", "sfft_version",
     "sfft_profile_enable", "sfft_profile_read", "sfft_median_combine", "sfft_aperture_stats", "sfft_resample_affine", "sfft_resample_mask_affine",
-    "sfft_cut_stamps", "sfft_multi_template_difference", "sfft_solve_static",
+    "sfft_cut_stamps", "sfft_multi_template_difference", "sfft_multi_template_difference_plans", "sfft_solve_static",
 ]
 
 SOLVE_STATIC_MAX_N = 768   # SFFT_SOLVE_STATIC_MAX_N (include/sfft.h)
@@ -90,6 +90,8 @@ def load_library():
     lib.sfft_cut_stamps.restype = i32
     lib.sfft_multi_template_difference.argtypes = [vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp]
     lib.sfft_multi_template_difference.restype = i32
+    lib.sfft_multi_template_difference_plans.argtypes = [vp, i32, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp]
+    lib.sfft_multi_template_difference_plans.restype = i32
     lib.sfft_aperture_stats.argtypes = [vp, vp, i32, i32, vp, vp, i32, ctypes.c_double, vp, vp, vp]
     lib.sfft_aperture_stats.restype = i32
     lib.sfft_resample_affine.argtypes = [vp, i32, i32, vp, i32, vp, i32, i32, vp, vp]
@@ -227,10 +229,12 @@ class SfftPlan:
         _check(self._lib, self._lib.sfft_subtract_prepare(
             self._p, _dev_ptr(R, torch.float64, self.H * self.W, "R"), _stream_handle(stream)), "sfft_subtract_prepare")
 
-    def multi_template_difference(self, Rs, S, mask, scales, stream=None):
+    def multi_template_difference(self, Rs, S, mask, scales, stream=None, helpers=()):
         """sfft_multi_template_difference: S against every template of Rs with one
         common mask, then the median of the scaled differences.  Returns (out, Dk, coeffs, info) with
-        Dk [n, H, W], coeffs [n, N], info [n]."""
+        Dk [n, H, W], coeffs [n, N], info [n].  helpers: further SfftPlan objects of the same
+        configuration; template k then runs on plan k % (1 + len(helpers))
+        (sfft_multi_template_difference_plans), bitwise the same results."""
         import torch
         n, P = len(Rs), self.H * self.W
         dev = S.device
@@ -240,11 +244,13 @@ class SfftPlan:
         coeffs = torch.empty((n, self.N), dtype=torch.float64, device=dev)
         info = torch.zeros(n, dtype=torch.int32, device=dev)
         out = torch.empty((self.H, self.W), dtype=torch.float64, device=dev)
-        _check(self._lib, self._lib.sfft_multi_template_difference(
-            self._p, ptrs, _dev_ptr(S, torch.float64, P, "S"), _dev_ptr(mask, torch.uint8, P, "mask"), sc, n,
+        plans = [self, *helpers]
+        pl = (ctypes.c_void_p * len(plans))(*[q._p for q in plans])
+        _check(self._lib, self._lib.sfft_multi_template_difference_plans(
+            pl, len(plans), ptrs, _dev_ptr(S, torch.float64, P, "S"), _dev_ptr(mask, torch.uint8, P, "mask"), sc, n,
             _dev_ptr(Dk, torch.float64, n * P, "Dk"), _dev_ptr(coeffs, torch.float64, n * self.N, "coeffs"),
             _dev_ptr(info, torch.int32, n, "info"), _dev_ptr(out, torch.float64, P, "out"),
-            _stream_handle(stream)), "sfft_multi_template_difference")
+            _stream_handle(stream)), "sfft_multi_template_difference_plans")
         return out, Dk, coeffs, info
 
     def difference(self, R, S, mask, stream=None):

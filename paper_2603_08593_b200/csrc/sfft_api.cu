@@ -70,6 +70,9 @@ static void plan_free(sfft_plan* p) {
   cudaFree(p->mom); cudaFree(p->spCount); cudaFree(p->spOff); cudaFree(p->spList); cudaFree(p->fmFlag); cudaFree(p->fmList); cudaFree(p->kbPart); cudaFree(p->kbCorr); cudaFree(p->kbStrip); cudaFree(p->Lw); cudaFree(p->exScratch); cudaFree(p->exRows); cudaFree(p->exBar); cudaFree(p->xsPlan); cudaFree(p->xsColCnt); cudaFree(p->xsRowFull); cudaFree(p->xsColFull); cudaFree(p->xsSrcIdxY); cudaFree(p->xsSrcIdxX); cudaFree(p->xsZ); cudaFree(p->xsQ); cudaFree(p->xsCnt); cudaFree(p->xsOff); cudaFree(p->xsList); cudaFree(p->cholBar); cudaFree(p->mtA); cudaFree(p->mtB); cudaFree(p->Etab); cudaFree(p->Mhat);
   free(p->h_pairs);
   if (p->side) cudaStreamDestroy(p->side);
+  if (p->work) cudaStreamDestroy(p->work);
+  if (p->evWork) cudaEventDestroy(p->evWork);
+  if (p->evBuilt) cudaEventDestroy(p->evBuilt);
   if (p->evFork) cudaEventDestroy(p->evFork);
   if (p->evJoin) cudaEventDestroy(p->evJoin);
   if (p->evRow) cudaEventDestroy(p->evRow);
@@ -172,6 +175,9 @@ sfft_status sfft_plan_create(sfft_plan** out, int H, int W, int w, int DK, int D
   int prLo = 0, prHi = 0;   // the side stream's small kernels take free slots ahead of the big grids
   cudaDeviceGetStreamPriorityRange(&prLo, &prHi);
   if (cudaStreamCreateWithPriority(&p->side, cudaStreamNonBlocking, prHi) != cudaSuccess ||
+      cudaStreamCreateWithPriority(&p->work, cudaStreamNonBlocking, prLo) != cudaSuccess ||
+      cudaEventCreateWithFlags(&p->evWork, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&p->evBuilt, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->evFork, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->evJoin, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->evRow, cudaEventDisableTiming) != cudaSuccess ||
@@ -396,42 +402,95 @@ sfft_status sfft_subtract_prepare(sfft_plan* p, const double* R, void* stream) {
   return subtract_prepare_impl(p, R, (cudaStream_t)stream);
 }
 
+// One template of the multi-template mode on plan p and stream st: build (the science image's row transform
+// and moments reused when reuseS), prepare, solve, subtract.  *nlTot receives the launches.
+// after: the previous template's "build enqueued and finished" event when that template runs on another plan
+// (the builds are throughput-bound, so they run one after the other and each solve falls beside the NEXT
+// template's build instead of beside its peers' solves); p->evBuilt is recorded after this build.
+static sfft_status mt_chain(sfft_plan* p, const double* Rk, const double* S, const unsigned char* mask, bool reuseS,
+                            double* ck, int* infok, double* Dcur, cudaStream_t st, cudaEvent_t after, int* nlTot) {
+  if (after) SFFT_CUDA_TRY(cudaStreamWaitEvent(st, after, 0));
+  sfft_status s = build_system_impl(p, Rk, S, mask, p->mtA, p->mtB, st, reuseS);
+  if (s != SFFT_OK) return s;
+  SFFT_CUDA_TRY(cudaEventRecord(p->evBuilt, st));
+  *nlTot += p->launches[0];
+  // the coefficient-independent row transforms of the subtraction run beside the latency-bound solve
+  s = subtract_prepare_impl(p, Rk, st);
+  if (s != SFFT_OK) return s;
+  int nl = 0;
+  { ProfScope ps(p, 5, st); s = sfft_launch_solve(p, p->mtA, p->mtB, ck, infok, st, &nl); }
+  if (s != SFFT_OK) return fail_joined(p, st, s);
+  *nlTot += nl;
+  nl = p->launches[2];
+  s = sfft_launch_subtract(p, Rk, S, ck, Dcur, st, &nl);
+  if (s != SFFT_OK) return s;
+  *nlTot += nl;
+  return SFFT_OK;
+}
+
+static bool mt_args_ok(const sfft_plan* p, const double* const* R, const double* S, const unsigned char* mask,
+                       const double* scale, int n, const double* Dk, const double* coeffs, const double* out) {
+  if (!p || !R || !S || !scale || !Dk || !coeffs || !out || n < 1 || n > SFFT_MAX_TEMPLATES) return false;
+  if (!aligned16(S) || !aligned16(Dk) || !aligned16(out) || (mask && !aligned16(mask))) return false;
+  const size_t npix = (size_t)p->H * p->W;
+  for (int k = 0; k < n; ++k)
+    if (!R[k] || !aligned16(R[k]) || R[k] == out || R[k] == S) return false;
+  if (out == S || (out >= Dk && out < Dk + (size_t)n * npix)) return false;
+  return true;
+}
+
 sfft_status sfft_multi_template_difference(sfft_plan* p, const double* const* R, const double* S,
                                            const unsigned char* mask, const double* scale, int n,
                                            double* Dk, double* coeffs, int* info, double* out, void* stream) {
-  if (!p || !R || !S || !scale || !Dk || !coeffs || !out || n < 1 || n > SFFT_MAX_TEMPLATES) return SFFT_ERR_INVALID_ARG;
-  if (!aligned16(S) || !aligned16(Dk) || !aligned16(out) || (mask && !aligned16(mask))) return SFFT_ERR_INVALID_ARG;
-  const size_t npix = (size_t)p->H * p->W;
-  for (int k = 0; k < n; ++k)
-    if (!R[k] || !aligned16(R[k]) || R[k] == out || R[k] == S) return SFFT_ERR_INVALID_ARG;
-  if (out == S || (out >= Dk && out < Dk + (size_t)n * npix)) return SFFT_ERR_INVALID_ARG;
+  return sfft_multi_template_difference_plans(&p, 1, R, S, mask, scale, n, Dk, coeffs, info, out, stream);
+}
+
+sfft_status sfft_multi_template_difference_plans(sfft_plan* const* plans, int nplans, const double* const* R,
+                                                 const double* S, const unsigned char* mask, const double* scale,
+                                                 int n, double* Dk, double* coeffs, int* info, double* out,
+                                                 void* stream) {
+  if (!plans || nplans < 1 || nplans > SFFT_MAX_TEMPLATES || !plans[0]) return SFFT_ERR_INVALID_ARG;
+  sfft_plan* p = plans[0];
+  if (!mt_args_ok(p, R, S, mask, scale, n, Dk, coeffs, out)) return SFFT_ERR_INVALID_ARG;
+  for (int q = 1; q < nplans; ++q) {
+    const sfft_plan* h = plans[q];
+    if (!h || h->H != p->H || h->W != p->W || h->w != p->w || h->DK != p->DK || h->DB != p->DB) return SFFT_ERR_INVALID_ARG;
+    for (int r = 0; r < q; ++r)
+      if (plans[r] == h) return SFFT_ERR_INVALID_ARG;
+  }
   if (cuda_error_pending()) return SFFT_ERR_CUDA;
   cudaStream_t st = (cudaStream_t)stream;
+  const size_t npix = (size_t)p->H * p->W;
+  const int np = nplans < n ? nplans : n;
+  // helper plans run their chains on their own work streams, forked from the caller stream here and joined
+  // back into it before the median (and on every failure path): no host synchronisation
+  if (np > 1) {
+    SFFT_CUDA_TRY(cudaEventRecord(p->evWork, st));
+    for (int q = 1; q < np; ++q) SFFT_CUDA_TRY(cudaStreamWaitEvent(plans[q]->work, p->evWork, 0));
+  }
+  auto join = [&]() {
+    bool ok = true;
+    for (int q = 1; q < np; ++q)
+      ok = cudaEventRecord(plans[q]->evWork, plans[q]->work) == cudaSuccess &&
+           cudaStreamWaitEvent(st, plans[q]->evWork, 0) == cudaSuccess && ok;
+    if (!ok) cudaGetLastError();
+    return ok;
+  };
   const double* dptr[SFFT_MAX_TEMPLATES];
   int nlTot = 0;
   for (int k = 0; k < n; ++k) {
+    sfft_plan* h = plans[k % np];
     double* Dcur = Dk + (size_t)k * npix;
-    sfft_status s = build_system_impl(p, R[k], S, mask, p->mtA, p->mtB, st, k > 0);
-    if (s != SFFT_OK) return s;
-    nlTot += p->launches[0];
-    // the coefficient-independent row transforms of the subtraction run beside the latency-bound solve
-    s = subtract_prepare_impl(p, R[k], st);
-    if (s != SFFT_OK) return s;
-    int nl = 0;
-    { ProfScope ps(p, 5, st); s = sfft_launch_solve(p, p->mtA, p->mtB, coeffs + (size_t)k * p->N, info ? info + k : nullptr, st, &nl); }
-    if (s != SFFT_OK) return fail_joined(p, st, s);
-    nlTot += nl;
-    nl = p->launches[2];
-    s = sfft_launch_subtract(p, R[k], S, coeffs + (size_t)k * p->N, Dcur, st, &nl);
-    if (s != SFFT_OK) return s;
-    nlTot += nl;
+    sfft_status s = mt_chain(h, R[k], S, mask, k >= np, coeffs + (size_t)k * p->N, info ? info + k : nullptr, Dcur,
+                             k % np == 0 ? st : h->work, (np > 1 && k > 0) ? plans[(k - 1) % np]->evBuilt : nullptr, &nlTot);
+    if (s != SFFT_OK) { join(); return s; }
     dptr[k] = Dcur;
   }
+  if (!join()) return SFFT_ERR_CUDA;
   sfft_status s = sfft_median_combine(dptr, scale, n, npix, out, stream);
   if (s != SFFT_OK) return s;
-  p->launches[0] = nlTot + 1;   // the whole chain is reported as one "build" count
-  p->launches[1] = 0;
-  p->launches[2] = 0;
+  for (int q = 0; q < np; ++q) { plans[q]->launches[0] = 0; plans[q]->launches[1] = 0; plans[q]->launches[2] = 0; }
+  p->launches[0] = nlTot + 1;   // the whole chain is reported as one "build" count of the first plan
   return SFFT_OK;
 }
 

@@ -157,6 +157,9 @@ struct sfft_plan {
   // (forked from and joined back into the caller stream with events; no host synchronisation)
   cudaStream_t side;
   cudaEvent_t evFork, evJoin, evRow, evPrep;
+  // sfft_multi_template_difference_plans: the chains a helper plan runs go to its own work stream
+  cudaStream_t work;
+  cudaEvent_t evWork, evBuilt;
   // sfft_subtract_prepare: the row spectra of xi^p R for the next sfft_subtract are already in T
   const double* prepR;
   int prepValid;

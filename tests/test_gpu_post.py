@@ -197,6 +197,52 @@ def test_multi_template_mode_parity_and_reuse(H, W, w, DK, DB, n, masked):
         assert torch.equal(median_combine(sep, scales), out)
 
 
+@pytest.mark.parametrize("H,W,w,DK,DB,n,nplans", [(1024, 64, 2, 2, 2, 5, 3), (64, 64, 2, 1, 1, 5, 2),
+                                                   (128, 256, 3, 2, 1, 3, 3), (1024, 32, 1, 0, 0, 2, 3)])
+def test_multi_template_mode_over_several_plans(H, W, w, DK, DB, n, nplans):
+    """sfft_multi_template_difference_plans (template k on plans[k % nplans], helper plans on their own
+    streams, each with the 16-CTA solve grid bench.py uses): every output bitwise equal to the
+    single-plan call, twice in a row (the second call finds the plans' scratch used by the first), and
+    the chain against the oracle at the parity tolerances.  nplans > n leaves the extra plans idle."""
+    from paper_2603_08593_b200 import SfftPlan
+    Rs, S, mask = _templates(7 * H + W + n, H, W, n)
+    scales = list(np.linspace(1.1, 0.9, n))
+    Dm_o, Ds_o, cs_o = po.multi_template_difference(Rs, S, mask, w, DK, DB, scales, workers=8)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    Rd, Sd, Md = [t(R) for R in Rs], t(S), t(mask)
+    sky = 30.0
+    plans = [SfftPlan(H, W, w, DK, DB) for _ in range(nplans)]
+    try:
+        ref = plans[0].multi_template_difference(Rd, Sd, Md, scales)
+        for pl in plans:
+            pl.set_solve_ctas(16)
+        st = torch.cuda.Stream()
+        st.wait_stream(torch.cuda.current_stream())
+        for rep in range(2):
+            with torch.cuda.stream(st):
+                got = plans[0].multi_template_difference(Rd, Sd, Md, scales, stream=st, helpers=plans[1:])
+                after = got[0] + 1.0          # work enqueued after the call sees the joined result
+            st.synchronize()
+            for a, b in zip(got, ref):
+                assert torch.equal(a, b)
+            assert torch.equal(after, ref[0] + 1.0)
+        out, Dk, coeffs, info = got
+        assert info.cpu().tolist() == [0] * n
+        for k in range(n):
+            assert np.max(np.abs(coeffs[k].cpu().numpy() - cs_o[k])) <= 1e-7 * np.max(np.abs(cs_o[k]))
+            assert np.max(np.abs(Dk[k].cpu().numpy() - Ds_o[k])) <= 1e-6 * sky
+        assert np.max(np.abs(out.cpu().numpy() - Dm_o)) <= 1e-6 * sky * max(scales)
+        # a helper of another configuration, or the same plan twice, is refused before anything is enqueued
+        with SfftPlan(H, W, w, DK, max(DB - 1, 0) if DB else 1) as other:
+            with pytest.raises(Exception):
+                plans[0].multi_template_difference(Rd, Sd, Md, scales, helpers=[other])
+        with pytest.raises(Exception):
+            plans[0].multi_template_difference(Rd, Sd, Md, scales, helpers=[plans[0]])
+    finally:
+        for pl in plans:
+            pl.close()
+
+
 def test_multi_template_mode_rejects_an_artefact_in_one_template():
     from paper_2603_08593_b200 import SfftPlan
     Rs, S, mask = _templates(77, 64, 64, 1)
