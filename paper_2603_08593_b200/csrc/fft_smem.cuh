@@ -200,12 +200,14 @@ struct FftCfg {
   static __host__ __device__ constexpr int phys(int n) { return n + (n >> PADSHIFT); }
 };
 
-// Butterfly index i -> (sequence, butterfly j).  SEQ_FAST: adjacent threads work on adjacent
-// sequences (the column kernels, where adjacent sequences are adjacent in global memory).
-template <int NB, bool SEQ_FAST>
-__device__ __forceinline__ void fft_map(int i, int nseq, int& seq, int& j) {
-  if (SEQ_FAST) { seq = i % nseq; j = i / nseq; }
-  else { seq = i / NB; j = i & (NB - 1); }
+// Butterfly m of thread tid -> (sequence, butterfly j).  SEQ_FAST: adjacent threads work on adjacent
+// sequences (the column kernels, where adjacent sequences are adjacent in global memory).  Otherwise a
+// sequence belongs to TPS = N/EPT consecutive threads in EVERY pass (butterflies j = t + m TPS of thread t), so
+// the threads of one sequence exchange data only among themselves and may meet at a barrier of their own.
+template <int NB, bool SEQ_FAST, int TPS>
+__device__ __forceinline__ void fft_map(int tid, int m, int nth, int nseq, int& seq, int& j) {
+  if (SEQ_FAST) { const int i = tid + m * nth; seq = i % nseq; j = i / nseq; }
+  else { seq = tid / TPS; j = (tid - seq * TPS) + m * TPS; }
 }
 
 // twiddle + butterfly + Stockham store of one radix-R butterfly held in v[]
@@ -276,21 +278,40 @@ __device__ __forceinline__ void fft_store(const cplx* v, cplx* base, int j) {
   for (int r = 0; r < R; ++r) base[C::phys(o + r * NS)] = v[r];
 }
 
+// Barrier policies of the passes: the whole CTA (default), or a named barrier over the threads of one group of
+// sequences (a kernel whose sequences are exchanged only inside such a group lets the groups drift apart).
+struct FftSyncCta {
+  __device__ __forceinline__ void operator()() const { __syncthreads(); }
+};
+template <int MAXID>
+struct FftSyncNamed {
+  int id, n;   // barrier 1..MAXID (immediate operands below, so the kernel reserves MAXID + 1 barriers, not 16); n threads, a multiple of 32
+  __device__ __forceinline__ void operator()() const {
+#define SFFT_BAR_CASE(I) case I: if constexpr (I <= MAXID) asm volatile("bar.sync " #I ", %0;\n" ::"r"(n) : "memory"); break;
+    switch (id) {
+      SFFT_BAR_CASE(1) SFFT_BAR_CASE(2) SFFT_BAR_CASE(3) SFFT_BAR_CASE(4)
+      SFFT_BAR_CASE(5) SFFT_BAR_CASE(6) SFFT_BAR_CASE(7) SFFT_BAR_CASE(8)
+      default: break;
+    }
+#undef SFFT_BAR_CASE
+  }
+};
+
 // Pass 0 from registers: the calling thread supplies v[r] = x[seq][j + r*N/EPT], r < EPT, for the
 // butterfly (seq, j) it chose (any one-to-one assignment of threads to butterflies).  Ends with a
 // barrier unless the transform has a single pass and NOSYNC is set.
-template <int N, int DIR>
-__device__ __forceinline__ void fft_first_from_regs(cplx* v, cplx* s, int seq, int j, int seq_stride) {
+template <int N, int DIR, typename Sync = FftSyncCta>
+__device__ __forceinline__ void fft_first_from_regs(cplx* v, cplx* s, int seq, int j, int seq_stride, Sync sync = Sync()) {
   using C = FftCfg<N>;
   Dft<C::EPT, DIR>::run(v);
   fft_store<N, C::EPT, 1>(v, s + seq * seq_stride, j);
-  __syncthreads();
+  sync();
 }
 
 // One in-place pass shared memory -> shared memory.
-template <int N, int R, int NS, int DIR, bool SEQ_FAST>
+template <int N, int R, int NS, int DIR, bool SEQ_FAST, typename Sync = FftSyncCta>
 __device__ __forceinline__ void fft_pass(cplx* s, int tid, int nth, int nseq, const cplx* __restrict__ tw,
-                                         const int seq_stride) {
+                                         const int seq_stride, Sync sync = Sync()) {
   using C = FftCfg<N>;
   constexpr int NB = N / R;        // butterflies per sequence
   constexpr int IT = C::EPT / R;   // butterflies per thread
@@ -300,26 +321,26 @@ __device__ __forceinline__ void fft_pass(cplx* s, int tid, int nth, int nseq, co
 #pragma unroll
   for (int m = 0; m < IT; ++m) {
     int seq, j;
-    fft_map<NB, SEQ_FAST>(tid + m * nth, nseq, seq, j);
+    fft_map<NB, SEQ_FAST, N / C::EPT>(tid, m, nth, nseq, seq, j);
     fft_twiddle_load<N, R, NS>(t[m], j, tw);
   }
 #pragma unroll
   for (int m = 0; m < IT; ++m) {
     int seq, j;
-    fft_map<NB, SEQ_FAST>(tid + m * nth, nseq, seq, j);
+    fft_map<NB, SEQ_FAST, N / C::EPT>(tid, m, nth, nseq, seq, j);
     const cplx* base = s + seq * seq_stride;
 #pragma unroll
     for (int r = 0; r < R; ++r) v[m][r] = base[C::phys(j + r * NB)];
   }
-  __syncthreads();
+  sync();
 #pragma unroll
   for (int m = 0; m < IT; ++m) {
     int seq, j;
-    fft_map<NB, SEQ_FAST>(tid + m * nth, nseq, seq, j);
+    fft_map<NB, SEQ_FAST, N / C::EPT>(tid, m, nth, nseq, seq, j);
     fft_twiddle_apply<N, R, NS, DIR>(v[m], t[m]);
     fft_store<N, R, NS>(v[m], s + seq * seq_stride, j);
   }
-  __syncthreads();
+  sync();
 }
 
 // Last pass, outputs left in registers: butterfly m of the thread is (seq[m], j[m]) from fft_map
@@ -334,13 +355,13 @@ __device__ __forceinline__ void fft_pass_to_regs(const cplx* s, cplx* v, int tid
 #pragma unroll
   for (int m = 0; m < IT; ++m) {
     int seq, j;
-    fft_map<NB, SEQ_FAST>(tid + m * nth, nseq, seq, j);
+    fft_map<NB, SEQ_FAST, N / C::EPT>(tid, m, nth, nseq, seq, j);
     fft_twiddle_load<N, R, NS>(t[m], j, tw);
   }
 #pragma unroll
   for (int m = 0; m < IT; ++m) {
     int seq, j;
-    fft_map<NB, SEQ_FAST>(tid + m * nth, nseq, seq, j);
+    fft_map<NB, SEQ_FAST, N / C::EPT>(tid, m, nth, nseq, seq, j);
     const cplx* base = s + seq * seq_stride;
 #pragma unroll
     for (int r = 0; r < R; ++r) v[m * R + r] = base[C::phys(j + r * NB)];
@@ -349,11 +370,11 @@ __device__ __forceinline__ void fft_pass_to_regs(const cplx* s, cplx* v, int tid
   for (int m = 0; m < IT; ++m) fft_twiddle_apply<N, R, NS, DIR>(v + m * R, t[m]);
 }
 
-template <int N, int PASS, int DIR, bool SEQ_FAST>
+template <int N, int PASS, int DIR, bool SEQ_FAST, typename Sync = FftSyncCta>
 __device__ __forceinline__ void fft_run_pass(cplx* s, int tid, int nth, int nseq, const cplx* __restrict__ tw,
-                                             int seq_stride) {
-  fft_pass<N, fft_radix(N, PASS), fft_pass_ns(N, PASS), DIR, SEQ_FAST>(s, tid, nth, nseq,
-                                                                       tw + fft_tw_off(N, PASS), seq_stride);
+                                             int seq_stride, Sync sync = Sync()) {
+  fft_pass<N, fft_radix(N, PASS), fft_pass_ns(N, PASS), DIR, SEQ_FAST, Sync>(s, tid, nth, nseq,
+                                                                             tw + fft_tw_off(N, PASS), seq_stride, sync);
 }
 template <int N, int PASS, int DIR, bool SEQ_FAST>
 __device__ __forceinline__ void fft_run_pass_to_regs(const cplx* s, cplx* v, int tid, int nth, int nseq,
@@ -367,15 +388,18 @@ __device__ __forceinline__ void fft_run_pass_to_regs(const cplx* s, cplx* v, int
 // v[r] = x[seq][j + r*N/EPT] for the caller's butterfly (seq, j) = fft_map<N/EPT, SEQ_FAST>(tid).
 // The CTA must have exactly nseq*N/EPT threads.  DIR = -1: X[k] = sum x[n] e^{-2 pi i nk/N};
 // +1: e^{+...}; unnormalised.  A barrier must separate earlier readers of s from this call.
-template <int N, int DIR, bool SEQ_FAST>
+// Sync: the barrier between passes; a named barrier over one sequence's threads is valid when SEQ_FAST is
+// false and a sequence's N/EPT threads are whole warps (they exchange data only among themselves); the
+// caller then owes a CTA-wide barrier before threads of other sequences read s.
+template <int N, int DIR, bool SEQ_FAST, typename Sync = FftSyncCta>
 __device__ __forceinline__ void fft_regs_to_smem(cplx* v, cplx* s, int tid, int nth, int nseq,
-                                                 const cplx* __restrict__ tw, int seq_stride) {
+                                                 const cplx* __restrict__ tw, int seq_stride, Sync sync = Sync()) {
   using C = FftCfg<N>;
   int seq, j;
-  fft_map<N / C::EPT, SEQ_FAST>(tid, nseq, seq, j);
-  fft_first_from_regs<N, DIR>(v, s, seq, j, seq_stride);
-  if constexpr (C::NPASS >= 2) fft_run_pass<N, 1, DIR, SEQ_FAST>(s, tid, nth, nseq, tw, seq_stride);
-  if constexpr (C::NPASS >= 3) fft_run_pass<N, 2, DIR, SEQ_FAST>(s, tid, nth, nseq, tw, seq_stride);
+  fft_map<N / C::EPT, SEQ_FAST, N / C::EPT>(tid, 0, nth, nseq, seq, j);
+  fft_first_from_regs<N, DIR, Sync>(v, s, seq, j, seq_stride, sync);
+  if constexpr (C::NPASS >= 2) fft_run_pass<N, 1, DIR, SEQ_FAST, Sync>(s, tid, nth, nseq, tw, seq_stride, sync);
+  if constexpr (C::NPASS >= 3) fft_run_pass<N, 2, DIR, SEQ_FAST, Sync>(s, tid, nth, nseq, tw, seq_stride, sync);
 }
 
 // Whole transform registers -> registers.  On return, with RL = fft_radix(N, NPASS-1) and
@@ -389,7 +413,7 @@ __device__ __forceinline__ void fft_regs_to_regs(cplx* v, cplx* s, int tid, int 
     Dft<C::EPT, DIR>::run(v);
   } else {
     int seq, j;
-    fft_map<N / C::EPT, SEQ_FAST>(tid, nseq, seq, j);
+    fft_map<N / C::EPT, SEQ_FAST, N / C::EPT>(tid, 0, nth, nseq, seq, j);
     fft_first_from_regs<N, DIR>(v, s, seq, j, seq_stride);
     if constexpr (C::NPASS == 2) {
       fft_run_pass_to_regs<N, 1, DIR, SEQ_FAST>(s, v, tid, nth, nseq, tw, seq_stride);

@@ -47,7 +47,7 @@ __global__ void __launch_bounds__(HH >= 4096 ? 512 : 256, MINB) k_col_fwd(ColFwd
   const int g = blockIdx.y;
   const double invH = 1.0 / (double)HH;
   int c0, j0;
-  fft_map<NB0, true>(tid, ncol, c0, j0);
+  fft_map<NB0, true, 1>(tid, 0, nth, ncol, c0, j0);
   const cplx* in = P.T + (size_t)P.grp_src[g] * HH * P.NC + kx0 + c0;
   const int nspec = P.grp_n[g];
   for (int is = 0; is < nspec; ++is) {
@@ -69,7 +69,7 @@ __global__ void __launch_bounds__(HH >= 4096 ? 512 : 256, MINB) k_col_fwd(ColFwd
 #pragma unroll
       for (int m = 0; m < ITL; ++m) {
         int c, j;
-        fft_map<NBL, true>(tid + m * nth, ncol, c, j);
+        fft_map<NBL, true, 1>(tid, m, nth, ncol, c, j);
 #pragma unroll
         for (int r = 0; r < RL; ++r) out[(size_t)(j + r * NBL) * P.pitch + c] = v[m * RL + r];
       }
@@ -81,7 +81,7 @@ __global__ void __launch_bounds__(HH >= 4096 ? 512 : 256, MINB) k_col_fwd(ColFwd
 #pragma unroll
       for (int m = 0; m < ITL; ++m) {
         int c, j;
-        fft_map<NBL, true>(tid + m * nth, ncol, c, j);
+        fft_map<NBL, true, 1>(tid, m, nth, ncol, c, j);
 #pragma unroll
         for (int r = 0; r < RL; ++r) {
           const int ky = j + r * NBL;

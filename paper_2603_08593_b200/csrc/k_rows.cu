@@ -203,7 +203,14 @@ __global__ void __launch_bounds__(256, MINB) k_row2_fwd(RowFwdParams P) {
       for (int i = 0; i < SFFT_MAX_DEG; ++i) redX[i][slot] = hi[i];
     }
   }
-  fft_regs_to_smem<NC, -1, false>(v, s, tid, nth, nseq, P.twP, C::SEQ_STRIDE);
+  if constexpr (TPR >= 32 && 256 / TPR <= 8) {
+    // a row's TPR threads (whole warps) exchange data only among themselves until the split: the passes meet
+    // at a named barrier per row, so the rows of the CTA drift apart; one CTA barrier before the split
+    fft_regs_to_smem<NC, -1, false>(v, s, tid, nth, nseq, P.twP, C::SEQ_STRIDE, FftSyncNamed<256 / TPR>{1 + seq, TPR});
+    __syncthreads();
+  } else {
+    fft_regs_to_smem<NC, -1, false>(v, s, tid, nth, nseq, P.twP, C::SEQ_STRIDE);
+  }
 
   // split of both rows of the pair; this thread: half rr of tr's bins
   const cplx* sA = s + (2 * pr) * C::SEQ_STRIDE;
@@ -356,7 +363,7 @@ __global__ void __launch_bounds__(128, MINB) k_row_inv_sub(RowInvParams P) {
 #pragma unroll
   for (int m = 0; m < ITL; ++m) {
     int sq, j;
-    fft_map<NBL, false>(tid + m * nth, RB, sq, j);
+    fft_map<NBL, false, TPR>(tid, m, nth, RB, sq, j);
     const int y = y0 + sq;
     // background: B = sum_p cp[p] xi^p,  cp[p] = sum_q beta_(p,q) eta^q
     const double eta = (double)(2 * y + 1 - H) / (double)H;
