@@ -213,7 +213,7 @@ struct LagParams {
   const cplx* twW;
 };
 
-#define LAG_TH 256
+#define LAG_TH 128   // 507 CTAs of 4 warps at Full: one wave (256 threads: 1.7 waves, and twice the reduction work per kx)
 // LAG_MAXD = largest lag half-range of the instantiation: 10 (w <= 5) or 30 (w <= 15)
 
 // One CTA per (pair, lag row): lanes run along kx (coalesced reads of the lag row), every thread
@@ -255,9 +255,8 @@ __global__ void __launch_bounds__(LAG_TH) k_lag_idft(LagParams P) {
 #pragma unroll
       for (int dx = 1; dx <= LAG_MAXD; ++dx) {
         if (dx <= D) {
-          const double pc = y.x * t.x, qs = y.y * (-t.y);
-          ap[dx] += pc - qs;  // Re(y e^{+i th})
-          am[dx] += pc + qs;  // Re(y e^{-i th})
+          ap[dx] = fma(y.x, t.x, ap[dx]);   // sum Re y cos(dx th)
+          am[dx] = fma(y.y, t.y, am[dx]);   // -sum Im y sin(dx th);  Re(y e^{+-i dx th}) = their sum / difference
           t = cmul(t, t1[u]);
         }
       }
@@ -266,7 +265,8 @@ __global__ void __launch_bounds__(LAG_TH) k_lag_idft(LagParams P) {
   __shared__ double red[2][LAG_MAXD + 1][LAG_TH / 32];
 #pragma unroll
   for (int dx = 0; dx <= LAG_MAXD; ++dx) {
-    double a = ap[dx], b = am[dx];
+    double a = ap[dx] + am[dx], b = ap[dx] - am[dx];
+    if (dx == 0) { a = ap[0]; b = ap[0]; }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {
       a += __shfl_xor_sync(0xffffffffu, a, off);
@@ -350,11 +350,12 @@ __global__ void __launch_bounds__(256) k_gather(GatherParams P) {
   const int nK = L * P.TK;
   const int nKK = P.TK * (P.TK + 1) / 2;
   const size_t lag2 = (size_t)P.nLag * P.nLag;
-  const size_t total = (size_t)N * N + N;
-  for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total;
-       e += (size_t)gridDim.x * blockDim.x) {
-    if (e >= (size_t)N * N) {  // right-hand side
-      const int i = (int)(e - (size_t)N * N);
+  // grid: y = row of A (y = N: the right-hand side), x = blocks of 256 columns -- 32-bit index arithmetic only
+  const int row = blockIdx.y, col = blockIdx.x * 256 + threadIdx.x;
+  if (col >= N) return;
+  {
+    if (row == N) {  // right-hand side
+      const int i = col;
       double v;
       if (i < nK) {
         const int t = i / L, s = i - t * L;
@@ -365,9 +366,9 @@ __global__ void __launch_bounds__(256) k_gather(GatherParams P) {
         v = P.mom[P.nMomA * P.nMomA + (i - nK)];
       }
       P.b[i] = v;
-      continue;
+      return;
     }
-    const int i = (int)(e / N), j = (int)(e - (size_t)i * N);
+    const int i = row, j = col;
     double v;
     if (i < nK && j < nK) {
       int t = i / L, s = i - t * L, t2 = j / L, s2 = j - t2 * L;
@@ -399,7 +400,7 @@ __global__ void __launch_bounds__(256) k_gather(GatherParams P) {
       const int pa = P.monoB[a][0] + P.monoB[c][0], qa = P.monoB[a][1] + P.monoB[c][1];
       v = P.mom[pa * P.nMomA + qa];
     }
-    P.A[e] = v;
+    P.A[(size_t)i * N + j] = v;
   }
 }
 
@@ -473,9 +474,7 @@ sfft_status sfft_launch_lag_gather(sfft_plan* p, double* A, double* b, cudaStrea
   GP.kbStrip = p->kbStrip;
   for (int t = 0; t < p->TB; ++t) { GP.monoB[t][0] = p->monoB[t][0]; GP.monoB[t][1] = p->monoB[t][1]; }
   for (int t = 0; t < p->TK; ++t) { GP.monoK[t][0] = p->monoK[t][0]; GP.monoK[t][1] = p->monoK[t][1]; }
-  const size_t total = (size_t)p->N * p->N + p->N;
-  int blocks = (int)((total + 255) / 256);
-  if (blocks > p->num_sms * 16) blocks = p->num_sms * 16;
+  const dim3 blocks((p->N + 255) / 256, p->N + 1);   // y = row of A, y = N: the right-hand side
   k_gather<<<blocks, 256, 0, st>>>(GP);
   SFFT_LAUNCH_CHECK();
   ++*nl;
