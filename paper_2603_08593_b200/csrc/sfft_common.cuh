@@ -12,7 +12,9 @@
 #define SFFT_CR_CT 16        // k_cross: columns per CTA
 #define SFFT_CR_GP 21        // k_cross: pairs per CTA (threads = SFFT_CR_GP * SFFT_CR_CT)
 #define SFFT_CR_MAXSPEC 24   // k_cross: spectra a group may stage
+#ifndef SFFT_KB_NBLK
 #define SFFT_KB_NBLK 296     // x-CTAs of the kernel-background correction kernel (2 per SM)
+#endif
 #ifndef SFFT_T_G
 #define SFFT_T_G 4          // fused path: rows per group of the row-spectra layout T[img][y/G][kx][y%G] (2, 4 and 8 measured: 4 is best)
 #endif
