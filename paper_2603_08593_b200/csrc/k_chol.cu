@@ -258,10 +258,25 @@ k_chol_fused(const double* __restrict__ A, const double* __restrict__ b, double*
   {
     const size_t total = (size_t)(N + 1) * N;
     if (blockIdx.x == 0 && tid == 0 && info) *info = 0;
-    for (size_t e = (size_t)blockIdx.x * CH_THREADS + tid; e < total; e += (size_t)nblocks * CH_THREADS) {
-      const int i = (int)(e / N), j = (int)(e - (size_t)i * N);
-      if (i == N) Lw[(size_t)N * ld + j] = b[j];
-      else if (j <= i) Lw[(size_t)i * ld + j] = A[e];
+    // eight elements per thread and round, all requested before the first store (one memory latency per round)
+    const unsigned stride = nblocks * CH_THREADS;
+    for (unsigned e0 = blockIdx.x * CH_THREADS + tid; e0 < (unsigned)total; e0 += 8u * stride) {
+      double val[8];
+      int dst[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        const unsigned e = e0 + (unsigned)q * stride;
+        dst[q] = -1;
+        val[q] = 0.0;
+        if (e < (unsigned)total) {
+          const int i = (int)(e / (unsigned)N), j = (int)(e - (unsigned)i * (unsigned)N);
+          if (i == N) { dst[q] = N * ld + j; val[q] = b[j]; }
+          else if (j <= i) { dst[q] = i * ld + j; val[q] = A[e]; }
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < 8; ++q)
+        if (dst[q] >= 0) Lw[dst[q]] = val[q];
     }
   }
   CH_STAMP(0)
@@ -288,9 +303,19 @@ k_chol_fused(const double* __restrict__ A, const double* __restrict__ b, double*
         if (lane < nb) pre0 = ld_cg(src + lane);
         if (lane + CH_NB < nb) pre1 = ld_cg(src + lane + CH_NB);
       }
-      for (int e = tid; e < CH_PB * CH_PB; e += CH_THREADS) {
-        const int i = e >> 6, j = e & 63;
-        sd[i * CH_LDS + j] = (i < nb && j <= i) ? ld_cg(Lw + (size_t)(k0 + i) * ld + k0 + j) : (i == j ? 1.0 : 0.0);
+      {
+        // all of the thread's 16 elements are requested before the first one is stored: one L2 latency
+        double blk[CH_PB * CH_PB / CH_THREADS];
+#pragma unroll
+        for (int q = 0; q < CH_PB * CH_PB / CH_THREADS; ++q) {
+          const int e = tid + q * CH_THREADS, i = e >> 6, j = e & 63;
+          blk[q] = (i < nb && j <= i) ? ld_cg(Lw + (size_t)(k0 + i) * ld + k0 + j) : (i == j ? 1.0 : 0.0);
+        }
+#pragma unroll
+        for (int q = 0; q < CH_PB * CH_PB / CH_THREADS; ++q) {
+          const int e = tid + q * CH_THREADS, i = e >> 6, j = e & 63;
+          sd[i * CH_LDS + j] = blk[q];
+        }
       }
       const int bad = cta_potrf64(sd, ss, srd, colb, tid);
       if (bad >= 0 && bad < nb && blockIdx.x == storer && tid == 0 && info) atomicCAS(info, 0, k0 + bad + 1);
