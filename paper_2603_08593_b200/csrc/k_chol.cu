@@ -456,9 +456,17 @@ __global__ void __launch_bounds__(CHB_TH, 1) k_chol_back(const double* __restric
   const int nblk = (N + CHB_NB - 1) / CHB_NB;
   {
     const int k0 = (nblk - 1) * CHB_NB, nb = N - k0;
-    for (int e = tid; e < CHB_NB * CHB_NB; e += CHB_TH) {
-      const int i = e >> 6, j = e & 63;
-      ls[i * (CHB_NB + 1) + j] = (i < nb && j <= i) ? Lw[(size_t)(k0 + i) * ld + k0 + j] : (i == j ? 1.0 : 0.0);
+    constexpr int NQ0 = CHB_NB * CHB_NB / CHB_TH;
+    double blk[NQ0];   // all requested before the first store: one L2 latency
+#pragma unroll
+    for (int q = 0; q < NQ0; ++q) {
+      const int e = tid + q * CHB_TH, i = e >> 6, j = e & 63;
+      blk[q] = (i < nb && j <= i) ? Lw[(size_t)(k0 + i) * ld + k0 + j] : (i == j ? 1.0 : 0.0);
+    }
+#pragma unroll
+    for (int q = 0; q < NQ0; ++q) {
+      const int e = tid + q * CHB_TH;
+      ls[(e >> 6) * (CHB_NB + 1) + (e & 63)] = blk[q];
     }
   }
   __syncthreads();
