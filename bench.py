@@ -719,8 +719,8 @@ def run_cuda(args, rank, world, local_rank):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture of the final
 # kernels of this round, summarised in NCU_SOURCE (null where that capture holds no such kernel).
 NCU_SOURCE = "profiles/r02_ncu_full.md"
-NCU_TRAFFIC = {"build.colx": 283.2e6, "build.row_fwd": 364.4e6, "subtract.row_fwd": 208.5e6, "subtract.mix": 253.9e6,
-               "subtract.row_inv": 171.8e6, "solve": 4.6e6}
+NCU_TRAFFIC = {"build.colx": 282.8e6, "build.row_fwd": 363.4e6, "subtract.row_fwd": 209.1e6, "subtract.mix": 253.7e6,
+               "subtract.row_inv": 172.5e6, "solve": 4.6e6}
 
 
 def main():
