@@ -332,6 +332,17 @@ __global__ void __launch_bounds__(128, MINB) k_row_inv_sub(RowInvParams P) {
   const int y0 = blockIdx.x * RB;
   const int W = P.W, H = P.H;
   const cplx* in = P.Mhat + (size_t)(y0 + r) * NC;
+  // the science row is read only after the transform: ask L2 for it now (one request per 128-byte line)
+  if ((tid & 7) == 0) {
+#pragma unroll
+    for (int m = 0; m < ITL; ++m) {
+#pragma unroll
+      for (int rr = 0; rr < RL; ++rr) {
+        const double* a = P.S + (size_t)(y0 + r) * W + 2 * ((tid - r * TPR) + m * TPR + rr * NBL);
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+      }
+    }
+  }
   // merge: Z[k] = Xe + i Xo,  Xe = (X[k] + conj(X[NC-k]))/2,  Xo = (X[k] - conj(X[NC-k]))/2 * e^{+2 pi i k/W}
   cplx v[EPT];
   {
