@@ -43,6 +43,9 @@ struct RowFwdParams {
 #define ROW_LD(p) (*(p))
 #define ROW_ST(p, v) (*(p) = (v))
 #endif
+#ifndef SFFT_ROW_AHEAD
+#define SFFT_ROW_AHEAD 48   // k_row2_fwd: CTA-loads of row pairs between a CTA and the pair it prefetches into L2 (24..64 equal, 192 no gain)
+#endif
 #ifndef SFFT_ROW_MINB
 #define SFFT_ROW_MINB 3   // CTAs per SM the row kernels are compiled for
 #endif
@@ -131,6 +134,17 @@ __global__ void __launch_bounds__(256, MINB) k_row2_fwd(RowFwdParams P) {
   double2 raw[EPT];
 #pragma unroll
   for (int e = 0; e < EPT; ++e) raw[e] = ROW_LD(reinterpret_cast<const double2*>(src + 2 * (tr + e * TPR)));
+  // the rows of a pair that starts about one wave of CTAs later are requested from L2 now (one request per
+  // 128-byte line; R by the first image's CTA, S by the science image's, the mask with R)
+  {
+    const int pa = pairIdx + SFFT_ROW_AHEAD * (nseq >> 1);
+    if (2 * pa + 1 < H && (im == 0 || im >= P.nR)) {
+      const double* nb = (im < P.nR ? P.R : P.S) + (size_t)(2 * pa) * W;
+      for (int l = tid; l < (2 * W) / 16; l += nth) asm volatile("prefetch.global.L2 [%0];" ::"l"(nb + 16 * l));
+      if (im == 0 && P.mask)
+        for (int l = tid; l < (2 * W) / 128; l += nth) asm volatile("prefetch.global.L2 [%0];" ::"l"(P.mask + (size_t)(2 * pa) * W + 128 * l));
+    }
+  }
   // mask bits: bit 2e = element 2j masked, bit 2e+1 = element 2j+1 masked, j = tr + e*TPR
   unsigned mbits = 0u;
   if (P.mask) {
